@@ -1,0 +1,183 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs.
+
+This module serves BOTH the CPU oracle (``oracle/``) and the CUDA path.  It
+holds none of the method's arithmetic: no forces, no neighbor search, no
+integration.  It only lays atoms on an fcc lattice, draws counter-based random
+numbers and scales velocities to a temperature (input preparation the paper
+leaves to the LAMMPS input script, App. A).
+
+The workloads stand in for the LAMMPS bench input decks and the tabulated Cu
+EAM file the paper's runs used (neither is in the container); BASELINE.json's
+analytic Finnis-Sinclair-style potential replaces the table.
+
+Random numbers: counter-based, u = hash(seed, atom_id, stream) with SplitMix64
+mixing -> 53-bit uniform; Gaussians by Box-Muller.  Order independent.
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+
+import numpy as np
+
+# metal units
+KB_METAL = 8.617343e-5          # eV / K
+MVV2E_METAL = 1.0364269e-4      # amu (A/ps)^2 -> eV
+FTM2V_METAL = 1.0 / 1.0364269e-4
+
+PAIR_LJ = 1
+PAIR_EAM = 2
+PREC_FP64 = 0
+PREC_MIXED = 1
+
+_M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
+_GOLD = np.uint64(0x9E3779B97F4A7C15)
+_C1 = np.uint64(0xBF58476D1CE4E5B9)
+_C2 = np.uint64(0x94D049BB133111EB)
+_STREAM_MUL = np.uint64(0xD1B54A32D192ED03)
+
+
+def _splitmix64(z: np.ndarray) -> np.ndarray:
+    """One SplitMix64 output step on an array of uint64 counters."""
+    with np.errstate(over="ignore"):
+        z = (z + _GOLD) & _M64
+        z = ((z ^ (z >> np.uint64(30))) * _C1) & _M64
+        z = ((z ^ (z >> np.uint64(27))) * _C2) & _M64
+        return z ^ (z >> np.uint64(31))
+
+
+def hash_u64(seed: int, ids: np.ndarray, stream: int) -> np.ndarray:
+    """64-bit hash of (seed, atom id, stream)."""
+    ids = np.asarray(ids, dtype=np.uint64)
+    with np.errstate(over="ignore"):
+        s = _splitmix64(np.full(1, seed, dtype=np.uint64))[0]
+        k = (ids * _GOLD + np.uint64(stream) * _STREAM_MUL) & _M64
+        return _splitmix64(_splitmix64(k ^ s))
+
+
+def uniform01(seed: int, ids: np.ndarray, stream: int) -> np.ndarray:
+    """Uniform in [0, 1) with 53 random bits."""
+    return (hash_u64(seed, ids, stream) >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+
+
+def gaussian(seed: int, ids: np.ndarray, stream: int) -> np.ndarray:
+    """Standard normal by Box-Muller on streams (2*stream+16, 2*stream+17)."""
+    u1 = uniform01(seed, ids, 2 * stream + 16)
+    u2 = uniform01(seed, ids, 2 * stream + 17)
+    return np.sqrt(-2.0 * np.log1p(-u1)) * np.cos(2.0 * math.pi * u2)
+
+
+def fcc_lattice(n: int, a: float) -> tuple[np.ndarray, np.ndarray]:
+    """n x n x n fcc unit cells of edge a.  Atom index = ((iz*n+iy)*n+ix)*4+b.
+
+    Returns (positions [4n^3, 3] float64, box [3])."""
+    basis = np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.0], [0.5, 0.0, 0.5], [0.0, 0.5, 0.5]])
+    iz, iy, ix = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    cell = np.stack([ix.ravel(), iy.ravel(), iz.ravel()], axis=1).astype(np.float64)
+    x = (cell[:, None, :] + basis[None, :, :]).reshape(-1, 3) * a
+    return np.ascontiguousarray(x), np.array([n * a] * 3, dtype=np.float64)
+
+
+def thermal_velocities(seed: int, ids: np.ndarray, mass: np.ndarray, kT: float, mvv2e: float) -> np.ndarray:
+    """v ~ N(0, kT/m); subtract the centre-of-mass velocity; rescale so that
+    sum 1/2 m v^2 * mvv2e = 1/2 (3N-3) kT exactly."""
+    n = len(ids)
+    v = np.stack([gaussian(seed, ids, c) for c in range(3)], axis=1)
+    v *= np.sqrt(kT / (mass * mvv2e))[:, None]
+    v -= (mass[:, None] * v).sum(axis=0) / mass.sum()
+    ke = 0.5 * mvv2e * float((mass[:, None] * v * v).sum())
+    v *= math.sqrt(0.5 * (3 * n - 3) * kT / ke)
+    return np.ascontiguousarray(v)
+
+
+def uniform_displacements(seed: int, ids: np.ndarray, amplitude: float) -> np.ndarray:
+    """Each coordinate ~ U(-amplitude, +amplitude); streams 3..5."""
+    return np.stack([(2.0 * uniform01(seed, ids, 3 + c) - 1.0) * amplitude for c in range(3)], axis=1)
+
+
+def permutation(seed: int, n: int) -> np.ndarray:
+    """Seeded permutation: sort atoms by their 64-bit key (stream 6), ties by id."""
+    key = hash_u64(seed, np.arange(n, dtype=np.uint64), 6)
+    return np.lexsort((np.arange(n), key))
+
+
+@dataclasses.dataclass
+class Workload:
+    name: str
+    cfg: int
+    x: np.ndarray            # [N,3] float64, inside [0,L)
+    v: np.ndarray            # [N,3] float64
+    box: np.ndarray          # [3]
+    types: np.ndarray        # [N] int32 (all zero: single species)
+    mass: np.ndarray         # [ntypes]
+    style: int
+    params: tuple            # LJ: (eps, sigma); EAM: (A, p, B, q, r0)
+    rc: float
+    skin: float
+    dt: float
+    nsteps: int
+    precision: int
+    ftm2v: float
+    mvv2e: float
+    kT: float
+    seed: int
+
+    @property
+    def natoms(self) -> int:
+        return int(self.x.shape[0])
+
+
+LJ_RHO = 0.8442
+LJ_A = (4.0 / LJ_RHO) ** (1.0 / 3.0)
+CU_A = 3.615
+EAM_PARAMS = (0.0855, 10.96, 1.2240, 2.278, 2.556)   # A[eV], p, B[eV], q, r0[A]  (BASELINE.json cfg 4)
+
+# cfg -> (style, n_cells, rc, skin, dt, nsteps, precision, permuted)
+_TABLE = {
+    1: ("LJ 12-6 fluid 4,000 atoms fp64", PAIR_LJ, 10, 2.5, 0.3, 0.005, 100, PREC_FP64, False),
+    2: ("LJ 12-6 fluid 32,000 atoms mixed", PAIR_LJ, 20, 2.5, 0.3, 0.005, 1000, PREC_MIXED, False),
+    3: ("LJ 12-6 fluid 256,000 atoms rc=5.0 mixed", PAIR_LJ, 40, 5.0, 0.3, 0.005, 500, PREC_MIXED, False),
+    4: ("EAM Cu 256,000 atoms mixed", PAIR_EAM, 40, 4.95, 1.0, 0.001, 500, PREC_MIXED, False),
+    5: ("LJ 12-6 liquid 4,000,000 atoms permuted mixed", PAIR_LJ, 100, 2.5, 0.3, 0.005, 200, PREC_MIXED, True),
+}
+
+
+def make(cfg: int, n_override: int | None = None, seed_offset: int = 0) -> Workload:
+    """Build config ``cfg`` (1..5) of BASELINE.json.  ``n_override`` shrinks the
+    lattice (unit cells per edge) for tests; ``seed_offset`` decorrelates replicas."""
+    name, style, n, rc, skin, dt, nsteps, prec, permuted = _TABLE[cfg]
+    if n_override is not None:
+        n = int(n_override)
+    seed = 43300 + cfg + 1000 * seed_offset
+    if style == PAIR_LJ:
+        x, box = fcc_lattice(n, LJ_A)
+        mass = np.array([1.0])
+        kT, ftm2v, mvv2e = 1.44, 1.0, 1.0
+        params = (1.0, 1.0)
+    else:
+        x, box = fcc_lattice(n, CU_A)
+        mass = np.array([63.55])
+        kT, ftm2v, mvv2e = KB_METAL * 300.0, FTM2V_METAL, MVV2E_METAL
+        params = EAM_PARAMS
+    N = x.shape[0]
+    ids = np.arange(N, dtype=np.uint64)
+    if style == PAIR_EAM:
+        x = x + uniform_displacements(seed, ids, 0.05)
+        x -= np.floor(x / box) * box
+    v = thermal_velocities(seed, ids, np.full(N, mass[0]), kT, mvv2e)
+    if permuted:
+        p = permutation(seed, N)
+        x, v = np.ascontiguousarray(x[p]), np.ascontiguousarray(v[p])
+    return Workload(name=name, cfg=cfg, x=x, v=v, box=box, types=np.zeros(N, dtype=np.int32), mass=mass,
+                    style=style, params=params, rc=rc, skin=skin, dt=dt, nsteps=nsteps, precision=prec,
+                    ftm2v=ftm2v, mvv2e=mvv2e, kT=kT, seed=seed)
+
+
+def perturbed(w: Workload, amplitude: float, seed: int = 7) -> np.ndarray:
+    """Positions of ``w`` with seeded uniform displacements, wrapped into the box.
+    Force-parity snapshots need this: a perfect lattice has zero net force
+    (SURVEY.md §7 hard part 7)."""
+    ids = np.arange(w.natoms, dtype=np.uint64)
+    x = w.x + uniform_displacements(seed, ids, amplitude)
+    x -= np.floor(x / w.box) * w.box
+    return np.ascontiguousarray(x)
