@@ -1,0 +1,163 @@
+/*
+ * md_b200.h -- C ABI of the B200-native short-range molecular-dynamics hot path
+ *              of arXiv 1009.4330 (Trott, Winterfeld, Crozier, "General-purpose
+ *              molecular dynamics simulations on GPU-based clusters").
+ *
+ * The library (libmd_b200.so, hand-written CUDA for sm_100a) owns all device
+ * state of one periodic orthogonal box of N atoms and runs, on ONE GPU:
+ *
+ *   cell binning + counting sort + spatial reorder      ("spatially ordered")
+ *   Verlet neighbor-list build, full or half            (numneigh[i], neighbors[i][jj])
+ *   pair forces: LJ 12-6 and two-pass EAM               (App. A)
+ *     thread-per-atom (TpA, L88-104), sub-warp/warp-per-atom with shuffle
+ *     reduction (the paper's block-per-atom BpA, L105-122), direct cell list (L64-82),
+ *     chosen by a setup-time mini benchmark (L137)
+ *   velocity-Verlet NVE, positions/velocities/forces resident on the device (L50-58)
+ *   rebuild iff max_i |x_i - x0_i|^2 > (skin/2)^2, decided on the device.
+ *
+ * Conventions
+ *   - Every call returns MD_OK (0) or a negative MD_ERR_*; nothing throws or
+ *     aborts across the ABI.  md_last_error() gives the text of the last failure.
+ *   - The handle owns all device memory.  Caller buffers are only read or
+ *     written during the call; they may be HOST or DEVICE pointers (detected
+ *     with cudaPointerGetAttributes; pageable or pinned host memory both work).
+ *   - Per-atom arrays are N x 3 AoS doubles in the CALLER'S atom order; the
+ *     spatial permutation the library applies internally is invisible.
+ *   - All work is enqueued on the stream given to md_create (a cudaStream_t
+ *     passed as void*; NULL = the legacy default stream).  Calls that return
+ *     host scalars or fill host buffers synchronise that stream.
+ *   - Units are the caller's: accelerations are f/m * ftm2v, kinetic energy is
+ *     1/2 m v^2 * mvv2e (LJ reduced units: 1, 1; LAMMPS-metal: see md_set_units).
+ *   - Precision modes: MD_FP64 computes everything in double;
+ *     MD_MIXED computes pair terms in fp32 from tile-centred fp32 coordinates and
+ *     accumulates per-atom sums, energy and virial in fp64; positions,
+ *     velocities, forces, the list-build distance test and the integrator are
+ *     fp64 in both modes.
+ */
+#ifndef MD_B200_H
+#define MD_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct md_system md_system; /* opaque */
+
+/* error codes */
+#define MD_OK 0
+#define MD_ERR_BAD_ARGUMENT (-1)   /* NULL pointer, N <= 0, unknown enum, bad parameter count ... */
+#define MD_ERR_BOX_TOO_SMALL (-2)  /* some box edge < 3 (rc + skin): the 27-cell stencil would double count */
+#define MD_ERR_CUDA (-3)           /* a CUDA runtime call failed; text in md_last_error */
+#define MD_ERR_OVERFLOW (-4)       /* a tile or neighbor row outgrew its capacity even after re-planning */
+#define MD_ERR_NOT_READY (-5)      /* positions or pair style not set yet */
+#define MD_ERR_NONFINITE (-6)      /* a non-finite coordinate reached the binning kernel */
+
+/* precision modes */
+#define MD_FP64 0
+#define MD_MIXED 1
+
+/* pair styles */
+#define MD_PAIR_LJ126 1   /* params = {eps, sigma}:   u = 4 eps [(s/r)^12 - (s/r)^6], plain cut at rc (lj/cut, L256) */
+#define MD_PAIR_EAM_FS 2  /* params = {A, p, B, q, r0}: phi = A exp(-p(r/r0-1)), rho = exp(-q(r/r0-1)),
+                             F(rho) = -B sqrt(rho), F'(0) := 0; E = sum_i F(rho_i) + 1/2 sum_ij phi (L260) */
+
+/* neighbor-list kinds */
+#define MD_LIST_FULL 0    /* both (i,j) and (j,i): each kernel row writes only f[i] (L104) */
+#define MD_LIST_HALF 1    /* each pair once; -F scattered to j with atomics (Newton's third law, L76) */
+
+/* force-kernel variants */
+#define MD_KERNEL_AUTO 0     /* setup-time mini benchmark picks among TPA / SUBWARP / WARP (L137) */
+#define MD_KERNEL_TPA 1      /* one thread per atom (L88-104) */
+#define MD_KERNEL_SUBWARP 2  /* 8 lanes per atom, shuffle reduction */
+#define MD_KERNEL_WARP 3     /* 32 lanes per atom, shuffle reduction (the paper's BpA, L105-122) */
+#define MD_KERNEL_CELL 4     /* no list: every atom scans the 27-cell stencil of its tile (L64-82) */
+
+typedef struct md_stats {
+  int64_t natoms;
+  int64_t nsteps_total;        /* time steps integrated since md_create */
+  int64_t nbuilds;             /* neighbor-list builds since md_create */
+  int64_t nforce_evals;        /* force evaluations since md_create */
+  int32_t kernel_variant;      /* MD_KERNEL_* actually in use (AUTO resolved) */
+  int32_t list_kind;
+  int32_t precision;
+  int32_t lanes_per_atom;      /* 1, 8 or 32 */
+  int32_t ncells[3];           /* cell grid */
+  int32_t brick[3];            /* cells per tile edge (interior) */
+  int32_t ntiles;              /* thread blocks per force launch */
+  int32_t tile_capacity;       /* staged atoms a tile can hold */
+  int32_t max_tile_atoms;      /* largest staged count seen at the last build */
+  int32_t max_neighbors;       /* longest list row at the last build */
+  int32_t row_capacity;        /* list row capacity (entries) */
+  int32_t reserved_;
+  double mean_neighbors;       /* mean list row length at the last build */
+  double kinetic_energy;       /* 1/2 sum m v^2 mvv2e at the time of the call */
+  double ms_build;             /* device time of the last list build (bin+sort+build), CUDA events */
+  double ms_force;             /* device time of the last md_compute_forces */
+  double ms_run;               /* device time of the last md_run */
+  int64_t launches_last_run;   /* kernels launched by the last md_run */
+  int64_t launches_total;      /* kernels launched since md_create */
+} md_stats;
+
+/* Creates a system: orthogonal periodic box [0,Lx) x [0,Ly) x [0,Lz), N atoms with type ids in
+ * 0..ntypes-1 (caller order, host or device pointer) and per-type masses (host pointer).
+ * stream: a cudaStream_t (void*), NULL for the default stream.  (north_star md_create) */
+int md_create(md_system** out, const double box[3], int64_t N, const int32_t* types, int ntypes,
+              const double* mass, void* cuda_stream);
+void md_destroy(md_system* s);
+
+/* LJ reduced units: (1, 1).  LAMMPS-metal (A, eV, amu, ps): ftm2v = 1/1.0364269e-4, mvv2e = 1.0364269e-4. */
+int md_set_units(md_system* s, double ftm2v, double mvv2e);
+/* MD_FP64 or MD_MIXED.  Invalidates the neighbor list. */
+int md_set_precision(md_system* s, int mode);
+/* N x 3 doubles, caller order, host or device.  Positions may lie outside the box (they are wrapped at
+ * the next build).  Setting positions invalidates the neighbor list and the cached forces. */
+int md_set_positions(md_system* s, const double* x);
+int md_set_velocities(md_system* s, const double* v);
+/* One parameter set for all type pairs (single-species potentials; types select masses).
+ * Fails with MD_ERR_BOX_TOO_SMALL unless every box edge >= 3 (rc + skin).  (north_star md_set_pair) */
+int md_set_pair(md_system* s, int style, const double* params, int nparams, double rc, double skin);
+/* list_kind: MD_LIST_FULL | MD_LIST_HALF; kernel: MD_KERNEL_*.  HALF needs TPA.  Invalidates the list. */
+int md_set_neighbor(md_system* s, int list_kind, int kernel);
+
+/* Wrap into the box, bin into cells of edge >= rc+skin, counting-sort and reorder atoms, build the
+ * Verlet list from the 27-cell stencil (fp64 distance test r^2 < (rc+skin)^2), reset x0.
+ * (north_star (1),(2); md_build_neighbors) */
+int md_build_neighbors(md_system* s);
+
+/* Forces at the current positions (builds the list first if it is not valid).  f_out: N x 3 doubles in
+ * caller order, host or device, may be NULL.  energy_out: total potential energy (host double), may be
+ * NULL.  virial_out: xx,yy,zz,xy,xz,yz with W_ab = sum over pairs (each once) of D_a f_b (host), may be
+ * NULL.  (north_star md_compute_forces) */
+int md_compute_forces(md_system* s, double* f_out, double* energy_out, double virial_out[6]);
+
+/* nsteps of velocity-Verlet NVE with time step dt: v += dt/2 f/m ftm2v; x += dt v;
+ * [rebuild iff max |x-x0|^2 > (skin/2)^2]; f = F(x); v += dt/2 f/m ftm2v.  Asynchronous apart from the
+ * rebuild decisions.  (north_star md_run) */
+int md_run(md_system* s, int64_t nsteps, double dt);
+
+/* Current state in caller order (host or device buffers of N x 3 doubles).  Positions are as stored:
+ * inside the box at the last build, possibly slightly outside since. */
+int md_get_positions(md_system* s, double* x);
+int md_get_velocities(md_system* s, double* v);
+/* Forces of the last evaluation (md_compute_forces or the last step of md_run). */
+int md_get_forces(md_system* s, double* f);
+
+/* The current neighbor list in CALLER ids, for pair-set parity: numneigh[N] and neigh[N x stride]
+ * (host or device int32 buffers).  Rows longer than stride are truncated (numneigh still holds the true
+ * length).  Half lists hold each unordered pair in exactly one of the two rows. */
+int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride);
+
+/* Setup-time mini benchmark of PAPER.md L137: times nrep force evaluations with each of TPA, SUBWARP
+ * and WARP on the current positions, keeps the fastest, and reports the three times (ms per
+ * evaluation, indexed by MD_KERNEL_TPA..MD_KERNEL_WARP minus 1) if ms_out is not NULL. */
+int md_autotune(md_system* s, int nrep, double ms_out[3]);
+
+int md_get_stats(md_system* s, md_stats* out);
+const char* md_last_error(const md_system* s); /* s may be NULL: error of a failed md_create */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MD_B200_H */

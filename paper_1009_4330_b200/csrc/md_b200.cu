@@ -1,0 +1,679 @@
+// md_b200.cu -- host side of the C ABI declared in include/md_b200.h.
+// Every step of the hot path runs in the kernels of md_kernels.cuh; this file owns device memory,
+// plans tile geometry, launches, and marshals caller buffers.  There is no CPU fallback: any CUDA
+// failure is reported as MD_ERR_CUDA.
+#include "../../include/md_b200.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <string>
+
+#include "md_kernels.cuh"
+
+using namespace mdk;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct md_system_impl {
+  int64_t N = 0;
+  size_t ld = 0;   // leading dimension of SoA arrays (N rounded up to 32)
+  cudaStream_t stream = nullptr;
+  double box[3] = {0, 0, 0};
+  int ntypes = 0;
+  double ftm2v = 1.0, mvv2e = 1.0;
+  int precision = MD_FP64;
+  int style = 0;
+  double params[5] = {0, 0, 0, 0, 0};
+  double rc = 0, skin = 0;
+  int list_kind = MD_LIST_FULL;
+  int kernel_req = MD_KERNEL_TPA;
+  int kernel_eff = MD_KERNEL_TPA;
+  bool autotuned = false;
+  bool have_x = false, pair_set = false, planned = false, list_valid = false, forces_valid = false;
+  bool list_built_for_export = false;
+
+  // device arrays (sorted order, SoA with leading dimension ld)
+  double* x[2] = {nullptr, nullptr};
+  double* v[2] = {nullptr, nullptr};
+  int* id[2] = {nullptr, nullptr};
+  int* type[2] = {nullptr, nullptr};
+  int cur = 0;
+  double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
+  int *cell_of = nullptr, *rank = nullptr, *perm = nullptr, *numneigh = nullptr;
+  int *cell_count = nullptr, *cell_start = nullptr;
+  size_t cell_alloc = 0;
+  uint4* list = nullptr;
+  size_t list_words = 0;
+  double* mass_d = nullptr;
+  double* ev_partials = nullptr;
+  size_t ev_tiles_alloc = 0;
+  double* scalars_d = nullptr;   // 16 doubles: [0..7] energy/virial, [8] kinetic
+  double* io_d = nullptr;        // 3N doubles, staging for host pointers
+  int* io_i = nullptr;           // N ints staging
+  int* types_caller = nullptr;   // types in caller order (device)
+  Flags* flags_d = nullptr;
+  Flags* flags_h = nullptr;      // pinned
+  double* scalars_h = nullptr;   // pinned, 16 doubles
+
+  Geom g{};
+  PairParams P{};
+  double cap_scale_tile = 1.0, cap_scale_int = 1.0, cap_scale_row = 1.0;
+
+  // stats
+  int64_t nsteps_total = 0, nbuilds = 0, nforce = 0, launches = 0, launches_last_run = 0;
+  int max_tile_atoms = 0, max_row = 0;
+  double mean_row = 0;
+  double ms_build = 0, ms_force = 0, ms_run = 0;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr, ev3 = nullptr;
+
+  std::map<const void*, size_t> smem_set;
+  std::string err;
+};
+
+}  // namespace
+
+struct md_system : md_system_impl {};
+
+namespace {
+
+int fail(md_system* s, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (s) s->err = buf; else g_create_error = buf;
+  return code;
+}
+
+#define CK(call)                                                                                         \
+  do {                                                                                                   \
+    cudaError_t e_ = (call);                                                                             \
+    if (e_ != cudaSuccess) return fail(s, MD_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+  } while (0)
+
+template <class Kern, class... Args>
+cudaError_t launch(md_system* s, Kern kern, unsigned grid, unsigned block, size_t smem, Args... args) {
+  if (grid == 0) return cudaSuccess;
+  if (smem > 48 * 1024) {
+    const void* key = reinterpret_cast<const void*>(kern);
+    auto it = s->smem_set.find(key);
+    if (it == s->smem_set.end() || it->second < smem) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e != cudaSuccess) return e;
+      s->smem_set[key] = smem;
+    }
+  }
+  kern<<<grid, block, smem, s->stream>>>(args...);
+  s->launches++;
+  return cudaGetLastError();
+}
+
+inline unsigned blocks_for(int64_t n, int block) { return (unsigned)((n + block - 1) / block); }
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  cudaError_t e = cudaPointerGetAttributes(&a, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+template <class T>
+cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T)); }
+
+int lanes_for(int kernel) { return kernel == MD_KERNEL_SUBWARP ? 8 : (kernel == MD_KERNEL_WARP ? 32 : 1); }
+
+// ---- planning: cell grid, tile width, capacities -----------------------------------------------------
+size_t force_smem(const md_system* s, const Geom& g, bool half) {
+  size_t elem = s->precision == MD_FP64 ? sizeof(double4) : sizeof(float4);
+  return sizeof(TileTables) + (size_t)(g.tile_cap + 1) * elem + (half ? (size_t)(g.tile_cap + 1) * 4 : 0) + 16;
+}
+size_t build_smem(const Geom& g) { return sizeof(TileTables) + 3 * (size_t)(g.tile_cap + 1) * sizeof(double) + 16; }
+
+void fill_geom_for_b(const md_system* s, int b, Geom& g) {
+  double rl = s->rc + s->skin;
+  g.ncell = 1;
+  for (int d = 0; d < 3; ++d) {
+    g.L[d] = s->box[d];
+    g.nc[d] = (int)std::floor(s->box[d] / rl);
+    g.edge[d] = s->box[d] / g.nc[d];
+    g.inv_edge[d] = g.nc[d] / s->box[d];
+    g.b[d] = std::min(b, g.nc[d]);
+    g.nb[d] = (g.nc[d] + g.b[d] - 1) / g.b[d];
+    g.ncell *= g.nc[d];
+  }
+  g.ntiles = g.nb[0] * g.nb[1] * g.nb[2];
+  double per_cell = (double)s->N / g.ncell;
+  double staged = per_cell * (g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2);
+  double interior = per_cell * g.b[0] * g.b[1] * g.b[2];
+  g.tile_cap = (int)(staged * 1.2 * s->cap_scale_tile + 64);
+  g.tile_cap = (g.tile_cap + 7) & ~7;
+  g.interior_cap = (int)(interior * 1.25 * s->cap_scale_int + 32);
+  g.interior_cap = (g.interior_cap + 31) & ~31;
+  g.K = lanes_for(s->kernel_eff);
+  g.half = s->list_kind == MD_LIST_HALF ? 1 : 0;
+  double vol = s->box[0] * s->box[1] * s->box[2];
+  double mean_nb = 4.0 / 3.0 * M_PI * rl * rl * rl * s->N / vol * (g.half ? 0.5 : 1.0);
+  int unit = 8 * g.K;
+  g.row_cap = (int)(mean_nb * 1.5 * s->cap_scale_row + 24);
+  g.row_cap = ((g.row_cap + unit - 1) / unit) * unit;
+  g.chunk_cap = g.row_cap / unit;
+}
+
+int plan(md_system* s) {
+  double rl = s->rc + s->skin;
+  for (int d = 0; d < 3; ++d)
+    if (s->box[d] < 3.0 * rl) return fail(s, MD_ERR_BOX_TOO_SMALL, "box edge %d = %g < 3 (rc+skin) = %g", d, s->box[d], 3.0 * rl);
+  int forced = 0;
+  if (const char* e = getenv("MD_B200_BRICK")) forced = atoi(e);
+  double vol = s->box[0] * s->box[1] * s->box[2];
+  double lscale = std::cbrt(vol / (double)s->N);   // ~ nearest-neighbor distance
+  int best = 0;
+  Geom g{};
+  const size_t smem_soft = 100 * 1024, smem_hard = 200 * 1024;
+  for (int pass = 0; pass < 3 && !best; ++pass) {
+    // pass 0: all preferences; pass 1: drop the tile-count preference; pass 2: only hard limits
+    for (int b = 6; b >= 1; --b) {
+      if (forced && b != forced) continue;
+      fill_geom_for_b(s, b, g);
+      if ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) > MAX_TILE_CELLS) continue;
+      if (g.tile_cap + 1 > 65535) continue;
+      size_t sm = std::max(force_smem(s, g, g.half), build_smem(g));
+      if (sm > smem_hard) continue;
+      if (!forced && pass < 2) {
+        if (sm > smem_soft) continue;
+        double half_extent = 0;
+        for (int d = 0; d < 3; ++d) half_extent = std::max(half_extent, 0.5 * (g.b[d] + 2) * g.edge[d]);
+        if (s->precision == MD_MIXED && half_extent > 9.0 * lscale && b > 1) continue;   // fp32 tile coordinates
+        if (pass == 0 && g.ntiles < 2 * 148) continue;
+      }
+      best = b;
+      break;
+    }
+  }
+  if (!best) return fail(s, MD_ERR_OVERFLOW, "no tile width fits shared memory (density too high for cells of edge rc+skin)");
+  fill_geom_for_b(s, best, g);
+  s->g = g;
+  // pair constants
+  PairParams& P = s->P;
+  P = PairParams{};
+  P.rc2 = s->rc * s->rc;
+  if (s->style == MD_PAIR_LJ126) {
+    double eps = s->params[0], sg = s->params[1];
+    double s6 = std::pow(sg, 6), s12 = s6 * s6;
+    P.lj1 = 48.0 * eps * s12; P.lj2 = 24.0 * eps * s6; P.lj3 = 4.0 * eps * s12; P.lj4 = 4.0 * eps * s6;
+  } else {
+    P.A = s->params[0]; P.p = s->params[1]; P.B = s->params[2]; P.q = s->params[3];
+    P.inv_r0 = 1.0 / s->params[4]; P.p_r0 = P.p * P.inv_r0; P.q_r0 = P.q * P.inv_r0;
+  }
+  // (re)allocate what depends on the geometry
+  if ((size_t)g.ncell + 1 > s->cell_alloc) {
+    cudaFree(s->cell_count); cudaFree(s->cell_start);
+    s->cell_alloc = (size_t)g.ncell + 1;
+    CK(dalloc(&s->cell_count, s->cell_alloc));
+    CK(dalloc(&s->cell_start, s->cell_alloc));
+  }
+  size_t words = (size_t)g.ntiles * g.chunk_cap * g.interior_cap * g.K;
+  if (words > s->list_words) {
+    cudaFree(s->list);
+    s->list = nullptr; s->list_words = 0;
+    CK(dalloc(&s->list, words));
+    s->list_words = words;
+  }
+  if ((size_t)g.ntiles > s->ev_tiles_alloc) {
+    cudaFree(s->ev_partials);
+    s->ev_tiles_alloc = g.ntiles;
+    CK(dalloc(&s->ev_partials, (size_t)g.ntiles * 8));
+  }
+  s->planned = true;
+  s->list_valid = false;
+  return MD_OK;
+}
+
+// ---- build ------------------------------------------------------------------------------------------
+int build_list_only(md_system* s) {
+  const Geom& g = s->g;
+  double rl = s->rc + s->skin;
+  CK(launch(s, k_build_list, g.ntiles, BLOCK, build_smem(g), g, (const int*)s->cell_start, (const double*)s->x[s->cur], s->ld,
+            rl * rl, s->list, s->numneigh, s->flags_d));
+  return MD_OK;
+}
+
+int build(md_system* s, bool need_list) {
+  if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set before building");
+  for (int attempt = 0; attempt < 6; ++attempt) {
+    if (!s->planned) { int rc = plan(s); if (rc) return rc; }
+    const Geom& g = s->g;
+    const int N = (int)s->N;
+    CK(cudaEventRecord(s->ev2, s->stream));
+    CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
+    CK(cudaMemsetAsync(s->cell_count, 0, (size_t)(g.ncell + 1) * sizeof(int), s->stream));
+    int c = s->cur, o = 1 - c;
+    CK(launch(s, k_bin, blocks_for(N, 256), 256, 0, g, N, s->x[c], s->x[c] + s->ld, s->x[c] + 2 * s->ld, s->cell_of, s->rank,
+              s->cell_count, s->flags_d));
+    CK(launch(s, k_scan_cells, 1, 1024, 0, g.ncell, (const int*)s->cell_count, s->cell_start));
+    CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
+              s->perm));
+    CK(launch(s, k_sort_cells, blocks_for(g.ncell, 128), 128, 0, g.ncell, (const int*)s->cell_start, s->perm));
+    CK(launch(s, k_permute, blocks_for(N, 256), 256, 0, N, (const int*)s->perm, (const double*)s->x[c], (const double*)s->v[c],
+              (const int*)s->id[c], (const int*)s->type[c], s->x[o], s->v[o], s->id[o], s->type[o], s->x0, s->ld));
+    s->cur = o;
+    s->forces_valid = false;
+    bool do_list = need_list || s->kernel_eff != MD_KERNEL_CELL;
+    if (do_list) { int rc = build_list_only(s); if (rc) return rc; }
+    CK(cudaEventRecord(s->ev3, s->stream));
+    CK(cudaMemcpyAsync(s->flags_h, s->flags_d, sizeof(Flags), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    float ms = 0;
+    cudaEventElapsedTime(&ms, s->ev2, s->ev3);
+    s->ms_build = ms;
+    s->nbuilds++;
+    const Flags& F = *s->flags_h;
+    if (F.nonfinite) return fail(s, MD_ERR_NONFINITE, "a non-finite coordinate reached the binning kernel");
+    bool again = false;
+    if (do_list) {
+      if (F.need_tile_cap > g.tile_cap) { s->cap_scale_tile *= 1.1 * (double)F.need_tile_cap / g.tile_cap; again = true; }
+      if (F.need_interior_cap > g.interior_cap) { s->cap_scale_int *= 1.1 * (double)F.need_interior_cap / g.interior_cap; again = true; }
+      if (F.need_row_cap > g.row_cap) { s->cap_scale_row *= 1.1 * (double)F.need_row_cap / g.row_cap; again = true; }
+    }
+    if (again) { s->planned = false; continue; }
+    s->max_tile_atoms = F.max_tile_atoms;
+    s->max_row = F.max_row;
+    s->mean_row = (double)F.sum_rows / (double)s->N;
+    s->list_valid = true;
+    s->list_built_for_export = do_list;
+    return MD_OK;
+  }
+  return fail(s, MD_ERR_OVERFLOW, "tile or neighbor-row capacity still exceeded after re-planning");
+}
+
+// ---- force dispatch ------------------------------------------------------------------------------------
+template <typename T, class Body, int MODE, bool EV>
+int launch_force_variant(md_system* s, const ForceArgs& A) {
+  const Geom& g = s->g;
+  const bool half = g.half != 0;
+  size_t smem = force_smem(s, g, half && MODE == 0);
+  if (s->kernel_eff == MD_KERNEL_CELL) {
+    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false, true>, g.ntiles, BLOCK, smem, A));
+  } else if (half) {
+    if constexpr (MODE == 0) {
+      CK(cudaMemsetAsync(A.f, 0, 3 * s->ld * sizeof(double), s->stream));
+      CK(launch(s, k_tile_force<T, Body, 1, 0, EV, true, false>, g.ntiles, BLOCK, smem, A));
+    } else {
+      return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
+    }
+  } else if (g.K == 1) {
+    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false, false>, g.ntiles, BLOCK, smem, A));
+  } else if (g.K == 8) {
+    CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false, false>, g.ntiles, BLOCK, smem, A));
+  } else {
+    CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false, false>, g.ntiles, BLOCK, smem, A));
+  }
+  return MD_OK;
+}
+
+template <typename T, bool EV>
+int launch_force_T(md_system* s) {
+  const Geom& g = s->g;
+  ForceArgs A{};
+  A.g = g; A.P = s->P; A.cell_start = s->cell_start; A.x = s->x[s->cur]; A.ld = s->ld; A.list = s->list;
+  A.numneigh = s->numneigh; A.fp_in = nullptr; A.f = s->f; A.rho = s->rho; A.fp_out = s->fp; A.ev_partials = s->ev_partials;
+  if (s->style == MD_PAIR_LJ126) {
+    int rc = launch_force_variant<T, LJBody<T, EV>, 0, EV>(s, A);
+    if (rc) return rc;
+    if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
+  } else {
+    int rc = launch_force_variant<T, EamDensityBody<T>, 1, false>(s, A);   // pass 1: rho, F'(rho), sum F(rho)
+    if (rc) return rc;
+    if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
+    A.fp_in = s->fp;
+    rc = launch_force_variant<T, EamForceBody<T, EV>, 0, EV>(s, A);          // pass 2: forces
+    if (rc) return rc;
+    if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 1));
+  }
+  s->nforce++;
+  s->forces_valid = true;
+  return MD_OK;
+}
+
+int compute_forces_device(md_system* s, bool ev) {
+  if (s->precision == MD_FP64) return ev ? launch_force_T<double, true>(s) : launch_force_T<double, false>(s);
+  return ev ? launch_force_T<float, true>(s) : launch_force_T<float, false>(s);
+}
+
+int autotune(md_system* s, int nrep, double* ms_out);
+
+int ensure_list(md_system* s) {
+  if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set first");
+  if (s->kernel_req == MD_KERNEL_AUTO && !s->autotuned) {
+    int rc = autotune(s, 3, nullptr);
+    if (rc) return rc;
+  }
+  if (!s->list_valid) return build(s, false);
+  return MD_OK;
+}
+
+int autotune(md_system* s, int nrep, double* ms_out) {
+  if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set first");
+  if (s->list_kind == MD_LIST_HALF) { s->kernel_eff = MD_KERNEL_TPA; s->autotuned = true; s->planned = false; return MD_OK; }
+  if (nrep < 1) nrep = 1;
+  const int cand[3] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP};
+  double best_ms = 1e300;
+  int best = MD_KERNEL_TPA;
+  for (int k = 0; k < 3; ++k) {
+    s->kernel_eff = cand[k];
+    s->planned = false;
+    int rc = build(s, true);
+    if (rc) return rc;
+    rc = compute_forces_device(s, false);   // warm-up
+    if (rc) return rc;
+    CK(cudaEventRecord(s->ev0, s->stream));
+    for (int r = 0; r < nrep; ++r) { rc = compute_forces_device(s, false); if (rc) return rc; }
+    CK(cudaEventRecord(s->ev1, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    float ms = 0;
+    cudaEventElapsedTime(&ms, s->ev0, s->ev1);
+    double per = ms / nrep;
+    if (ms_out) ms_out[k] = per;
+    if (per < best_ms) { best_ms = per; best = cand[k]; }
+  }
+  s->kernel_eff = best;
+  s->autotuned = true;
+  s->planned = false;
+  s->list_valid = false;
+  return MD_OK;
+}
+
+// ---- caller-order I/O -----------------------------------------------------------------------------------
+int set_vec3(md_system* s, const double* in, double* dst) {
+  const double* src = in;
+  if (!is_device_ptr(in)) {
+    CK(cudaMemcpyAsync(s->io_d, in, 3 * (size_t)s->N * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    src = s->io_d;
+  }
+  CK(launch(s, k_scatter_in, blocks_for(s->N, 256), 256, 0, (int)s->N, (const int*)s->id[s->cur], src, dst, s->ld));
+  if (src == s->io_d) CK(cudaStreamSynchronize(s->stream));   // the caller may reuse its buffer
+  return MD_OK;
+}
+int get_vec3(md_system* s, const double* srcv, double* out) {
+  bool dev = is_device_ptr(out);
+  double* dst = dev ? out : s->io_d;
+  CK(launch(s, k_gather_out, blocks_for(s->N, 256), 256, 0, (int)s->N, (const int*)s->id[s->cur], srcv, dst, s->ld));
+  if (!dev) {
+    CK(cudaMemcpyAsync(out, s->io_d, 3 * (size_t)s->N * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
+  return MD_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+// C ABI
+// =====================================================================================================
+extern "C" {
+
+const char* md_last_error(const md_system* s) { return s ? s->err.c_str() : g_create_error.c_str(); }
+
+int md_create(md_system** out, const double box[3], int64_t N, const int32_t* types, int ntypes, const double* mass,
+              void* cuda_stream) {
+  md_system* s = nullptr;
+  if (!out || !box || !types || !mass || N <= 0 || ntypes <= 0 || N > 2000000000LL)
+    return fail(nullptr, MD_ERR_BAD_ARGUMENT, "md_create: bad argument");
+  for (int d = 0; d < 3; ++d)
+    if (!(box[d] > 0.0) || !std::isfinite(box[d])) return fail(nullptr, MD_ERR_BAD_ARGUMENT, "md_create: box edge must be positive");
+  for (int t = 0; t < ntypes; ++t)
+    if (!(mass[t] > 0.0)) return fail(nullptr, MD_ERR_BAD_ARGUMENT, "md_create: masses must be positive");
+  s = new md_system();
+  auto bail = [&](int code) { std::string e = s->err; md_destroy(s); g_create_error = e; return code; };
+  s->N = N;
+  s->ld = ((size_t)N + 31) & ~(size_t)31;
+  s->stream = (cudaStream_t)cuda_stream;
+  s->ntypes = ntypes;
+  for (int d = 0; d < 3; ++d) s->box[d] = box[d];
+#define CKC(call)                                                                                     \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess) { fail(s, MD_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); return bail(MD_ERR_CUDA); } \
+  } while (0)
+  for (int k = 0; k < 2; ++k) {
+    CKC(dalloc(&s->x[k], 3 * s->ld)); CKC(dalloc(&s->v[k], 3 * s->ld));
+    CKC(dalloc(&s->id[k], s->ld)); CKC(dalloc(&s->type[k], s->ld));
+    CKC(cudaMemsetAsync(s->x[k], 0, 3 * s->ld * sizeof(double), s->stream));
+    CKC(cudaMemsetAsync(s->v[k], 0, 3 * s->ld * sizeof(double), s->stream));
+  }
+  CKC(dalloc(&s->f, 3 * s->ld)); CKC(dalloc(&s->x0, 3 * s->ld)); CKC(dalloc(&s->rho, s->ld)); CKC(dalloc(&s->fp, s->ld));
+  CKC(cudaMemsetAsync(s->f, 0, 3 * s->ld * sizeof(double), s->stream));
+  CKC(dalloc(&s->cell_of, s->ld)); CKC(dalloc(&s->rank, s->ld)); CKC(dalloc(&s->perm, s->ld)); CKC(dalloc(&s->numneigh, s->ld));
+  CKC(dalloc(&s->mass_d, (size_t)ntypes)); CKC(dalloc(&s->scalars_d, 16)); CKC(dalloc(&s->io_d, 3 * s->ld));
+  CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
+  CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
+  CKC(cudaEventCreate(&s->ev0)); CKC(cudaEventCreate(&s->ev1)); CKC(cudaEventCreate(&s->ev2)); CKC(cudaEventCreate(&s->ev3));
+  CKC(cudaMemcpyAsync(s->mass_d, mass, ntypes * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+  CKC(cudaMemcpyAsync(s->types_caller, types, (size_t)N * sizeof(int), is_device_ptr(types) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+                      s->stream));
+  CKC(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
+  CKC(launch(s, k_iota, blocks_for(N, 256), 256, 0, (int)N, s->id[0]));
+  CKC(cudaMemcpyAsync(s->type[0], s->types_caller, (size_t)N * sizeof(int), cudaMemcpyDeviceToDevice, s->stream));
+  CKC(cudaStreamSynchronize(s->stream));
+#undef CKC
+  *out = s;
+  return MD_OK;
+}
+
+void md_destroy(md_system* s) {
+  if (!s) return;
+  for (int k = 0; k < 2; ++k) { cudaFree(s->x[k]); cudaFree(s->v[k]); cudaFree(s->id[k]); cudaFree(s->type[k]); }
+  cudaFree(s->f); cudaFree(s->x0); cudaFree(s->rho); cudaFree(s->fp); cudaFree(s->cell_of); cudaFree(s->rank); cudaFree(s->perm);
+  cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d);
+  cudaFree(s->ev_partials); cudaFree(s->scalars_d); cudaFree(s->io_d); cudaFree(s->io_i); cudaFree(s->types_caller); cudaFree(s->flags_d);
+  if (s->flags_h) cudaFreeHost(s->flags_h);
+  if (s->scalars_h) cudaFreeHost(s->scalars_h);
+  if (s->ev0) cudaEventDestroy(s->ev0);
+  if (s->ev1) cudaEventDestroy(s->ev1);
+  if (s->ev2) cudaEventDestroy(s->ev2);
+  if (s->ev3) cudaEventDestroy(s->ev3);
+  delete s;
+}
+
+int md_set_units(md_system* s, double ftm2v, double mvv2e) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  if (!(ftm2v > 0.0) || !(mvv2e > 0.0)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_units: factors must be positive");
+  s->ftm2v = ftm2v; s->mvv2e = mvv2e;
+  return MD_OK;
+}
+
+int md_set_precision(md_system* s, int mode) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  if (mode != MD_FP64 && mode != MD_MIXED) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_precision: unknown mode %d", mode);
+  if (mode != s->precision) { s->precision = mode; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; }
+  return MD_OK;
+}
+
+int md_set_positions(md_system* s, const double* x) {
+  if (!s || !x) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_positions: NULL") : MD_ERR_BAD_ARGUMENT;
+  int rc = set_vec3(s, x, s->x[s->cur]);
+  if (rc) return rc;
+  s->have_x = true; s->list_valid = false; s->forces_valid = false;
+  return MD_OK;
+}
+
+int md_set_velocities(md_system* s, const double* v) {
+  if (!s || !v) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_velocities: NULL") : MD_ERR_BAD_ARGUMENT;
+  return set_vec3(s, v, s->v[s->cur]);
+}
+
+int md_set_pair(md_system* s, int style, const double* params, int nparams, double rc, double skin) {
+  if (!s || !params) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: NULL") : MD_ERR_BAD_ARGUMENT;
+  int need = style == MD_PAIR_LJ126 ? 2 : (style == MD_PAIR_EAM_FS ? 5 : -1);
+  if (need < 0) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: unknown style %d", style);
+  if (nparams != need) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: style %d takes %d parameters, got %d", style, need, nparams);
+  if (!(rc > 0.0) || !(skin >= 0.0) || !std::isfinite(rc) || !std::isfinite(skin)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: bad rc/skin");
+  for (int k = 0; k < need; ++k)
+    if (!std::isfinite(params[k])) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: non-finite parameter");
+  if (style == MD_PAIR_EAM_FS && !(params[4] > 0.0)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: r0 must be positive");
+  if (style == MD_PAIR_EAM_FS && s->list_kind == MD_LIST_HALF) return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
+  for (int d = 0; d < 3; ++d)
+    if (s->box[d] < 3.0 * (rc + skin))
+      return fail(s, MD_ERR_BOX_TOO_SMALL, "box edge %d = %g < 3 (rc+skin) = %g", d, s->box[d], 3.0 * (rc + skin));
+  s->style = style;
+  for (int k = 0; k < 5; ++k) s->params[k] = k < need ? params[k] : 0.0;
+  s->rc = rc; s->skin = skin;
+  s->pair_set = true; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false;
+  return MD_OK;
+}
+
+int md_set_neighbor(md_system* s, int list_kind, int kernel) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  if (list_kind != MD_LIST_FULL && list_kind != MD_LIST_HALF) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown list kind");
+  if (kernel < MD_KERNEL_AUTO || kernel > MD_KERNEL_CELL) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown kernel");
+  if (list_kind == MD_LIST_HALF && !(kernel == MD_KERNEL_TPA || kernel == MD_KERNEL_AUTO))
+    return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: a half list needs MD_KERNEL_TPA");
+  if (list_kind == MD_LIST_HALF && s->style == MD_PAIR_EAM_FS) return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
+  s->list_kind = list_kind;
+  s->kernel_req = kernel;
+  s->kernel_eff = kernel == MD_KERNEL_AUTO ? MD_KERNEL_TPA : kernel;
+  s->autotuned = false;
+  s->planned = false; s->list_valid = false; s->forces_valid = false;
+  return MD_OK;
+}
+
+int md_build_neighbors(md_system* s) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  if (s->kernel_req == MD_KERNEL_AUTO && !s->autotuned) {
+    int rc = autotune(s, 3, nullptr);
+    if (rc) return rc;
+  }
+  return build(s, false);
+}
+
+int md_autotune(md_system* s, int nrep, double ms_out[3]) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  return autotune(s, nrep, ms_out);
+}
+
+int md_compute_forces(md_system* s, double* f_out, double* energy_out, double virial_out[6]) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  int rc = ensure_list(s);
+  if (rc) return rc;
+  bool ev = energy_out || virial_out;
+  CK(cudaEventRecord(s->ev0, s->stream));
+  rc = compute_forces_device(s, ev);
+  if (rc) return rc;
+  CK(cudaEventRecord(s->ev1, s->stream));
+  if (f_out) { rc = get_vec3(s, s->f, f_out); if (rc) return rc; }
+  if (ev) {
+    CK(cudaMemcpyAsync(s->scalars_h, s->scalars_d, 8 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    if (energy_out) *energy_out = s->scalars_h[0];
+    if (virial_out) for (int k = 0; k < 6; ++k) virial_out[k] = s->scalars_h[1 + k];
+  }
+  if (cudaEventQuery(s->ev1) == cudaSuccess) { float ms = 0; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->ms_force = ms; }
+  return MD_OK;
+}
+
+int md_run(md_system* s, int64_t nsteps, double dt) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  if (nsteps < 0 || !std::isfinite(dt)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_run: bad nsteps/dt");
+  int rc = ensure_list(s);
+  if (rc) return rc;
+  int64_t launches0 = s->launches;
+  CK(cudaEventRecord(s->ev0, s->stream));
+  if (!s->forces_valid) { rc = compute_forces_device(s, false); if (rc) return rc; }
+  const int N = (int)s->N;
+  const double trigger = 0.25 * s->skin * s->skin;
+  const double hdtf = 0.5 * dt * s->ftm2v;
+  for (int64_t step = 0; step < nsteps; ++step) {
+    int c = s->cur;
+    CK(launch(s, k_initial_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->x[c], s->v[c], (const double*)s->f, (const double*)s->x0,
+              (const int*)s->type[c], (const double*)s->mass_d, dt, hdtf, s->flags_d));
+    CK(cudaMemcpyAsync(&s->flags_h->max_disp2_bits, &s->flags_d->max_disp2_bits, sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                       s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    double d2;
+    memcpy(&d2, &s->flags_h->max_disp2_bits, sizeof d2);
+    if (d2 > trigger) { rc = build(s, false); if (rc) return rc; }
+    rc = compute_forces_device(s, false);
+    if (rc) return rc;
+    c = s->cur;
+    CK(launch(s, k_final_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->v[c], (const double*)s->f, (const int*)s->type[c],
+              (const double*)s->mass_d, hdtf));
+    s->nsteps_total++;
+  }
+  CK(cudaEventRecord(s->ev1, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  float ms = 0;
+  cudaEventElapsedTime(&ms, s->ev0, s->ev1);
+  s->ms_run = ms;
+  s->launches_last_run = s->launches - launches0;
+  return MD_OK;
+}
+
+int md_get_positions(md_system* s, double* x) {
+  if (!s || !x) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_positions: NULL") : MD_ERR_BAD_ARGUMENT;
+  if (!s->have_x) return fail(s, MD_ERR_NOT_READY, "positions not set");
+  return get_vec3(s, s->x[s->cur], x);
+}
+int md_get_velocities(md_system* s, double* v) {
+  if (!s || !v) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_velocities: NULL") : MD_ERR_BAD_ARGUMENT;
+  return get_vec3(s, s->v[s->cur], v);
+}
+int md_get_forces(md_system* s, double* f) {
+  if (!s || !f) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_forces: NULL") : MD_ERR_BAD_ARGUMENT;
+  if (!s->forces_valid) return fail(s, MD_ERR_NOT_READY, "no valid forces: call md_compute_forces or md_run first");
+  return get_vec3(s, s->f, f);
+}
+
+int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride) {
+  if (!s || !numneigh || !neigh || stride <= 0) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_neighbors: bad argument") : MD_ERR_BAD_ARGUMENT;
+  int rc = ensure_list(s);
+  if (rc) return rc;
+  if (!s->list_built_for_export) { rc = build(s, true); if (rc) return rc; }
+  const Geom& g = s->g;
+  bool dev_n = is_device_ptr(numneigh), dev_l = is_device_ptr(neigh);
+  int *dn = numneigh, *dl = neigh;
+  if (!dev_n) dn = s->io_i;
+  if (!dev_l) CK(cudaMalloc((void**)&dl, (size_t)s->N * stride * sizeof(int)));
+  size_t smem = sizeof(TileTables) + (size_t)(g.tile_cap + 1) * sizeof(int) + 16;
+  cudaError_t e = launch(s, k_export_list, g.ntiles, BLOCK, smem, g, (const int*)s->cell_start, (const int*)s->id[s->cur],
+                         (const uint4*)s->list, (const int*)s->numneigh, dn, dl, (long long)stride);
+  if (e == cudaSuccess && !dev_n) e = cudaMemcpyAsync(numneigh, dn, (size_t)s->N * sizeof(int), cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess && !dev_l) e = cudaMemcpyAsync(neigh, dl, (size_t)s->N * stride * sizeof(int), cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (!dev_l) cudaFree(dl);
+  if (e != cudaSuccess) return fail(s, MD_ERR_CUDA, "md_get_neighbors: %s", cudaGetErrorString(e));
+  return MD_OK;
+}
+
+int md_get_stats(md_system* s, md_stats* out) {
+  if (!s || !out) return MD_ERR_BAD_ARGUMENT;
+  memset(out, 0, sizeof *out);
+  out->natoms = s->N; out->nsteps_total = s->nsteps_total; out->nbuilds = s->nbuilds; out->nforce_evals = s->nforce;
+  out->kernel_variant = s->kernel_eff; out->list_kind = s->list_kind; out->precision = s->precision;
+  out->lanes_per_atom = lanes_for(s->kernel_eff);
+  if (s->planned) {
+    for (int d = 0; d < 3; ++d) { out->ncells[d] = s->g.nc[d]; out->brick[d] = s->g.b[d]; }
+    out->ntiles = s->g.ntiles; out->tile_capacity = s->g.tile_cap; out->row_capacity = s->g.row_cap;
+  }
+  out->max_tile_atoms = s->max_tile_atoms; out->max_neighbors = s->max_row; out->mean_neighbors = s->mean_row;
+  CK(cudaMemsetAsync(s->scalars_d + 8, 0, sizeof(double), s->stream));
+  CK(launch(s, k_kinetic, std::min<unsigned>(blocks_for(s->N, 256), 1184u), 256, 0, (int)s->N, s->ld, (const double*)s->v[s->cur],
+            (const int*)s->type[s->cur], (const double*)s->mass_d, s->scalars_d + 8));
+  CK(cudaMemcpyAsync(s->scalars_h + 8, s->scalars_d + 8, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  out->kinetic_energy = s->scalars_h[8] * s->mvv2e;
+  out->ms_build = s->ms_build; out->ms_force = s->ms_force; out->ms_run = s->ms_run;
+  out->launches_last_run = s->launches_last_run; out->launches_total = s->launches;
+  return MD_OK;
+}
+
+}  // extern "C"
