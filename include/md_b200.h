@@ -98,6 +98,11 @@ typedef struct md_stats {
   double ms_run;               /* device time of the last md_run */
   int64_t launches_last_run;   /* kernels launched by the last md_run */
   int64_t launches_total;      /* kernels launched since md_create */
+  /* phase timers of the last md_run (CUDA events on the library's stream, inside the run) */
+  double ms_force_sampled;     /* summed device time of the force launches of the sampled steps */
+  int64_t nforce_sampled;      /* how many steps were sampled (every ceil(nsteps/128)-th) */
+  double ms_build_in_run;      /* summed device time of the list builds (bin+sort+reorder+build) */
+  int64_t nbuilds_in_run;      /* list builds inside the last md_run */
 } md_stats;
 
 /* Creates a system: orthogonal periodic box [0,Lx) x [0,Ly) x [0,Lz), N atoms with type ids in

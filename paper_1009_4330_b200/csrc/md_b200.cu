@@ -74,6 +74,10 @@ struct md_system_impl {
   double mean_row = 0;
   double ms_build = 0, ms_force = 0, ms_run = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr, ev3 = nullptr;
+  static constexpr int NSAMPLE = 128;          // sampled force timings per md_run
+  cudaEvent_t pev[2 * NSAMPLE] = {};
+  double ms_force_sampled = 0, ms_build_in_run = 0;
+  int64_t nforce_sampled = 0, nbuilds_in_run = 0;
 
   std::map<const void*, size_t> smem_set;
   std::string err;
@@ -458,6 +462,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
   CKC(cudaEventCreate(&s->ev0)); CKC(cudaEventCreate(&s->ev1)); CKC(cudaEventCreate(&s->ev2)); CKC(cudaEventCreate(&s->ev3));
+  for (int k = 0; k < 2 * md_system_impl::NSAMPLE; ++k) CKC(cudaEventCreate(&s->pev[k]));
   CKC(cudaMemcpyAsync(s->mass_d, mass, ntypes * sizeof(double), cudaMemcpyHostToDevice, s->stream));
   CKC(cudaMemcpyAsync(s->types_caller, types, (size_t)N * sizeof(int), is_device_ptr(types) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
                       s->stream));
@@ -482,6 +487,7 @@ void md_destroy(md_system* s) {
   if (s->ev1) cudaEventDestroy(s->ev1);
   if (s->ev2) cudaEventDestroy(s->ev2);
   if (s->ev3) cudaEventDestroy(s->ev3);
+  for (cudaEvent_t e : s->pev) if (e) cudaEventDestroy(e);
   delete s;
 }
 
@@ -584,14 +590,19 @@ int md_compute_forces(md_system* s, double* f_out, double* energy_out, double vi
 int md_run(md_system* s, int64_t nsteps, double dt) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (nsteps < 0 || !std::isfinite(dt)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_run: bad nsteps/dt");
+  int64_t launches0 = s->launches, builds0 = s->nbuilds;
+  s->ms_build_in_run = 0;
+  CK(cudaEventRecord(s->ev0, s->stream));
+  const bool had_list = s->list_valid;
   int rc = ensure_list(s);
   if (rc) return rc;
-  int64_t launches0 = s->launches;
-  CK(cudaEventRecord(s->ev0, s->stream));
+  if (!had_list) s->ms_build_in_run += s->ms_build;
   if (!s->forces_valid) { rc = compute_forces_device(s, false); if (rc) return rc; }
   const int N = (int)s->N;
   const double trigger = 0.25 * s->skin * s->skin;
   const double hdtf = 0.5 * dt * s->ftm2v;
+  const int64_t sample_every = (nsteps + md_system_impl::NSAMPLE - 1) / md_system_impl::NSAMPLE;
+  int nsampled = 0;
   for (int64_t step = 0; step < nsteps; ++step) {
     int c = s->cur;
     CK(launch(s, k_initial_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->x[c], s->v[c], (const double*)s->f, (const double*)s->x0,
@@ -601,9 +612,12 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
     CK(cudaStreamSynchronize(s->stream));
     double d2;
     memcpy(&d2, &s->flags_h->max_disp2_bits, sizeof d2);
-    if (d2 > trigger) { rc = build(s, false); if (rc) return rc; }
+    if (d2 > trigger) { rc = build(s, false); if (rc) return rc; s->ms_build_in_run += s->ms_build; }
+    const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
+    if (sample) CK(cudaEventRecord(s->pev[2 * nsampled], s->stream));
     rc = compute_forces_device(s, false);
     if (rc) return rc;
+    if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
     c = s->cur;
     CK(launch(s, k_final_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->v[c], (const double*)s->f, (const int*)s->type[c],
               (const double*)s->mass_d, hdtf));
@@ -614,6 +628,14 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   float ms = 0;
   cudaEventElapsedTime(&ms, s->ev0, s->ev1);
   s->ms_run = ms;
+  s->ms_force_sampled = 0;
+  for (int k = 0; k < nsampled; ++k) {
+    float t = 0;
+    CK(cudaEventElapsedTime(&t, s->pev[2 * k], s->pev[2 * k + 1]));
+    s->ms_force_sampled += t;
+  }
+  s->nforce_sampled = nsampled;
+  s->nbuilds_in_run = s->nbuilds - builds0;
   s->launches_last_run = s->launches - launches0;
   return MD_OK;
 }
@@ -673,6 +695,8 @@ int md_get_stats(md_system* s, md_stats* out) {
   out->kinetic_energy = s->scalars_h[8] * s->mvv2e;
   out->ms_build = s->ms_build; out->ms_force = s->ms_force; out->ms_run = s->ms_run;
   out->launches_last_run = s->launches_last_run; out->launches_total = s->launches;
+  out->ms_force_sampled = s->ms_force_sampled; out->nforce_sampled = s->nforce_sampled;
+  out->ms_build_in_run = s->ms_build_in_run; out->nbuilds_in_run = s->nbuilds_in_run;
   return MD_OK;
 }
 

@@ -40,6 +40,8 @@ class md_stats(ctypes.Structure):
         ("reserved_", ctypes.c_int32), ("mean_neighbors", ctypes.c_double), ("kinetic_energy", ctypes.c_double),
         ("ms_build", ctypes.c_double), ("ms_force", ctypes.c_double), ("ms_run", ctypes.c_double),
         ("launches_last_run", ctypes.c_int64), ("launches_total", ctypes.c_int64),
+        ("ms_force_sampled", ctypes.c_double), ("nforce_sampled", ctypes.c_int64),
+        ("ms_build_in_run", ctypes.c_double), ("nbuilds_in_run", ctypes.c_int64),
     ]
 
     def as_dict(self) -> dict:
