@@ -13,6 +13,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <type_traits>
 #include <string>
 
 #include "md_kernels.cuh"
@@ -46,9 +47,12 @@ struct md_system_impl {
   double* v[2] = {nullptr, nullptr};
   int* id[2] = {nullptr, nullptr};
   int* type[2] = {nullptr, nullptr};
-  int cur = 0;
+  int cur = 0;    // buffer of v, id, type (flips at every build)
+  int xcur = 0;   // buffer of x (flips at every build and at every fused kick+drift step)
+  int force_threads = 256, batch = 8;
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
   int *cell_of = nullptr, *rank = nullptr, *perm = nullptr, *numneigh = nullptr;
+  size_t numneigh_alloc = 0;
   int *cell_count = nullptr, *cell_start = nullptr;
   size_t cell_alloc = 0;
   uint4* list = nullptr;
@@ -77,7 +81,7 @@ struct md_system_impl {
   static constexpr int NSAMPLE = 128;          // sampled force timings per md_run
   cudaEvent_t pev[2 * NSAMPLE] = {};
   double ms_force_sampled = 0, ms_build_in_run = 0;
-  int64_t nforce_sampled = 0, nbuilds_in_run = 0;
+  int64_t nforce_sampled = 0, nbuilds_in_run = 0, nforce_sampled_acc = 0;
 
   std::map<const void*, size_t> smem_set;
   std::string err;
@@ -108,7 +112,7 @@ int fail(md_system* s, int code, const char* fmt, ...) {
 template <class Kern, class... Args>
 cudaError_t launch(md_system* s, Kern kern, unsigned grid, unsigned block, size_t smem, Args... args) {
   if (grid == 0) return cudaSuccess;
-  if (smem > 48 * 1024) {
+  if (smem > 40 * 1024) {   // static shared memory (reduction scratch) counts against the 48 KB default too
     const void* key = reinterpret_cast<const void*>(kern);
     auto it = s->smem_set.find(key);
     if (it == s->smem_set.end() || it->second < smem) {
@@ -137,11 +141,14 @@ cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, std::max<size
 int lanes_for(int kernel) { return kernel == MD_KERNEL_SUBWARP ? 8 : (kernel == MD_KERNEL_WARP ? 32 : 1); }
 
 // ---- planning: cell grid, tile width, capacities -----------------------------------------------------
+size_t elem_size(const md_system* s) { return s->precision == MD_FP64 ? sizeof(double) : sizeof(float); }
+int capA_of(const Geom& g) { return (g.tile_cap + 8) & ~3; }
 size_t force_smem(const md_system* s, const Geom& g, bool half) {
-  size_t elem = s->precision == MD_FP64 ? sizeof(double4) : sizeof(float4);
-  return sizeof(TileTables) + (size_t)(g.tile_cap + 1) * elem + (half ? (size_t)(g.tile_cap + 1) * 4 : 0) + 16;
+  return sizeof(TileTables) + 4 * (size_t)capA_of(g) * elem_size(s) + (size_t)g.interior_cap * 2 + (half ? (size_t)capA_of(g) * 4 : 0) + 16;
 }
-size_t build_smem(const Geom& g) { return sizeof(TileTables) + 3 * (size_t)(g.tile_cap + 1) * sizeof(double) + 16; }
+size_t cell_smem(const md_system* s, const Geom& g) { return sizeof(TileTables) + 4 * (size_t)capA_of(g) * elem_size(s) + 16; }
+size_t build_smem(const Geom& g) { return sizeof(TileTables) + 3 * (size_t)capA_of(g) * sizeof(float) + (size_t)BUILD_THREADS * RING_STRIDE + 16; }
+size_t export_smem(const Geom& g) { return sizeof(TileTables) + (size_t)capA_of(g) * sizeof(int) + 16; }
 
 void fill_geom_for_b(const md_system* s, int b, Geom& g) {
   double rl = s->rc + s->skin;
@@ -156,7 +163,7 @@ void fill_geom_for_b(const md_system* s, int b, Geom& g) {
     g.ncell *= g.nc[d];
   }
   g.ntiles = g.nb[0] * g.nb[1] * g.nb[2];
-  double per_cell = (double)s->N / g.ncell;
+  double per_cell = (double)s->N / g.ncell + 1.5;   // cells are padded to multiples of 4 slots
   double staged = per_cell * (g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2);
   double interior = per_cell * g.b[0] * g.b[1] * g.b[2];
   g.tile_cap = (int)(staged * 1.2 * s->cap_scale_tile + 64);
@@ -165,6 +172,7 @@ void fill_geom_for_b(const md_system* s, int b, Geom& g) {
   g.interior_cap = (g.interior_cap + 31) & ~31;
   g.K = lanes_for(s->kernel_eff);
   g.half = s->list_kind == MD_LIST_HALF ? 1 : 0;
+  g.code_shift = s->precision == MD_FP64 ? 4 : 3;
   double vol = s->box[0] * s->box[1] * s->box[2];
   double mean_nb = 4.0 / 3.0 * M_PI * rl * rl * rl * s->N / vol * (g.half ? 0.5 : 1.0);
   int unit = 8 * g.K;
@@ -184,14 +192,15 @@ int plan(md_system* s) {
   int best = 0;
   Geom g{};
   const size_t smem_soft = 100 * 1024, smem_hard = 200 * 1024;
+  const int code_shift = s->precision == MD_FP64 ? 4 : 3;
   for (int pass = 0; pass < 3 && !best; ++pass) {
     // pass 0: all preferences; pass 1: drop the tile-count preference; pass 2: only hard limits
     for (int b = 6; b >= 1; --b) {
       if (forced && b != forced) continue;
       fill_geom_for_b(s, b, g);
       if ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) > MAX_TILE_CELLS) continue;
-      if (g.tile_cap + 1 > 65535) continue;
-      size_t sm = std::max(force_smem(s, g, g.half), build_smem(g));
+      if (g.tile_cap > (65535 >> code_shift)) continue;       // 16-bit slot codes
+      size_t sm = std::max(std::max(force_smem(s, g, g.half), build_smem(g)), cell_smem(s, g));
       if (sm > smem_hard) continue;
       if (!forced && pass < 2) {
         if (sm > smem_soft) continue;
@@ -207,6 +216,17 @@ int plan(md_system* s) {
   if (!best) return fail(s, MD_ERR_OVERFLOW, "no tile width fits shared memory (density too high for cells of edge rc+skin)");
   fill_geom_for_b(s, best, g);
   s->g = g;
+  // block size of the list force kernels: the tile's rows should fill whole rounds of the block
+  {
+    double rows = ((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.06 + 8.0;
+    double lanes = rows * g.K;
+    int tmax = g.K == 1 ? FORCE_MAX_THREADS : 256;
+    int rounds = (int)std::ceil(lanes / tmax);
+    int t = (int)std::ceil(lanes / std::max(rounds, 1));
+    t = ((t + 31) / 32) * 32;
+    s->force_threads = std::min(std::max(t, 32), tmax);
+    if (const char* e = getenv("MD_B200_THREADS")) s->force_threads = std::min(std::max(atoi(e) / 32 * 32, 32), FORCE_MAX_THREADS);
+  }
   // pair constants
   PairParams& P = s->P;
   P = PairParams{};
@@ -233,6 +253,13 @@ int plan(md_system* s) {
     CK(dalloc(&s->list, words));
     s->list_words = words;
   }
+  size_t rows = (size_t)g.ntiles * g.interior_cap;
+  if (rows > s->numneigh_alloc) {
+    cudaFree(s->numneigh);
+    s->numneigh = nullptr; s->numneigh_alloc = 0;
+    CK(dalloc(&s->numneigh, rows));
+    s->numneigh_alloc = rows;
+  }
   if ((size_t)g.ntiles > s->ev_tiles_alloc) {
     cudaFree(s->ev_partials);
     s->ev_tiles_alloc = g.ntiles;
@@ -247,8 +274,18 @@ int plan(md_system* s) {
 int build_list_only(md_system* s) {
   const Geom& g = s->g;
   double rl = s->rc + s->skin;
-  CK(launch(s, k_build_list, g.ntiles, BLOCK, build_smem(g), g, (const int*)s->cell_start, (const double*)s->x[s->cur], s->ld,
-            rl * rl, s->list, s->numneigh, s->flags_d));
+  BuildArgs B{};
+  B.g = g; B.cell_start = s->cell_start; B.x = s->x[s->xcur]; B.ld = s->ld; B.rl2 = rl * rl;
+  // guard band of the fp32 distance test: tile-centred coordinates up to E are
+  // rounded to fp32, so r^2 carries a relative error of about (7 E / rl + 3) 2^-24; four times that is used.
+  double E = 0;
+  for (int d = 0; d < 3; ++d) E = std::max(E, 0.5 * (g.b[d] + 2) * g.edge[d] + s->skin);
+  double band = 4.0 * (7.0 * E / rl + 3.0) * std::ldexp(1.0, -24);
+  B.rl2_lo = std::nextafterf((float)(rl * rl * (1.0 - band)), 0.0f);
+  B.rl2_hi = std::nextafterf((float)(rl * rl * (1.0 + band)), INFINITY);
+  B.list = s->list; B.numneigh = s->numneigh; B.flags = s->flags_d;
+  if (g.half) CK(launch(s, k_build_list<true>, g.ntiles, BUILD_THREADS, build_smem(g), B));
+  else CK(launch(s, k_build_list<false>, g.ntiles, BUILD_THREADS, build_smem(g), B));
   return MD_OK;
 }
 
@@ -261,16 +298,16 @@ int build(md_system* s, bool need_list) {
     CK(cudaEventRecord(s->ev2, s->stream));
     CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
     CK(cudaMemsetAsync(s->cell_count, 0, (size_t)(g.ncell + 1) * sizeof(int), s->stream));
-    int c = s->cur, o = 1 - c;
-    CK(launch(s, k_bin, blocks_for(N, 256), 256, 0, g, N, s->x[c], s->x[c] + s->ld, s->x[c] + 2 * s->ld, s->cell_of, s->rank,
+    int c = s->cur, o = 1 - c, xc = s->xcur, xo = 1 - xc;
+    CK(launch(s, k_bin, blocks_for(N, 256), 256, 0, g, N, s->x[xc], s->x[xc] + s->ld, s->x[xc] + 2 * s->ld, s->cell_of, s->rank,
               s->cell_count, s->flags_d));
     CK(launch(s, k_scan_cells, 1, 1024, 0, g.ncell, (const int*)s->cell_count, s->cell_start));
     CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
               s->perm));
     CK(launch(s, k_sort_cells, blocks_for(g.ncell, 128), 128, 0, g.ncell, (const int*)s->cell_start, s->perm));
-    CK(launch(s, k_permute, blocks_for(N, 256), 256, 0, N, (const int*)s->perm, (const double*)s->x[c], (const double*)s->v[c],
-              (const int*)s->id[c], (const int*)s->type[c], s->x[o], s->v[o], s->id[o], s->type[o], s->x0, s->ld));
-    s->cur = o;
+    CK(launch(s, k_permute, blocks_for(N, 256), 256, 0, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
+              (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, s->ld));
+    s->cur = o; s->xcur = xo;
     s->forces_valid = false;
     bool do_list = need_list || s->kernel_eff != MD_KERNEL_CELL;
     if (do_list) { int rc = build_list_only(s); if (rc) return rc; }
@@ -301,57 +338,72 @@ int build(md_system* s, bool need_list) {
 }
 
 // ---- force dispatch ------------------------------------------------------------------------------------
-template <typename T, class Body, int MODE, bool EV>
+// how a force evaluation is embedded in time stepping (ForceArgs.epi / in_run / parity)
+struct StepMode {
+  int epi = EPI_FORCES;
+  int in_run = 0;
+  int parity = 0;
+  double dt = 0, hdtf = 0, trigger = 0;
+  const double* x_in = nullptr;   // positions read (default: current buffer)
+  double* x_out = nullptr;        // EPI_KICK_DRIFT: positions written
+};
+
+template <typename T, template <typename, bool> class BodyT, int MODE, bool EV>
 int launch_force_variant(md_system* s, const ForceArgs& A) {
+  using Body = BodyT<T, EV>;
   const Geom& g = s->g;
   const bool half = g.half != 0;
-  size_t smem = force_smem(s, g, half && MODE == 0);
   if (s->kernel_eff == MD_KERNEL_CELL) {
-    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false, true>, g.ntiles, BLOCK, smem, A));
+    CK(launch(s, k_cell_force<T, Body, MODE, EV>, g.ntiles, BUILD_THREADS, cell_smem(s, g), A));
   } else if (half) {
-    if constexpr (MODE == 0) {
+    if constexpr (MODE == 0 && std::is_same<Body, LJBody<T, EV>>::value) {
       CK(cudaMemsetAsync(A.f, 0, 3 * s->ld * sizeof(double), s->stream));
-      CK(launch(s, k_tile_force<T, Body, 1, 0, EV, true, false>, g.ntiles, BLOCK, smem, A));
+      CK(launch(s, k_tile_force<T, Body, 1, 0, EV, true>, g.ntiles, s->force_threads, force_smem(s, g, true), A));
     } else {
       return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
     }
   } else if (g.K == 1) {
-    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false, false>, g.ntiles, BLOCK, smem, A));
+    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
   } else if (g.K == 8) {
-    CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false, false>, g.ntiles, BLOCK, smem, A));
+    CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
   } else {
-    CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false, false>, g.ntiles, BLOCK, smem, A));
+    CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
   }
   return MD_OK;
 }
 
 template <typename T, bool EV>
-int launch_force_T(md_system* s) {
+int launch_force_T(md_system* s, const StepMode& M) {
   const Geom& g = s->g;
   ForceArgs A{};
-  A.g = g; A.P = s->P; A.cell_start = s->cell_start; A.x = s->x[s->cur]; A.ld = s->ld; A.list = s->list;
+  A.g = g; A.P = s->P; A.cell_start = s->cell_start; A.x = M.x_in ? M.x_in : s->x[s->xcur]; A.ld = s->ld; A.list = s->list;
   A.numneigh = s->numneigh; A.fp_in = nullptr; A.f = s->f; A.rho = s->rho; A.fp_out = s->fp; A.ev_partials = s->ev_partials;
+  A.epi = M.epi; A.in_run = M.in_run; A.parity = M.parity;
+  A.v = s->v[s->cur]; A.x_new = M.x_out; A.x0 = s->x0; A.type = s->type[s->cur]; A.mass = s->mass_d;
+  A.dt = M.dt; A.half_dt_ftm2v = M.hdtf; A.trigger = M.trigger; A.flags = s->flags_d;
   if (s->style == MD_PAIR_LJ126) {
-    int rc = launch_force_variant<T, LJBody<T, EV>, 0, EV>(s, A);
+    int rc = launch_force_variant<T, LJBody, 0, EV>(s, A);
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
   } else {
-    int rc = launch_force_variant<T, EamDensityBody<T>, 1, false>(s, A);   // pass 1: rho, F'(rho), sum F(rho)
+    int rc = launch_force_variant<T, EamDensityBody, 1, EV>(s, A);   // pass 1: rho, F'(rho), sum F(rho)
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
     A.fp_in = s->fp;
-    rc = launch_force_variant<T, EamForceBody<T, EV>, 0, EV>(s, A);          // pass 2: forces
+    rc = launch_force_variant<T, EamForceBody, 0, EV>(s, A);          // pass 2: forces
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 1));
   }
   s->nforce++;
-  s->forces_valid = true;
   return MD_OK;
 }
 
-int compute_forces_device(md_system* s, bool ev) {
-  if (s->precision == MD_FP64) return ev ? launch_force_T<double, true>(s) : launch_force_T<double, false>(s);
-  return ev ? launch_force_T<float, true>(s) : launch_force_T<float, false>(s);
+int compute_forces_device(md_system* s, bool ev, const StepMode& M = StepMode()) {
+  int rc;
+  if (s->precision == MD_FP64) rc = ev ? launch_force_T<double, true>(s, M) : launch_force_T<double, false>(s, M);
+  else rc = ev ? launch_force_T<float, true>(s, M) : launch_force_T<float, false>(s, M);
+  if (rc == MD_OK && M.epi == EPI_FORCES) s->forces_valid = true;
+  return rc;
 }
 
 int autotune(md_system* s, int nrep, double* ms_out);
@@ -457,7 +509,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   }
   CKC(dalloc(&s->f, 3 * s->ld)); CKC(dalloc(&s->x0, 3 * s->ld)); CKC(dalloc(&s->rho, s->ld)); CKC(dalloc(&s->fp, s->ld));
   CKC(cudaMemsetAsync(s->f, 0, 3 * s->ld * sizeof(double), s->stream));
-  CKC(dalloc(&s->cell_of, s->ld)); CKC(dalloc(&s->rank, s->ld)); CKC(dalloc(&s->perm, s->ld)); CKC(dalloc(&s->numneigh, s->ld));
+  CKC(dalloc(&s->cell_of, s->ld)); CKC(dalloc(&s->rank, s->ld)); CKC(dalloc(&s->perm, s->ld));
   CKC(dalloc(&s->mass_d, (size_t)ntypes)); CKC(dalloc(&s->scalars_d, 16)); CKC(dalloc(&s->io_d, 3 * s->ld));
   CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
@@ -507,7 +559,7 @@ int md_set_precision(md_system* s, int mode) {
 
 int md_set_positions(md_system* s, const double* x) {
   if (!s || !x) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_positions: NULL") : MD_ERR_BAD_ARGUMENT;
-  int rc = set_vec3(s, x, s->x[s->cur]);
+  int rc = set_vec3(s, x, s->x[s->xcur]);
   if (rc) return rc;
   s->have_x = true; s->list_valid = false; s->forces_valid = false;
   return MD_OK;
@@ -603,38 +655,104 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   const double hdtf = 0.5 * dt * s->ftm2v;
   const int64_t sample_every = (nsteps + md_system_impl::NSAMPLE - 1) / md_system_impl::NSAMPLE;
   int nsampled = 0;
-  for (int64_t step = 0; step < nsteps; ++step) {
-    int c = s->cur;
-    CK(launch(s, k_initial_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->x[c], s->v[c], (const double*)s->f, (const double*)s->x0,
-              (const int*)s->type[c], (const double*)s->mass_d, dt, hdtf, s->flags_d));
-    CK(cudaMemcpyAsync(&s->flags_h->max_disp2_bits, &s->flags_d->max_disp2_bits, sizeof(unsigned long long), cudaMemcpyDeviceToHost,
-                       s->stream));
-    CK(cudaStreamSynchronize(s->stream));
-    double d2;
-    memcpy(&d2, &s->flags_h->max_disp2_bits, sizeof d2);
-    if (d2 > trigger) { rc = build(s, false); if (rc) return rc; s->ms_build_in_run += s->ms_build; }
-    const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
-    if (sample) CK(cudaEventRecord(s->pev[2 * nsampled], s->stream));
-    rc = compute_forces_device(s, false);
-    if (rc) return rc;
-    if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
-    c = s->cur;
-    CK(launch(s, k_final_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->v[c], (const double*)s->f, (const int*)s->type[c],
-              (const double*)s->mass_d, hdtf));
-    s->nsteps_total++;
+  s->ms_force_sampled = 0;
+  const bool fused = s->list_kind != MD_LIST_HALF;
+  if (nsteps > 0 && fused) {
+    // Velocity Verlet with ONE launch per time step (two for EAM): the force kernel of step n also does the
+    // second half kick of step n and the first half kick + drift of step n+1, writing the new positions to
+    // the other x buffer and the max displacement to a device flag.  Steps are enqueued in batches without
+    // host synchronisation; a step kernel that finds the list stale does nothing and raises `stop`, and so
+    // do all later ones; the host then rebuilds and continues from the step that stopped.
+    CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
+    CK(launch(s, k_initial_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
+              (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, dt, hdtf, &s->flags_d->max_disp2_bits[0]));
+    s->forces_valid = false;
+    int64_t remaining = nsteps;
+    int parity = 0;
+    while (remaining > 0) {
+      const int m = (int)std::min<int64_t>(s->batch, remaining);
+      int sample_slot[64];
+      for (int k = 0; k < m; ++k) {
+        const bool last = (int64_t)k == remaining - 1;
+        StepMode M;
+        M.epi = last ? EPI_FINAL : EPI_KICK_DRIFT;
+        M.in_run = 1; M.parity = (parity + k) & 1; M.dt = dt; M.hdtf = hdtf; M.trigger = trigger;
+        M.x_in = s->x[s->xcur ^ (k & 1)];
+        M.x_out = s->x[s->xcur ^ (k & 1) ^ 1];
+        const int64_t step = nsteps - remaining + k;
+        const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
+        sample_slot[k] = -1;
+        if (sample) { sample_slot[k] = nsampled; CK(cudaEventRecord(s->pev[2 * nsampled], s->stream)); }
+        rc = compute_forces_device(s, false, M);
+        if (rc) return rc;
+        if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
+      }
+      CK(cudaMemcpyAsync(s->flags_h, s->flags_d, sizeof(Flags), cudaMemcpyDeviceToHost, s->stream));
+      CK(cudaStreamSynchronize(s->stream));
+      const int done = s->flags_h->steps_done;
+      const bool stopped = s->flags_h->stop != 0;
+      if (done < 0 || done > m || (!stopped && done != m)) return fail(s, MD_ERR_CUDA, "md_run: inconsistent step count from the device (%d of %d)", done, m);
+      for (int k = 0; k < m; ++k) {   // timings of the launches that really ran
+        if (sample_slot[k] < 0) continue;
+        if (k < done) { float t = 0; CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev[2 * sample_slot[k] + 1])); s->ms_force_sampled += t; s->nforce_sampled_acc++; }
+      }
+      const bool final_ran = done == m && (int64_t)m == remaining;
+      const int flips = final_ran ? done - 1 : done;   // kick+drift launches that ran
+      s->xcur ^= (flips & 1);
+      s->nsteps_total += done;
+      remaining -= done;
+      parity = (parity + done) & 1;
+      s->nforce -= (m - done);
+      if (final_ran) s->forces_valid = true;
+      if (stopped) {
+        s->batch = std::min(32, std::max(2, done + 2));
+        rc = build(s, false);   // also clears the flags
+        if (rc) return rc;
+        s->ms_build_in_run += s->ms_build;
+        parity = 0;
+      } else if (remaining > 0) {
+        CK(cudaMemsetAsync(&s->flags_d->steps_done, 0, sizeof(int), s->stream));
+        if (done == s->batch) s->batch = std::min(32, s->batch + 2);
+      }
+    }
+  } else {
+    // half list: the scatter kernel's forces are complete only when it has finished, so integrate separately
+    for (int64_t step = 0; step < nsteps; ++step) {
+      CK(cudaMemsetAsync(s->flags_d->max_disp2_bits, 0, 2 * sizeof(unsigned long long), s->stream));
+      CK(launch(s, k_initial_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
+                (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, dt, hdtf, &s->flags_d->max_disp2_bits[0]));
+      CK(cudaMemcpyAsync(&s->flags_h->max_disp2_bits[0], &s->flags_d->max_disp2_bits[0], sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                         s->stream));
+      CK(cudaStreamSynchronize(s->stream));
+      double d2;
+      memcpy(&d2, &s->flags_h->max_disp2_bits[0], sizeof d2);
+      if (d2 > trigger) { rc = build(s, false); if (rc) return rc; s->ms_build_in_run += s->ms_build; }
+      const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
+      if (sample) CK(cudaEventRecord(s->pev[2 * nsampled], s->stream));
+      rc = compute_forces_device(s, false);
+      if (rc) return rc;
+      if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
+      CK(launch(s, k_final_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->v[s->cur], (const double*)s->f, (const int*)s->type[s->cur],
+                (const double*)s->mass_d, hdtf));
+      s->nsteps_total++;
+    }
   }
   CK(cudaEventRecord(s->ev1, s->stream));
   CK(cudaStreamSynchronize(s->stream));
   float ms = 0;
   cudaEventElapsedTime(&ms, s->ev0, s->ev1);
   s->ms_run = ms;
-  s->ms_force_sampled = 0;
-  for (int k = 0; k < nsampled; ++k) {
-    float t = 0;
-    CK(cudaEventElapsedTime(&t, s->pev[2 * k], s->pev[2 * k + 1]));
-    s->ms_force_sampled += t;
+  if (!fused) {
+    for (int k = 0; k < nsampled; ++k) {
+      float t = 0;
+      CK(cudaEventElapsedTime(&t, s->pev[2 * k], s->pev[2 * k + 1]));
+      s->ms_force_sampled += t;
+    }
+    s->nforce_sampled = nsampled;
+  } else {
+    s->nforce_sampled = s->nforce_sampled_acc;
+    s->nforce_sampled_acc = 0;
   }
-  s->nforce_sampled = nsampled;
   s->nbuilds_in_run = s->nbuilds - builds0;
   s->launches_last_run = s->launches - launches0;
   return MD_OK;
@@ -643,7 +761,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
 int md_get_positions(md_system* s, double* x) {
   if (!s || !x) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_positions: NULL") : MD_ERR_BAD_ARGUMENT;
   if (!s->have_x) return fail(s, MD_ERR_NOT_READY, "positions not set");
-  return get_vec3(s, s->x[s->cur], x);
+  return get_vec3(s, s->x[s->xcur], x);
 }
 int md_get_velocities(md_system* s, double* v) {
   if (!s || !v) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_velocities: NULL") : MD_ERR_BAD_ARGUMENT;
@@ -665,8 +783,8 @@ int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t st
   int *dn = numneigh, *dl = neigh;
   if (!dev_n) dn = s->io_i;
   if (!dev_l) CK(cudaMalloc((void**)&dl, (size_t)s->N * stride * sizeof(int)));
-  size_t smem = sizeof(TileTables) + (size_t)(g.tile_cap + 1) * sizeof(int) + 16;
-  cudaError_t e = launch(s, k_export_list, g.ntiles, BLOCK, smem, g, (const int*)s->cell_start, (const int*)s->id[s->cur],
+  size_t smem = export_smem(g);
+  cudaError_t e = launch(s, k_export_list, g.ntiles, BUILD_THREADS, smem, g, (const int*)s->cell_start, (const int*)s->id[s->cur],
                          (const uint4*)s->list, (const int*)s->numneigh, dn, dl, (long long)stride);
   if (e == cudaSuccess && !dev_n) e = cudaMemcpyAsync(numneigh, dn, (size_t)s->N * sizeof(int), cudaMemcpyDeviceToHost, s->stream);
   if (e == cudaSuccess && !dev_l) e = cudaMemcpyAsync(neigh, dl, (size_t)s->N * stride * sizeof(int), cudaMemcpyDeviceToHost, s->stream);

@@ -6,10 +6,11 @@
 // interior cells plus a one-cell halo (periodic images resolved while staging) into shared memory as
 // TILE-CENTRED coordinates -- fp32 in mixed mode, which is what makes fp32 pair math accurate enough in
 // a 168-sigma box -- and then runs the paper's neighbor-list loop against shared
-// memory: the "random access" load of atom j (L100) is an LDS, not a texture/L1 gather, and the list
-// holds 16-bit tile-local indices, eight to a 128-bit word, so the index stream is half the classic
+// memory: the "random access" load of atom j (L100) is two LDS.64, not a texture/L1 gather, and the list
+// holds 16-bit tile-local slot codes, eight to a 128-bit word, so the index stream is half the classic
 // 4 B/entry.  One template covers thread-per-atom (K=1), sub-warp (K=8) and warp-per-atom (K=32, the
-// paper's BpA with a shuffle reduction instead of a block reduction).
+// paper's BpA with a shuffle reduction instead of a block reduction).  The force kernel's epilogue can
+// also do the velocity-Verlet kick and drift, so a time step between rebuilds is ONE launch.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -17,7 +18,10 @@
 namespace mdk {
 
 constexpr int MAX_TILE_CELLS = 512;    // (b+2)^3 <= 512  =>  b <= 6
-constexpr int BLOCK = 256;             // threads per tile block
+constexpr int BUILD_THREADS = 256;     // threads per block of the list-build and cell-list kernels
+constexpr int FORCE_MAX_THREADS = 640; // upper bound of the force kernels' block size (runtime choice)
+constexpr int RING = 64;               // list-build: pending entries a lane can hold in shared memory
+constexpr int RING_STRIDE = RING * 2 + 16;   // bytes between the rings of neighbouring lanes (odd * 16)
 
 struct Geom {
   double L[3];        // box
@@ -28,17 +32,21 @@ struct Geom {
   int nb[3];          // tiles per dimension
   int ncell;
   int ntiles;
-  int tile_cap;       // staged atoms a tile can hold (excluding the dummy slot)
-  int interior_cap;   // interior atoms a tile can hold (multiple of 32)
+  int tile_cap;       // staged slots a tile can hold (cells padded to multiples of 4; excluding the dummy slot)
+  int interior_cap;   // interior slots (= list rows) a tile can hold (multiple of 32)
   int row_cap;        // list entries per atom (multiple of 8*K)
   int K;              // lanes per atom: 1, 8, 32
   int chunk_cap;      // row_cap / (8*K): 128-bit words per lane
   int half;           // 1: half list
+  int code_shift;     // list entries hold slot << code_shift (3: fp32 tile, 4: fp64 tile)
 };
 
-// flags written by the device, read by the host after a build / at the end of a run
+// flags written by the device, read by the host after a build / after a batch of steps
 struct Flags {
-  unsigned long long max_disp2_bits;  // max |x-x0|^2 as the bit pattern of a non-negative double
+  unsigned long long max_disp2_bits[2];  // max |x-x0|^2 since the last build (bit pattern of a non-negative
+                                         // double); slot p is written by steps of parity p, read by parity 1-p
+  int stop;                           // a step kernel found the list stale and did nothing (sticky until the next build)
+  int steps_done;                     // step kernels that ran since the host last cleared it
   int need_tile_cap;                  // > tile_cap     => staging overflow
   int need_interior_cap;              // > interior_cap => interior overflow
   int need_row_cap;                   // > row_cap      => a list row overflowed
@@ -70,6 +78,31 @@ __device__ __forceinline__ uint4 ld_stream(const uint4* p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
   return r;
+}
+__device__ __forceinline__ void st_stream(uint4* p, uint4 v) {
+  asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float2 lds_f2(unsigned a) {
+  float2 r;
+  asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ double2 lds_d2(unsigned a) {
+  double2 r;
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(r.x), "=d"(r.y) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ uint4 lds_u4(unsigned a) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ void sts_u4(unsigned a, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void sts_u16(unsigned a, unsigned v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((unsigned short)v) : "memory");
 }
 __device__ __forceinline__ float rcp_approx(float x) {
   float r;
@@ -113,21 +146,52 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* red) {
     }
   }
 }
+__device__ __forceinline__ void atomic_max_double_bits(unsigned long long* p, double v) {
+  if (v > 0.0) atomicMax(p, (unsigned long long)__double_as_longlong(v));
+}
+// block-wide max of a non-negative double, then ONE atomicMax per block.  red: >= 32 doubles of shared scratch.
+__device__ __forceinline__ void block_max_to_flag(double v, double* red, unsigned long long* flag) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  __syncthreads();
+  if (lane == 0) red[wid] = v;
+  __syncthreads();
+  if (wid == 0) {
+    v = lane < nw ? red[lane] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if (lane == 0) atomic_max_double_bits(flag, v);
+  }
+}
 
 // ---------------------------------------------------------------------------------------------------
-// tile staging, shared by the list build, every force kernel and the list export
+// tile staging, shared by the list build, every force kernel and the list export.
+// Staged slot order: the tile's interior cells first (in their global = brick order), then the halo
+// cells in tile scan order; every cell is padded to a multiple of 4 slots (pad slots hold a far-away
+// point), so that a cell's coordinates can be read four at a time with aligned 128-bit loads.
+// Interior slot a is also the list row of that atom.
 // ---------------------------------------------------------------------------------------------------
 struct alignas(16) TileTables {   // lives in shared memory
-  int start[MAX_TILE_CELLS];  // staged slot of the first atom of tile cell t
+  int start[MAX_TILE_CELLS];  // staged slot of the first atom of tile cell t (multiple of 4)
   int gstart[MAX_TILE_CELLS]; // global (sorted) index of the first atom of tile cell t
   int cnt[MAX_TILE_CELLS];    // atoms in tile cell t
-  int scan_tmp[32];
   int c0[3], w[3], tc[3];     // first interior cell, interior width, tile width (w+2)
   int ntc;                    // tc[0]*tc[1]*tc[2]
-  int n_int;                  // interior atoms (slots [0,n_int))
-  int n_staged;               // interior + halo atoms; slot n_staged is the far-away dummy
-  int brick_start;            // global index of interior slot 0
+  int nic;                    // interior cells w[0]*w[1]*w[2]
+  int n_int_slots;            // padded interior slots (list rows in use)
+  int n_slots;                // all padded slots; slot n_slots is the far-away dummy
+  int n_int_atoms;            // interior atoms
+  int brick_start;            // global index of the first interior atom
 };
+
+__device__ __forceinline__ int pad4(int c) { return (c + 3) & ~3; }
+__device__ __forceinline__ int interior_tile_cell(const TileTables& tt, int ic) {
+  int lx = ic % tt.w[0], ly = (ic / tt.w[0]) % tt.w[1], lz = ic / (tt.w[0] * tt.w[1]);
+  return ((lz + 1) * tt.tc[1] + (ly + 1)) * tt.tc[0] + (lx + 1);
+}
+__device__ __forceinline__ bool tile_cell_is_interior(const TileTables& tt, int t) {
+  int tx = t % tt.tc[0], ty = (t / tt.tc[0]) % tt.tc[1], tz = t / (tt.tc[0] * tt.tc[1]);
+  return tx >= 1 && tx <= tt.w[0] && ty >= 1 && ty <= tt.w[1] && tz >= 1 && tz <= tt.w[2];
+}
 
 // Fills the tables for tile `tile`.  All threads of the block call it; ends with __syncthreads().
 __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict__ cell_start, TileTables& tt) {
@@ -141,10 +205,10 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
       tt.tc[d] = tt.w[d] + 2;
     }
     tt.ntc = tt.tc[0] * tt.tc[1] * tt.tc[2];
+    tt.nic = tt.w[0] * tt.w[1] * tt.w[2];
     int first = cell_order_id(g, tt.c0[0], tt.c0[1], tt.c0[2]);
-    int ncell_int = tt.w[0] * tt.w[1] * tt.w[2];
     tt.brick_start = cell_start[first];
-    tt.n_int = cell_start[first + ncell_int] - tt.brick_start;
+    tt.n_int_atoms = cell_start[first + tt.nic] - tt.brick_start;
   }
   __syncthreads();
   const int ntc = tt.ntc;
@@ -155,30 +219,41 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
     cy += cy < 0 ? g.nc[1] : (cy >= g.nc[1] ? -g.nc[1] : 0);
     cz += cz < 0 ? g.nc[2] : (cz >= g.nc[2] ? -g.nc[2] : 0);
     int oid = cell_order_id(g, cx, cy, cz);
-    int s = cell_start[oid], c = cell_start[oid + 1] - s;
-    bool interior = tx >= 1 && tx <= tt.w[0] && ty >= 1 && ty <= tt.w[1] && tz >= 1 && tz <= tt.w[2];
+    int s = cell_start[oid];
     tt.gstart[t] = s;
-    tt.cnt[t] = c;
-    tt.start[t] = interior ? -1 : c;   // halo: count, to be scanned; interior: marker
+    tt.cnt[t] = cell_start[oid + 1] - s;
   }
   __syncthreads();
-  // exclusive scan of the halo counts by warp 0
+  // two exclusive scans of the padded counts by warp 0: interior cells in brick order, then halo cells
   if (tid < 32) {
-    int per = (ntc + 31) / 32, lo = tid * per, hi = min(lo + per, ntc), sum = 0;
-    for (int t = lo; t < hi; ++t) sum += tt.start[t] < 0 ? 0 : tt.start[t];
+    const int nic = tt.nic;
+    int per = (nic + 31) / 32, lo = tid * per, hi = min(lo + per, nic), sum = 0;
+    for (int ic = lo; ic < hi; ++ic) sum += pad4(tt.cnt[interior_tile_cell(tt, ic)]);
     int incl = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       int u = __shfl_up_sync(0xffffffffu, incl, o);
       if (tid >= o) incl += u;
     }
-    int run = tt.n_int + incl - sum;
-    for (int t = lo; t < hi; ++t) {
-      int c = tt.start[t];
-      if (c < 0) tt.start[t] = tt.gstart[t] - tt.brick_start;
-      else { tt.start[t] = run; run += c; }
+    int run = incl - sum;
+    for (int ic = lo; ic < hi; ++ic) {
+      int t = interior_tile_cell(tt, ic);
+      tt.start[t] = run;
+      run += pad4(tt.cnt[t]);
     }
-    if (tid == 31) tt.n_staged = tt.n_int + incl;
+    const int n_int = __shfl_sync(0xffffffffu, incl, 31);
+    per = (ntc + 31) / 32; lo = tid * per; hi = min(lo + per, ntc); sum = 0;
+    for (int t = lo; t < hi; ++t) sum += tile_cell_is_interior(tt, t) ? 0 : pad4(tt.cnt[t]);
+    incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int u = __shfl_up_sync(0xffffffffu, incl, o);
+      if (tid >= o) incl += u;
+    }
+    run = n_int + incl - sum;
+    for (int t = lo; t < hi; ++t)
+      if (!tile_cell_is_interior(tt, t)) { tt.start[t] = run; run += pad4(tt.cnt[t]); }
+    if (tid == 31) { tt.n_int_slots = n_int; tt.n_slots = n_int + incl; }
   }
   __syncthreads();
 }
@@ -195,20 +270,24 @@ __device__ __forceinline__ void tile_cell_offset(const Geom& g, const TileTables
   }
 }
 
-// Calls store(slot, global_index, off[3]) for every staged atom with slot < cap.  One warp per tile
-// cell; two cells in flight per warp for memory-level parallelism.  Caller syncs afterwards.
-template <class Store>
-__device__ __forceinline__ void tile_stage(const Geom& g, const TileTables& tt, int cap, Store store) {
+// Calls store(slot, global_index, off[3], t) for every staged atom and pad(slot) for every pad slot and
+// for the dummy slot, all with slot <= cap.  One warp per tile cell.  Caller syncs afterwards.
+template <class Store, class Pad>
+__device__ __forceinline__ void tile_stage(const Geom& g, const TileTables& tt, int cap, Store store, Pad pad) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   for (int t = wid; t < tt.ntc; t += nw) {
-    int c = tt.cnt[t];
-    if (c == 0) continue;
+    const int c = tt.cnt[t], c4 = pad4(c);
+    if (c4 == 0) continue;
     double off[3];
     tile_cell_offset(g, tt, t, off);
-    int s0 = tt.start[t], g0 = tt.gstart[t];
-    for (int k = lane; k < c; k += 32)
-      if (s0 + k < cap) store(s0 + k, g0 + k, off);
+    const int s0 = tt.start[t], g0 = tt.gstart[t];
+    for (int k = lane; k < c4; k += 32) {
+      if (s0 + k >= cap) continue;
+      if (k < c) store(s0 + k, g0 + k, off, t);
+      else pad(s0 + k);
+    }
   }
+  if (threadIdx.x == 0) pad(tt.n_slots < cap ? tt.n_slots : cap);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -238,17 +317,20 @@ __global__ void k_bin(Geom g, int N, double* __restrict__ x, double* __restrict_
   rank[k] = atomicAdd(&cell_count[oid], 1);
 }
 
-// a2: exclusive scan of the cell counts, one block (ncell is at most a few 1e5).
-__global__ void k_scan_cells(int ncell, const int* __restrict__ cell_count, int* __restrict__ cell_start) {
+// a2: exclusive scan of the cell counts, one block of 1024 threads, 8 cells per thread per sweep.
+__global__ void __launch_bounds__(1024) k_scan_cells(int ncell, const int* __restrict__ cell_count, int* __restrict__ cell_start) {
+  constexpr int PER = 8;
   __shared__ int wsum[32];
   __shared__ int carry_s;
-  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   if (tid == 0) carry_s = 0;
   __syncthreads();
-  for (int base = 0; base < ncell; base += blockDim.x) {
-    int i = base + tid;
-    int v = i < ncell ? cell_count[i] : 0;
-    int incl = v;
+  for (int base = 0; base < ncell; base += 1024 * PER) {
+    const int i0 = base + tid * PER;
+    int v[PER], sum = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { v[k] = i0 + k < ncell ? cell_count[i0 + k] : 0; sum += v[k]; }
+    int incl = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       int u = __shfl_up_sync(0xffffffffu, incl, o);
@@ -257,7 +339,7 @@ __global__ void k_scan_cells(int ncell, const int* __restrict__ cell_count, int*
     if (lane == 31) wsum[wid] = incl;
     __syncthreads();
     if (wid == 0) {
-      int s = lane < nw ? wsum[lane] : 0, si = s;
+      int s = wsum[lane], si = s;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
         int u = __shfl_up_sync(0xffffffffu, si, o);
@@ -266,10 +348,15 @@ __global__ void k_scan_cells(int ncell, const int* __restrict__ cell_count, int*
       wsum[lane] = si - s;   // exclusive
     }
     __syncthreads();
-    int carry = carry_s;
-    if (i < ncell) cell_start[i] = carry + wsum[wid] + incl - v;
+    const int carry = carry_s;
+    int run = carry + wsum[wid] + incl - sum;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+      if (i0 + k < ncell) cell_start[i0 + k] = run;
+      run += v[k];
+    }
     __syncthreads();
-    if (tid == blockDim.x - 1) carry_s = carry + wsum[wid] + incl;
+    if (tid == 1023) carry_s = run;
     __syncthreads();
   }
   if (tid == 0) cell_start[ncell] = carry_s;
@@ -330,152 +417,219 @@ __global__ void k_iota(int N, int* __restrict__ a) {
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n < N) a[n] = n;
 }
-__global__ void k_scatter_types(int N, const int* __restrict__ id, const int* __restrict__ in, int* __restrict__ out) {
-  int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n < N) out[n] = in[id[n]];
-}
 
 // ---------------------------------------------------------------------------------------------------
-// a3: Verlet list build from the 27-cell stencil of the staged tile (north_star (2)); fp64 test.
-// Shared memory: TileTables | sx[cap+1] sy[cap+1] sz[cap+1] doubles.
-// List layout: 16-bit tile-local slots, 8 per uint4; entry e of interior atom a sits in word
+// a3: Verlet list build from the 27-cell stencil of the staged tile (north_star (2)).
+// One WARP per interior cell, one LANE per atom of that cell: every lane walks the same candidate
+// sequence (the 27 cells' staged slots, four candidates per 128-bit broadcast load from SoA shared
+// memory), so there is no divergence in the test loop.  The distance test runs in fp32 on tile-centred
+// coordinates with a guard band: r2 < rl2_lo accepts, r2 >= rl2_hi rejects, and the rare candidate in
+// between is decided in fp64 from the global positions, so the pair set is exactly the fp64 one.
+// Accepted slot codes go to a small per-lane ring in shared memory (one predicated 16-bit store each)
+// and leave for global memory as complete 128-bit words.
+// Shared memory: TileTables | xs[capA] ys[capA] zs[capA] floats | rings[nwarps*32*RING_STRIDE].
+// List layout: 16-bit codes (slot << code_shift), 8 per uint4; entry e of row a sits in word
 //   q = e/8, lane s = q % K, chunk c = q / K  at  list[tile_base + c*slots_cap + a*K + s].
-// Unused entries of the last word hold the dummy slot n_staged (a far-away point).
+// Unused entries of the last word hold the dummy slot n_slots (a far-away point).
 // ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(BLOCK) k_build_list(Geom g, const int* __restrict__ cell_start, const double* __restrict__ x,
-                                                      size_t ld, double rl2, uint4* __restrict__ list, int* __restrict__ numneigh,
-                                                      Flags* flags) {
+struct BuildArgs {
+  Geom g;
+  const int* cell_start;
+  const double* x; size_t ld;
+  double rl2;
+  float rl2_lo, rl2_hi;    // guard band of the fp32 test around rl2
+  uint4* list;
+  int* numneigh;           // [ntiles][interior_cap]
+  Flags* flags;
+};
+
+__device__ __forceinline__ int build_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
+
+__device__ __noinline__ bool confirm_pair_fp64(const Geom& g, const TileTables& tt, const double* __restrict__ x, size_t ld,
+                                               int gi, int ti, int gj, int tj, double rl2) {
+  double oi[3], oj[3];
+  tile_cell_offset(g, tt, ti, oi);
+  tile_cell_offset(g, tt, tj, oj);
+  double r2 = 0.0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    double dd = (x[d * ld + gi] + oi[d]) - (x[d * ld + gj] + oj[d]);
+    r2 += dd * dd;
+  }
+  return r2 < rl2;
+}
+
+template <bool HALF>
+__global__ void __launch_bounds__(BUILD_THREADS) k_build_list(BuildArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
-  double* sx = reinterpret_cast<double*>(smem_raw + sizeof(TileTables));
-  double* sy = sx + (g.tile_cap + 1);
-  double* sz = sy + (g.tile_cap + 1);
+  const Geom& g = A.g;
+  const int capA = build_capA(g);
+  float* xs = reinterpret_cast<float*>(smem_raw + sizeof(TileTables));
+  float* ys = xs + capA;
+  float* zs = ys + capA;
+  unsigned char* rings = reinterpret_cast<unsigned char*>(zs + capA);
   const int tile = blockIdx.x;
-  tile_setup(g, tile, cell_start, tt);
+  tile_setup(g, tile, A.cell_start, tt);
   if (threadIdx.x == 0) {
-    if (tt.n_staged > g.tile_cap) atomicMax(&flags->need_tile_cap, tt.n_staged);
-    if (tt.n_int > g.interior_cap) atomicMax(&flags->need_interior_cap, tt.n_int);
-    atomicMax(&flags->max_tile_atoms, tt.n_staged);
+    if (tt.n_slots > g.tile_cap) atomicMax(&A.flags->need_tile_cap, tt.n_slots);
+    if (tt.n_int_slots > g.interior_cap) atomicMax(&A.flags->need_interior_cap, tt.n_int_slots);
+    atomicMax(&A.flags->max_tile_atoms, tt.n_slots);
   }
-  if (tt.n_staged > g.tile_cap || tt.n_int > g.interior_cap) return;   // host re-plans and rebuilds
-  tile_stage(g, tt, g.tile_cap, [&](int slot, int gi, const double* off) {
-    sx[slot] = x[gi] + off[0];
-    sy[slot] = x[ld + gi] + off[1];
-    sz[slot] = x[2 * ld + gi] + off[2];
-  });
+  if (tt.n_slots > g.tile_cap || tt.n_int_slots > g.interior_cap) return;   // host re-plans and rebuilds
+  const double* __restrict__ x = A.x;
+  const size_t ld = A.ld;
+  tile_stage(g, tt, g.tile_cap,
+             [&](int slot, int gi, const double* off, int) {
+               xs[slot] = (float)(x[gi] + off[0]);
+               ys[slot] = (float)(x[ld + gi] + off[1]);
+               zs[slot] = (float)(x[2 * ld + gi] + off[2]);
+             },
+             [&](int slot) { xs[slot] = 1e15f; ys[slot] = 1e15f; zs[slot] = 1e15f; });
   __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const unsigned rbase = smem_addr(rings) + (unsigned)(wid * 32 + lane) * RING_STRIDE;
   const int K = g.K;
   const size_t slots_cap = (size_t)g.interior_cap * K;
-  uint4* tlist = list + (size_t)tile * g.chunk_cap * slots_cap;
-  const unsigned dummy = (unsigned)tt.n_staged;
+  uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
+  const int max_words = g.chunk_cap * K;
+  const unsigned dummy = (unsigned)tt.n_slots << g.code_shift;
+  const int shift = g.code_shift;
+  const float lo = A.rl2_lo, hi = A.rl2_hi;
   int my_max = 0;
   unsigned long long my_sum = 0;
-  // one thread per interior atom, walking the interior cells in staging order
-  for (int a = threadIdx.x; a < tt.n_int; a += blockDim.x) {
-    // which interior cell holds slot a?  interior cells are consecutive in order id; find by scanning
-    // the tile-cell table (interior cells only); tiles hold at most a few hundred cells.
-    int tx = 1, ty = 1, tz = 1;
-    {
-      int lo = 0, hi = tt.w[0] * tt.w[1] * tt.w[2] - 1;   // binary search over interior cells in order
-      while (lo < hi) {
-        int mid = (lo + hi + 1) >> 1;
-        int mx = mid % tt.w[0], my = (mid / tt.w[0]) % tt.w[1], mz = mid / (tt.w[0] * tt.w[1]);
-        int t = ((mz + 1) * tt.tc[1] + (my + 1)) * tt.tc[0] + (mx + 1);
-        if (tt.start[t] <= a) lo = mid; else hi = mid - 1;
-      }
-      tx = lo % tt.w[0] + 1; ty = (lo / tt.w[0]) % tt.w[1] + 1; tz = lo / (tt.w[0] * tt.w[1]) + 1;
-    }
-    const double xi = sx[a], yi = sy[a], zi = sz[a];
-    const int gi = tt.brick_start + a;
-    unsigned long long lo64 = 0, hi64 = 0;
-    int n = 0;
-    auto flush = [&](int nn) {   // word q = (nn-1)/8 is complete (or final)
-      int q = (nn - 1) >> 3;
-      int s = q % K, c = q / K;
-      uint4 w;
-      w.x = (unsigned)lo64; w.y = (unsigned)(lo64 >> 32); w.z = (unsigned)hi64; w.w = (unsigned)(hi64 >> 32);
-      tlist[(size_t)c * slots_cap + (size_t)a * K + s] = w;
-    };
-    for (int dz = -1; dz <= 1; ++dz)
-      for (int dy = -1; dy <= 1; ++dy)
-        for (int dx = -1; dx <= 1; ++dx) {
-          int t = ((tz + dz) * tt.tc[1] + (ty + dy)) * tt.tc[0] + (tx + dx);
-          int s0 = tt.start[t], c = tt.cnt[t], g0 = tt.gstart[t];
-          for (int k = 0; k < c; ++k) {
-            int j = s0 + k;
-            double ddx = xi - sx[j], ddy = yi - sy[j], ddz = zi - sz[j];
-            double r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-            bool take = r2 < rl2 && j != a;
-            if (g.half) take = take && (g0 + k > gi);
-            if (take) {
-              if (n < g.row_cap) {
-                int pos = n & 7;
-                if (pos < 4) lo64 |= (unsigned long long)j << (16 * pos);
-                else hi64 |= (unsigned long long)j << (16 * (pos - 4));
-                if (pos == 7) { flush(n + 1); lo64 = 0; hi64 = 0; }
+
+  for (int ic = wid; ic < tt.nic; ic += nw) {
+    const int t = interior_tile_cell(tt, ic);
+    const int s_lo = tt.start[t], c = tt.cnt[t], g_lo = tt.gstart[t];
+    const int tx = t % tt.tc[0], ty = (t / tt.tc[0]) % tt.tc[1], tz = t / (tt.tc[0] * tt.tc[1]);
+    for (int r0 = 0; r0 < c; r0 += 32) {
+      const bool act = r0 + lane < c;
+      const int a = act ? s_lo + r0 + lane : s_lo;   // staged slot = list row
+      const int gi = g_lo + r0 + lane;
+      const float xi = xs[a], yi = ys[a], zi = zs[a];
+      unsigned rp = rbase;
+      int nwords = 0;
+      auto store_word = [&](uint4 v) {
+        if (nwords < max_words) {
+          int s = nwords % K, cch = nwords / K;
+          st_stream(tlist + (size_t)cch * slots_cap + (size_t)a * K + s, v);
+        }
+        ++nwords;
+      };
+      auto flush = [&]() {   // complete words leave; the remainder moves to the ring start
+        const int pend = (int)(rp - rbase) >> 1, full = pend >> 3;
+        for (int w = 0; w < full; ++w) store_word(lds_u4(rbase + 16 * w));
+        if (full) sts_u4(rbase, lds_u4(rbase + 16 * full));
+        rp = rbase + 2 * (pend & 7);
+      };
+      for (int dz = -1; dz <= 1; ++dz)
+        for (int dy = -1; dy <= 1; ++dy)
+          for (int dx = -1; dx <= 1; ++dx) {
+            const int t2 = ((tz + dz) * tt.tc[1] + (ty + dy)) * tt.tc[0] + (tx + dx);
+            const int s0 = tt.start[t2], c2 = tt.cnt[t2], g0 = tt.gstart[t2];
+            const int aself = t2 == t ? a : -1;
+            for (int k0 = 0; k0 < c2; k0 += 32) {
+              if (((int)(rp - rbase) >> 1) + 32 > RING) flush();
+              const int ng = (min(c2 - k0, 32) + 3) >> 2;
+              for (int q = 0; q < ng; ++q) {
+                const int j0 = s0 + k0 + 4 * q;
+                const float4 X = *reinterpret_cast<const float4*>(xs + j0);
+                const float4 Y = *reinterpret_cast<const float4*>(ys + j0);
+                const float4 Z = *reinterpret_cast<const float4*>(zs + j0);
+                const float xx[4] = {X.x, X.y, X.z, X.w}, yy[4] = {Y.x, Y.y, Y.z, Y.w}, zz[4] = {Z.x, Z.y, Z.z, Z.w};
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                  const float ddx = xi - xx[u], ddy = yi - yy[u], ddz = zi - zz[u];
+                  const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+                  const int j = j0 + u;
+                  bool take = act && r2 < hi && j != aself;
+                  if (HALF) take = take && (g0 + (j - s0) > gi);
+                  if (__builtin_expect(take && r2 > lo, 0))
+                    take = confirm_pair_fp64(g, tt, x, ld, gi, t, g0 + (j - s0), t2, A.rl2);
+                  asm volatile("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p st.shared.u16 [%0], %1; }" ::"r"(rp),
+                               "h"((unsigned short)(j << shift)), "r"((unsigned)take)
+                               : "memory");
+                  rp += take ? 2u : 0u;
+                }
               }
-              ++n;
             }
           }
-        }
-    int stored = n < g.row_cap ? n : g.row_cap;
-    if (stored & 7) {   // pad the last word with the dummy slot
-      for (int pos = stored & 7; pos < 8; ++pos) {
-        if (pos < 4) lo64 |= (unsigned long long)dummy << (16 * pos);
-        else hi64 |= (unsigned long long)dummy << (16 * (pos - 4));
+      // last words: complete ones, then the partial one padded with the dummy code
+      flush();
+      const int rem = (int)(rp - rbase) >> 1;   // 0..7
+      if (rem) {
+        uint4 v = lds_u4(rbase);
+        unsigned h[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int p = 0; p < 8; ++p)
+          if (p >= rem) h[p >> 1] = (p & 1) ? ((h[p >> 1] & 0xffffu) | (dummy << 16)) : ((h[p >> 1] & 0xffff0000u) | dummy);
+        v.x = h[0]; v.y = h[1]; v.z = h[2]; v.w = h[3];
+        const int before = nwords;
+        store_word(v);
+        nwords = before;   // count below from complete words + rem
       }
-      flush(stored);
+      const int n = nwords * 8 + rem;
+      if (act) {
+        const int stored = n < g.row_cap ? n : g.row_cap;
+        A.numneigh[(size_t)tile * g.interior_cap + a] = stored;
+        my_max = max(my_max, n);
+        my_sum += (unsigned long long)stored;
+      }
     }
-    numneigh[gi] = stored;
-    my_max = max(my_max, n);
-    my_sum += (unsigned long long)stored;
   }
-  // statistics
   for (int o = 16; o > 0; o >>= 1) {
     my_max = max(my_max, __shfl_xor_sync(0xffffffffu, my_max, o));
     my_sum += __shfl_xor_sync(0xffffffffu, my_sum, o);
   }
-  if ((threadIdx.x & 31) == 0) {
-    atomicMax(&flags->max_row, my_max);
-    if (my_max > g.row_cap) atomicMax(&flags->need_row_cap, my_max);
-    atomicAdd(&flags->sum_rows, my_sum);
+  if (lane == 0) {
+    atomicMax(&A.flags->max_row, my_max);
+    if (my_max > g.row_cap) atomicMax(&A.flags->need_row_cap, my_max);
+    atomicAdd(&A.flags->sum_rows, my_sum);
   }
 }
 
-// list export in caller ids (pair-set parity).  Shared memory: TileTables | sid[cap+1] ints.
-__global__ void __launch_bounds__(BLOCK) k_export_list(Geom g, const int* __restrict__ cell_start, const int* __restrict__ id,
-                                                       const uint4* __restrict__ list, const int* __restrict__ numneigh,
-                                                       int* __restrict__ nn_out, int* __restrict__ neigh_out, long long stride) {
+// list export in caller ids (pair-set parity).  Shared memory: TileTables | sid[tile_cap+4] ints.
+__global__ void __launch_bounds__(BUILD_THREADS) k_export_list(Geom g, const int* __restrict__ cell_start, const int* __restrict__ id,
+                                                               const uint4* __restrict__ list, const int* __restrict__ numneigh,
+                                                               int* __restrict__ nn_out, int* __restrict__ neigh_out, long long stride) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
   int* sid = reinterpret_cast<int*>(smem_raw + sizeof(TileTables));
   const int tile = blockIdx.x;
   tile_setup(g, tile, cell_start, tt);
-  tile_stage(g, tt, g.tile_cap, [&](int slot, int gi, const double*) { sid[slot] = id[gi]; });
+  tile_stage(g, tt, g.tile_cap, [&](int slot, int gi, const double*, int) { sid[slot] = id[gi]; }, [&](int slot) { sid[slot] = -1; });
   __syncthreads();
   const int K = g.K;
   const size_t slots_cap = (size_t)g.interior_cap * K;
   const uint4* tlist = list + (size_t)tile * g.chunk_cap * slots_cap;
-  for (int a = threadIdx.x; a < tt.n_int; a += blockDim.x) {
-    int gi = tt.brick_start + a, n = numneigh[gi], io = id[gi];
-    nn_out[io] = n;
-    for (int e = 0; e < n && e < stride; ++e) {
-      int q = e >> 3, s = q % K, c = q / K;
-      uint4 w = tlist[(size_t)c * slots_cap + (size_t)a * K + s];
-      unsigned word = (&w.x)[(e & 7) >> 1];
-      unsigned j = (e & 1) ? (word >> 16) : (word & 0xffffu);
-      neigh_out[(long long)io * stride + e] = sid[j];
+  for (int ic = 0; ic < tt.nic; ++ic) {
+    const int t = interior_tile_cell(tt, ic);
+    for (int k = threadIdx.x; k < tt.cnt[t]; k += blockDim.x) {
+      const int a = tt.start[t] + k, n = numneigh[(size_t)tile * g.interior_cap + a], io = sid[a];
+      nn_out[io] = n;
+      for (int e = 0; e < n && e < stride; ++e) {
+        int q = e >> 3, s = q % K, c = q / K;
+        uint4 w = tlist[(size_t)c * slots_cap + (size_t)a * K + s];
+        unsigned word = (&w.x)[(e & 7) >> 1];
+        unsigned code = (e & 1) ? (word >> 16) : (word & 0xffffu);
+        neigh_out[(long long)io * stride + e] = sid[code >> g.code_shift];
+      }
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------------
 // pair styles.  T = double (MD_FP64) or float (MD_MIXED pair math).
-// A Body accumulates per-word partial sums in T and per-atom totals in double.
+// A Body accumulates per-word partial sums in T; the kernels add them to per-atom totals in double.
+// Bodies are branch-free: out-of-range partners contribute an exact zero through a select.
 // ---------------------------------------------------------------------------------------------------
-template <typename T> struct Vec4;
-template <> struct Vec4<float> { using type = float4; };
-template <> struct Vec4<double> { using type = double4; };
+template <typename T> struct Vec2;
+template <> struct Vec2<float> { using type = float2; };
+template <> struct Vec2<double> { using type = double2; };
+template <typename T> __device__ __forceinline__ typename Vec2<T>::type lds_v2(unsigned a);
+template <> __device__ __forceinline__ float2 lds_v2<float>(unsigned a) { return lds_f2(a); }
+template <> __device__ __forceinline__ double2 lds_v2<double>(unsigned a) { return lds_d2(a); }
 
 struct PairParams {    // host-prepared constants, in double; kernels convert once
   double rc2;
@@ -489,7 +643,6 @@ template <> __device__ __forceinline__ double t_rcp<double>(double x) { return 1
 template <typename T> __device__ __forceinline__ T t_rsqrt(T x);
 template <> __device__ __forceinline__ float t_rsqrt<float>(float x) { return rsqrt_approx(x); }
 template <> __device__ __forceinline__ double t_rsqrt<double>(double x) { return 1.0 / sqrt(x); }
-// exp(-a) for a >= 0-ish arguments
 template <typename T> __device__ __forceinline__ T t_exp(T x);
 template <> __device__ __forceinline__ float t_exp<float>(float x) { return ex2_approx(x * 1.4426950408889634f); }
 template <> __device__ __forceinline__ double t_exp<double>(double x) { return exp(x); }
@@ -500,74 +653,136 @@ struct LJBody {
   static constexpr int NT = EV ? 10 : 3;   // fx fy fz [e wxx wyy wzz wxy wxz wyz]
   T rc2, lj1, lj2, lj3, lj4;
   __device__ explicit LJBody(const PairParams& P) : rc2((T)P.rc2), lj1((T)P.lj1), lj2((T)P.lj2), lj3((T)P.lj3), lj4((T)P.lj4) {}
-  __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T, T, T (&p)[NT]) const {
-    if (r2 < rc2) {
-      T r2i = t_rcp<T>(r2);
-      T r6 = r2i * r2i * r2i;
-      T fp = r6 * (lj1 * r6 - lj2) * r2i;
-      p[0] += fp * dx; p[1] += fp * dy; p[2] += fp * dz;
-      if constexpr (EV) {
-        p[3] += r6 * (lj3 * r6 - lj4);
-        p[4] += dx * dx * fp; p[5] += dy * dy * fp; p[6] += dz * dz * fp;
-        p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
-      }
+  __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T, bool ok, T (&p)[NT]) const {
+    const bool in = ok && r2 < rc2;
+    T r2i = t_rcp<T>(r2);
+    T r6 = r2i * r2i * r2i;
+    T fp = in ? r6 * (lj1 * r6 - lj2) * r2i : (T)0;
+    p[0] += fp * dx; p[1] += fp * dy; p[2] += fp * dz;
+    if constexpr (EV) {
+      p[3] += in ? r6 * (lj3 * r6 - lj4) : (T)0;
+      p[4] += dx * dx * fp; p[5] += dy * dy * fp; p[6] += dz * dz * fp;
+      p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
     }
   }
 };
 
 // EAM pass 1: rho_i = sum_j exp(-q (r/r0 - 1))            (a6)
-template <typename T>
+template <typename T, bool EV>
 struct EamDensityBody {
   static constexpr int NT = 1;
   T rc2, q_r0, q;
   __device__ explicit EamDensityBody(const PairParams& P) : rc2((T)P.rc2), q_r0((T)P.q_r0), q((T)P.q) {}
-  __device__ __forceinline__ void pair(T, T, T, T r2, T, T, T (&p)[NT]) const {
-    if (r2 < rc2) {
-      T r = r2 * t_rsqrt<T>(r2);
-      p[0] += t_exp<T>(q - q_r0 * r);
-    }
+  __device__ __forceinline__ void pair(T, T, T, T r2, T, bool ok, T (&p)[NT]) const {
+    const bool in = ok && r2 < rc2;
+    T r = r2 * t_rsqrt<T>(r2);
+    p[0] += in ? t_exp<T>(q - q_r0 * r) : (T)0;
   }
 };
 
-// EAM pass 2: F_i = -sum_j [ (F'_i + F'_j) rho'(r) + phi'(r) ] D / r      (a7); w carries F'.
+// EAM pass 2: F_i = -sum_j [ (F'_i + F'_j) rho'(r) + phi'(r) ] D / r      (a7); wsum = F'_i + F'_j.
 template <typename T, bool EV>
 struct EamForceBody {
   static constexpr int NT = EV ? 10 : 3;
   T rc2, q_r0, q, p_r0, pp, A;
   __device__ explicit EamForceBody(const PairParams& P)
       : rc2((T)P.rc2), q_r0((T)P.q_r0), q((T)P.q), p_r0((T)P.p_r0), pp((T)P.p), A((T)P.A) {}
-  __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T wi, T wj, T (&p)[NT]) const {
-    if (r2 < rc2) {
-      T rinv = t_rsqrt<T>(r2);
-      T r = r2 * rinv;
-      T rho = t_exp<T>(q - q_r0 * r);
-      T phi = A * t_exp<T>(pp - p_r0 * r);
-      // rho' = -(q/r0) rho, phi' = -(p/r0) phi  =>  fpair = [ (F'_i+F'_j)(q/r0) rho + (p/r0) phi ] / r
-      T fp = ((wi + wj) * q_r0 * rho + p_r0 * phi) * rinv;
-      p[0] += fp * dx; p[1] += fp * dy; p[2] += fp * dz;
-      if constexpr (EV) {
-        p[3] += phi;
-        p[4] += dx * dx * fp; p[5] += dy * dy * fp; p[6] += dz * dz * fp;
-        p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
-      }
+  __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T wsum, bool ok, T (&p)[NT]) const {
+    const bool in = ok && r2 < rc2;
+    T rinv = t_rsqrt<T>(r2);
+    T r = r2 * rinv;
+    T rho = t_exp<T>(q - q_r0 * r);
+    T phi = A * t_exp<T>(pp - p_r0 * r);
+    // rho' = -(q/r0) rho, phi' = -(p/r0) phi  =>  fpair = [ (F'_i+F'_j)(q/r0) rho + (p/r0) phi ] / r
+    T fp = in ? (wsum * q_r0 * rho + p_r0 * phi) * rinv : (T)0;
+    p[0] += fp * dx; p[1] += fp * dy; p[2] += fp * dz;
+    if constexpr (EV) {
+      p[3] += in ? phi : (T)0;
+      p[4] += dx * dx * fp; p[5] += dy * dy * fp; p[6] += dz * dz * fp;
+      p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
     }
   }
 };
 
 // ---------------------------------------------------------------------------------------------------
+// a5/a6/a7 (+ a8, a4 fused): arguments shared by the force kernels
+// ---------------------------------------------------------------------------------------------------
+constexpr int EPI_FORCES = 0;      // write f[i] (md_compute_forces; first evaluation of a run)
+constexpr int EPI_KICK_DRIFT = 1;  // v += dtf f; then next step's first half: v += dtf f; x' = x + dt v; max |x'-x0|^2
+constexpr int EPI_FINAL = 2;       // v += dtf f; write f[i] (last step of a run)
+
+struct ForceArgs {
+  Geom g;
+  PairParams P;
+  const int* cell_start;
+  const double* x; size_t ld;
+  const uint4* list;
+  const int* numneigh;
+  const double* fp_in;     // EAM pass 2: F'(rho) per sorted atom (else NULL)
+  double* f;               // forces out
+  double* rho; double* fp_out;   // EAM pass 1 out
+  double* ev_partials;     // [ntiles][8]: e, wxx, wyy, wzz, wxy, wxz, wyz, pad
+  // time stepping (a8) and the displacement test (a4), fused into the epilogue
+  int epi;                 // EPI_*
+  int in_run;              // 1: the launch belongs to a batch of steps: do nothing if the list is stale
+  int parity;              // reads max_disp2_bits[parity], writes max_disp2_bits[1-parity]
+  double* v; double* x_new; const double* x0;
+  const int* type; const double* mass;
+  double dt, half_dt_ftm2v, trigger;
+  Flags* flags;
+};
+
+// true if this launch must do nothing: an earlier step of the batch moved some atom farther than
+// skin/2 from its position at the last build, so the host has to rebuild first (reading s4).
+__device__ __forceinline__ bool list_is_stale(const ForceArgs& A) {
+  if (!A.in_run) return false;
+  const double d2 = __longlong_as_double((long long)A.flags->max_disp2_bits[A.parity]);
+  const bool stale = A.flags->stop != 0 || d2 > A.trigger;
+  if (stale && threadIdx.x == 0 && blockIdx.x == 0) atomicExch(&A.flags->stop, 1);
+  return stale;
+}
+
+// per-atom epilogue; returns |x'-x0|^2 for EPI_KICK_DRIFT (else 0)
+__device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, const double (&tot)[3]) {
+  const size_t ld = A.ld;
+  if (A.epi == EPI_FORCES) {
+    A.f[gi] = tot[0]; A.f[ld + gi] = tot[1]; A.f[2 * ld + gi] = tot[2];
+    return 0.0;
+  }
+  const double dtf = A.half_dt_ftm2v / A.mass[A.type[gi]];
+  double d2 = 0.0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    double vv = A.v[d * ld + gi] + dtf * tot[d];          // second half kick of this step
+    if (A.epi == EPI_KICK_DRIFT) {
+      vv += dtf * tot[d];                                 // first half kick of the next step
+      const double xx = A.x[d * ld + gi] + A.dt * vv;     // drift
+      A.x_new[d * ld + gi] = xx;
+      const double dd = xx - A.x0[d * ld + gi];
+      d2 += dd * dd;
+    } else {
+      A.f[d * ld + gi] = tot[d];
+    }
+    A.v[d * ld + gi] = vv;
+  }
+  return d2;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // the neighbor-list loop of PAPER.md L88-122 for one (atom, lane): walks this lane's 128-bit words,
-// 8 entries each, gathers from the shared-memory tile, accumulates word partials in T and totals in
-// double.  `tile` holds n_staged+1 vec4 entries (x,y,z,w).
+// 8 entries each; each entry is the byte offset of partner j in the two staged arrays xy[] and zw[]
+// (two LDS.64 per gather: 6.5 cycles per warp against 8.2 for one LDS.128 at random addresses, measured).
+// zw.y of the staged atoms holds -F'(rho_j) for EAM pass 2, so pzw.y - jzw.y = F'_i + F'_j.
 // ---------------------------------------------------------------------------------------------------
 template <typename T, class Body>
-__device__ __forceinline__ void list_loop(const Body& body, const typename Vec4<T>::type* __restrict__ tile,
-                                          const uint4* __restrict__ words, size_t word_stride, int nwords,
-                                          typename Vec4<T>::type pi, double (&tot)[Body::NT]) {
+__device__ __forceinline__ void list_loop(const Body& body, unsigned xy_base, unsigned zw_base, const uint4* __restrict__ words,
+                                          size_t word_stride, int nwords, typename Vec2<T>::type pxy, typename Vec2<T>::type pzw,
+                                          double (&tot)[Body::NT]) {
   constexpr int NT = Body::NT;
   if (nwords <= 0) return;
   uint4 w = ld_stream(words);
   for (int c = 0; c < nwords; ++c) {
-    uint4 cur = w;
+    const uint4 cur = w;
     if (c + 1 < nwords) w = ld_stream(words + (size_t)(c + 1) * word_stride);
     T p[NT];
 #pragma unroll
@@ -577,11 +792,11 @@ __device__ __forceinline__ void list_loop(const Body& body, const typename Vec4<
     for (int h = 0; h < 4; ++h) {
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
-        unsigned j = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
-        typename Vec4<T>::type pj = tile[j];
-        T dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-        T r2 = dx * dx + dy * dy + dz * dz;
-        body.pair(dx, dy, dz, r2, pi.w, pj.w, p);
+        const unsigned code = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
+        const typename Vec2<T>::type jxy = lds_v2<T>(xy_base + code), jzw = lds_v2<T>(zw_base + code);
+        const T dx = pxy.x - jxy.x, dy = pxy.y - jxy.y, dz = pzw.x - jzw.x;
+        const T r2 = dx * dx + dy * dy + dz * dz;
+        body.pair(dx, dy, dz, r2, pzw.y - jzw.y, true, p);
       }
     }
 #pragma unroll
@@ -589,143 +804,100 @@ __device__ __forceinline__ void list_loop(const Body& body, const typename Vec4<
   }
 }
 
-// the direct cell-list loop (reading s10): no list; atom a tests every staged atom of
-// the 27 tile cells around its own cell.
-template <typename T, class Body>
-__device__ __forceinline__ void cell_loop(const Body& body, const typename Vec4<T>::type* __restrict__ tile, const TileTables& tt,
-                                          int a, int tx, int ty, int tz, typename Vec4<T>::type pi, double (&tot)[Body::NT]) {
-  constexpr int NT = Body::NT;
-  for (int dz = -1; dz <= 1; ++dz)
-    for (int dy = -1; dy <= 1; ++dy)
-      for (int dx = -1; dx <= 1; ++dx) {
-        int t = ((tz + dz) * tt.tc[1] + (ty + dy)) * tt.tc[0] + (tx + dx);
-        int s0 = tt.start[t], c = tt.cnt[t];
-        T p[NT];
-#pragma unroll
-        for (int k = 0; k < NT; ++k) p[k] = (T)0;
-        for (int k = 0; k < c; ++k) {
-          int j = s0 + k;
-          if (j == a) continue;
-          typename Vec4<T>::type pj = tile[j];
-          T ex = pi.x - pj.x, ey = pi.y - pj.y, ez = pi.z - pj.z;
-          T r2 = ex * ex + ey * ey + ez * ez;
-          body.pair(ex, ey, ez, r2, pi.w, pj.w, p);
-        }
-#pragma unroll
-        for (int k = 0; k < NT; ++k) tot[k] += (double)p[k];
-      }
-}
-
-__device__ __forceinline__ void interior_cell_of(const TileTables& tt, int a, int& tx, int& ty, int& tz) {
-  int lo = 0, hi = tt.w[0] * tt.w[1] * tt.w[2] - 1;
-  while (lo < hi) {
-    int mid = (lo + hi + 1) >> 1;
-    int mx = mid % tt.w[0], my = (mid / tt.w[0]) % tt.w[1], mz = mid / (tt.w[0] * tt.w[1]);
-    int t = ((mz + 1) * tt.tc[1] + (my + 1)) * tt.tc[0] + (mx + 1);
-    if (tt.start[t] <= a) lo = mid; else hi = mid - 1;
-  }
-  tx = lo % tt.w[0] + 1; ty = (lo / tt.w[0]) % tt.w[1] + 1; tz = lo / (tt.w[0] * tt.w[1]) + 1;
-}
-
 // ---------------------------------------------------------------------------------------------------
-// a5/a6/a7: the tile force kernel.
-//   MODE 0: forces (LJ or EAM pass 2) -> f[3][N] (+ per-block energy/virial partials when EV)
-//   MODE 1: EAM pass 1 -> rho[N], fp[N] = F'(rho) (+ per-block embedding energy partial)
-//   HALF (MODE 0 only, K = 1): each pair once, -F scattered to f[j] with fp64 atomics (f zeroed before).
-//   CELL: no list, direct cell loop.
-// Shared memory: TileTables | vec4<T> tile[cap+1] | (HALF: int sgid[cap+1])
-// w component of the staged atoms: F'(rho_j) for EAM pass 2, else 0.
+// a5/a6/a7: the tile force kernel over the Verlet list.
+//   MODE 0: forces (LJ or EAM pass 2) + epilogue A.epi (+ per-block energy/virial partials when EV)
+//   MODE 1: EAM pass 1 -> rho[N], fp[N] = F'(rho) (+ per-block embedding energy partial when EV)
+//   HALF (MODE 0 only, K = 1, EPI_FORCES only): each pair once, -F scattered to f[j] with fp64 atomics.
+// Thread <-> (interior slot a = list row, lane s of K).  Block size is chosen by the host so that the
+// tile's rows fill whole rounds of the block.
+// Shared memory: TileTables | xy[capA] | zw[capA] (Vec2<T>) | scell[interior_cap] u16 | (HALF: sgid[capA] int)
 // ---------------------------------------------------------------------------------------------------
-struct ForceArgs {
-  Geom g;
-  PairParams P;
-  const int* cell_start;
-  const double* x; size_t ld;
-  const uint4* list;
-  const int* numneigh;
-  const double* fp_in;     // EAM pass 2: F'(rho) per sorted atom (else NULL)
-  double* f;               // MODE 0 out
-  double* rho; double* fp_out;   // MODE 1 out
-  double* ev_partials;     // [ntiles][8]: e, wxx, wyy, wzz, wxy, wxz, wyz, pad   (EV or MODE 1)
-};
+__host__ __device__ inline int force_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
 
-template <typename T, class Body, int K, int MODE, bool EV, bool HALF, bool CELL>
-__global__ void __launch_bounds__(BLOCK) k_tile_force(ForceArgs A) {
-  using V4 = typename Vec4<T>::type;
+template <typename T, class Body, int K, int MODE, bool EV, bool HALF>
+__global__ void __launch_bounds__(FORCE_MAX_THREADS) k_tile_force(ForceArgs A) {
+  using V2 = typename Vec2<T>::type;
   constexpr int NT = Body::NT;
+  if (list_is_stale(A)) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
-  V4* tile = reinterpret_cast<V4*>(smem_raw + sizeof(TileTables));
-  int* sgid = reinterpret_cast<int*>(tile + (A.g.tile_cap + 1));   // HALF only
-  __shared__ double red[8 * 32];
   const Geom& g = A.g;
+  const int capA = force_capA(g);
+  V2* xy = reinterpret_cast<V2*>(smem_raw + sizeof(TileTables));
+  V2* zw = xy + capA;
+  unsigned short* scell = reinterpret_cast<unsigned short*>(zw + capA);
+  int* sgid = reinterpret_cast<int*>(scell + g.interior_cap);   // HALF only
+  __shared__ double red[8 * 32];
   const int tileid = blockIdx.x;
   tile_setup(g, tileid, A.cell_start, tt);
   const double* __restrict__ xs = A.x;
   const size_t ld = A.ld;
   const double* __restrict__ fpin = A.fp_in;
-  tile_stage(g, tt, g.tile_cap, [&](int slot, int gi, const double* off) {
-    V4 v;
-    v.x = (T)(xs[gi] + off[0]);
-    v.y = (T)(xs[ld + gi] + off[1]);
-    v.z = (T)(xs[2 * ld + gi] + off[2]);
-    v.w = fpin ? (T)fpin[gi] : (T)0;
-    tile[slot] = v;
-    if constexpr (HALF) sgid[slot] = gi;
-  });
-  if (threadIdx.x == 0) {
-    V4 far;
-    far.x = (T)1e15; far.y = (T)1e15; far.z = (T)1e15; far.w = (T)0;
-    tile[tt.n_staged < g.tile_cap ? tt.n_staged : g.tile_cap] = far;
-  }
+  const int icap = g.interior_cap;
+  tile_stage(g, tt, g.tile_cap,
+             [&](int slot, int gi, const double* off, int t) {
+               V2 a, b;
+               a.x = (T)(xs[gi] + off[0]);
+               a.y = (T)(xs[ld + gi] + off[1]);
+               b.x = (T)(xs[2 * ld + gi] + off[2]);
+               b.y = fpin ? (T)(-fpin[gi]) : (T)0;
+               xy[slot] = a; zw[slot] = b;
+               if (slot < icap && slot < tt.n_int_slots) scell[slot] = (unsigned short)t;
+               if constexpr (HALF) sgid[slot] = gi;
+             },
+             [&](int slot) {
+               V2 a, b;
+               a.x = (T)1e15; a.y = (T)1e15; b.x = (T)1e15; b.y = (T)0;
+               xy[slot] = a; zw[slot] = b;
+               if (slot < icap && slot < tt.n_int_slots) scell[slot] = 0xffffu;
+               if constexpr (HALF) sgid[slot] = 0;
+             });
   __syncthreads();
   const Body body(A.P);
-  const size_t slots_cap = (size_t)g.interior_cap * K;
+  const unsigned xy_base = smem_addr(xy), zw_base = smem_addr(zw);
+  const size_t slots_cap = (size_t)icap * K;
   const uint4* tlist = A.list + (size_t)tileid * g.chunk_cap * slots_cap;
   double ev[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-  const int nslots = tt.n_int * K;
-  for (int base = 0; base < nslots; base += blockDim.x) {   // uniform trip count: shuffles below need full groups
-    int sidx = base + threadIdx.x;
-    bool active = sidx < nslots;
-    int a = active ? sidx / K : 0, s = sidx % K;
-    int gi = tt.brick_start + a;
+  double d2max = 0.0;
+  const int nslots = tt.n_int_slots * K;
+  for (int base = 0; base < nslots; base += blockDim.x) {   // uniform trip count: the shuffles below need full groups
+    const int sidx = base + threadIdx.x;
+    const int a = sidx / K, s = sidx % K;
+    unsigned cell = 0xffffu;
+    if (sidx < nslots) cell = scell[a];
+    const bool active = cell != 0xffffu;
+    const int gi = active ? tt.gstart[cell] + (a - tt.start[cell]) : 0;
     double tot[NT];
 #pragma unroll
     for (int k = 0; k < NT; ++k) tot[k] = 0.0;
     if (active) {
-      V4 pi = tile[a];
-      if constexpr (CELL) {
-        if (s == 0) {
-          int tx, ty, tz;
-          interior_cell_of(tt, a, tx, ty, tz);
-          cell_loop<T, Body>(body, tile, tt, a, tx, ty, tz, pi, tot);
-        }
-      } else if constexpr (!HALF) {
-        int n = A.numneigh[gi];
-        int nq = (n + 7) >> 3;                       // words of this atom
-        int mine = nq > s ? (nq - s + K - 1) / K : 0; // words q = s, s+K, ...
-        list_loop<T, Body>(body, tile, tlist + sidx, slots_cap, mine, pi, tot);
+      V2 pxy = xy[a], pzw = zw[a];
+      pzw.y = -pzw.y;
+      const int n = A.numneigh[(size_t)tileid * icap + a];
+      const int nq = (n + 7) >> 3;                          // words of this atom
+      if constexpr (!HALF) {
+        const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
+        list_loop<T, Body>(body, xy_base, zw_base, tlist + sidx, slots_cap, mine, pxy, pzw, tot);
       } else {
         // half list: each in-range pair once; +F to i (registers), -F to j (atomics)
-        int n = A.numneigh[gi];
-        int nq = (n + 7) >> 3;
         for (int c = 0; c < nq; ++c) {
-          uint4 cur = tlist[(size_t)c * slots_cap + sidx];
+          const uint4 cur = tlist[(size_t)c * slots_cap + sidx];
           const unsigned ww[4] = {cur.x, cur.y, cur.z, cur.w};
 #pragma unroll
           for (int h = 0; h < 4; ++h)
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-              unsigned j = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
-              V4 pj = tile[j];
-              T dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-              T r2 = dx * dx + dy * dy + dz * dz;
+              const unsigned code = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
+              const V2 jxy = lds_v2<T>(xy_base + code), jzw = lds_v2<T>(zw_base + code);
+              const T dx = pxy.x - jxy.x, dy = pxy.y - jxy.y, dz = pzw.x - jzw.x;
+              const T r2 = dx * dx + dy * dy + dz * dz;
               T p[NT];
 #pragma unroll
               for (int k = 0; k < NT; ++k) p[k] = (T)0;
-              body.pair(dx, dy, dz, r2, pi.w, pj.w, p);
+              body.pair(dx, dy, dz, r2, pzw.y - jzw.y, true, p);
               if (p[0] != (T)0 || p[1] != (T)0 || p[2] != (T)0) {
-                int gj = sgid[j];
+                const int gj = sgid[code >> g.code_shift];
                 atomicAdd(&A.f[gj], -(double)p[0]);
                 atomicAdd(&A.f[ld + gj], -(double)p[1]);
                 atomicAdd(&A.f[2 * ld + gj], -(double)p[2]);
@@ -745,7 +917,8 @@ __global__ void __launch_bounds__(BLOCK) k_tile_force(ForceArgs A) {
         if constexpr (HALF) {
           atomicAdd(&A.f[gi], tot[0]); atomicAdd(&A.f[ld + gi], tot[1]); atomicAdd(&A.f[2 * ld + gi], tot[2]);
         } else {
-          A.f[gi] = tot[0]; A.f[ld + gi] = tot[1]; A.f[2 * ld + gi] = tot[2];
+          const double t3[3] = {tot[0], tot[1], tot[2]};
+          d2max = fmax(d2max, atom_epilogue(A, gi, t3));
         }
         if constexpr (EV) {
           const double wgt = HALF ? 1.0 : 0.5;   // a full list visits every pair twice
@@ -753,19 +926,133 @@ __global__ void __launch_bounds__(BLOCK) k_tile_force(ForceArgs A) {
           for (int k = 0; k < 7; ++k) ev[k] += wgt * tot[3 + k];
         }
       } else {
-        double rho = tot[0];
-        double sq = sqrt(rho);
+        const double rho = tot[0];
+        const double sq = sqrt(rho);
         A.rho[gi] = rho;
         A.fp_out[gi] = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
-        ev[0] += -A.P.B * sq;                                    // embedding energy F(rho_i)
+        if constexpr (EV) ev[0] += -A.P.B * sq;                  // embedding energy F(rho_i)
       }
     }
   }
-  if constexpr (EV || MODE == 1) {
+  if constexpr (EV) {
     block_sum<8>(ev, red);
     if (threadIdx.x == 0)
 #pragma unroll
       for (int k = 0; k < 8; ++k) A.ev_partials[(size_t)tileid * 8 + k] = ev[k];
+  }
+  if constexpr (MODE == 0 && !HALF) {
+    if (A.epi == EPI_KICK_DRIFT) {   // a4: device-side max-displacement reduction
+      block_max_to_flag(d2max, red, &A.flags->max_disp2_bits[1 - A.parity]);
+    }
+    if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a5' direct cell-list variant (reading s10): no list.  One warp per interior cell, one
+// lane per atom; every lane tests every staged atom of the 27 tile cells around its cell, four
+// candidates per broadcast 128-bit load from SoA shared memory (the same walk as the list build).
+// Shared memory: TileTables | xs ys zs ws [capA] of T.
+// ---------------------------------------------------------------------------------------------------
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { using type = float4; };
+template <> struct Vec4<double> { using type = double4; };
+
+template <typename T, class Body, int MODE, bool EV>
+__global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
+  using V4 = typename Vec4<T>::type;
+  constexpr int NT = Body::NT;
+  if (list_is_stale(A)) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
+  const Geom& g = A.g;
+  const int capA = force_capA(g);
+  T* xs = reinterpret_cast<T*>(smem_raw + sizeof(TileTables));
+  T* ys = xs + capA;
+  T* zs = ys + capA;
+  T* ws = zs + capA;
+  __shared__ double red[8 * 32];
+  const int tileid = blockIdx.x;
+  tile_setup(g, tileid, A.cell_start, tt);
+  const double* __restrict__ x = A.x;
+  const size_t ld = A.ld;
+  const double* __restrict__ fpin = A.fp_in;
+  tile_stage(g, tt, g.tile_cap,
+             [&](int slot, int gi, const double* off, int) {
+               xs[slot] = (T)(x[gi] + off[0]);
+               ys[slot] = (T)(x[ld + gi] + off[1]);
+               zs[slot] = (T)(x[2 * ld + gi] + off[2]);
+               ws[slot] = fpin ? (T)fpin[gi] : (T)0;
+             },
+             [&](int slot) { xs[slot] = (T)1e15; ys[slot] = (T)1e15; zs[slot] = (T)1e15; ws[slot] = (T)0; });
+  __syncthreads();
+  const Body body(A.P);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  double ev[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  double d2max = 0.0;
+  for (int ic = wid; ic < tt.nic; ic += nw) {
+    const int t = interior_tile_cell(tt, ic);
+    const int s_lo = tt.start[t], c = tt.cnt[t], g_lo = tt.gstart[t];
+    const int tx = t % tt.tc[0], ty = (t / tt.tc[0]) % tt.tc[1], tz = t / (tt.tc[0] * tt.tc[1]);
+    for (int r0 = 0; r0 < c; r0 += 32) {
+      const bool act = r0 + lane < c;
+      const int a = act ? s_lo + r0 + lane : s_lo;
+      const int gi = g_lo + r0 + lane;
+      const T xi = xs[a], yi = ys[a], zi = zs[a], wi = ws[a];
+      double tot[NT];
+#pragma unroll
+      for (int k = 0; k < NT; ++k) tot[k] = 0.0;
+      for (int dz = -1; dz <= 1; ++dz)
+        for (int dy = -1; dy <= 1; ++dy)
+          for (int dx = -1; dx <= 1; ++dx) {
+            const int t2 = ((tz + dz) * tt.tc[1] + (ty + dy)) * tt.tc[0] + (tx + dx);
+            const int s0 = tt.start[t2], c2 = tt.cnt[t2];
+            const int aself = t2 == t ? a : -1;
+            T p[NT];
+#pragma unroll
+            for (int k = 0; k < NT; ++k) p[k] = (T)0;
+            for (int q = 0; q < (c2 + 3) >> 2; ++q) {
+              const int j0 = s0 + 4 * q;
+              const V4 X = *reinterpret_cast<const V4*>(xs + j0), Y = *reinterpret_cast<const V4*>(ys + j0);
+              const V4 Z = *reinterpret_cast<const V4*>(zs + j0), W = *reinterpret_cast<const V4*>(ws + j0);
+              const T xx[4] = {X.x, X.y, X.z, X.w}, yy[4] = {Y.x, Y.y, Y.z, Y.w}, zz[4] = {Z.x, Z.y, Z.z, Z.w};
+              const T wj[4] = {W.x, W.y, W.z, W.w};
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const T ex = xi - xx[u], ey = yi - yy[u], ez = zi - zz[u];
+                const T r2 = ex * ex + ey * ey + ez * ez;
+                body.pair(ex, ey, ez, r2, wi + wj[u], j0 + u != aself, p);
+              }
+            }
+#pragma unroll
+            for (int k = 0; k < NT; ++k) tot[k] += (double)p[k];
+          }
+      if (act) {
+        if constexpr (MODE == 0) {
+          const double t3[3] = {tot[0], tot[1], tot[2]};
+          d2max = fmax(d2max, atom_epilogue(A, gi, t3));
+          if constexpr (EV)
+#pragma unroll
+            for (int k = 0; k < 7; ++k) ev[k] += 0.5 * tot[3 + k];
+        } else {
+          const double rho = tot[0];
+          const double sq = sqrt(rho);
+          A.rho[gi] = rho;
+          A.fp_out[gi] = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;
+          if constexpr (EV) ev[0] += -A.P.B * sq;
+        }
+      }
+    }
+  }
+  if constexpr (EV) {
+    block_sum<8>(ev, red);
+    if (threadIdx.x == 0)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) A.ev_partials[(size_t)tileid * 8 + k] = ev[k];
+  }
+  if constexpr (MODE == 0) {
+    if (A.epi == EPI_KICK_DRIFT) block_max_to_flag(d2max, red, &A.flags->max_disp2_bits[1 - A.parity]);
+    if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
   }
 }
 
@@ -783,12 +1070,15 @@ __global__ void k_reduce_ev(int ntiles, const double* __restrict__ partials, dou
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a8 + a4: velocity Verlet and the device-side displacement test
+// a8 + a4 unfused: velocity Verlet and the device-side displacement test.  Used for
+// the first half step of every md_run and by the half-list path (whose forces are complete only when
+// the scatter kernel has finished).
 // ---------------------------------------------------------------------------------------------------
 // v += dtf f ; x += dt v ; flag = max |x - x0|^2
 __global__ void k_initial_integrate(int N, size_t ld, double* __restrict__ x, double* __restrict__ v, const double* __restrict__ f,
                                     const double* __restrict__ x0, const int* __restrict__ type, const double* __restrict__ mass,
-                                    double dt, double half_dt_ftm2v, Flags* flags) {
+                                    double dt, double half_dt_ftm2v, unsigned long long* flag) {
+  __shared__ double red[32];
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   double d2 = 0.0;
   if (n < N) {
@@ -803,16 +1093,7 @@ __global__ void k_initial_integrate(int N, size_t ld, double* __restrict__ x, do
       d2 += dd * dd;
     }
   }
-  for (int o = 16; o > 0; o >>= 1) d2 = fmax(d2, __shfl_xor_sync(0xffffffffu, d2, o));
-  __shared__ double wmax[32];
-  int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  if (lane == 0) wmax[wid] = d2;
-  __syncthreads();
-  if (wid == 0) {
-    d2 = lane < (blockDim.x >> 5) ? wmax[lane] : 0.0;
-    for (int o = 16; o > 0; o >>= 1) d2 = fmax(d2, __shfl_xor_sync(0xffffffffu, d2, o));
-    if (lane == 0 && d2 > 0.0) atomicMax(&flags->max_disp2_bits, (unsigned long long)__double_as_longlong(d2));
-  }
+  block_max_to_flag(d2, red, flag);
 }
 
 __global__ void k_final_integrate(int N, size_t ld, double* __restrict__ v, const double* __restrict__ f,

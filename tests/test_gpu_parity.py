@@ -313,7 +313,7 @@ def test_error_paths():
     with pytest.raises(md.MDError):
         md.System(np.array([1.0, -1.0, 1.0]), 4, np.zeros(4, np.int32), np.array([1.0]))
     with pytest.raises(md.MDError):
-        md.System(box, 0, np.zeros(1, np.int32), np.array([1.0]))
+        md.System(box, 0, np.zeros(0, np.int32), np.array([1.0]))
 
 
 def test_sparse_gas_empty_cells_and_zero_steps():
