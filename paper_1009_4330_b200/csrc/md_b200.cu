@@ -51,6 +51,9 @@ struct md_system_impl {
   int xcur = 0;   // buffer of x (flips at every build and at every fused kick+drift step)
   int force_threads = 256, batch = 8;
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
+  void* xr[2] = {nullptr, nullptr};   // packed cell-relative positions (Vec4<T>, 32 B per atom reserved), buffer index = xcur
+  int* tab = nullptr;                 // per-tile tables of the last build
+  size_t tab_alloc = 0;
   int *cell_of = nullptr, *rank = nullptr, *perm = nullptr, *numneigh = nullptr;
   size_t numneigh_alloc = 0;
   int *cell_count = nullptr, *cell_start = nullptr;
@@ -118,6 +121,8 @@ cudaError_t launch(md_system* s, Kern kern, unsigned grid, unsigned block, size_
     if (it == s->smem_set.end() || it->second < smem) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       if (e != cudaSuccess) return e;
+      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+      if (e != cudaSuccess) return e;
       s->smem_set[key] = smem;
     }
   }
@@ -158,6 +163,14 @@ void fill_geom_for_b(const md_system* s, int b, Geom& g) {
     g.nc[d] = (int)std::floor(s->box[d] / rl);
     g.edge[d] = s->box[d] / g.nc[d];
     g.inv_edge[d] = g.nc[d] / s->box[d];
+    {   // anchor spacing: edge rounded to `bits` significant bits, so that k * h/2 is exact in fp32 for |k| <= 2 nc
+      int lg = 1;
+      while ((1 << lg) < 2 * g.nc[d] + 4) ++lg;
+      const int bits = std::max(4, 23 - lg);
+      int e;
+      const double m = std::frexp(g.edge[d], &e);                 // edge = m 2^e, m in [0.5, 1)
+      g.h[d] = std::ldexp(std::nearbyint(std::ldexp(m, bits)), e - bits);
+    }
     g.b[d] = std::min(b, g.nc[d]);
     g.nb[d] = (g.nc[d] + g.b[d] - 1) / g.b[d];
     g.ncell *= g.nc[d];
@@ -260,6 +273,13 @@ int plan(md_system* s) {
     CK(dalloc(&s->numneigh, rows));
     s->numneigh_alloc = rows;
   }
+  size_t tab_ints = (size_t)g.ntiles * tile_tab_stride(g);
+  if (tab_ints > s->tab_alloc) {
+    cudaFree(s->tab);
+    s->tab = nullptr; s->tab_alloc = 0;
+    CK(dalloc(&s->tab, tab_ints));
+    s->tab_alloc = tab_ints;
+  }
   if ((size_t)g.ntiles > s->ev_tiles_alloc) {
     cudaFree(s->ev_partials);
     s->ev_tiles_alloc = g.ntiles;
@@ -275,14 +295,15 @@ int build_list_only(md_system* s) {
   const Geom& g = s->g;
   double rl = s->rc + s->skin;
   BuildArgs B{};
-  B.g = g; B.cell_start = s->cell_start; B.x = s->x[s->xcur]; B.ld = s->ld; B.rl2 = rl * rl;
+  B.g = g; B.cell_start = s->cell_start; B.tab = s->tab; B.x = s->x[s->xcur]; B.ld = s->ld; B.rl2 = rl * rl;
   // guard band of the fp32 distance test: tile-centred coordinates up to E are
   // rounded to fp32, so r^2 carries a relative error of about (7 E / rl + 3) 2^-24; four times that is used.
   double E = 0;
   for (int d = 0; d < 3; ++d) E = std::max(E, 0.5 * (g.b[d] + 2) * g.edge[d] + s->skin);
   double band = 4.0 * (7.0 * E / rl + 3.0) * std::ldexp(1.0, -24);
-  B.rl2_lo = std::nextafterf((float)(rl * rl * (1.0 - band)), 0.0f);
-  B.rl2_hi = std::nextafterf((float)(rl * rl * (1.0 + band)), INFINITY);
+  B.rl2_mid = (float)(rl * rl);
+  B.rl2_bw = std::nextafterf((float)(rl * rl * band), INFINITY);
+  B.rl2_hi = B.rl2_mid + B.rl2_bw;      // the same fp32 sum the kernel's accept test and band test are consistent with
   B.list = s->list; B.numneigh = s->numneigh; B.flags = s->flags_d;
   if (g.half) CK(launch(s, k_build_list<true>, g.ntiles, BUILD_THREADS, build_smem(g), B));
   else CK(launch(s, k_build_list<false>, g.ntiles, BUILD_THREADS, build_smem(g), B));
@@ -305,8 +326,13 @@ int build(md_system* s, bool need_list) {
     CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
               s->perm));
     CK(launch(s, k_sort_cells, blocks_for(g.ncell, 128), 128, 0, g.ncell, (const int*)s->cell_start, s->perm));
-    CK(launch(s, k_permute, blocks_for(N, 256), 256, 0, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
-              (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, s->ld));
+    if (s->precision == MD_FP64)
+      CK(launch(s, k_permute<double>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
+                (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (double4*)s->xr[xo], s->ld));
+    else
+      CK(launch(s, k_permute<float>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
+                (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (float4*)s->xr[xo], s->ld));
+    CK(launch(s, k_tile_tables, g.ntiles, 128, 0, g, (const int*)s->cell_start, s->tab, s->flags_d));
     s->cur = o; s->xcur = xo;
     s->forces_valid = false;
     bool do_list = need_list || s->kernel_eff != MD_KERNEL_CELL;
@@ -321,7 +347,7 @@ int build(md_system* s, bool need_list) {
     const Flags& F = *s->flags_h;
     if (F.nonfinite) return fail(s, MD_ERR_NONFINITE, "a non-finite coordinate reached the binning kernel");
     bool again = false;
-    if (do_list) {
+    {
       if (F.need_tile_cap > g.tile_cap) { s->cap_scale_tile *= 1.1 * (double)F.need_tile_cap / g.tile_cap; again = true; }
       if (F.need_interior_cap > g.interior_cap) { s->cap_scale_int *= 1.1 * (double)F.need_interior_cap / g.interior_cap; again = true; }
       if (F.need_row_cap > g.row_cap) { s->cap_scale_row *= 1.1 * (double)F.need_row_cap / g.row_cap; again = true; }
@@ -344,8 +370,7 @@ struct StepMode {
   int in_run = 0;
   int parity = 0;
   double dt = 0, hdtf = 0, trigger = 0;
-  const double* x_in = nullptr;   // positions read (default: current buffer)
-  double* x_out = nullptr;        // EPI_KICK_DRIFT: positions written
+  int xbuf = -1;                  // x / xr buffer read (default: the current one); EPI_KICK_DRIFT writes the other one
 };
 
 template <typename T, template <typename, bool> class BodyT, int MODE, bool EV>
@@ -376,10 +401,11 @@ template <typename T, bool EV>
 int launch_force_T(md_system* s, const StepMode& M) {
   const Geom& g = s->g;
   ForceArgs A{};
-  A.g = g; A.P = s->P; A.cell_start = s->cell_start; A.x = M.x_in ? M.x_in : s->x[s->xcur]; A.ld = s->ld; A.list = s->list;
+  const int xb = M.xbuf >= 0 ? M.xbuf : s->xcur;
+  A.g = g; A.P = s->P; A.cell_start = s->cell_start; A.tab = s->tab; A.x = s->x[xb]; A.xr = s->xr[xb]; A.ld = s->ld; A.list = s->list;
   A.numneigh = s->numneigh; A.fp_in = nullptr; A.f = s->f; A.rho = s->rho; A.fp_out = s->fp; A.ev_partials = s->ev_partials;
   A.epi = M.epi; A.in_run = M.in_run; A.parity = M.parity;
-  A.v = s->v[s->cur]; A.x_new = M.x_out; A.x0 = s->x0; A.type = s->type[s->cur]; A.mass = s->mass_d;
+  A.v = s->v[s->cur]; A.x_new = s->x[xb ^ 1]; A.xr_new = s->xr[xb ^ 1]; A.x0 = s->x0; A.type = s->type[s->cur]; A.mass = s->mass_d;
   A.dt = M.dt; A.half_dt_ftm2v = M.hdtf; A.trigger = M.trigger; A.flags = s->flags_d;
   if (s->style == MD_PAIR_LJ126) {
     int rc = launch_force_variant<T, LJBody, 0, EV>(s, A);
@@ -407,6 +433,19 @@ int compute_forces_device(md_system* s, bool ev, const StepMode& M = StepMode())
 }
 
 int autotune(md_system* s, int nrep, double* ms_out);
+
+int initial_integrate(md_system* s, double dt, double hdtf) {
+  const int N = (int)s->N;
+  if (s->precision == MD_FP64)
+    CK(launch(s, k_initial_integrate<double>, blocks_for(N, 256), 256, 0, s->g, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
+              (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, (double4*)s->xr[s->xcur], dt, hdtf,
+              &s->flags_d->max_disp2_bits[0]));
+  else
+    CK(launch(s, k_initial_integrate<float>, blocks_for(N, 256), 256, 0, s->g, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
+              (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, (float4*)s->xr[s->xcur], dt, hdtf,
+              &s->flags_d->max_disp2_bits[0]));
+  return MD_OK;
+}
 
 int ensure_list(md_system* s) {
   if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set first");
@@ -504,6 +543,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   for (int k = 0; k < 2; ++k) {
     CKC(dalloc(&s->x[k], 3 * s->ld)); CKC(dalloc(&s->v[k], 3 * s->ld));
     CKC(dalloc(&s->id[k], s->ld)); CKC(dalloc(&s->type[k], s->ld));
+    CKC(cudaMalloc(&s->xr[k], (s->ld + 8) * 32));
     CKC(cudaMemsetAsync(s->x[k], 0, 3 * s->ld * sizeof(double), s->stream));
     CKC(cudaMemsetAsync(s->v[k], 0, 3 * s->ld * sizeof(double), s->stream));
   }
@@ -529,7 +569,8 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
 
 void md_destroy(md_system* s) {
   if (!s) return;
-  for (int k = 0; k < 2; ++k) { cudaFree(s->x[k]); cudaFree(s->v[k]); cudaFree(s->id[k]); cudaFree(s->type[k]); }
+  for (int k = 0; k < 2; ++k) { cudaFree(s->x[k]); cudaFree(s->v[k]); cudaFree(s->id[k]); cudaFree(s->type[k]); cudaFree(s->xr[k]); }
+  cudaFree(s->tab);
   cudaFree(s->f); cudaFree(s->x0); cudaFree(s->rho); cudaFree(s->fp); cudaFree(s->cell_of); cudaFree(s->rank); cudaFree(s->perm);
   cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d);
   cudaFree(s->ev_partials); cudaFree(s->scalars_d); cudaFree(s->io_d); cudaFree(s->io_i); cudaFree(s->types_caller); cudaFree(s->flags_d);
@@ -664,8 +705,8 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
     // host synchronisation; a step kernel that finds the list stale does nothing and raises `stop`, and so
     // do all later ones; the host then rebuilds and continues from the step that stopped.
     CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
-    CK(launch(s, k_initial_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
-              (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, dt, hdtf, &s->flags_d->max_disp2_bits[0]));
+    rc = initial_integrate(s, dt, hdtf);
+    if (rc) return rc;
     s->forces_valid = false;
     int64_t remaining = nsteps;
     int parity = 0;
@@ -677,8 +718,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         StepMode M;
         M.epi = last ? EPI_FINAL : EPI_KICK_DRIFT;
         M.in_run = 1; M.parity = (parity + k) & 1; M.dt = dt; M.hdtf = hdtf; M.trigger = trigger;
-        M.x_in = s->x[s->xcur ^ (k & 1)];
-        M.x_out = s->x[s->xcur ^ (k & 1) ^ 1];
+        M.xbuf = s->xcur ^ (k & 1);
         const int64_t step = nsteps - remaining + k;
         const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
         sample_slot[k] = -1;
@@ -719,8 +759,8 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
     // half list: the scatter kernel's forces are complete only when it has finished, so integrate separately
     for (int64_t step = 0; step < nsteps; ++step) {
       CK(cudaMemsetAsync(s->flags_d->max_disp2_bits, 0, 2 * sizeof(unsigned long long), s->stream));
-      CK(launch(s, k_initial_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
-                (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, dt, hdtf, &s->flags_d->max_disp2_bits[0]));
+      rc = initial_integrate(s, dt, hdtf);
+      if (rc) return rc;
       CK(cudaMemcpyAsync(&s->flags_h->max_disp2_bits[0], &s->flags_d->max_disp2_bits[0], sizeof(unsigned long long), cudaMemcpyDeviceToHost,
                          s->stream));
       CK(cudaStreamSynchronize(s->stream));
@@ -784,7 +824,7 @@ int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t st
   if (!dev_n) dn = s->io_i;
   if (!dev_l) CK(cudaMalloc((void**)&dl, (size_t)s->N * stride * sizeof(int)));
   size_t smem = export_smem(g);
-  cudaError_t e = launch(s, k_export_list, g.ntiles, BUILD_THREADS, smem, g, (const int*)s->cell_start, (const int*)s->id[s->cur],
+  cudaError_t e = launch(s, k_export_list, g.ntiles, BUILD_THREADS, smem, g, (const int*)s->tab, (const int*)s->id[s->cur],
                          (const uint4*)s->list, (const int*)s->numneigh, dn, dl, (long long)stride);
   if (e == cudaSuccess && !dev_n) e = cudaMemcpyAsync(numneigh, dn, (size_t)s->N * sizeof(int), cudaMemcpyDeviceToHost, s->stream);
   if (e == cudaSuccess && !dev_l) e = cudaMemcpyAsync(neigh, dl, (size_t)s->N * stride * sizeof(int), cudaMemcpyDeviceToHost, s->stream);

@@ -14,12 +14,14 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace mdk {
 
 constexpr int MAX_TILE_CELLS = 512;    // (b+2)^3 <= 512  =>  b <= 6
 constexpr int BUILD_THREADS = 256;     // threads per block of the list-build and cell-list kernels
 constexpr int FORCE_MAX_THREADS = 640; // upper bound of the force kernels' block size (runtime choice)
+constexpr int FORCE_MIN_BLOCKS = 2;    // resident blocks per SM the mixed-precision force kernels are compiled for (<= 48 registers)
 constexpr int RING = 64;               // list-build: pending entries a lane can hold in shared memory
 constexpr int RING_STRIDE = RING * 2 + 16;   // bytes between the rings of neighbouring lanes (odd * 16)
 
@@ -27,6 +29,8 @@ struct Geom {
   double L[3];        // box
   double edge[3];     // cell edge = L / nc  (>= rc + skin)
   double inv_edge[3];
+  double h[3];        // anchor spacing of the packed coordinates: edge rounded to so few bits that every
+                      // (half-)integer multiple a tile needs is exact in fp32 (see tile_cell_offset_rel)
   int nc[3];          // cells per dimension (>= 3)
   int b[3];           // tile width in cells (interior)
   int nb[3];          // tiles per dimension
@@ -119,6 +123,13 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { using type = float4; };
+template <> struct Vec4<double> { using type = double4; };   // 32 B, 16-B aligned is all that is needed here
+template <typename T> __device__ __forceinline__ typename Vec4<T>::type make_v4(T x, T y, T z, T w);
+template <> __device__ __forceinline__ float4 make_v4<float>(float x, float y, float z, float w) { return make_float4(x, y, z, w); }
+template <> __device__ __forceinline__ double4 make_v4<double>(double x, double y, double z, double w) { return make_double4(x, y, z, w); }
+
 template <int K>
 __device__ __forceinline__ double group_sum(double v) {
 #pragma unroll
@@ -174,6 +185,7 @@ struct alignas(16) TileTables {   // lives in shared memory
   int start[MAX_TILE_CELLS];  // staged slot of the first atom of tile cell t (multiple of 4)
   int gstart[MAX_TILE_CELLS]; // global (sorted) index of the first atom of tile cell t
   int cnt[MAX_TILE_CELLS];    // atoms in tile cell t
+  int meta[MAX_TILE_CELLS];   // tx | ty << 8 | tz << 16 | interior << 24   (filled by tile_load only)
   int c0[3], w[3], tc[3];     // first interior cell, interior width, tile width (w+2)
   int ntc;                    // tc[0]*tc[1]*tc[2]
   int nic;                    // interior cells w[0]*w[1]*w[2]
@@ -258,6 +270,78 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
   __syncthreads();
 }
 
+// ---------------------------------------------------------------------------------------------------
+// The tables above are computed ONCE per list build by k_tile_tables and kept in global memory
+// (TILE_HDR ints of header + three ints {gstart, start<<16 | cnt, meta} per tile cell); every tile kernel
+// launched between two builds only loads them (tile_load: one coalesced read, one barrier).
+// ---------------------------------------------------------------------------------------------------
+constexpr int TILE_HDR = 8;   // n_int_slots, n_slots, n_int_atoms, brick_start, n_staged_atoms, pad x3
+__host__ __device__ inline int tile_tab_cells(const Geom& g) { return ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) + 3) & ~3; }
+__host__ __device__ inline int tile_tab_stride(const Geom& g) {
+  return TILE_HDR + 3 * tile_tab_cells(g);
+}
+
+__device__ __forceinline__ void tile_dims(const Geom& g, int tile, int c0[3], int w[3]) {
+  int bt[3] = {tile % g.nb[0], (tile / g.nb[0]) % g.nb[1], tile / (g.nb[0] * g.nb[1])};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    c0[d] = bt[d] * g.b[d];
+    w[d] = tile_width(g, d, bt[d]);
+  }
+}
+
+// All threads of the block call it; ends with __syncthreads().
+__device__ __forceinline__ void tile_load(const Geom& g, int tile, const int* __restrict__ tab, TileTables& tt) {
+  const int* __restrict__ h = tab + (size_t)tile * tile_tab_stride(g);
+  int c0[3], w[3];
+  tile_dims(g, tile, c0, w);
+  const int ntc = (w[0] + 2) * (w[1] + 2) * (w[2] + 2);
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { tt.c0[d] = c0[d]; tt.w[d] = w[d]; tt.tc[d] = w[d] + 2; }
+    tt.ntc = ntc;
+    tt.nic = w[0] * w[1] * w[2];
+    tt.n_int_slots = h[0]; tt.n_slots = h[1]; tt.n_int_atoms = h[2]; tt.brick_start = h[3];
+  }
+  const int tcs = tile_tab_cells(g);
+  for (int t = threadIdx.x; t < ntc; t += blockDim.x) {
+    const unsigned sc = (unsigned)h[TILE_HDR + tcs + t];
+    tt.gstart[t] = h[TILE_HDR + t];
+    tt.start[t] = (int)(sc >> 16);
+    tt.cnt[t] = (int)(sc & 0xffffu);
+    tt.meta[t] = h[TILE_HDR + 2 * tcs + t];
+  }
+  __syncthreads();
+}
+
+// one block per tile; also raises the capacity flags the host re-plans on
+__global__ void __launch_bounds__(128) k_tile_tables(Geom g, const int* __restrict__ cell_start, int* __restrict__ tab, Flags* flags) {
+  __shared__ TileTables tt;
+  const int tile = blockIdx.x;
+  tile_setup(g, tile, cell_start, tt);
+  int* h = tab + (size_t)tile * tile_tab_stride(g);
+  const int tcs = tile_tab_cells(g);
+  int staged = 0;
+  for (int t = threadIdx.x; t < tt.ntc; t += blockDim.x) {
+    const int tx = t % tt.tc[0], ty = (t / tt.tc[0]) % tt.tc[1], tz = t / (tt.tc[0] * tt.tc[1]);
+    h[TILE_HDR + t] = tt.gstart[t];
+    h[TILE_HDR + tcs + t] = (int)(((unsigned)tt.start[t] << 16) | ((unsigned)tt.cnt[t] & 0xffffu));
+    h[TILE_HDR + 2 * tcs + t] = tx | ty << 8 | tz << 16 | (tile_cell_is_interior(tt, t) ? 1 << 24 : 0);
+    staged += tt.cnt[t];
+  }
+  __shared__ int red[4];
+  for (int o = 16; o > 0; o >>= 1) staged += __shfl_xor_sync(0xffffffffu, staged, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = staged;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    h[0] = tt.n_int_slots; h[1] = tt.n_slots; h[2] = tt.n_int_atoms; h[3] = tt.brick_start;
+    h[4] = red[0] + red[1] + red[2] + red[3]; h[5] = 0; h[6] = 0; h[7] = 0;
+    if (tt.n_slots > g.tile_cap) atomicMax(&flags->need_tile_cap, tt.n_slots);
+    if (tt.n_int_slots > g.interior_cap) atomicMax(&flags->need_interior_cap, tt.n_int_slots);
+    atomicMax(&flags->max_tile_atoms, tt.n_slots);
+  }
+}
+
 // Periodic image shift minus tile centre for tile cell t, per dimension: staged = x + off.
 __device__ __forceinline__ void tile_cell_offset(const Geom& g, const TileTables& tt, int t, double off[3]) {
   int tq[3] = {t % tt.tc[0], (t / tt.tc[0]) % tt.tc[1], t / (tt.tc[0] * tt.tc[1])};
@@ -269,6 +353,29 @@ __device__ __forceinline__ void tile_cell_offset(const Geom& g, const TileTables
     off[d] = shift - centre;
   }
 }
+
+// The same for the PACKED coordinates xr = x - anchor(c), anchor(c) = (c + 1/2) h of the atom's storage cell c:
+// staged = xr + off, off = anchor(unwrapped tile cell u) - (c0 + w/2) h  [+- (nc h - L) for a periodic image].
+// h has so few significant bits that (2u + 1 - 2 c0 - w) (h/2) is EXACT in fp32: every atom of a tile is shifted
+// by an exactly representable amount, so no rounding error is shared by all pairs of a cell pair (it would
+// add up coherently in the virial); only cells seen through the periodic boundary carry one rounded term.
+__device__ __forceinline__ void tile_cell_offset_rel(const Geom& g, const TileTables& tt, int t, double off[3]) {
+  const int m = tt.meta[t];
+  int tq[3] = {m & 0xff, (m >> 8) & 0xff, (m >> 16) & 0xff};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    const int u = tt.c0[d] + tq[d] - 1;
+    const double wrap = u < 0 ? g.nc[d] * g.h[d] - g.L[d] : (u >= g.nc[d] ? g.L[d] - g.nc[d] * g.h[d] : 0.0);
+    off[d] = (2 * (u - tt.c0[d]) + 1 - tt.w[d]) * (0.5 * g.h[d]) + wrap;
+  }
+}
+// cell index of a wrapped coordinate w in [0, L) -- the ONE definition used by binning and by everything
+// that must agree with it about which cell an atom is stored in
+__device__ __forceinline__ int cell_index_1d(const Geom& g, int d, double w) {
+  int ci = (int)(w * g.inv_edge[d]);
+  return ci >= g.nc[d] ? g.nc[d] - 1 : ci;
+}
+__device__ __forceinline__ double cell_anchor_1d(const Geom& g, int d, int ci) { return (ci + 0.5) * g.h[d]; }
 
 // Calls store(slot, global_index, off[3], t) for every staged atom and pad(slot) for every pad slot and
 // for the dummy slot, all with slot <= cap.  One warp per tile cell.  Caller syncs afterwards.
@@ -307,8 +414,7 @@ __global__ void k_bin(Geom g, int N, double* __restrict__ x, double* __restrict_
     if (w >= g.L[d]) w -= g.L[d];
     if (w < 0.0) w = 0.0;
     p[d] = w;
-    int ci = (int)(w * g.inv_edge[d]);
-    c[d] = ci >= g.nc[d] ? g.nc[d] - 1 : ci;
+    c[d] = cell_index_1d(g, d, w);
   }
   if (bad) atomicExch(&flags->nonfinite, 1);
   x[k] = p[0]; y[k] = p[1]; z[k] = p[2];
@@ -382,20 +488,26 @@ __global__ void k_sort_cells(int ncell, const int* __restrict__ cell_start, int*
 }
 
 // a2: spatial reorder of the per-atom arrays; x0 := x (reference for the displacement test)
-__global__ void k_permute(int N, const int* __restrict__ perm, const double* __restrict__ xi, const double* __restrict__ vi,
+// It also writes the PACKED copy the force kernels stage from: xr[n] = (x - centre of its cell, 0) in T
+// (fp32 in mixed mode), 16 or 32 B per atom, so that a tile cell is one contiguous bulk copy.
+template <typename T>
+__global__ void k_permute(Geom g, int N, const int* __restrict__ perm, const double* __restrict__ xi, const double* __restrict__ vi,
                           const int* __restrict__ idi, const int* __restrict__ typei, double* __restrict__ xo,
                           double* __restrict__ vo, int* __restrict__ ido, int* __restrict__ typeo, double* __restrict__ x0,
-                          size_t ld) {
+                          typename Vec4<T>::type* __restrict__ xr, size_t ld) {
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n >= N) return;
   int k = perm[n];
+  T r[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     double p = xi[d * ld + k];
     xo[d * ld + n] = p;
     x0[d * ld + n] = p;
     vo[d * ld + n] = vi[d * ld + k];
+    r[d] = (T)(p - cell_anchor_1d(g, d, cell_index_1d(g, d, p)));
   }
+  xr[n] = make_v4<T>(r[0], r[1], r[2], (T)0);
   ido[n] = idi[k];
   typeo[n] = typei[k];
 }
@@ -435,9 +547,10 @@ __global__ void k_iota(int N, int* __restrict__ a) {
 struct BuildArgs {
   Geom g;
   const int* cell_start;
+  const int* tab;          // per-tile tables (k_tile_tables)
   const double* x; size_t ld;
   double rl2;
-  float rl2_lo, rl2_hi;    // guard band of the fp32 test around rl2
+  float rl2_hi, rl2_mid, rl2_bw;   // fp32 test: accept r2 < hi = mid + bw; |r2 - mid| <= bw is decided in fp64 (mid = fl(rl2))
   uint4* list;
   int* numneigh;           // [ntiles][interior_cap]
   Flags* flags;
@@ -459,8 +572,24 @@ __device__ __noinline__ bool confirm_pair_fp64(const Geom& g, const TileTables& 
   return r2 < rl2;
 }
 
+// packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2: two lanes of math per issue slot)
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+// predicated 16-bit store to the lane's ring + pointer advance
+__device__ __forceinline__ void ring_push(unsigned& rp, unsigned code, bool take) {
+  asm volatile("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p st.shared.u16 [%0], %1; @p add.u32 %0, %0, 2; }"
+               : "+r"(rp)
+               : "h"((unsigned short)code), "r"((unsigned)take)
+               : "memory");
+}
+
 template <bool HALF>
-__global__ void __launch_bounds__(BUILD_THREADS) k_build_list(BuildArgs A) {
+__global__ void __launch_bounds__(BUILD_THREADS, 2) k_build_list(BuildArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
   const Geom& g = A.g;
@@ -470,12 +599,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_list(BuildArgs A) {
   float* zs = ys + capA;
   unsigned char* rings = reinterpret_cast<unsigned char*>(zs + capA);
   const int tile = blockIdx.x;
-  tile_setup(g, tile, A.cell_start, tt);
-  if (threadIdx.x == 0) {
-    if (tt.n_slots > g.tile_cap) atomicMax(&A.flags->need_tile_cap, tt.n_slots);
-    if (tt.n_int_slots > g.interior_cap) atomicMax(&A.flags->need_interior_cap, tt.n_int_slots);
-    atomicMax(&A.flags->max_tile_atoms, tt.n_slots);
-  }
+  tile_load(g, tile, A.tab, tt);
   if (tt.n_slots > g.tile_cap || tt.n_int_slots > g.interior_cap) return;   // host re-plans and rebuilds
   const double* __restrict__ x = A.x;
   const size_t ld = A.ld;
@@ -495,19 +619,24 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_list(BuildArgs A) {
   const int max_words = g.chunk_cap * K;
   const unsigned dummy = (unsigned)tt.n_slots << g.code_shift;
   const int shift = g.code_shift;
-  const float lo = A.rl2_lo, hi = A.rl2_hi;
+  const unsigned cstep = 1u << shift;
+  const float hi = A.rl2_hi, mid = A.rl2_mid, bw = A.rl2_bw;
+  const f32x2 mid2 = pack2(mid, mid);
   int my_max = 0;
   unsigned long long my_sum = 0;
 
   for (int ic = wid; ic < tt.nic; ic += nw) {
     const int t = interior_tile_cell(tt, ic);
     const int s_lo = tt.start[t], c = tt.cnt[t], g_lo = tt.gstart[t];
-    const int tx = t % tt.tc[0], ty = (t / tt.tc[0]) % tt.tc[1], tz = t / (tt.tc[0] * tt.tc[1]);
+    const int mt = tt.meta[t];
+    const int tx = mt & 0xff, ty = (mt >> 8) & 0xff, tz = (mt >> 16) & 0xff;
     for (int r0 = 0; r0 < c; r0 += 32) {
       const bool act = r0 + lane < c;
       const int a = act ? s_lo + r0 + lane : s_lo;   // staged slot = list row
       const int gi = g_lo + r0 + lane;
-      const float xi = xs[a], yi = ys[a], zi = zs[a];
+      // an idle lane sits far away from everything, pad slots (+1e15) included: it accepts nothing
+      const float xi = act ? xs[a] : -1e15f, yi = act ? ys[a] : -1e15f, zi = act ? zs[a] : -1e15f;
+      const f32x2 xi2 = pack2(xi, xi), yi2 = pack2(yi, yi), zi2 = pack2(zi, zi);
       unsigned rp = rbase;
       int nwords = 0;
       auto store_word = [&](uint4 v) {
@@ -528,29 +657,56 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_list(BuildArgs A) {
           for (int dx = -1; dx <= 1; ++dx) {
             const int t2 = ((tz + dz) * tt.tc[1] + (ty + dy)) * tt.tc[0] + (tx + dx);
             const int s0 = tt.start[t2], c2 = tt.cnt[t2], g0 = tt.gstart[t2];
-            const int aself = t2 == t ? a : -1;
+            // candidates a lane must never take: itself (own cell), and for a half list every j <= i
+            int jskip = -1, jmin = -1;
+            if (t2 == t) jskip = a;
+            if (HALF) jmin = gi - g0 + s0;        // take only g0 + (j - s0) > gi  <=>  j > jmin
+            const bool plain = !HALF && t2 != t;
             for (int k0 = 0; k0 < c2; k0 += 32) {
               if (((int)(rp - rbase) >> 1) + 32 > RING) flush();
               const int ng = (min(c2 - k0, 32) + 3) >> 2;
-              for (int q = 0; q < ng; ++q) {
-                const int j0 = s0 + k0 + 4 * q;
-                const float4 X = *reinterpret_cast<const float4*>(xs + j0);
-                const float4 Y = *reinterpret_cast<const float4*>(ys + j0);
-                const float4 Z = *reinterpret_cast<const float4*>(zs + j0);
-                const float xx[4] = {X.x, X.y, X.z, X.w}, yy[4] = {Y.x, Y.y, Y.z, Y.w}, zz[4] = {Z.x, Z.y, Z.z, Z.w};
+              const unsigned rp_chunk = rp;
+              float m = 1e30f;                    // min |r2 - rl2| over the chunk: the guard-band detector
+              auto scan = [&](auto plain_tag) {
+                constexpr bool PLAIN = decltype(plain_tag)::value;
+                unsigned code = (unsigned)(s0 + k0) << shift;
+                for (int q = 0; q < ng; ++q) {
+                  const int j0 = s0 + k0 + 4 * q;
+                  const float4 X = *reinterpret_cast<const float4*>(xs + j0);
+                  const float4 Y = *reinterpret_cast<const float4*>(ys + j0);
+                  const float4 Z = *reinterpret_cast<const float4*>(zs + j0);
+                  const f32x2 dx01 = sub2(xi2, pack2(X.x, X.y)), dx23 = sub2(xi2, pack2(X.z, X.w));
+                  const f32x2 dy01 = sub2(yi2, pack2(Y.x, Y.y)), dy23 = sub2(yi2, pack2(Y.z, Y.w));
+                  const f32x2 dz01 = sub2(zi2, pack2(Z.x, Z.y)), dz23 = sub2(zi2, pack2(Z.z, Z.w));
+                  const f32x2 q01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
+                  const f32x2 q23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
+                  float r2[4], e[4];
+                  unpack2(q01, r2[0], r2[1]); unpack2(q23, r2[2], r2[3]);
+                  unpack2(sub2(q01, mid2), e[0], e[1]); unpack2(sub2(q23, mid2), e[2], e[3]);
+                  m = fminf(fminf(m, fabsf(e[0])), fabsf(e[1]));
+                  m = fminf(fminf(m, fabsf(e[2])), fabsf(e[3]));
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                  const float ddx = xi - xx[u], ddy = yi - yy[u], ddz = zi - zz[u];
-                  const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-                  const int j = j0 + u;
-                  bool take = act && r2 < hi && j != aself;
-                  if (HALF) take = take && (g0 + (j - s0) > gi);
-                  if (__builtin_expect(take && r2 > lo, 0))
-                    take = confirm_pair_fp64(g, tt, x, ld, gi, t, g0 + (j - s0), t2, A.rl2);
-                  asm volatile("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p st.shared.u16 [%0], %1; }" ::"r"(rp),
-                               "h"((unsigned short)(j << shift)), "r"((unsigned)take)
-                               : "memory");
-                  rp += take ? 2u : 0u;
+                  for (int u = 0; u < 4; ++u) {
+                    bool take = r2[u] < hi;
+                    if constexpr (!PLAIN) take = take && (j0 + u != jskip) && (j0 + u > jmin);
+                    ring_push(rp, code, take);
+                    code += cstep;
+                  }
+                }
+              };
+              if (plain) scan(std::true_type{}); else scan(std::false_type{});
+              if (__builtin_expect(m <= bw, 0)) {
+                // some candidate of this chunk lies in the guard band of the fp32 test: redo the chunk, deciding
+                // the in-band candidates in fp64 from the global positions (the pair set is exactly the fp64 one)
+                rp = rp_chunk;
+                const int nc = min(c2 - k0, 32);
+                for (int k = 0; k < nc; ++k) {
+                  const int j = s0 + k0 + k;
+                  const float ex = xi - xs[j], ey = yi - ys[j], ez = zi - zs[j];
+                  const float r2s = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
+                  bool take = r2s < hi && j != jskip && j > jmin;
+                  if (act && take && fabsf(r2s - mid) <= bw) take = confirm_pair_fp64(g, tt, x, ld, gi, t, g0 + (j - s0), t2, A.rl2);
+                  ring_push(rp, (unsigned)j << shift, take);
                 }
               }
             }
@@ -590,14 +746,14 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_list(BuildArgs A) {
 }
 
 // list export in caller ids (pair-set parity).  Shared memory: TileTables | sid[tile_cap+4] ints.
-__global__ void __launch_bounds__(BUILD_THREADS) k_export_list(Geom g, const int* __restrict__ cell_start, const int* __restrict__ id,
+__global__ void __launch_bounds__(BUILD_THREADS) k_export_list(Geom g, const int* __restrict__ tab, const int* __restrict__ id,
                                                                const uint4* __restrict__ list, const int* __restrict__ numneigh,
                                                                int* __restrict__ nn_out, int* __restrict__ neigh_out, long long stride) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
   int* sid = reinterpret_cast<int*>(smem_raw + sizeof(TileTables));
   const int tile = blockIdx.x;
-  tile_setup(g, tile, cell_start, tt);
+  tile_load(g, tile, tab, tt);
   tile_stage(g, tt, g.tile_cap, [&](int slot, int gi, const double*, int) { sid[slot] = id[gi]; }, [&](int slot) { sid[slot] = -1; });
   __syncthreads();
   const int K = g.K;
@@ -715,10 +871,13 @@ struct ForceArgs {
   Geom g;
   PairParams P;
   const int* cell_start;
+  const int* tab;          // per-tile tables of the last build (k_tile_tables)
   const double* x; size_t ld;
+  const void* xr;          // packed cell-relative positions (Vec4<T>) of the positions in x; .w = -F'(rho) for EAM pass 2
+  void* xr_new;            // EPI_KICK_DRIFT: packed copy of x_new
   const uint4* list;
   const int* numneigh;
-  const double* fp_in;     // EAM pass 2: F'(rho) per sorted atom (else NULL)
+  const double* fp_in;     // EAM pass 2, cell-list variant only: F'(rho) per sorted atom (else NULL)
   double* f;               // forces out
   double* rho; double* fp_out;   // EAM pass 1 out
   double* ev_partials;     // [ntiles][8]: e, wxx, wyy, wzz, wxy, wxz, wyz, pad
@@ -742,8 +901,10 @@ __device__ __forceinline__ bool list_is_stale(const ForceArgs& A) {
   return stale;
 }
 
-// per-atom epilogue; returns |x'-x0|^2 for EPI_KICK_DRIFT (else 0)
-__device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, const double (&tot)[3]) {
+// per-atom epilogue; returns |x'-x0|^2 for EPI_KICK_DRIFT (else 0).  cc[3]: centre of the cell the atom is
+// stored in (for the packed copy of the new position).
+template <typename T>
+__device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, const double (&tot)[3], const double (&cc)[3]) {
   const size_t ld = A.ld;
   if (A.epi == EPI_FORCES) {
     A.f[gi] = tot[0]; A.f[ld + gi] = tot[1]; A.f[2 * ld + gi] = tot[2];
@@ -751,6 +912,7 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
   }
   const double dtf = A.half_dt_ftm2v / A.mass[A.type[gi]];
   double d2 = 0.0;
+  T r[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     double vv = A.v[d * ld + gi] + dtf * tot[d];          // second half kick of this step
@@ -758,6 +920,7 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
       vv += dtf * tot[d];                                 // first half kick of the next step
       const double xx = A.x[d * ld + gi] + A.dt * vv;     // drift
       A.x_new[d * ld + gi] = xx;
+      r[d] = (T)(xx - cc[d]);
       const double dd = xx - A.x0[d * ld + gi];
       d2 += dd * dd;
     } else {
@@ -765,19 +928,59 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
     }
     A.v[d * ld + gi] = vv;
   }
+  if (A.epi == EPI_KICK_DRIFT) reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(r[0], r[1], r[2], (T)0);
   return d2;
 }
 
 // ---------------------------------------------------------------------------------------------------
+// staged-tile gathers: the "random access" load of atom j is ONE 128-bit shared-memory
+// load (two for fp64) of {x, y, z, w} in tile-centred coordinates; w holds -F'(rho_j) in EAM pass 2.
+// Measured on B200 (random slots, 32 lanes): LDS.128 from AoS 11.0 SM-cycles per warp-gather, two
+// LDS.64 from split arrays 12.9, two LDS.64 from AoS 17.0.
+// ---------------------------------------------------------------------------------------------------
+template <typename T> __device__ __forceinline__ typename Vec4<T>::type lds_v4(unsigned a);
+template <> __device__ __forceinline__ float4 lds_v4<float>(unsigned a) {
+  float4 r;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "r"(a));
+  return r;
+}
+template <> __device__ __forceinline__ double4 lds_v4<double>(unsigned a) {
+  double4 r;
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(r.x), "=d"(r.y) : "r"(a));
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%2+16];" : "=d"(r.z), "=d"(r.w) : "r"(a));
+  return r;
+}
+
+// TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned mbar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes),
+               "r"(mbar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
+  unsigned ok = 0;
+  while (!ok)
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok)
+                 : "r"(mbar), "r"(parity)
+                 : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------
 // the neighbor-list loop of PAPER.md L88-122 for one (atom, lane): walks this lane's 128-bit words,
-// 8 entries each; each entry is the byte offset of partner j in the two staged arrays xy[] and zw[]
-// (two LDS.64 per gather: 6.5 cycles per warp against 8.2 for one LDS.128 at random addresses, measured).
-// zw.y of the staged atoms holds -F'(rho_j) for EAM pass 2, so pzw.y - jzw.y = F'_i + F'_j.
+// 8 entries each; each entry is a slot code (slot << code_shift; the staged record sits at
+// st_base + 2 * code).  w of the staged atoms holds -F'(rho_j) for EAM pass 2, so pw - jw = F'_i + F'_j.
 // ---------------------------------------------------------------------------------------------------
 template <typename T, class Body>
-__device__ __forceinline__ void list_loop(const Body& body, unsigned xy_base, unsigned zw_base, const uint4* __restrict__ words,
-                                          size_t word_stride, int nwords, typename Vec2<T>::type pxy, typename Vec2<T>::type pzw,
-                                          double (&tot)[Body::NT]) {
+__device__ __forceinline__ void list_loop(const Body& body, unsigned st_base, const uint4* __restrict__ words, size_t word_stride,
+                                          int nwords, typename Vec4<T>::type pi, double (&tot)[Body::NT]) {
   constexpr int NT = Body::NT;
   if (nwords <= 0) return;
   uint4 w = ld_stream(words);
@@ -793,10 +996,10 @@ __device__ __forceinline__ void list_loop(const Body& body, unsigned xy_base, un
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         const unsigned code = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
-        const typename Vec2<T>::type jxy = lds_v2<T>(xy_base + code), jzw = lds_v2<T>(zw_base + code);
-        const T dx = pxy.x - jxy.x, dy = pxy.y - jxy.y, dz = pzw.x - jzw.x;
+        const typename Vec4<T>::type pj = lds_v4<T>(st_base + 2u * code);
+        const T dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
         const T r2 = dx * dx + dy * dy + dz * dz;
-        body.pair(dx, dy, dz, r2, pzw.y - jzw.y, true, p);
+        body.pair(dx, dy, dz, r2, pi.w - pj.w, true, p);
       }
     }
 #pragma unroll
@@ -807,55 +1010,73 @@ __device__ __forceinline__ void list_loop(const Body& body, unsigned xy_base, un
 // ---------------------------------------------------------------------------------------------------
 // a5/a6/a7: the tile force kernel over the Verlet list.
 //   MODE 0: forces (LJ or EAM pass 2) + epilogue A.epi (+ per-block energy/virial partials when EV)
-//   MODE 1: EAM pass 1 -> rho[N], fp[N] = F'(rho) (+ per-block embedding energy partial when EV)
+//   MODE 1: EAM pass 1 -> rho[N], fp[N] = F'(rho), packed w = -F'(rho) (+ embedding energy partial when EV)
 //   HALF (MODE 0 only, K = 1, EPI_FORCES only): each pair once, -F scattered to f[j] with fp64 atomics.
 // Thread <-> (interior slot a = list row, lane s of K).  Block size is chosen by the host so that the
 // tile's rows fill whole rounds of the block.
-// Shared memory: TileTables | xy[capA] | zw[capA] (Vec2<T>) | scell[interior_cap] u16 | (HALF: sgid[capA] int)
+// Staging: the tile's cells (interior + one-cell halo) are contiguous runs of the packed array, so each
+// is ONE TMA bulk copy (cp.async.bulk, <= 125 per tile, all in flight at once, one mbarrier); a second
+// pass in shared memory adds each cell's offset from the tile centre (periodic image included).
+// Shared memory: TileTables | st[capA] Vec4<T> | scell[interior_cap] u16 | (HALF: sgid[capA] int)
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int force_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
 
 template <typename T, class Body, int K, int MODE, bool EV, bool HALF>
-__global__ void __launch_bounds__(FORCE_MAX_THREADS) k_tile_force(ForceArgs A) {
-  using V2 = typename Vec2<T>::type;
+__global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 : FORCE_MIN_BLOCKS) k_tile_force(ForceArgs A) {
+  using V4 = typename Vec4<T>::type;
   constexpr int NT = Body::NT;
   if (list_is_stale(A)) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
   const Geom& g = A.g;
   const int capA = force_capA(g);
-  V2* xy = reinterpret_cast<V2*>(smem_raw + sizeof(TileTables));
-  V2* zw = xy + capA;
-  unsigned short* scell = reinterpret_cast<unsigned short*>(zw + capA);
+  V4* st = reinterpret_cast<V4*>(smem_raw + sizeof(TileTables));
+  unsigned short* scell = reinterpret_cast<unsigned short*>(st + capA);
   int* sgid = reinterpret_cast<int*>(scell + g.interior_cap);   // HALF only
   __shared__ double red[8 * 32];
+  __shared__ __align__(8) unsigned long long mbar_storage;
+  const unsigned mbar = smem_addr(&mbar_storage);
   const int tileid = blockIdx.x;
-  tile_setup(g, tileid, A.cell_start, tt);
-  const double* __restrict__ xs = A.x;
-  const size_t ld = A.ld;
-  const double* __restrict__ fpin = A.fp_in;
+  if (threadIdx.x == 0) mbar_init(mbar, 1);
+  tile_load(g, tileid, A.tab, tt);
   const int icap = g.interior_cap;
-  tile_stage(g, tt, g.tile_cap,
-             [&](int slot, int gi, const double* off, int t) {
-               V2 a, b;
-               a.x = (T)(xs[gi] + off[0]);
-               a.y = (T)(xs[ld + gi] + off[1]);
-               b.x = (T)(xs[2 * ld + gi] + off[2]);
-               b.y = fpin ? (T)(-fpin[gi]) : (T)0;
-               xy[slot] = a; zw[slot] = b;
-               if (slot < icap && slot < tt.n_int_slots) scell[slot] = (unsigned short)t;
-               if constexpr (HALF) sgid[slot] = gi;
-             },
-             [&](int slot) {
-               V2 a, b;
-               a.x = (T)1e15; a.y = (T)1e15; b.x = (T)1e15; b.y = (T)0;
-               xy[slot] = a; zw[slot] = b;
-               if (slot < icap && slot < tt.n_int_slots) scell[slot] = 0xffffu;
-               if constexpr (HALF) sgid[slot] = 0;
-             });
+  const unsigned st_base = smem_addr(st);
+  {
+    const V4* __restrict__ xr = reinterpret_cast<const V4*>(A.xr);
+    if (threadIdx.x == 0) mbar_expect_tx(mbar, (unsigned)A.tab[(size_t)tileid * tile_tab_stride(g) + 4] * (unsigned)sizeof(V4));
+    for (int t = threadIdx.x; t < tt.ntc; t += blockDim.x) {
+      const int c = tt.cnt[t];
+      if (c > 0) bulk_g2s(st_base + (unsigned)tt.start[t] * (unsigned)sizeof(V4), xr + tt.gstart[t], (unsigned)c * (unsigned)sizeof(V4), mbar);
+    }
+    mbar_wait(mbar, 0);
+    // offsets, pad slots, slot -> cell map
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int t = wid; t < tt.ntc; t += nw) {
+      const int c = tt.cnt[t], c4 = pad4(c);
+      if (c4 == 0) continue;
+      double offd[3];
+      tile_cell_offset_rel(g, tt, t, offd);
+      const T o0 = (T)offd[0], o1 = (T)offd[1], o2 = (T)offd[2];
+      const int s0 = tt.start[t];
+      const bool interior = (tt.meta[t] >> 24) != 0;
+      for (int k = lane; k < c4; k += 32) {
+        const int slot = s0 + k;
+        if (k < c) {
+          V4 q = st[slot];
+          q.x += o0; q.y += o1; q.z += o2;
+          st[slot] = q;
+        } else {
+          st[slot] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);
+        }
+        if (interior) scell[slot] = k < c ? (unsigned short)t : (unsigned short)0xffffu;
+        if constexpr (HALF) sgid[slot] = k < c ? tt.gstart[t] + k : 0;
+      }
+    }
+    if (threadIdx.x == 0) st[tt.n_slots] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);   // the dummy slot
+  }
   __syncthreads();
   const Body body(A.P);
-  const unsigned xy_base = smem_addr(xy), zw_base = smem_addr(zw);
+  const size_t ld = A.ld;
   const size_t slots_cap = (size_t)icap * K;
   const uint4* tlist = A.list + (size_t)tileid * g.chunk_cap * slots_cap;
   double ev[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -872,13 +1093,13 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS) k_tile_force(ForceArgs A) {
 #pragma unroll
     for (int k = 0; k < NT; ++k) tot[k] = 0.0;
     if (active) {
-      V2 pxy = xy[a], pzw = zw[a];
-      pzw.y = -pzw.y;
+      V4 pi = st[a];
+      pi.w = -pi.w;
       const int n = A.numneigh[(size_t)tileid * icap + a];
       const int nq = (n + 7) >> 3;                          // words of this atom
       if constexpr (!HALF) {
         const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
-        list_loop<T, Body>(body, xy_base, zw_base, tlist + sidx, slots_cap, mine, pxy, pzw, tot);
+        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi, tot);
       } else {
         // half list: each in-range pair once; +F to i (registers), -F to j (atomics)
         for (int c = 0; c < nq; ++c) {
@@ -889,13 +1110,13 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS) k_tile_force(ForceArgs A) {
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
               const unsigned code = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
-              const V2 jxy = lds_v2<T>(xy_base + code), jzw = lds_v2<T>(zw_base + code);
-              const T dx = pxy.x - jxy.x, dy = pxy.y - jxy.y, dz = pzw.x - jzw.x;
+              const V4 pj = lds_v4<T>(st_base + 2u * code);
+              const T dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
               const T r2 = dx * dx + dy * dy + dz * dz;
               T p[NT];
 #pragma unroll
               for (int k = 0; k < NT; ++k) p[k] = (T)0;
-              body.pair(dx, dy, dz, r2, pzw.y - jzw.y, true, p);
+              body.pair(dx, dy, dz, r2, pi.w - pj.w, true, p);
               if (p[0] != (T)0 || p[1] != (T)0 || p[2] != (T)0) {
                 const int gj = sgid[code >> g.code_shift];
                 atomicAdd(&A.f[gj], -(double)p[0]);
@@ -918,7 +1139,14 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS) k_tile_force(ForceArgs A) {
           atomicAdd(&A.f[gi], tot[0]); atomicAdd(&A.f[ld + gi], tot[1]); atomicAdd(&A.f[2 * ld + gi], tot[2]);
         } else {
           const double t3[3] = {tot[0], tot[1], tot[2]};
-          d2max = fmax(d2max, atom_epilogue(A, gi, t3));
+          double cc[3] = {0.0, 0.0, 0.0};
+          if (A.epi == EPI_KICK_DRIFT) {
+            const int m = tt.meta[cell];
+            const int tq[3] = {m & 0xff, (m >> 8) & 0xff, (m >> 16) & 0xff};
+#pragma unroll
+            for (int d = 0; d < 3; ++d) cc[d] = cell_anchor_1d(g, d, tt.c0[d] + tq[d] - 1);
+          }
+          d2max = fmax(d2max, atom_epilogue<T>(A, gi, t3, cc));
         }
         if constexpr (EV) {
           const double wgt = HALF ? 1.0 : 0.5;   // a full list visits every pair twice
@@ -928,8 +1156,10 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS) k_tile_force(ForceArgs A) {
       } else {
         const double rho = tot[0];
         const double sq = sqrt(rho);
+        const double fpv = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
         A.rho[gi] = rho;
-        A.fp_out[gi] = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
+        A.fp_out[gi] = fpv;
+        reinterpret_cast<T*>(const_cast<void*>(A.xr))[4 * (size_t)gi + 3] = (T)(-fpv);   // read back as pj.w by pass 2
         if constexpr (EV) ev[0] += -A.P.B * sq;                  // embedding energy F(rho_i)
       }
     }
@@ -954,10 +1184,6 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS) k_tile_force(ForceArgs A) {
 // candidates per broadcast 128-bit load from SoA shared memory (the same walk as the list build).
 // Shared memory: TileTables | xs ys zs ws [capA] of T.
 // ---------------------------------------------------------------------------------------------------
-template <typename T> struct Vec4;
-template <> struct Vec4<float> { using type = float4; };
-template <> struct Vec4<double> { using type = double4; };
-
 template <typename T, class Body, int MODE, bool EV>
 __global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
   using V4 = typename Vec4<T>::type;
@@ -973,7 +1199,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
   T* ws = zs + capA;
   __shared__ double red[8 * 32];
   const int tileid = blockIdx.x;
-  tile_setup(g, tileid, A.cell_start, tt);
+  tile_load(g, tileid, A.tab, tt);
   const double* __restrict__ x = A.x;
   const size_t ld = A.ld;
   const double* __restrict__ fpin = A.fp_in;
@@ -1030,7 +1256,9 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
       if (act) {
         if constexpr (MODE == 0) {
           const double t3[3] = {tot[0], tot[1], tot[2]};
-          d2max = fmax(d2max, atom_epilogue(A, gi, t3));
+          const double cc[3] = {cell_anchor_1d(g, 0, tt.c0[0] + tx - 1), cell_anchor_1d(g, 1, tt.c0[1] + ty - 1),
+                                cell_anchor_1d(g, 2, tt.c0[2] + tz - 1)};
+          d2max = fmax(d2max, atom_epilogue<T>(A, gi, t3, cc));
           if constexpr (EV)
 #pragma unroll
             for (int k = 0; k < 7; ++k) ev[k] += 0.5 * tot[3 + k];
@@ -1075,23 +1303,30 @@ __global__ void k_reduce_ev(int ntiles, const double* __restrict__ partials, dou
 // the scatter kernel has finished).
 // ---------------------------------------------------------------------------------------------------
 // v += dtf f ; x += dt v ; flag = max |x - x0|^2
-__global__ void k_initial_integrate(int N, size_t ld, double* __restrict__ x, double* __restrict__ v, const double* __restrict__ f,
+// The atom's storage cell is the cell of x0 (its wrapped position at the last build); the packed copy xr is
+// kept in step with x.
+template <typename T>
+__global__ void k_initial_integrate(Geom g, int N, size_t ld, double* __restrict__ x, double* __restrict__ v, const double* __restrict__ f,
                                     const double* __restrict__ x0, const int* __restrict__ type, const double* __restrict__ mass,
-                                    double dt, double half_dt_ftm2v, unsigned long long* flag) {
+                                    typename Vec4<T>::type* __restrict__ xr, double dt, double half_dt_ftm2v, unsigned long long* flag) {
   __shared__ double red[32];
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   double d2 = 0.0;
   if (n < N) {
     double dtf = half_dt_ftm2v / mass[type[n]];
+    T r[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
       double vv = v[d * ld + n] + dtf * f[d * ld + n];
       double xx = x[d * ld + n] + dt * vv;
       v[d * ld + n] = vv;
       x[d * ld + n] = xx;
-      double dd = xx - x0[d * ld + n];
+      const double p0 = x0[d * ld + n];
+      double dd = xx - p0;
       d2 += dd * dd;
+      r[d] = (T)(xx - cell_anchor_1d(g, d, cell_index_1d(g, d, p0)));
     }
+    xr[n] = make_v4<T>(r[0], r[1], r[2], (T)0);
   }
   block_max_to_flag(d2, red, flag);
 }
