@@ -1,0 +1,110 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (MD_KERNEL_AUTO, full
+list, the config's own precision), on the same seeded inputs.
+
+At these sizes the oracle cannot enumerate all pairs by brute force, so the comparison is
+  * sampled atoms, one by one: orc_forces_sample / orc_neighbors_sample scan ALL N atoms per sampled atom
+    (the plain definition, any N); the GPU's forces and list rows of those atoms are compared with them;
+  * every atom: the oracle's O(N) list route (itself pinned to the brute force in test_oracle_pins.py)
+    recomputes forces, energy and virial from the GPU's OWN fp64 positions after a piece of the run
+    that crosses several list rebuilds (same-input snapshot, SURVEY.md §8(c) "GPU vs oracle").
+Tolerances: north_star -- mixed: relative RMS force error <= 1e-5, energy <= 1e-6 relative; fp64: 1e-12;
+pair sets identical outside the 1e-9 band around rc+skin.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1009_4330_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+NSAMPLE = 48
+
+
+def _rel_rms(f, ref):
+    return float(np.sqrt(((f - ref) ** 2).sum() / (ref ** 2).sum()))
+
+
+def _sample_ids(N, seed):
+    u = wl.uniform01(seed, np.arange(NSAMPLE, dtype=np.uint64), 9)
+    return np.unique((u * N).astype(np.int64))
+
+
+@pytest.mark.parametrize("cfg,steps", [(2, 40), (3, 12), (4, 30), (5, 14)])
+def test_full_size_run_snapshot_matches_oracle(cfg, steps):
+    import torch
+    from paper_1009_4330_b200 import md
+    w = wl.make(cfg)
+    N = w.natoms
+    s = md.from_workload(w, kernel=md.MD_KERNEL_AUTO)          # what bench.py launches
+    s.md_run(steps, w.dt)
+    st = s.md_get_stats()
+    assert st["nsteps_total"] == steps
+    if w.style == wl.PAIR_LJ:
+        assert st["nbuilds_in_run"] >= 2                        # the piece crossed displacement-triggered rebuilds
+    x = np.zeros((N, 3)); f_run = np.zeros((N, 3))
+    s.md_get_positions(x); s.md_get_forces(f_run)
+    f = np.zeros((N, 3))
+    E, W = s.md_compute_forces(f, energy=True, virial=True)    # same positions, the list the run left behind
+    fo, Eo, Wo, _, _ = oracle.forces(x, w.box, w.style, w.params, w.rc)
+    assert np.isfinite(f).all()
+    assert _rel_rms(f, fo) < 1e-5, _rel_rms(f, fo)
+    assert _rel_rms(f_run, fo) < 1e-5
+    assert abs(E - Eo) < 1e-6 * abs(Eo), (E, Eo)
+    assert np.abs(W[:3] - Wo[:3]).max() < 1e-5 * np.abs(Wo[:3]).max()
+    # sampled atoms by the plain definition (full scan over all N)
+    ids = _sample_ids(N, w.seed)
+    fs, _ = oracle.forces_sample(x, w.box, w.style, w.params, w.rc, ids)
+    scale = np.sqrt((fo ** 2).sum(axis=1).mean())
+    assert np.abs(f[ids] - fs).max() < 3e-5 * scale
+    assert np.abs(fo[ids] - fs).max() < 1e-10 * scale          # the oracle's two routes agree
+    # the list the run left behind is still valid: every pair inside rc at the CURRENT positions is in it
+    stride = int(st["max_neighbors"]) + 8
+    nn = torch.zeros(N, dtype=torch.int32, device="cuda")
+    nb = torch.full((N, stride), -1, dtype=torch.int32, device="cuda")
+    s.md_get_neighbors(nn, nb, stride)
+    idt = torch.from_numpy(ids).cuda()
+    nn_s, nb_s = nn[idt].cpu().numpy(), nb[idt].cpu().numpy()
+    cnt, inside = oracle.neighbors_sample(x, w.box, w.rc - 1e-9, ids, stride=2048)
+    for k in range(len(ids)):
+        have = set(nb_s[k, :nn_s[k]].tolist())
+        assert len(have) == nn_s[k]
+        assert set(inside[k, :cnt[k]].tolist()) <= have
+    del nn, nb
+    s.close()
+
+
+@pytest.mark.parametrize("cfg", [3, 5])
+def test_full_size_list_rows_match_full_scan(cfg):
+    """Pair-set parity at build time: sampled rows of the freshly built list against a full scan."""
+    import torch
+    from paper_1009_4330_b200 import md
+    w = wl.make(cfg)
+    N = w.natoms
+    x = wl.perturbed(w, 0.1)
+    s = md.from_workload(w, kernel=md.MD_KERNEL_AUTO, x=x)
+    s.md_build_neighbors()
+    st = s.md_get_stats()
+    stride = int(st["max_neighbors"]) + 8
+    nn = torch.zeros(N, dtype=torch.int32, device="cuda")
+    nb = torch.full((N, stride), -1, dtype=torch.int32, device="cuda")
+    s.md_get_neighbors(nn, nb, stride)
+    total = int(nn.sum().item())
+    assert abs(total / N - st["mean_neighbors"]) < 1e-9 * total / N + 1e-6
+    ids = _sample_ids(N, w.seed + 1)
+    idt = torch.from_numpy(ids).cuda()
+    nn_s, nb_s = nn[idt].cpu().numpy(), nb[idt].cpu().numpy()
+    rl, band = w.rc + w.skin, 1e-9
+    c_in, sure = oracle.neighbors_sample(x, w.box, rl - band, ids, stride=2048)
+    c_out, maybe = oracle.neighbors_sample(x, w.box, rl + band, ids, stride=2048)
+    for k in range(len(ids)):
+        have = set(nb_s[k, :nn_s[k]].tolist())
+        assert len(have) == nn_s[k]
+        assert set(sure[k, :c_in[k]].tolist()) <= have <= set(maybe[k, :c_out[k]].tolist())
+    # a full list is symmetric: row lengths of the partners include the sampled atom
+    k = 0
+    partners = torch.from_numpy(nb_s[k, :nn_s[k]].astype(np.int64)).cuda()
+    rows = nb[partners]
+    assert bool((rows == int(ids[k])).any(dim=1).all().item())
+    del nn, nb
+    s.close()
