@@ -149,10 +149,13 @@ int lanes_for(int kernel) { return kernel == MD_KERNEL_SUBWARP ? 8 : (kernel == 
 size_t elem_size(const md_system* s) { return s->precision == MD_FP64 ? sizeof(double) : sizeof(float); }
 int capA_of(const Geom& g) { return (g.tile_cap + 8) & ~3; }
 size_t force_smem(const md_system* s, const Geom& g, bool half) {
-  return sizeof(TileTables) + 4 * (size_t)capA_of(g) * elem_size(s) + (size_t)g.interior_cap * 2 + (half ? (size_t)capA_of(g) * 4 : 0) + 16;
+  return sizeof(TileTables) + 4 * (size_t)(capA_of(g) + tile_tab_cells(g)) * elem_size(s) + (size_t)g.interior_cap * 2 +
+         (size_t)((tile_tab_quads(g) + 7) & ~7) * 2 + (half ? (size_t)capA_of(g) * 4 : 0) + 16;
 }
 size_t cell_smem(const md_system* s, const Geom& g) { return sizeof(TileTables) + 4 * (size_t)capA_of(g) * elem_size(s) + 16; }
-size_t build_smem(const Geom& g) { return sizeof(TileTables) + 3 * (size_t)capA_of(g) * sizeof(float) + (size_t)BUILD_THREADS * RING_STRIDE + 16; }
+size_t build_smem(const Geom& g) {
+  return sizeof(TileTables) + (size_t)tile_tab_cells(g) * 16 + BUILD_TASK_INTS * sizeof(int) + 3 * (size_t)capA_of(g) * sizeof(float) + (size_t)BUILD_THREADS * RING_STRIDE + 16;
+}
 size_t export_smem(const Geom& g) { return sizeof(TileTables) + (size_t)capA_of(g) * sizeof(int) + 16; }
 
 void fill_geom_for_b(const md_system* s, int b, Geom& g) {
@@ -256,7 +259,7 @@ int plan(md_system* s) {
   if ((size_t)g.ncell + 1 > s->cell_alloc) {
     cudaFree(s->cell_count); cudaFree(s->cell_start);
     s->cell_alloc = (size_t)g.ncell + 1;
-    CK(dalloc(&s->cell_count, s->cell_alloc));
+    CK(dalloc(&s->cell_count, s->cell_alloc + s->cell_alloc / SCAN_BLOCK + 2));   // + the scan's block sums
     CK(dalloc(&s->cell_start, s->cell_alloc));
   }
   size_t words = (size_t)g.ntiles * g.chunk_cap * g.interior_cap * g.K;
@@ -296,6 +299,7 @@ int build_list_only(md_system* s) {
   double rl = s->rc + s->skin;
   BuildArgs B{};
   B.g = g; B.cell_start = s->cell_start; B.tab = s->tab; B.x = s->x[s->xcur]; B.ld = s->ld; B.rl2 = rl * rl;
+  B.xr = s->xr[s->xcur]; B.xr_double = s->precision == MD_FP64 ? 1 : 0;
   // guard band of the fp32 distance test: tile-centred coordinates up to E are
   // rounded to fp32, so r^2 carries a relative error of about (7 E / rl + 3) 2^-24; four times that is used.
   double E = 0;
@@ -305,8 +309,21 @@ int build_list_only(md_system* s) {
   B.rl2_bw = std::nextafterf((float)(rl * rl * band), INFINITY);
   B.rl2_hi = B.rl2_mid + B.rl2_bw;      // the same fp32 sum the kernel's accept test and band test are consistent with
   B.list = s->list; B.numneigh = s->numneigh; B.flags = s->flags_d;
-  if (g.half) CK(launch(s, k_build_list<true>, g.ntiles, BUILD_THREADS, build_smem(g), B));
-  else CK(launch(s, k_build_list<false>, g.ntiles, BUILD_THREADS, build_smem(g), B));
+  const bool s4 = g.code_shift == 4;
+  const size_t sm = build_smem(g);
+  if (g.half) {
+    if (s4) CK(launch(s, k_build_list<true, 0, 4>, g.ntiles, BUILD_THREADS, sm, B));
+    else CK(launch(s, k_build_list<true, 0, 3>, g.ntiles, BUILD_THREADS, sm, B));
+  } else if (g.K == 1) {
+    if (s4) CK(launch(s, k_build_list<false, 0, 4>, g.ntiles, BUILD_THREADS, sm, B));
+    else CK(launch(s, k_build_list<false, 0, 3>, g.ntiles, BUILD_THREADS, sm, B));
+  } else if (g.K == 8) {
+    if (s4) CK(launch(s, k_build_list<false, 3, 4>, g.ntiles, BUILD_THREADS, sm, B));
+    else CK(launch(s, k_build_list<false, 3, 3>, g.ntiles, BUILD_THREADS, sm, B));
+  } else {
+    if (s4) CK(launch(s, k_build_list<false, 5, 4>, g.ntiles, BUILD_THREADS, sm, B));
+    else CK(launch(s, k_build_list<false, 5, 3>, g.ntiles, BUILD_THREADS, sm, B));
+  }
   return MD_OK;
 }
 
@@ -322,7 +339,13 @@ int build(md_system* s, bool need_list) {
     int c = s->cur, o = 1 - c, xc = s->xcur, xo = 1 - xc;
     CK(launch(s, k_bin, blocks_for(N, 256), 256, 0, g, N, s->x[xc], s->x[xc] + s->ld, s->x[xc] + 2 * s->ld, s->cell_of, s->rank,
               s->cell_count, s->flags_d));
-    CK(launch(s, k_scan_cells, 1, 1024, 0, g.ncell, (const int*)s->cell_count, s->cell_start));
+    {
+      // block sums live in the tail of cell_count's allocation (cell_alloc has SCAN slack, see plan())
+      const unsigned nblk = blocks_for(g.ncell, SCAN_BLOCK);
+      int* bsum = s->cell_count + (g.ncell + 1);
+      CK(launch(s, k_scan_block_sums, nblk, 1024, 0, g.ncell, (const int*)s->cell_count, bsum));
+      CK(launch(s, k_scan_cells, nblk, 1024, 0, g.ncell, (const int*)s->cell_count, (const int*)bsum, s->cell_start));
+    }
     CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
               s->perm));
     CK(launch(s, k_sort_cells, blocks_for(g.ncell, 128), 128, 0, g.ncell, (const int*)s->cell_start, s->perm));

@@ -18,11 +18,13 @@
 
 namespace mdk {
 
-constexpr int MAX_TILE_CELLS = 512;    // (b+2)^3 <= 512  =>  b <= 6
+constexpr int MAX_TILE_CELLS = 216;    // (b+2)^3 <= 216  =>  b <= 4
 constexpr int BUILD_THREADS = 256;     // threads per block of the list-build and cell-list kernels
 constexpr int FORCE_MAX_THREADS = 640; // upper bound of the force kernels' block size (runtime choice)
 constexpr int FORCE_MIN_BLOCKS = 2;    // resident blocks per SM the mixed-precision force kernels are compiled for (<= 48 registers)
-constexpr int RING = 64;               // list-build: pending entries a lane can hold in shared memory
+constexpr int BUILD_MIN_BLOCKS = 3;    // resident blocks per SM the list-build kernel is compiled for (<= 85 registers)
+constexpr int BUILD_TASK_INTS = 72;     // list-build: room for the first-task table of <= 64 interior cells (+1), 16-byte multiple
+constexpr int RING = 48;               // list-build: pending entries a lane can hold in shared memory (>= 32 + 8)
 constexpr int RING_STRIDE = RING * 2 + 16;   // bytes between the rings of neighbouring lanes (odd * 16)
 
 struct Geom {
@@ -277,8 +279,11 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
 // ---------------------------------------------------------------------------------------------------
 constexpr int TILE_HDR = 8;   // n_int_slots, n_slots, n_int_atoms, brick_start, n_staged_atoms, pad x3
 __host__ __device__ inline int tile_tab_cells(const Geom& g) { return ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) + 3) & ~3; }
+// after the per-cell ints: one u16 per QUAD of staged slots (cells are padded to 4 slots, so a quad belongs to
+// one tile cell) = the tile cell of that quad; lets the force kernel post-process the staged tile slot-parallel
+__host__ __device__ inline int tile_tab_quads(const Geom& g) { return (g.tile_cap >> 2) + 2; }
 __host__ __device__ inline int tile_tab_stride(const Geom& g) {
-  return TILE_HDR + 3 * tile_tab_cells(g);
+  return TILE_HDR + 3 * tile_tab_cells(g) + ((tile_tab_quads(g) + 1) >> 1);
 }
 
 __device__ __forceinline__ void tile_dims(const Geom& g, int tile, int c0[3], int w[3]) {
@@ -328,6 +333,9 @@ __global__ void __launch_bounds__(128) k_tile_tables(Geom g, const int* __restri
     h[TILE_HDR + tcs + t] = (int)(((unsigned)tt.start[t] << 16) | ((unsigned)tt.cnt[t] & 0xffffu));
     h[TILE_HDR + 2 * tcs + t] = tx | ty << 8 | tz << 16 | (tile_cell_is_interior(tt, t) ? 1 << 24 : 0);
     staged += tt.cnt[t];
+    unsigned short* qc = reinterpret_cast<unsigned short*>(h + TILE_HDR + 3 * tcs);
+    const int q0 = tt.start[t] >> 2, q1 = min((tt.start[t] + pad4(tt.cnt[t])) >> 2, tile_tab_quads(g));
+    for (int q = q0; q < q1; ++q) qc[q] = (unsigned short)t;
   }
   __shared__ int red[4];
   for (int o = 16; o > 0; o >>= 1) staged += __shfl_xor_sync(0xffffffffu, staged, o);
@@ -423,49 +431,67 @@ __global__ void k_bin(Geom g, int N, double* __restrict__ x, double* __restrict_
   rank[k] = atomicAdd(&cell_count[oid], 1);
 }
 
-// a2: exclusive scan of the cell counts, one block of 1024 threads, 8 cells per thread per sweep.
-__global__ void __launch_bounds__(1024) k_scan_cells(int ncell, const int* __restrict__ cell_count, int* __restrict__ cell_start) {
-  constexpr int PER = 8;
+// a2: exclusive scan of the cell counts in two launches: per-block sums of SCAN_BLOCK cells, then every block
+// adds up the sums of the blocks before it (there are few) and scans its own cells.
+constexpr int SCAN_PER = 8;
+constexpr int SCAN_BLOCK = 1024 * SCAN_PER;
+__global__ void __launch_bounds__(1024) k_scan_block_sums(int ncell, const int* __restrict__ cell_count, int* __restrict__ block_sum) {
+  __shared__ int wsum[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int i0 = blockIdx.x * SCAN_BLOCK + tid * SCAN_PER;
+  int sum = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_PER; ++k) sum += i0 + k < ncell ? cell_count[i0 + k] : 0;
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if (lane == 0) wsum[wid] = sum;
+  __syncthreads();
+  if (wid == 0) {
+    int v = wsum[lane];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) block_sum[blockIdx.x] = v;
+  }
+}
+__global__ void __launch_bounds__(1024) k_scan_cells(int ncell, const int* __restrict__ cell_count, const int* __restrict__ block_sum,
+                                                     int* __restrict__ cell_start) {
   __shared__ int wsum[32];
   __shared__ int carry_s;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  if (tid == 0) carry_s = 0;
+  if (wid == 0) {   // sum of the blocks before this one
+    int v = 0;
+    for (int b = lane; b < (int)blockIdx.x; b += 32) v += block_sum[b];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) carry_s = v;
+  }
   __syncthreads();
-  for (int base = 0; base < ncell; base += 1024 * PER) {
-    const int i0 = base + tid * PER;
-    int v[PER], sum = 0;
+  const int i0 = blockIdx.x * SCAN_BLOCK + tid * SCAN_PER;
+  int v[SCAN_PER], sum = 0;
 #pragma unroll
-    for (int k = 0; k < PER; ++k) { v[k] = i0 + k < ncell ? cell_count[i0 + k] : 0; sum += v[k]; }
-    int incl = sum;
+  for (int k = 0; k < SCAN_PER; ++k) { v[k] = i0 + k < ncell ? cell_count[i0 + k] : 0; sum += v[k]; }
+  int incl = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int u = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += u;
+  }
+  if (lane == 31) wsum[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    int s = wsum[lane], si = s;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      int u = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += u;
+      int u = __shfl_up_sync(0xffffffffu, si, o);
+      if (lane >= o) si += u;
     }
-    if (lane == 31) wsum[wid] = incl;
-    __syncthreads();
-    if (wid == 0) {
-      int s = wsum[lane], si = s;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        int u = __shfl_up_sync(0xffffffffu, si, o);
-        if (lane >= o) si += u;
-      }
-      wsum[lane] = si - s;   // exclusive
-    }
-    __syncthreads();
-    const int carry = carry_s;
-    int run = carry + wsum[wid] + incl - sum;
-#pragma unroll
-    for (int k = 0; k < PER; ++k) {
-      if (i0 + k < ncell) cell_start[i0 + k] = run;
-      run += v[k];
-    }
-    __syncthreads();
-    if (tid == 1023) carry_s = run;
-    __syncthreads();
+    wsum[lane] = si - s;   // exclusive
   }
-  if (tid == 0) cell_start[ncell] = carry_s;
+  __syncthreads();
+  int run = carry_s + wsum[wid] + incl - sum;
+#pragma unroll
+  for (int k = 0; k < SCAN_PER; ++k) {
+    if (i0 + k < ncell) cell_start[i0 + k] = run;
+    run += v[k];
+  }
+  if (i0 <= ncell - 1 && ncell - 1 < i0 + SCAN_PER) cell_start[ncell] = run;   // the thread that owns the last cell
 }
 
 __global__ void k_fill_perm(int N, const int* __restrict__ cell_of, const int* __restrict__ rank,
@@ -549,6 +575,8 @@ struct BuildArgs {
   const int* cell_start;
   const int* tab;          // per-tile tables (k_tile_tables)
   const double* x; size_t ld;
+  const void* xr;          // packed cell-relative positions (float4, or double4 when xr_double) of the positions in x
+  int xr_double;
   double rl2;
   float rl2_hi, rl2_mid, rl2_bw;   // fp32 test: accept r2 < hi = mid + bw; |r2 - mid| <= bw is decided in fp64 (mid = fl(rl2))
   uint4* list;
@@ -579,70 +607,217 @@ __device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mo
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+// 128-bit shared load as two packed pairs {a0,a1} {a2,a3}: the pairs are ready for the f32x2 ops, no moves
+__device__ __forceinline__ void lds_2x2(unsigned a, f32x2& p01, f32x2& p23) {
+  asm volatile("ld.shared.v2.u64 {%0,%1}, [%2];" : "=l"(p01), "=l"(p23) : "r"(a));
+}
 
-// predicated 16-bit store to the lane's ring + pointer advance
+// ring push of a candidate pair: for each half of r2 = {r2_a, r2_b}: if (r2 < hi) { ring[rp] = code (16 bit); rp += 2 }
+// The compare lives in the asm so that it feeds the two predicated instructions directly (FSETP, @P STS.U16, @P IADD).
+__device__ __forceinline__ void ring_push2(unsigned& rp, unsigned code_a, unsigned code_b, f32x2 r2, float hi) {
+  asm volatile(
+      "{ .reg .pred p; .reg .f32 a, b; .reg .b16 c, d;\n"
+      "  mov.b64 {a, b}, %3;\n"
+      "  mov.b32 {c, d}, %1;\n"
+      "  setp.lt.f32 p, a, %4;\n"
+      "  @p st.shared.u16 [%0], c;\n"
+      "  @p add.u32 %0, %0, 2;\n"
+      "  mov.b32 {c, d}, %2;\n"
+      "  setp.lt.f32 p, b, %4;\n"
+      "  @p st.shared.u16 [%0], c;\n"
+      "  @p add.u32 %0, %0, 2; }"
+      : "+r"(rp)
+      : "r"(code_a), "r"(code_b), "l"(r2), "f"(hi)
+      : "memory");
+}
+// the same with one more condition per candidate: its code differs from `self` (the lane's own atom)
+__device__ __forceinline__ void ring_push2_self(unsigned& rp, unsigned code_a, unsigned code_b, f32x2 r2, float hi, unsigned self) {
+  asm volatile(
+      "{ .reg .pred p; .reg .f32 a, b; .reg .b16 c, d;\n"
+      "  mov.b64 {a, b}, %3;\n"
+      "  mov.b32 {c, d}, %1;\n"
+      "  setp.lt.f32 p, a, %4;\n"
+      "  setp.ne.and.u32 p, %1, %5, p;\n"
+      "  @p st.shared.u16 [%0], c;\n"
+      "  @p add.u32 %0, %0, 2;\n"
+      "  mov.b32 {c, d}, %2;\n"
+      "  setp.lt.f32 p, b, %4;\n"
+      "  setp.ne.and.u32 p, %2, %5, p;\n"
+      "  @p st.shared.u16 [%0], c;\n"
+      "  @p add.u32 %0, %0, 2; }"
+      : "+r"(rp)
+      : "r"(code_a), "r"(code_b), "l"(r2), "f"(hi), "r"(self)
+      : "memory");
+}
+// predicated 16-bit store to the lane's ring + pointer advance (slow paths)
 __device__ __forceinline__ void ring_push(unsigned& rp, unsigned code, bool take) {
-  asm volatile("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p st.shared.u16 [%0], %1; @p add.u32 %0, %0, 2; }"
+  asm volatile("{ .reg .pred p; .reg .b16 c, d; mov.b32 {c, d}, %1; setp.ne.u32 p, %2, 0; @p st.shared.u16 [%0], c; @p add.u32 %0, %0, 2; }"
                : "+r"(rp)
-               : "h"((unsigned short)code), "r"((unsigned)take)
+               : "r"(code), "r"((unsigned)take)
                : "memory");
 }
 
-template <bool HALF>
-__global__ void __launch_bounds__(BUILD_THREADS, 2) k_build_list(BuildArgs A) {
+// The careful scan of `ncand` candidates starting at staged slot j0 of tile cell t2 (global index g0 at j0) for
+// the lane's atom (tile-centred position xi, yi, zi; global index gi; tile cell t; act: the lane holds an atom):
+// the same fp32 accept test as the fast loop, plus the exclusions (never slot jskip, only slots > jmin), plus an
+// fp64 decision from the global positions for every candidate inside the guard band.  Used for the own cell of a
+// half list and to redo a segment in which the fast loop saw an in-band candidate.  Everything is passed by value
+// or lives in shared memory (gs: a shared copy of the geometry), so the kernel keeps no stack frame for it.
+struct BuildBand { double rl2; float hi, mid, bw; };
+__device__ __noinline__ unsigned build_scan_careful(const Geom& gs, const TileTables& tt, const double* __restrict__ x, size_t ld,
+                                                    BuildBand bd, const float* xs, const float* ys, const float* zs, float xi, float yi,
+                                                    float zi, int act, int gi, int t, int jskip, int jmin, unsigned rp, int j0,
+                                                    int ncand, int g0, int t2, int shift) {
+  for (int k = 0; k < ncand; ++k) {
+    const int j = j0 + k;
+    const float ex = xi - xs[j], ey = yi - ys[j], ez = zi - zs[j];
+    const float r2s = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
+    bool take = r2s < bd.hi && j != jskip && j > jmin;
+    if (act && take && fabsf(r2s - bd.mid) <= bd.bw) take = confirm_pair_fp64(gs, tt, x, ld, gi, t, g0 + k, t2, bd.rl2);
+    ring_push(rp, (unsigned)j << shift, take);
+  }
+  return rp;
+}
+
+// The fast scan of nq quads of candidates (staged slots off/4 ..) for one lane: packed fp32 distance test, accepted
+// codes to the lane's ring, m = min |r2 - rl2| (the guard-band detector).  SELF: the candidates are the lane's own
+// cell, skip the code `self`.
+template <bool SELF, int SHIFT>
+__device__ __forceinline__ void build_scan_fast(unsigned& rp, float& m, unsigned xs_a, unsigned ys_a, unsigned zs_a, unsigned off,
+                                                unsigned code, int nq, f32x2 xi2, f32x2 yi2, f32x2 zi2, f32x2 mid2, float hi,
+                                                unsigned self) {
+#pragma unroll 2
+  for (int q = 0; q < nq; ++q) {
+    f32x2 X01, X23, Y01, Y23, Z01, Z23;
+    lds_2x2(xs_a + off, X01, X23);
+    lds_2x2(ys_a + off, Y01, Y23);
+    lds_2x2(zs_a + off, Z01, Z23);
+    const f32x2 dx01 = sub2(xi2, X01), dx23 = sub2(xi2, X23);
+    const f32x2 dy01 = sub2(yi2, Y01), dy23 = sub2(yi2, Y23);
+    const f32x2 dz01 = sub2(zi2, Z01), dz23 = sub2(zi2, Z23);
+    const f32x2 q01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
+    const f32x2 q23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
+    float e0, e1, e2, e3;
+    unpack2(sub2(q01, mid2), e0, e1);
+    unpack2(sub2(q23, mid2), e2, e3);
+    m = fminf(fminf(m, fabsf(e0)), fabsf(e1));
+    m = fminf(fminf(m, fabsf(e2)), fabsf(e3));
+    if constexpr (SELF) {
+      ring_push2_self(rp, code, code + (1u << SHIFT), q01, hi, self);
+      ring_push2_self(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi, self);
+    } else {
+      ring_push2(rp, code, code + (1u << SHIFT), q01, hi);
+      ring_push2(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi);
+    }
+    off += 16;
+    code += 4u << SHIFT;
+  }
+}
+
+// Shared memory: TileTables | offs[tile cells] float4 | xs[capA] ys[capA] zs[capA] floats | rings[nwarps*32*RING_STRIDE].
+template <bool HALF, int LOGK, int SHIFT>
+__global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_BLOCKS) k_build_list(BuildArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
   const Geom& g = A.g;
+  constexpr int K = 1 << LOGK;
   const int capA = build_capA(g);
-  float* xs = reinterpret_cast<float*>(smem_raw + sizeof(TileTables));
+  float4* offs = reinterpret_cast<float4*>(smem_raw + sizeof(TileTables));
+  int* task0 = reinterpret_cast<int*>(offs + tile_tab_cells(g));   // [nic + 1] first task of each interior cell
+  float* xs = reinterpret_cast<float*>(task0 + BUILD_TASK_INTS);
   float* ys = xs + capA;
   float* zs = ys + capA;
   unsigned char* rings = reinterpret_cast<unsigned char*>(zs + capA);
   const int tile = blockIdx.x;
+  __shared__ Geom gs;   // for the slow paths: a reference to kernel parameters would cost a stack copy
+  __shared__ int soff[27];   // tile-cell index offsets of the 27-cell stencil (the same for every cell of the tile)
+  if (threadIdx.x == 0) gs = A.g;
   tile_load(g, tile, A.tab, tt);
+  if (threadIdx.x < 27) {
+    const int dx = (int)threadIdx.x % 3 - 1, dy = ((int)threadIdx.x / 3) % 3 - 1, dz = (int)threadIdx.x / 9 - 1;
+    soff[threadIdx.x] = (dz * tt.tc[1] + dy) * tt.tc[0] + dx;
+  }
   if (tt.n_slots > g.tile_cap || tt.n_int_slots > g.interior_cap) return;   // host re-plans and rebuilds
-  const double* __restrict__ x = A.x;
-  const size_t ld = A.ld;
-  tile_stage(g, tt, g.tile_cap,
-             [&](int slot, int gi, const double* off, int) {
-               xs[slot] = (float)(x[gi] + off[0]);
-               ys[slot] = (float)(x[ld + gi] + off[1]);
-               zs[slot] = (float)(x[2 * ld + gi] + off[2]);
-             },
-             [&](int slot) { xs[slot] = 1e15f; ys[slot] = 1e15f; zs[slot] = 1e15f; });
+  // a task = 32 consecutive rows (atoms) of one interior cell; tasks are dealt to the warps round robin, so a tile
+  // of one big cell (rc = 5 sigma: ~150 atoms per cell) still keeps several warps busy
+  if (threadIdx.x == 0) {
+    int run = 0;
+    for (int ic = 0; ic < tt.nic; ++ic) { task0[ic] = run; run += (tt.cnt[interior_tile_cell(tt, ic)] + 31) >> 5; }
+    task0[tt.nic] = run;
+  }
+  // staging: tile-centred fp32 coordinates = packed cell-relative coordinate + the cell's offset (the same values the
+  // force kernels stage), one thread per quad of slots, SoA so that four candidates are one broadcast 128-bit load
+  for (int t = threadIdx.x; t < tt.ntc; t += blockDim.x) {
+    double od[3];
+    tile_cell_offset_rel(g, tt, t, od);
+    offs[t] = make_float4((float)od[0], (float)od[1], (float)od[2], 0.f);
+  }
+  __syncthreads();
+  {
+    const unsigned short* __restrict__ qc =
+        reinterpret_cast<const unsigned short*>(A.tab + (size_t)tile * tile_tab_stride(g) + TILE_HDR + 3 * tile_tab_cells(g));
+    const int nq = tt.n_slots >> 2;
+    for (int q = threadIdx.x; q < nq; q += blockDim.x) {
+      const int t = qc[q];
+      const int c = tt.cnt[t], k0 = 4 * q - tt.start[t], gb = tt.gstart[t] + k0;
+      const float4 o = offs[t];
+      float xv[4], yv[4], zv[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (k0 + u < c) {
+          if (A.xr_double) {
+            const double4 v = reinterpret_cast<const double4*>(A.xr)[gb + u];
+            xv[u] = (float)v.x + o.x; yv[u] = (float)v.y + o.y; zv[u] = (float)v.z + o.z;
+          } else {
+            const float4 v = reinterpret_cast<const float4*>(A.xr)[gb + u];
+            xv[u] = v.x + o.x; yv[u] = v.y + o.y; zv[u] = v.z + o.z;
+          }
+        } else {
+          xv[u] = 1e15f; yv[u] = 1e15f; zv[u] = 1e15f;
+        }
+      }
+      *reinterpret_cast<float4*>(xs + 4 * q) = make_float4(xv[0], xv[1], xv[2], xv[3]);
+      *reinterpret_cast<float4*>(ys + 4 * q) = make_float4(yv[0], yv[1], yv[2], yv[3]);
+      *reinterpret_cast<float4*>(zs + 4 * q) = make_float4(zv[0], zv[1], zv[2], zv[3]);
+    }
+    if (threadIdx.x == 0) { xs[tt.n_slots] = 1e15f; ys[tt.n_slots] = 1e15f; zs[tt.n_slots] = 1e15f; }   // the dummy slot
+  }
   __syncthreads();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const unsigned rbase = smem_addr(rings) + (unsigned)(wid * 32 + lane) * RING_STRIDE;
-  const int K = g.K;
-  const size_t slots_cap = (size_t)g.interior_cap * K;
+  const size_t slots_cap = (size_t)g.interior_cap << LOGK;
   uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
-  const int max_words = g.chunk_cap * K;
-  const unsigned dummy = (unsigned)tt.n_slots << g.code_shift;
-  const int shift = g.code_shift;
-  const unsigned cstep = 1u << shift;
-  const float hi = A.rl2_hi, mid = A.rl2_mid, bw = A.rl2_bw;
-  const f32x2 mid2 = pack2(mid, mid);
+  const int max_words = g.chunk_cap << LOGK;
+  const unsigned dummy = (unsigned)tt.n_slots << SHIFT;
+  const float hi = A.rl2_hi, bw = A.rl2_bw;
+  const BuildBand bd = {A.rl2, A.rl2_hi, A.rl2_mid, A.rl2_bw};
+  const f32x2 mid2 = pack2(A.rl2_mid, A.rl2_mid);
+  const unsigned xs_a = smem_addr(xs), ys_a = smem_addr(ys), zs_a = smem_addr(zs);
   int my_max = 0;
   unsigned long long my_sum = 0;
 
-  for (int ic = wid; ic < tt.nic; ic += nw) {
+  const int ntasks = task0[tt.nic];
+  int ic = 0;
+#pragma unroll 1
+  for (int task = wid; task < ntasks; task += nw) {
+    while (task0[ic + 1] <= task) ++ic;
     const int t = interior_tile_cell(tt, ic);
     const int s_lo = tt.start[t], c = tt.cnt[t], g_lo = tt.gstart[t];
-    const int mt = tt.meta[t];
-    const int tx = mt & 0xff, ty = (mt >> 8) & 0xff, tz = (mt >> 16) & 0xff;
-    for (int r0 = 0; r0 < c; r0 += 32) {
+    {
+      const int r0 = (task - task0[ic]) << 5;
       const bool act = r0 + lane < c;
       const int a = act ? s_lo + r0 + lane : s_lo;   // staged slot = list row
       const int gi = g_lo + r0 + lane;
       // an idle lane sits far away from everything, pad slots (+1e15) included: it accepts nothing
       const float xi = act ? xs[a] : -1e15f, yi = act ? ys[a] : -1e15f, zi = act ? zs[a] : -1e15f;
       const f32x2 xi2 = pack2(xi, xi), yi2 = pack2(yi, yi), zi2 = pack2(zi, zi);
+      const unsigned selfcode = (unsigned)a << SHIFT;
       unsigned rp = rbase;
       int nwords = 0;
       auto store_word = [&](uint4 v) {
         if (nwords < max_words) {
-          int s = nwords % K, cch = nwords / K;
-          st_stream(tlist + (size_t)cch * slots_cap + (size_t)a * K + s, v);
+          const int s = nwords & (K - 1), cch = nwords >> LOGK;
+          st_stream(tlist + (size_t)cch * slots_cap + ((size_t)a << LOGK) + s, v);
         }
         ++nwords;
       };
@@ -652,77 +827,48 @@ __global__ void __launch_bounds__(BUILD_THREADS, 2) k_build_list(BuildArgs A) {
         if (full) sts_u4(rbase, lds_u4(rbase + 16 * full));
         rp = rbase + 2 * (pend & 7);
       };
-      for (int dz = -1; dz <= 1; ++dz)
-        for (int dy = -1; dy <= 1; ++dy)
-          for (int dx = -1; dx <= 1; ++dx) {
-            const int t2 = ((tz + dz) * tt.tc[1] + (ty + dy)) * tt.tc[0] + (tx + dx);
-            const int s0 = tt.start[t2], c2 = tt.cnt[t2], g0 = tt.gstart[t2];
-            // candidates a lane must never take: itself (own cell), and for a half list every j <= i
-            int jskip = -1, jmin = -1;
-            if (t2 == t) jskip = a;
-            if (HALF) jmin = gi - g0 + s0;        // take only g0 + (j - s0) > gi  <=>  j > jmin
-            const bool plain = !HALF && t2 != t;
-            for (int k0 = 0; k0 < c2; k0 += 32) {
-              if (((int)(rp - rbase) >> 1) + 32 > RING) flush();
-              const int ng = (min(c2 - k0, 32) + 3) >> 2;
-              const unsigned rp_chunk = rp;
-              float m = 1e30f;                    // min |r2 - rl2| over the chunk: the guard-band detector
-              auto scan = [&](auto plain_tag) {
-                constexpr bool PLAIN = decltype(plain_tag)::value;
-                unsigned code = (unsigned)(s0 + k0) << shift;
-                for (int q = 0; q < ng; ++q) {
-                  const int j0 = s0 + k0 + 4 * q;
-                  const float4 X = *reinterpret_cast<const float4*>(xs + j0);
-                  const float4 Y = *reinterpret_cast<const float4*>(ys + j0);
-                  const float4 Z = *reinterpret_cast<const float4*>(zs + j0);
-                  const f32x2 dx01 = sub2(xi2, pack2(X.x, X.y)), dx23 = sub2(xi2, pack2(X.z, X.w));
-                  const f32x2 dy01 = sub2(yi2, pack2(Y.x, Y.y)), dy23 = sub2(yi2, pack2(Y.z, Y.w));
-                  const f32x2 dz01 = sub2(zi2, pack2(Z.x, Z.y)), dz23 = sub2(zi2, pack2(Z.z, Z.w));
-                  const f32x2 q01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
-                  const f32x2 q23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
-                  float r2[4], e[4];
-                  unpack2(q01, r2[0], r2[1]); unpack2(q23, r2[2], r2[3]);
-                  unpack2(sub2(q01, mid2), e[0], e[1]); unpack2(sub2(q23, mid2), e[2], e[3]);
-                  m = fminf(fminf(m, fabsf(e[0])), fabsf(e[1]));
-                  m = fminf(fminf(m, fabsf(e[2])), fabsf(e[3]));
-#pragma unroll
-                  for (int u = 0; u < 4; ++u) {
-                    bool take = r2[u] < hi;
-                    if constexpr (!PLAIN) take = take && (j0 + u != jskip) && (j0 + u > jmin);
-                    ring_push(rp, code, take);
-                    code += cstep;
-                  }
-                }
-              };
-              if (plain) scan(std::true_type{}); else scan(std::false_type{});
+#pragma unroll 1
+      for (int sc = 0; sc < 27; ++sc) {
+          {
+            const int t2 = t + soff[sc];          // the 27 cells around tile cell t
+            const int s0 = tt.start[t2], c2 = tt.cnt[t2];
+            const bool own = t2 == t;
+            // half list: keep (i, j) iff j follows i in the sorted order; a cell is a contiguous range of that
+            // order, so for another cell the answer is the same for all of its atoms
+            if (HALF && !own && tt.gstart[t2] < g_lo) continue;
+#pragma unroll 1
+            for (int k0 = 0; k0 < c2; k0 += 32) {   // segments of <= 32 candidates: what the ring is guaranteed to take
+              if ((int)(rp - rbase) > 2 * (RING - 32)) flush();
+              const int ncand = min(c2 - k0, 32);
+              if (HALF && own) {
+                // own cell: slot order is the sorted order
+                rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, a, a, rp, s0 + k0, ncand,
+                                        tt.gstart[t2] + k0, t2, SHIFT);
+                continue;
+              }
+              const unsigned rp_seg = rp;
+              const int nq = (ncand + 3) >> 2;
+              const unsigned off = 4u * (unsigned)(s0 + k0);
+              const unsigned code = (unsigned)(s0 + k0) << SHIFT;
+              float m = 1e30f;
+              if (own) build_scan_fast<true, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, xi2, yi2, zi2, mid2, hi, selfcode);
+              else build_scan_fast<false, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, xi2, yi2, zi2, mid2, hi, selfcode);
               if (__builtin_expect(m <= bw, 0)) {
-                // some candidate of this chunk lies in the guard band of the fp32 test: redo the chunk, deciding
+                // some candidate of this segment lies in the guard band of the fp32 test: redo the segment, deciding
                 // the in-band candidates in fp64 from the global positions (the pair set is exactly the fp64 one)
-                rp = rp_chunk;
-                const int nc = min(c2 - k0, 32);
-                for (int k = 0; k < nc; ++k) {
-                  const int j = s0 + k0 + k;
-                  const float ex = xi - xs[j], ey = yi - ys[j], ez = zi - zs[j];
-                  const float r2s = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
-                  bool take = r2s < hi && j != jskip && j > jmin;
-                  if (act && take && fabsf(r2s - mid) <= bw) take = confirm_pair_fp64(g, tt, x, ld, gi, t, g0 + (j - s0), t2, A.rl2);
-                  ring_push(rp, (unsigned)j << shift, take);
-                }
+                rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, own ? a : -1, -1, rp_seg, s0 + k0,
+                                        ncand, tt.gstart[t2] + k0, t2, SHIFT);
               }
             }
           }
+        }
       // last words: complete ones, then the partial one padded with the dummy code
       flush();
       const int rem = (int)(rp - rbase) >> 1;   // 0..7
       if (rem) {
-        uint4 v = lds_u4(rbase);
-        unsigned h[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-        for (int p = 0; p < 8; ++p)
-          if (p >= rem) h[p >> 1] = (p & 1) ? ((h[p >> 1] & 0xffffu) | (dummy << 16)) : ((h[p >> 1] & 0xffff0000u) | dummy);
-        v.x = h[0]; v.y = h[1]; v.z = h[2]; v.w = h[3];
+        for (int p = rem; p < 8; ++p) sts_u16(rbase + 2 * p, dummy);
         const int before = nwords;
-        store_word(v);
+        store_word(lds_u4(rbase));
         nwords = before;   // count below from complete words + rem
       }
       const int n = nwords * 8 + rem;
@@ -980,13 +1126,18 @@ __device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
 // ---------------------------------------------------------------------------------------------------
 template <typename T, class Body>
 __device__ __forceinline__ void list_loop(const Body& body, unsigned st_base, const uint4* __restrict__ words, size_t word_stride,
-                                          int nwords, typename Vec4<T>::type pi, double (&tot)[Body::NT]) {
+                                          int nwords, typename Vec4<T>::type pi, double (&tot)[Body::NT], uint4 w0, bool have_w0) {
   constexpr int NT = Body::NT;
   if (nwords <= 0) return;
-  uint4 w = ld_stream(words);
+  // two words in flight ahead of the one being processed: a word is ~200 issue slots of work for the warp,
+  // less than one DRAM round trip when the SM is busy with other warps
+  uint4 w = have_w0 ? w0 : ld_stream(words);
+  uint4 wn = w;
+  if (nwords > 1) wn = ld_stream(words + word_stride);
   for (int c = 0; c < nwords; ++c) {
     const uint4 cur = w;
-    if (c + 1 < nwords) w = ld_stream(words + (size_t)(c + 1) * word_stride);
+    w = wn;
+    if (c + 2 < nwords) wn = ld_stream(words + (size_t)(c + 2) * word_stride);
     T p[NT];
 #pragma unroll
     for (int k = 0; k < NT; ++k) p[k] = (T)0;
@@ -1017,7 +1168,7 @@ __device__ __forceinline__ void list_loop(const Body& body, unsigned st_base, co
 // Staging: the tile's cells (interior + one-cell halo) are contiguous runs of the packed array, so each
 // is ONE TMA bulk copy (cp.async.bulk, <= 125 per tile, all in flight at once, one mbarrier); a second
 // pass in shared memory adds each cell's offset from the tile centre (periodic image included).
-// Shared memory: TileTables | st[capA] Vec4<T> | scell[interior_cap] u16 | (HALF: sgid[capA] int)
+// Shared memory: TileTables | st[capA] Vec4<T> | offs[tile cells] Vec4<T> | scell[interior_cap] u16 | qcell[quads] u16 | (HALF: sgid[capA] int)
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int force_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
 
@@ -1031,8 +1182,10 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
   const Geom& g = A.g;
   const int capA = force_capA(g);
   V4* st = reinterpret_cast<V4*>(smem_raw + sizeof(TileTables));
-  unsigned short* scell = reinterpret_cast<unsigned short*>(st + capA);
-  int* sgid = reinterpret_cast<int*>(scell + g.interior_cap);   // HALF only
+  V4* offs = st + capA;                                           // per tile cell: offset of its atoms from the tile centre
+  unsigned short* scell = reinterpret_cast<unsigned short*>(offs + tile_tab_cells(g));
+  unsigned short* qcell = scell + g.interior_cap;                 // per quad of staged slots: its tile cell
+  int* sgid = reinterpret_cast<int*>(qcell + ((tile_tab_quads(g) + 7) & ~7));   // HALF only
   __shared__ double red[8 * 32];
   __shared__ __align__(8) unsigned long long mbar_storage;
   const unsigned mbar = smem_addr(&mbar_storage);
@@ -1041,36 +1194,56 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
   tile_load(g, tileid, A.tab, tt);
   const int icap = g.interior_cap;
   const unsigned st_base = smem_addr(st);
+  int n_first = 0;
+  uint4 w_first = make_uint4(0, 0, 0, 0);
   {
     const V4* __restrict__ xr = reinterpret_cast<const V4*>(A.xr);
-    if (threadIdx.x == 0) mbar_expect_tx(mbar, (unsigned)A.tab[(size_t)tileid * tile_tab_stride(g) + 4] * (unsigned)sizeof(V4));
+    const int* __restrict__ htab = A.tab + (size_t)tileid * tile_tab_stride(g);
+    if (threadIdx.x == 0) mbar_expect_tx(mbar, (unsigned)htab[4] * (unsigned)sizeof(V4));
     for (int t = threadIdx.x; t < tt.ntc; t += blockDim.x) {
       const int c = tt.cnt[t];
       if (c > 0) bulk_g2s(st_base + (unsigned)tt.start[t] * (unsigned)sizeof(V4), xr + tt.gstart[t], (unsigned)c * (unsigned)sizeof(V4), mbar);
-    }
-    mbar_wait(mbar, 0);
-    // offsets, pad slots, slot -> cell map
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int t = wid; t < tt.ntc; t += nw) {
-      const int c = tt.cnt[t], c4 = pad4(c);
-      if (c4 == 0) continue;
       double offd[3];
       tile_cell_offset_rel(g, tt, t, offd);
-      const T o0 = (T)offd[0], o1 = (T)offd[1], o2 = (T)offd[2];
-      const int s0 = tt.start[t];
+      offs[t] = make_v4<T>((T)offd[0], (T)offd[1], (T)offd[2], (T)0);
+    }
+    // while the bulk copies fly: this thread's row length and first list word of the first round, ...
+    if constexpr (!HALF) {
+      if ((int)threadIdx.x < icap * K) {
+        n_first = A.numneigh[(size_t)tileid * icap + threadIdx.x / K];
+        w_first = ld_stream(A.list + (size_t)tileid * g.chunk_cap * ((size_t)icap * K) + threadIdx.x);
+      }
+    }
+    // ... and the quad -> tile cell map of this tile
+    const int nq = tt.n_slots >> 2;
+    {
+      const unsigned* __restrict__ qsrc = reinterpret_cast<const unsigned*>(htab + TILE_HDR + 3 * tile_tab_cells(g));
+      unsigned* qdst = reinterpret_cast<unsigned*>(qcell);
+      for (int k = threadIdx.x; k < (nq + 1) >> 1; k += blockDim.x) qdst[k] = qsrc[k];
+    }
+    __syncthreads();
+    mbar_wait(mbar, 0);
+    // offsets, pad slots, slot -> cell map: one thread per quad of slots
+    for (int q = threadIdx.x; q < nq; q += blockDim.x) {
+      const int t = qcell[q];
+      const int c = tt.cnt[t], k0 = 4 * q - tt.start[t];
+      const V4 o = offs[t];
       const bool interior = (tt.meta[t] >> 24) != 0;
-      for (int k = lane; k < c4; k += 32) {
-        const int slot = s0 + k;
-        if (k < c) {
-          V4 q = st[slot];
-          q.x += o0; q.y += o1; q.z += o2;
-          st[slot] = q;
+      unsigned sc[2] = {0xffffffffu, 0xffffffffu};
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int slot = 4 * q + u;
+        if (k0 + u < c) {
+          V4 v = st[slot];
+          v.x += o.x; v.y += o.y; v.z += o.z;
+          st[slot] = v;
+          sc[u >> 1] = (u & 1) ? ((sc[u >> 1] & 0xffffu) | ((unsigned)t << 16)) : ((sc[u >> 1] & 0xffff0000u) | (unsigned)t);
         } else {
           st[slot] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);
         }
-        if (interior) scell[slot] = k < c ? (unsigned short)t : (unsigned short)0xffffu;
-        if constexpr (HALF) sgid[slot] = k < c ? tt.gstart[t] + k : 0;
+        if constexpr (HALF) sgid[slot] = k0 + u < c ? tt.gstart[t] + k0 + u : 0;
       }
+      if (interior) *reinterpret_cast<uint2*>(scell + 4 * q) = make_uint2(sc[0], sc[1]);
     }
     if (threadIdx.x == 0) st[tt.n_slots] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);   // the dummy slot
   }
@@ -1095,11 +1268,26 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
     if (active) {
       V4 pi = st[a];
       pi.w = -pi.w;
-      const int n = A.numneigh[(size_t)tileid * icap + a];
+      const int n = (!HALF && base == 0) ? n_first : A.numneigh[(size_t)tileid * icap + a];
       const int nq = (n + 7) >> 3;                          // words of this atom
       if constexpr (!HALF) {
+        if constexpr (MODE == 0) {
+          if (A.epi != EPI_FORCES) {   // the epilogue's operands: start them towards L2 now
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + gi));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + ld + gi));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + 2 * ld + gi));
+            if (A.epi == EPI_KICK_DRIFT) {
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x + ld + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x + 2 * ld + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x0 + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x0 + ld + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x0 + 2 * ld + gi));
+            }
+          }
+        }
         const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
-        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi, tot);
+        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi, tot, w_first, base == 0);
       } else {
         // half list: each in-range pair once; +F to i (registers), -F to j (atomics)
         for (int c = 0; c < nq; ++c) {
@@ -1172,7 +1360,10 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
   }
   if constexpr (MODE == 0 && !HALF) {
     if (A.epi == EPI_KICK_DRIFT) {   // a4: device-side max-displacement reduction
-      block_max_to_flag(d2max, red, &A.flags->max_disp2_bits[1 - A.parity]);
+      // only a displacement beyond the trigger matters to the next step (list_is_stale), so a warp reports its
+      // maximum only then: no block barrier at the end of the kernel, and in most steps no atomic at all
+      for (int o = 16; o > 0; o >>= 1) d2max = fmax(d2max, __shfl_xor_sync(0xffffffffu, d2max, o));
+      if ((threadIdx.x & 31) == 0 && d2max > A.trigger) atomic_max_double_bits(&A.flags->max_disp2_bits[1 - A.parity], d2max);
     }
     if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
   }
