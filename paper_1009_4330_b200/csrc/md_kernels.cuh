@@ -22,7 +22,10 @@ constexpr int MAX_TILE_CELLS = 216;    // (b+2)^3 <= 216  =>  b <= 4
 constexpr int BUILD_THREADS = 256;     // threads per block of the list-build and cell-list kernels
 constexpr int FORCE_MAX_THREADS = 640; // upper bound of the force kernels' block size (runtime choice)
 constexpr int FORCE_MIN_BLOCKS = 2;    // resident blocks per SM the mixed-precision force kernels are compiled for (<= 48 registers)
-constexpr int BUILD_MIN_BLOCKS = 3;    // resident blocks per SM the list-build kernel is compiled for (<= 85 registers)
+#ifndef MDK_BUILD_MIN_BLOCKS
+#define MDK_BUILD_MIN_BLOCKS 3
+#endif
+constexpr int BUILD_MIN_BLOCKS = MDK_BUILD_MIN_BLOCKS;    // resident blocks per SM the list-build kernel is compiled for (<= 85 registers)
 constexpr int BUILD_TASK_INTS = 72;     // list-build: room for the first-task table of <= 64 interior cells (+1), 16-byte multiple
 constexpr int RING = 48;               // list-build: pending entries a lane can hold in shared memory (>= 32 + 8)
 constexpr int RING_STRIDE = RING * 2 + 16;   // bytes between the rings of neighbouring lanes (odd * 16)
@@ -178,16 +181,19 @@ __device__ __forceinline__ void block_max_to_flag(double v, double* red, unsigne
 
 // ---------------------------------------------------------------------------------------------------
 // tile staging, shared by the list build, every force kernel and the list export.
-// Staged slot order: the tile's interior cells first (in their global = brick order), then the halo
-// cells in tile scan order; every cell is padded to a multiple of 4 slots (pad slots hold a far-away
-// point), so that a cell's coordinates can be read four at a time with aligned 128-bit loads.
-// Interior slot a is also the list row of that atom.
+// Staged slot order: the tile's cells (interior + halo) in tile scan order, x fastest; every cell is padded to a
+// multiple of 4 slots (pad slots hold a far-away point), so that a cell's coordinates can be read four at a time
+// with aligned 128-bit loads, and the three x-neighbours of a stencil row are ONE contiguous run of slots.
+// List rows number the interior atoms only (same cell order, same padding): row = rstart[t] + k for atom k of
+// interior tile cell t, whose staged slot is start[t] + k.
 // ---------------------------------------------------------------------------------------------------
 struct alignas(16) TileTables {   // lives in shared memory
   int start[MAX_TILE_CELLS];  // staged slot of the first atom of tile cell t (multiple of 4)
   int gstart[MAX_TILE_CELLS]; // global (sorted) index of the first atom of tile cell t
   int cnt[MAX_TILE_CELLS];    // atoms in tile cell t
   int meta[MAX_TILE_CELLS];   // tx | ty << 8 | tz << 16 | interior << 24   (filled by tile_load only)
+  int rstart[MAX_TILE_CELLS]; // interior cells: list row of the cell's first atom (multiple of 4); rows number the
+                              // interior atoms only, in the same cell order
   int c0[3], w[3], tc[3];     // first interior cell, interior width, tile width (w+2)
   int ntc;                    // tc[0]*tc[1]*tc[2]
   int nic;                    // interior cells w[0]*w[1]*w[2]
@@ -238,52 +244,45 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
     tt.cnt[t] = cell_start[oid + 1] - s;
   }
   __syncthreads();
-  // two exclusive scans of the padded counts by warp 0: interior cells in brick order, then halo cells
+  // two exclusive scans of the padded counts by warp 0: all tile cells in scan order (slots), interior cells (rows)
   if (tid < 32) {
-    const int nic = tt.nic;
-    int per = (nic + 31) / 32, lo = tid * per, hi = min(lo + per, nic), sum = 0;
-    for (int ic = lo; ic < hi; ++ic) sum += pad4(tt.cnt[interior_tile_cell(tt, ic)]);
-    int incl = sum;
+    int per = (ntc + 31) / 32, lo = tid * per, hi = min(lo + per, ntc), sum = 0, isum = 0;
+    for (int t = lo; t < hi; ++t) {
+      const int c4 = pad4(tt.cnt[t]);
+      sum += c4;
+      if (tile_cell_is_interior(tt, t)) isum += c4;
+    }
+    int incl = sum, iincl = isum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      int u = __shfl_up_sync(0xffffffffu, incl, o);
-      if (tid >= o) incl += u;
+      int u = __shfl_up_sync(0xffffffffu, incl, o), v = __shfl_up_sync(0xffffffffu, iincl, o);
+      if (tid >= o) { incl += u; iincl += v; }
     }
-    int run = incl - sum;
-    for (int ic = lo; ic < hi; ++ic) {
-      int t = interior_tile_cell(tt, ic);
+    int run = incl - sum, irun = iincl - isum;
+    for (int t = lo; t < hi; ++t) {
+      const int c4 = pad4(tt.cnt[t]);
       tt.start[t] = run;
-      run += pad4(tt.cnt[t]);
+      run += c4;
+      if (tile_cell_is_interior(tt, t)) { tt.rstart[t] = irun; irun += c4; } else tt.rstart[t] = 0;
     }
-    const int n_int = __shfl_sync(0xffffffffu, incl, 31);
-    per = (ntc + 31) / 32; lo = tid * per; hi = min(lo + per, ntc); sum = 0;
-    for (int t = lo; t < hi; ++t) sum += tile_cell_is_interior(tt, t) ? 0 : pad4(tt.cnt[t]);
-    incl = sum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      int u = __shfl_up_sync(0xffffffffu, incl, o);
-      if (tid >= o) incl += u;
-    }
-    run = n_int + incl - sum;
-    for (int t = lo; t < hi; ++t)
-      if (!tile_cell_is_interior(tt, t)) { tt.start[t] = run; run += pad4(tt.cnt[t]); }
-    if (tid == 31) { tt.n_int_slots = n_int; tt.n_slots = n_int + incl; }
+    if (tid == 31) { tt.n_int_slots = iincl; tt.n_slots = incl; }
   }
   __syncthreads();
 }
 
 // ---------------------------------------------------------------------------------------------------
 // The tables above are computed ONCE per list build by k_tile_tables and kept in global memory
-// (TILE_HDR ints of header + three ints {gstart, start<<16 | cnt, meta} per tile cell); every tile kernel
+// (TILE_HDR ints of header + four ints {gstart, start<<16 | cnt, meta, rstart} per tile cell); every tile kernel
 // launched between two builds only loads them (tile_load: one coalesced read, one barrier).
 // ---------------------------------------------------------------------------------------------------
+constexpr int TILE_CELL_INTS = 4;   // ints per tile cell in the table
 constexpr int TILE_HDR = 8;   // n_int_slots, n_slots, n_int_atoms, brick_start, n_staged_atoms, pad x3
 __host__ __device__ inline int tile_tab_cells(const Geom& g) { return ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) + 3) & ~3; }
 // after the per-cell ints: one u16 per QUAD of staged slots (cells are padded to 4 slots, so a quad belongs to
 // one tile cell) = the tile cell of that quad; lets the force kernel post-process the staged tile slot-parallel
 __host__ __device__ inline int tile_tab_quads(const Geom& g) { return (g.tile_cap >> 2) + 2; }
 __host__ __device__ inline int tile_tab_stride(const Geom& g) {
-  return TILE_HDR + 3 * tile_tab_cells(g) + ((tile_tab_quads(g) + 1) >> 1);
+  return TILE_HDR + TILE_CELL_INTS * tile_tab_cells(g) + ((tile_tab_quads(g) + 1) >> 1);
 }
 
 __device__ __forceinline__ void tile_dims(const Geom& g, int tile, int c0[3], int w[3]) {
@@ -315,6 +314,7 @@ __device__ __forceinline__ void tile_load(const Geom& g, int tile, const int* __
     tt.start[t] = (int)(sc >> 16);
     tt.cnt[t] = (int)(sc & 0xffffu);
     tt.meta[t] = h[TILE_HDR + 2 * tcs + t];
+    tt.rstart[t] = h[TILE_HDR + 3 * tcs + t];
   }
   __syncthreads();
 }
@@ -332,8 +332,9 @@ __global__ void __launch_bounds__(128) k_tile_tables(Geom g, const int* __restri
     h[TILE_HDR + t] = tt.gstart[t];
     h[TILE_HDR + tcs + t] = (int)(((unsigned)tt.start[t] << 16) | ((unsigned)tt.cnt[t] & 0xffffu));
     h[TILE_HDR + 2 * tcs + t] = tx | ty << 8 | tz << 16 | (tile_cell_is_interior(tt, t) ? 1 << 24 : 0);
+    h[TILE_HDR + 3 * tcs + t] = tt.rstart[t];
     staged += tt.cnt[t];
-    unsigned short* qc = reinterpret_cast<unsigned short*>(h + TILE_HDR + 3 * tcs);
+    unsigned short* qc = reinterpret_cast<unsigned short*>(h + TILE_HDR + TILE_CELL_INTS * tcs);
     const int q0 = tt.start[t] >> 2, q1 = min((tt.start[t] + pad4(tt.cnt[t])) >> 2, tile_tab_quads(g));
     for (int q = q0; q < q1; ++q) qc[q] = (unsigned short)t;
   }
@@ -657,23 +658,26 @@ __device__ __forceinline__ void ring_push(unsigned& rp, unsigned code, bool take
                : "memory");
 }
 
-// The careful scan of `ncand` candidates starting at staged slot j0 of tile cell t2 (global index g0 at j0) for
-// the lane's atom (tile-centred position xi, yi, zi; global index gi; tile cell t; act: the lane holds an atom):
-// the same fp32 accept test as the fast loop, plus the exclusions (never slot jskip, only slots > jmin), plus an
-// fp64 decision from the global positions for every candidate inside the guard band.  Used for the own cell of a
-// half list and to redo a segment in which the fast loop saw an in-band candidate.  Everything is passed by value
-// or lives in shared memory (gs: a shared copy of the geometry), so the kernel keeps no stack frame for it.
+// The careful scan of the `nslot` staged slots from j0 on (a piece of a run of consecutive tile cells; tc is a
+// cell at or before the one holding j0) for the lane's atom (tile-centred position xi, yi, zi; global index gi;
+// tile cell t; act: the lane holds an atom): the same fp32 accept test as the fast loop, plus the exclusions
+// (never slot jskip, only slots > jmin), plus an fp64 decision from the global positions for every candidate
+// inside the guard band.  Used for the own cell of a half list and to redo a piece in which the fast loop saw
+// an in-band candidate.  Everything is passed by value or lives in shared memory (gs: a shared copy of the
+// geometry), so the kernel keeps no stack frame for it.
 struct BuildBand { double rl2; float hi, mid, bw; };
 __device__ __noinline__ unsigned build_scan_careful(const Geom& gs, const TileTables& tt, const double* __restrict__ x, size_t ld,
                                                     BuildBand bd, const float* xs, const float* ys, const float* zs, float xi, float yi,
                                                     float zi, int act, int gi, int t, int jskip, int jmin, unsigned rp, int j0,
-                                                    int ncand, int g0, int t2, int shift) {
-  for (int k = 0; k < ncand; ++k) {
-    const int j = j0 + k;
+                                                    int nslot, int tc, int shift) {
+  for (int j = j0; j < j0 + nslot; ++j) {
+    while (j >= tt.start[tc] + pad4(tt.cnt[tc])) ++tc;
+    const int k = j - tt.start[tc];
     const float ex = xi - xs[j], ey = yi - ys[j], ez = zi - zs[j];
     const float r2s = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
-    bool take = r2s < bd.hi && j != jskip && j > jmin;
-    if (act && take && fabsf(r2s - bd.mid) <= bd.bw) take = confirm_pair_fp64(gs, tt, x, ld, gi, t, g0 + k, t2, bd.rl2);
+    bool take = r2s < bd.hi && j != jskip && j > jmin;     // pad slots (k >= cnt) are far away: never taken
+    if (act && take && k < tt.cnt[tc] && fabsf(r2s - bd.mid) <= bd.bw)
+      take = confirm_pair_fp64(gs, tt, x, ld, gi, t, tt.gstart[tc] + k, tc, bd.rl2);
     ring_push(rp, (unsigned)j << shift, take);
   }
   return rp;
@@ -755,7 +759,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_BLOCKS) k_build_list(
   __syncthreads();
   {
     const unsigned short* __restrict__ qc =
-        reinterpret_cast<const unsigned short*>(A.tab + (size_t)tile * tile_tab_stride(g) + TILE_HDR + 3 * tile_tab_cells(g));
+        reinterpret_cast<const unsigned short*>(A.tab + (size_t)tile * tile_tab_stride(g) + TILE_HDR + TILE_CELL_INTS * tile_tab_cells(g));
     const int nq = tt.n_slots >> 2;
     for (int q = threadIdx.x; q < nq; q += blockDim.x) {
       const int t = qc[q];
@@ -802,16 +806,18 @@ __global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_BLOCKS) k_build_list(
   for (int task = wid; task < ntasks; task += nw) {
     while (task0[ic + 1] <= task) ++ic;
     const int t = interior_tile_cell(tt, ic);
-    const int s_lo = tt.start[t], c = tt.cnt[t], g_lo = tt.gstart[t];
+    const int c = tt.cnt[t], g_lo = tt.gstart[t];
     {
       const int r0 = (task - task0[ic]) << 5;
       const bool act = r0 + lane < c;
-      const int a = act ? s_lo + r0 + lane : s_lo;   // staged slot = list row
+      const int kin = act ? r0 + lane : 0;
+      const int a = tt.rstart[t] + kin;             // list row
+      const int aslot = tt.start[t] + kin;          // staged slot
       const int gi = g_lo + r0 + lane;
       // an idle lane sits far away from everything, pad slots (+1e15) included: it accepts nothing
-      const float xi = act ? xs[a] : -1e15f, yi = act ? ys[a] : -1e15f, zi = act ? zs[a] : -1e15f;
+      const float xi = act ? xs[aslot] : -1e15f, yi = act ? ys[aslot] : -1e15f, zi = act ? zs[aslot] : -1e15f;
       const f32x2 xi2 = pack2(xi, xi), yi2 = pack2(yi, yi), zi2 = pack2(zi, zi);
-      const unsigned selfcode = (unsigned)a << SHIFT;
+      const unsigned selfcode = (unsigned)aslot << SHIFT;
       unsigned rp = rbase;
       int nwords = 0;
       auto store_word = [&](uint4 v) {
@@ -827,41 +833,50 @@ __global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_BLOCKS) k_build_list(
         if (full) sts_u4(rbase, lds_u4(rbase + 16 * full));
         rp = rbase + 2 * (pend & 7);
       };
+      // Full list: 9 runs, one per (dy, dz): the cells x-1, x, x+1 are consecutive tile cells, hence one contiguous
+      // range of staged slots (pad slots in between are far away and never taken).  Half list: 27 one-cell runs,
+      // because a whole cell is kept or dropped (below).
+      constexpr int NRUN = HALF ? 27 : 9;
 #pragma unroll 1
-      for (int sc = 0; sc < 27; ++sc) {
-          {
-            const int t2 = t + soff[sc];          // the 27 cells around tile cell t
-            const int s0 = tt.start[t2], c2 = tt.cnt[t2];
-            const bool own = t2 == t;
-            // half list: keep (i, j) iff j follows i in the sorted order; a cell is a contiguous range of that
-            // order, so for another cell the answer is the same for all of its atoms
-            if (HALF && !own && tt.gstart[t2] < g_lo) continue;
+      for (int sc = 0; sc < NRUN; ++sc) {
+        int tfirst, s0, s1;
+        bool own;
+        if constexpr (HALF) {
+          tfirst = t + soff[sc];
+          own = tfirst == t;
+          // keep (i, j) iff j follows i in the sorted order; a cell is a contiguous range of that order, so for
+          // another cell the answer is the same for all of its atoms
+          if (!own && tt.gstart[tfirst] < g_lo) continue;
+          s0 = tt.start[tfirst];
+          s1 = s0 + pad4(tt.cnt[tfirst]);
+        } else {
+          const int tc = t + soff[3 * sc + 1];
+          tfirst = tc - 1;
+          own = sc == 4;
+          s0 = tt.start[tc - 1];
+          s1 = tt.start[tc + 1] + pad4(tt.cnt[tc + 1]);
+        }
 #pragma unroll 1
-            for (int k0 = 0; k0 < c2; k0 += 32) {   // segments of <= 32 candidates: what the ring is guaranteed to take
-              if ((int)(rp - rbase) > 2 * (RING - 32)) flush();
-              const int ncand = min(c2 - k0, 32);
-              if (HALF && own) {
-                // own cell: slot order is the sorted order
-                rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, a, a, rp, s0 + k0, ncand,
-                                        tt.gstart[t2] + k0, t2, SHIFT);
-                continue;
-              }
-              const unsigned rp_seg = rp;
-              const int nq = (ncand + 3) >> 2;
-              const unsigned off = 4u * (unsigned)(s0 + k0);
-              const unsigned code = (unsigned)(s0 + k0) << SHIFT;
-              float m = 1e30f;
-              if (own) build_scan_fast<true, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, xi2, yi2, zi2, mid2, hi, selfcode);
-              else build_scan_fast<false, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, xi2, yi2, zi2, mid2, hi, selfcode);
-              if (__builtin_expect(m <= bw, 0)) {
-                // some candidate of this segment lies in the guard band of the fp32 test: redo the segment, deciding
-                // the in-band candidates in fp64 from the global positions (the pair set is exactly the fp64 one)
-                rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, own ? a : -1, -1, rp_seg, s0 + k0,
-                                        ncand, tt.gstart[t2] + k0, t2, SHIFT);
-              }
-            }
+        for (int j0 = s0; j0 < s1; j0 += 32) {   // pieces of <= 32 slots: what the ring is guaranteed to take
+          if ((int)(rp - rbase) > 2 * (RING - 32)) flush();
+          const int nq = min(8, (s1 - j0) >> 2);
+          if (HALF && own) {
+            // own cell: slot order is the sorted order
+            rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, aslot, aslot, rp, j0, 4 * nq, tfirst, SHIFT);
+            continue;
+          }
+          const unsigned rp_seg = rp;
+          float m = 1e30f;
+          if (own) build_scan_fast<true, SHIFT>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
+          else build_scan_fast<false, SHIFT>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
+          if (__builtin_expect(m <= bw, 0)) {
+            // some candidate of this piece lies in the guard band of the fp32 test: redo the piece, deciding the
+            // in-band candidates in fp64 from the global positions (the pair set is exactly the fp64 one)
+            rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, own ? aslot : -1, -1, rp_seg, j0, 4 * nq,
+                                    tfirst, SHIFT);
           }
         }
+      }
       // last words: complete ones, then the partial one padded with the dummy code
       flush();
       const int rem = (int)(rp - rbase) >> 1;   // 0..7
@@ -908,7 +923,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_export_list(Geom g, const int
   for (int ic = 0; ic < tt.nic; ++ic) {
     const int t = interior_tile_cell(tt, ic);
     for (int k = threadIdx.x; k < tt.cnt[t]; k += blockDim.x) {
-      const int a = tt.start[t] + k, n = numneigh[(size_t)tile * g.interior_cap + a], io = sid[a];
+      const int a = tt.rstart[t] + k, n = numneigh[(size_t)tile * g.interior_cap + a], io = sid[tt.start[t] + k];
       nn_out[io] = n;
       for (int e = 0; e < n && e < stride; ++e) {
         int q = e >> 3, s = q % K, c = q / K;
@@ -1217,7 +1232,7 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
     // ... and the quad -> tile cell map of this tile
     const int nq = tt.n_slots >> 2;
     {
-      const unsigned* __restrict__ qsrc = reinterpret_cast<const unsigned*>(htab + TILE_HDR + 3 * tile_tab_cells(g));
+      const unsigned* __restrict__ qsrc = reinterpret_cast<const unsigned*>(htab + TILE_HDR + TILE_CELL_INTS * tile_tab_cells(g));
       unsigned* qdst = reinterpret_cast<unsigned*>(qcell);
       for (int k = threadIdx.x; k < (nq + 1) >> 1; k += blockDim.x) qdst[k] = qsrc[k];
     }
@@ -1243,7 +1258,7 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
         }
         if constexpr (HALF) sgid[slot] = k0 + u < c ? tt.gstart[t] + k0 + u : 0;
       }
-      if (interior) *reinterpret_cast<uint2*>(scell + 4 * q) = make_uint2(sc[0], sc[1]);
+      if (interior) *reinterpret_cast<uint2*>(scell + tt.rstart[t] + k0) = make_uint2(sc[0], sc[1]);   // indexed by list row
     }
     if (threadIdx.x == 0) st[tt.n_slots] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);   // the dummy slot
   }
@@ -1261,12 +1276,13 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
     unsigned cell = 0xffffu;
     if (sidx < nslots) cell = scell[a];
     const bool active = cell != 0xffffu;
-    const int gi = active ? tt.gstart[cell] + (a - tt.start[cell]) : 0;
+    const int kin = active ? a - tt.rstart[cell] : 0;       // index of the atom within its cell
+    const int gi = active ? tt.gstart[cell] + kin : 0;
     double tot[NT];
 #pragma unroll
     for (int k = 0; k < NT; ++k) tot[k] = 0.0;
     if (active) {
-      V4 pi = st[a];
+      V4 pi = st[tt.start[cell] + kin];
       pi.w = -pi.w;
       const int n = (!HALF && base == 0) ? n_first : A.numneigh[(size_t)tileid * icap + a];
       const int nq = (n + 7) >> 3;                          // words of this atom
