@@ -15,8 +15,9 @@ value     whole-job atom-timesteps/s, inputs already resident in HBM (device buf
           md_set_positions / md_set_velocities), CUDA events on the library's stream, max over ranks
 e2e       the same through the C ABI with HOST (pinned) buffers: H2D of x and v, md_run, D2H of the
           final positions and the kinetic energy, every step, inside the timed region
-roofline  dominant kernel = the pair-force tile kernel; algorithmic bytes per launch / its mean launch
-          duration (CUDA events inside md_run, sampled steps of the timed region)
+roofline  dominant kernel = the pair-force tile kernel; SURVEY.md 8(d)'s algorithmic bytes per launch / its
+          mean launch duration (CUDA events on the library's stream inside md_run, sampled steps of the
+          timed region); traffic = measured DRAM bytes per launch from profiles/traffic.json
 cpu_baseline   the oracle (oracle/md_oracle.c, as it stands) on the host cores, bounded sample
 
 N > 1: independent replicas, one per GPU, no data-path collective ("scaling": "weak").
@@ -114,24 +115,24 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------
 # algorithmic bytes of the dominant kernel: the pair-force tile kernel
 # ---------------------------------------------------------------------------------------------------------
-def force_kernel_bytes(natoms: int, mean_neighbors: float, style: int) -> float:
-    """Bytes one force evaluation MUST move with this library's data layout, per launch group:
-    per atom: the neighbor-index stream (16-bit tile-local indices: 2 B per list entry), numneigh (4 B),
-    the atom's own fp64 position (24 B) and the fp64 force store (24 B).  Halo re-staging, padding of the
-    128-bit index words and L2 re-reads are NOT counted (they are waste, visible in ``traffic``).
-    EAM runs two list passes: indices + numneigh + positions twice, plus rho/F' stores (16 B) and the F'
-    read (8 B) instead of one force store.  SURVEY.md §8(d) charges a classic int32 list at 4 B per
-    entry; that figure is reported beside this one as ``survey_bytes``."""
-    per_atom = 2.0 * mean_neighbors + 4 + 24 + 24
-    if style == wl.PAIR_EAM:
-        per_atom = 2 * (2.0 * mean_neighbors + 4 + 24) + 16 + 8 + 24
-    return per_atom * natoms
-
-
 def survey_force_bytes(natoms: int, mean_neighbors: float, style: int) -> float:
+    """ALGORITHMIC bytes of one force evaluation as SURVEY.md §8(d) charges them: per atom the
+    neighbor-index stream at 4 B per full-list entry, numneigh (4 B), the atom's own fp64 position (24 B) and
+    the fp64 force store (24 B); gathered neighbor positions are charged to cache, not HBM (the optimistic
+    ceiling of §8(d), which the measured DRAM traffic confirms).  EAM runs two list passes: indices +
+    numneigh + own position twice, plus the rho / F' stores (16 B) and the F' read (8 B)."""
     per_atom = 4.0 * mean_neighbors + 4 + 24 + 24
     if style == wl.PAIR_EAM:
         per_atom = 2 * (4.0 * mean_neighbors + 4 + 24) + 16 + 8 + 24
+    return per_atom * natoms
+
+
+def layout_force_bytes(natoms: int, mean_neighbors: float, style: int) -> float:
+    """The same with THIS library's list layout (16-bit tile-local slot codes: 2 B per entry) -- what the
+    kernel itself must move; reported beside the SURVEY figure, never as ``achieved``."""
+    per_atom = 2.0 * mean_neighbors + 4 + 24 + 24
+    if style == wl.PAIR_EAM:
+        per_atom = 2 * (2.0 * mean_neighbors + 4 + 24) + 16 + 8 + 24
     return per_atom * natoms
 
 
@@ -268,9 +269,9 @@ def run_ours(args, rk) -> None:
     # roofline of the dominant kernel: sampled force launches inside the timed md_run
     nf = max(1, st["nforce_sampled"])
     ms_force = st["ms_force_sampled"] / nf
-    fbytes = force_kernel_bytes(w.natoms, st["mean_neighbors"], w.style)
     sbytes = survey_force_bytes(w.natoms, st["mean_neighbors"], w.style)
-    achieved = fbytes / (ms_force * 1e-3) / 1e9 if ms_force > 0 else 0.0
+    lbytes = layout_force_bytes(w.natoms, st["mean_neighbors"], w.style)
+    achieved = sbytes / (ms_force * 1e-3) / 1e9 if ms_force > 0 else 0.0
     nruns = max(1, args.steps)
     ms_per_step = 1e3 * tmax / nruns
     roofline = {
@@ -278,11 +279,15 @@ def run_ours(args, rk) -> None:
         "traffic": None, "peak_source": peak_src,
         "kernel": "k_tile_force<%s,%s,K=%d>" % ("float" if w.precision == wl.PREC_MIXED else "double",
                                                  "LJ" if w.style == wl.PAIR_LJ else "EAM density+force", st["lanes_per_atom"]),
-        "algorithmic_bytes_per_launch": fbytes, "survey_bytes_per_launch": sbytes,
-        "achieved_with_survey_bytes": sbytes / (ms_force * 1e-3) / 1e9 if ms_force > 0 else 0.0,
+        "algorithmic_bytes_per_launch": sbytes,
+        "algorithmic_bytes_definition": "SURVEY.md 8(d): (4 B x list entries + 52 B) per atom (EAM: two passes), DESIGN.md 6",
+        "own_layout_bytes_per_launch": lbytes,
+        "achieved_with_own_layout_bytes": lbytes / (ms_force * 1e-3) / 1e9 if ms_force > 0 else 0.0,
         "ms_per_launch": ms_force, "launches_sampled": st["nforce_sampled"],
         "share_of_step": {"force": ms_force * w.nsteps / (1e3 * tmax / nruns) if tmax > 0 else None,
                           "build": st["ms_build_in_run"] / (1e3 * tmax / nruns) if tmax > 0 else None},
+        "binding_resource_measured": "shared-memory data pipe (random 128-bit gathers of staged neighbor positions), "
+                                     "see profiles/ and DESIGN.md 6",
     }
     if not rk.is_root:
         return
@@ -290,6 +295,7 @@ def run_ours(args, rk) -> None:
     try:
         with open(traffic_file) as fh:
             roofline["traffic"] = json.load(fh).get("cfg%d" % args.cfg, {}).get("dram_bytes_per_launch")
+            roofline["traffic_source"] = "profiles/traffic.json (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
     except Exception:
         pass
     per_config = {}
@@ -307,7 +313,7 @@ def run_ours(args, rk) -> None:
                 "ms_per_pass": sum(r["ms"]) / len(r["ms"]), "time_steps": wc.nsteps, "builds": sc["nbuilds_in_run"],
                 "variant": md.KERNEL_NAMES[sc["kernel_variant"]], "mean_neighbors": sc["mean_neighbors"],
                 "force_ms_per_launch": msf,
-                "force_GBps": force_kernel_bytes(wc.natoms, sc["mean_neighbors"], wc.style) / (msf * 1e-3) / 1e9 if msf > 0 else None,
+                "force_GBps": survey_force_bytes(wc.natoms, sc["mean_neighbors"], wc.style) / (msf * 1e-3) / 1e9 if msf > 0 else None,
                 "l2_flushed_between_passes": r["flushed_l2"]}
     cpu = oracle_sample(args.cfg) if (rk.world == 1 and not args.no_cpu_baseline) else None
     line = {
