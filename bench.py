@@ -276,6 +276,7 @@ def run_ours(args, rk) -> None:
     ms_per_step = 1e3 * tmax / nruns
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+        "frac_of_nominal_8TBps": achieved / 8000.0,
         "traffic": None, "peak_source": peak_src,
         "kernel": "k_tile_force<%s,%s,K=%d>" % ("float" if w.precision == wl.PREC_MIXED else "double",
                                                  "LJ" if w.style == wl.PAIR_LJ else "EAM density+force", st["lanes_per_atom"]),
@@ -315,6 +316,18 @@ def run_ours(args, rk) -> None:
                 "force_ms_per_launch": msf,
                 "force_GBps": survey_force_bytes(wc.natoms, sc["mean_neighbors"], wc.style) / (msf * 1e-3) / 1e9 if msf > 0 else None,
                 "l2_flushed_between_passes": r["flushed_l2"]}
+        # the paper's comparison (Eq. 1): neighbor-list kernel against the direct cell-list kernel, and
+        # the half list (Newton's third law, atomics), on the bench workload itself
+        for name, kv, lk in (("cell_list", md.MD_KERNEL_CELL, md.MD_LIST_FULL), ("half_list_tpa", md.MD_KERNEL_TPA, md.MD_LIST_HALF)):
+            if w.style != wl.PAIR_LJ:
+                continue
+            r = time_workload(torch, md, w, stream, 1, 1, kv, lk, host_io=False)
+            sc = r["stats"]
+            msf = sc["ms_force_sampled"] / max(1, sc["nforce_sampled"])
+            per_config["cfg%d_%s" % (args.cfg, name)] = {
+                "workload": w.name, "value": w.natoms * w.nsteps * len(r["ms"]) / (sum(r["ms"]) * 1e-3), "unit": UNIT,
+                "ms_per_pass": sum(r["ms"]) / len(r["ms"]), "time_steps": w.nsteps, "builds": sc["nbuilds_in_run"],
+                "variant": md.KERNEL_NAMES[sc["kernel_variant"]], "force_ms_per_launch": msf, "passes_timed": 1}
     cpu = oracle_sample(args.cfg) if (rk.world == 1 and not args.no_cpu_baseline) else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": rk.world, "steps": args.steps, "warmup": args.warmup,

@@ -83,6 +83,47 @@ def test_full_list_pair_set_matches_brute_force(cfg, n, amp, kernel):
     assert st["mean_neighbors"] == pytest.approx(nn.mean(), rel=1e-12)
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("kernel,list_kind", [(1, 0), (2, 0), (1, 1)])
+def test_pairs_at_the_list_radius_are_decided_in_fp64(kernel, list_kind, precision):
+    """The build's distance test runs in fp32 with a guard band; every candidate inside the band must be decided
+    in fp64.  Dimers are planted at r = rl (1 +- d) with d from 1e-5 down to 3e-9 (far inside the fp32 band,
+    outside the 1e-9 exclusion of the comparison), in random orientations, all over a periodic box, so that the
+    partner sits in any of the 27 stencil cells and across the periodic boundary."""
+    rc, skin = 2.5, 0.3
+    rl = rc + skin
+    box = np.array([31.0, 29.0, 33.0])
+    nd = 600
+    ids = np.arange(nd, dtype=np.uint64)
+    centre = np.stack([wl.uniform01(11, ids, c) for c in range(3)], axis=1) * box
+    u = np.stack([wl.gaussian(11, ids, 3 + c) for c in range(3)], axis=1)
+    u /= np.linalg.norm(u, axis=1)[:, None]
+    deltas = np.array([1e-5, 1e-6, 1e-7, 1e-8, 3e-9])
+    d = deltas[np.arange(nd) % 5] * np.where((np.arange(nd) // 5) % 2 == 0, 1.0, -1.0)
+    x = np.concatenate([centre, centre + u * (rl * (1.0 + d))[:, None]])      # partner may lie outside the box
+    N = 2 * nd
+    s = md.System(box, N, np.zeros(N, np.int32), np.array([1.0]))
+    s.md_set_precision(precision)
+    s.md_set_neighbor(list_kind, kernel)
+    s.md_set_pair(md.MD_PAIR_LJ126, (1.0, 1.0), rc, skin)
+    s.md_set_positions(x)
+    s.md_build_neighbors()
+    nn, nb = _gpu_rows(s, N, 64)
+    got = {(min(i, int(j)), max(i, int(j))) for i in range(N) for j in nb[i, :nn[i]]}
+    sure, fuzzy = _oracle_pairs(x, box, rl)
+    assert sure <= got and got <= (sure | fuzzy)
+    # the planted dimers themselves: inside iff d < 0, judged from the fp64 coordinates actually passed in
+    xw = x - np.floor(x / box) * box
+    dd = xw[:nd] - xw[nd:]
+    dd -= box * np.round(dd / box)
+    r = np.sqrt((dd ** 2).sum(axis=1))
+    decided = np.abs(r - rl) > 1e-9
+    assert decided.sum() > 0.9 * nd
+    for k in np.nonzero(decided)[0]:
+        assert ((k, nd + k) in got) == (r[k] < rl), (k, r[k] - rl)
+    s.close()
+
+
 def test_half_list_holds_each_pair_once():
     w, x, s = _system(1, 7, 0.15, md.MD_FP64, md.MD_KERNEL_TPA, list_kind=md.MD_LIST_HALF)
     s.md_build_neighbors()
