@@ -154,9 +154,11 @@ int md_get_forces(md_system* s, double* f);
  * length).  Half lists hold each unordered pair in exactly one of the two rows. */
 int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride);
 
-/* Setup-time mini benchmark of PAPER.md L137: times nrep force evaluations with each of TPA, SUBWARP
- * and WARP on the current positions, keeps the fastest, and reports the three times (ms per
- * evaluation, indexed by MD_KERNEL_TPA..MD_KERNEL_WARP minus 1) if ms_out is not NULL. */
+/* Setup-time mini benchmark of PAPER.md L137: on the current positions, builds the list and times nrep
+ * force evaluations with each of TPA, SUBWARP and WARP, at the planner's tile width and its two
+ * neighbours; keeps the combination with the lowest (force evaluation + 1/8 list build) time, and
+ * reports the best force time of each variant (ms per evaluation, indexed by MD_KERNEL_TPA..MD_KERNEL_WARP
+ * minus 1) if ms_out is not NULL.  MD_KERNEL_AUTO runs it once before the first build. */
 int md_autotune(md_system* s, int nrep, double ms_out[3]);
 
 int md_get_stats(md_system* s, md_stats* out);

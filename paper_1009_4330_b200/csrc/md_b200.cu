@@ -50,6 +50,7 @@ struct md_system_impl {
   int cur = 0;    // buffer of v, id, type (flips at every build)
   int xcur = 0;   // buffer of x (flips at every build and at every fused kick+drift step)
   int force_threads = 256, batch = 8;
+  int brick_forced = 0;   // tile width in cells fixed by the autotuner (0: the planner's choice)
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
   void* xr[2] = {nullptr, nullptr};   // packed cell-relative positions (Vec4<T>, 32 B per atom reserved), buffer index = xcur
   int* tab = nullptr;                 // per-tile tables of the last build
@@ -201,7 +202,7 @@ int plan(md_system* s) {
   double rl = s->rc + s->skin;
   for (int d = 0; d < 3; ++d)
     if (s->box[d] < 3.0 * rl) return fail(s, MD_ERR_BOX_TOO_SMALL, "box edge %d = %g < 3 (rc+skin) = %g", d, s->box[d], 3.0 * rl);
-  int forced = 0;
+  int forced = s->brick_forced;
   if (const char* e = getenv("MD_B200_BRICK")) forced = atoi(e);
   double vol = s->box[0] * s->box[1] * s->box[2];
   double lscale = std::cbrt(vol / (double)s->N);   // ~ nearest-neighbor distance
@@ -484,27 +485,43 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set first");
   if (s->list_kind == MD_LIST_HALF) { s->kernel_eff = MD_KERNEL_TPA; s->autotuned = true; s->planned = false; return MD_OK; }
   if (nrep < 1) nrep = 1;
+  // The setup-time mini benchmark of PAPER.md L137, over lanes per atom (1, 8, 32) and, because the best tile
+  // width depends on how many tiles the box yields, over the planner's width and its two neighbours.  Score of a
+  // candidate: one force evaluation plus an eighth of a list build (a typical rebuild interval).
   const int cand[3] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP};
-  double best_ms = 1e300;
-  int best = MD_KERNEL_TPA;
-  for (int k = 0; k < 3; ++k) {
-    s->kernel_eff = cand[k];
-    s->planned = false;
-    int rc = build(s, true);
-    if (rc) return rc;
-    rc = compute_forces_device(s, false);   // warm-up
-    if (rc) return rc;
-    CK(cudaEventRecord(s->ev0, s->stream));
-    for (int r = 0; r < nrep; ++r) { rc = compute_forces_device(s, false); if (rc) return rc; }
-    CK(cudaEventRecord(s->ev1, s->stream));
-    CK(cudaStreamSynchronize(s->stream));
-    float ms = 0;
-    cudaEventElapsedTime(&ms, s->ev0, s->ev1);
-    double per = ms / nrep;
-    if (ms_out) ms_out[k] = per;
-    if (per < best_ms) { best_ms = per; best = cand[k]; }
+  s->brick_forced = 0;
+  s->kernel_eff = MD_KERNEL_TPA;
+  s->planned = false;
+  int rc = plan(s);
+  if (rc) return rc;
+  const int b0 = std::max(s->g.b[0], std::max(s->g.b[1], s->g.b[2]));
+  double best_score = 1e300;
+  int best = MD_KERNEL_TPA, best_b = 0;
+  if (ms_out) for (int k = 0; k < 3; ++k) ms_out[k] = 1e300;
+  for (int b = std::max(1, b0 - 1); b <= std::min(4, b0 + 1); ++b) {
+    for (int k = 0; k < 3; ++k) {
+      s->kernel_eff = cand[k];
+      s->brick_forced = b == b0 ? 0 : b;
+      s->planned = false;
+      rc = build(s, true);
+      if (rc == MD_ERR_OVERFLOW && b != b0) continue;   // this width does not fit shared memory
+      if (rc) return rc;
+      const double ms_build = s->ms_build;
+      rc = compute_forces_device(s, false);   // warm-up
+      if (rc) return rc;
+      CK(cudaEventRecord(s->ev0, s->stream));
+      for (int r = 0; r < nrep; ++r) { rc = compute_forces_device(s, false); if (rc) return rc; }
+      CK(cudaEventRecord(s->ev1, s->stream));
+      CK(cudaStreamSynchronize(s->stream));
+      float ms = 0;
+      cudaEventElapsedTime(&ms, s->ev0, s->ev1);
+      const double per = ms / nrep, score = per + ms_build / 8.0;
+      if (ms_out && per < ms_out[k]) ms_out[k] = per;
+      if (score < best_score) { best_score = score; best = cand[k]; best_b = s->brick_forced; }
+    }
   }
   s->kernel_eff = best;
+  s->brick_forced = best_b;
   s->autotuned = true;
   s->planned = false;
   s->list_valid = false;
@@ -617,7 +634,7 @@ int md_set_units(md_system* s, double ftm2v, double mvv2e) {
 int md_set_precision(md_system* s, int mode) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (mode != MD_FP64 && mode != MD_MIXED) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_precision: unknown mode %d", mode);
-  if (mode != s->precision) { s->precision = mode; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; }
+  if (mode != s->precision) { s->precision = mode; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->brick_forced = 0; }
   return MD_OK;
 }
 
@@ -650,7 +667,7 @@ int md_set_pair(md_system* s, int style, const double* params, int nparams, doub
   s->style = style;
   for (int k = 0; k < 5; ++k) s->params[k] = k < need ? params[k] : 0.0;
   s->rc = rc; s->skin = skin;
-  s->pair_set = true; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false;
+  s->pair_set = true; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->brick_forced = 0;
   return MD_OK;
 }
 
@@ -664,7 +681,7 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel) {
   s->list_kind = list_kind;
   s->kernel_req = kernel;
   s->kernel_eff = kernel == MD_KERNEL_AUTO ? MD_KERNEL_TPA : kernel;
-  s->autotuned = false;
+  s->autotuned = false; s->brick_forced = 0;
   s->planned = false; s->list_valid = false; s->forces_valid = false;
   return MD_OK;
 }
