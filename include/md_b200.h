@@ -68,11 +68,12 @@ typedef struct md_system md_system; /* opaque */
 #define MD_LIST_HALF 1    /* each pair once; -F scattered to j with atomics (Newton's third law, L76) */
 
 /* force-kernel variants */
-#define MD_KERNEL_AUTO 0     /* setup-time mini benchmark picks among TPA / SUBWARP / WARP (L137) */
+#define MD_KERNEL_AUTO 0     /* setup-time mini benchmark picks among TPA / SUBWARP4 / SUBWARP / WARP (L137) */
 #define MD_KERNEL_TPA 1      /* one thread per atom (L88-104) */
 #define MD_KERNEL_SUBWARP 2  /* 8 lanes per atom, shuffle reduction */
 #define MD_KERNEL_WARP 3     /* 32 lanes per atom, shuffle reduction (the paper's BpA, L105-122) */
 #define MD_KERNEL_CELL 4     /* no list: every atom scans the 27-cell stencil of its tile (L64-82) */
+#define MD_KERNEL_SUBWARP4 5 /* 4 lanes per atom, shuffle reduction: fills the SM when a tile holds few atoms with long rows */
 
 typedef struct md_stats {
   int64_t natoms;
@@ -82,7 +83,7 @@ typedef struct md_stats {
   int32_t kernel_variant;      /* MD_KERNEL_* actually in use (AUTO resolved) */
   int32_t list_kind;
   int32_t precision;
-  int32_t lanes_per_atom;      /* 1, 8 or 32 */
+  int32_t lanes_per_atom;      /* 1, 4, 8 or 32 */
   int32_t ncells[3];           /* cell grid */
   int32_t brick[3];            /* cells per tile edge (interior) */
   int32_t ntiles;              /* thread blocks per force launch */
@@ -155,11 +156,11 @@ int md_get_forces(md_system* s, double* f);
 int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride);
 
 /* Setup-time mini benchmark of PAPER.md L137: on the current positions, builds the list and times nrep
- * force evaluations with each of TPA, SUBWARP and WARP, at the planner's tile width and its two
+ * force evaluations with each of TPA, SUBWARP, WARP and SUBWARP4, at the planner's tile width and its two
  * neighbours; keeps the combination with the lowest (force evaluation + 1/8 list build) time, and
- * reports the best force time of each variant (ms per evaluation, indexed by MD_KERNEL_TPA..MD_KERNEL_WARP
- * minus 1) if ms_out is not NULL.  MD_KERNEL_AUTO runs it once before the first build. */
-int md_autotune(md_system* s, int nrep, double ms_out[3]);
+ * reports the best force time of each variant (ms per evaluation, in the order TPA, SUBWARP, WARP,
+ * SUBWARP4) if ms_out is not NULL.  MD_KERNEL_AUTO runs it once before the first build. */
+int md_autotune(md_system* s, int nrep, double ms_out[4]);
 
 int md_get_stats(md_system* s, md_stats* out);
 const char* md_last_error(const md_system* s); /* s may be NULL: error of a failed md_create */

@@ -50,6 +50,7 @@ struct md_system_impl {
   int cur = 0;    // buffer of v, id, type (flips at every build)
   int xcur = 0;   // buffer of x (flips at every build and at every fused kick+drift step)
   int force_threads = 256, batch = 8;
+  bool force_timing_pending = false;
   int brick_forced = 0;   // tile width in cells fixed by the autotuner (0: the planner's choice)
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
   void* xr[2] = {nullptr, nullptr};   // packed cell-relative positions (Vec4<T>, 32 B per atom reserved), buffer index = xcur
@@ -144,7 +145,7 @@ bool is_device_ptr(const void* p) {
 template <class T>
 cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T)); }
 
-int lanes_for(int kernel) { return kernel == MD_KERNEL_SUBWARP ? 8 : (kernel == MD_KERNEL_WARP ? 32 : 1); }
+int lanes_for(int kernel) { return kernel == MD_KERNEL_SUBWARP ? 8 : (kernel == MD_KERNEL_WARP ? 32 : (kernel == MD_KERNEL_SUBWARP4 ? 4 : 1)); }
 
 // ---- planning: cell grid, tile width, capacities -----------------------------------------------------
 size_t elem_size(const md_system* s) { return s->precision == MD_FP64 ? sizeof(double) : sizeof(float); }
@@ -237,7 +238,7 @@ int plan(md_system* s) {
   {
     double rows = ((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.06 + 8.0;
     double lanes = rows * g.K;
-    int tmax = g.K == 1 ? FORCE_MAX_THREADS : 256;
+    int tmax = FORCE_MAX_THREADS;
     int rounds = (int)std::ceil(lanes / tmax);
     int t = (int)std::ceil(lanes / std::max(rounds, 1));
     t = ((t + 31) / 32) * 32;
@@ -318,6 +319,9 @@ int build_list_only(md_system* s) {
   } else if (g.K == 1) {
     if (s4) CK(launch(s, k_build_list<false, 0, 4>, g.ntiles, BUILD_THREADS, sm, B));
     else CK(launch(s, k_build_list<false, 0, 3>, g.ntiles, BUILD_THREADS, sm, B));
+  } else if (g.K == 4) {
+    if (s4) CK(launch(s, k_build_list<false, 2, 4>, g.ntiles, BUILD_THREADS, sm, B));
+    else CK(launch(s, k_build_list<false, 2, 3>, g.ntiles, BUILD_THREADS, sm, B));
   } else if (g.K == 8) {
     if (s4) CK(launch(s, k_build_list<false, 3, 4>, g.ntiles, BUILD_THREADS, sm, B));
     else CK(launch(s, k_build_list<false, 3, 3>, g.ntiles, BUILD_THREADS, sm, B));
@@ -413,6 +417,8 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
     }
   } else if (g.K == 1) {
     CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
+  } else if (g.K == 4) {
+    CK(launch(s, k_tile_force<T, Body, 4, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
   } else if (g.K == 8) {
     CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
   } else {
@@ -488,7 +494,8 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   // The setup-time mini benchmark of PAPER.md L137, over lanes per atom (1, 8, 32) and, because the best tile
   // width depends on how many tiles the box yields, over the planner's width and its two neighbours.  Score of a
   // candidate: one force evaluation plus an eighth of a list build (a typical rebuild interval).
-  const int cand[3] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP};
+  const int cand[4] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_SUBWARP4};
+  s->force_timing_pending = false;   // ev0 / ev1 are reused below
   s->brick_forced = 0;
   s->kernel_eff = MD_KERNEL_TPA;
   s->planned = false;
@@ -497,9 +504,12 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   const int b0 = std::max(s->g.b[0], std::max(s->g.b[1], s->g.b[2]));
   double best_score = 1e300;
   int best = MD_KERNEL_TPA, best_b = 0;
-  if (ms_out) for (int k = 0; k < 3; ++k) ms_out[k] = 1e300;
-  for (int b = std::max(1, b0 - 1); b <= std::min(4, b0 + 1); ++b) {
-    for (int k = 0; k < 3; ++k) {
+  if (ms_out) for (int k = 0; k < 4; ++k) ms_out[k] = 1e300;
+  // with thousands of tiles the planner's (shared-memory driven) width is right and the SMs are full either way;
+  // the width matters when the box yields few tiles
+  const bool sweep_b = s->g.ntiles < 2048;
+  for (int b = sweep_b ? std::max(1, b0 - 1) : b0; b <= (sweep_b ? std::min(4, b0 + 1) : b0); ++b) {
+    for (int k = 0; k < 4; ++k) {
       s->kernel_eff = cand[k];
       s->brick_forced = b == b0 ? 0 : b;
       s->planned = false;
@@ -674,7 +684,7 @@ int md_set_pair(md_system* s, int style, const double* params, int nparams, doub
 int md_set_neighbor(md_system* s, int list_kind, int kernel) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (list_kind != MD_LIST_FULL && list_kind != MD_LIST_HALF) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown list kind");
-  if (kernel < MD_KERNEL_AUTO || kernel > MD_KERNEL_CELL) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown kernel");
+  if (kernel < MD_KERNEL_AUTO || kernel > MD_KERNEL_SUBWARP4) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown kernel");
   if (list_kind == MD_LIST_HALF && !(kernel == MD_KERNEL_TPA || kernel == MD_KERNEL_AUTO))
     return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: a half list needs MD_KERNEL_TPA");
   if (list_kind == MD_LIST_HALF && s->style == MD_PAIR_EAM_FS) return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
@@ -695,7 +705,7 @@ int md_build_neighbors(md_system* s) {
   return build(s, false);
 }
 
-int md_autotune(md_system* s, int nrep, double ms_out[3]) {
+int md_autotune(md_system* s, int nrep, double ms_out[4]) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   return autotune(s, nrep, ms_out);
 }
@@ -716,7 +726,7 @@ int md_compute_forces(md_system* s, double* f_out, double* energy_out, double vi
     if (energy_out) *energy_out = s->scalars_h[0];
     if (virial_out) for (int k = 0; k < 6; ++k) virial_out[k] = s->scalars_h[1 + k];
   }
-  if (cudaEventQuery(s->ev1) == cudaSuccess) { float ms = 0; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->ms_force = ms; }
+  s->force_timing_pending = true;   // read by md_get_stats once the stream has drained (the call may not have synchronised)
   return MD_OK;
 }
 
@@ -724,6 +734,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (nsteps < 0 || !std::isfinite(dt)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_run: bad nsteps/dt");
   int64_t launches0 = s->launches, builds0 = s->nbuilds;
+  s->force_timing_pending = false;   // ev0 / ev1 are reused below
   s->ms_build_in_run = 0;
   CK(cudaEventRecord(s->ev0, s->stream));
   const bool had_list = s->list_valid;
@@ -891,6 +902,11 @@ int md_get_stats(md_system* s, md_stats* out) {
   CK(cudaMemcpyAsync(s->scalars_h + 8, s->scalars_d + 8, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
   out->kinetic_energy = s->scalars_h[8] * s->mvv2e;
+  if (s->force_timing_pending) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, s->ev0, s->ev1) == cudaSuccess) s->ms_force = ms;
+    s->force_timing_pending = false;
+  }
   out->ms_build = s->ms_build; out->ms_force = s->ms_force; out->ms_run = s->ms_run;
   out->launches_last_run = s->launches_last_run; out->launches_total = s->launches;
   out->ms_force_sampled = s->ms_force_sampled; out->nforce_sampled = s->nforce_sampled;

@@ -137,7 +137,7 @@ def test_half_list_holds_each_pair_once():
 
 # ---- forces, energy, virial: small boxes, every kernel variant, against the O(N^2) definition --------------
 
-VARIANTS = [("tpa", 1, 0), ("subwarp8", 2, 0), ("warp", 3, 0), ("cell", 4, 0), ("half", 1, 1)]
+VARIANTS = [("tpa", 1, 0), ("subwarp4", 5, 0), ("subwarp8", 2, 0), ("warp", 3, 0), ("cell", 4, 0), ("half", 1, 1)]
 
 
 @pytest.mark.parametrize("name,kernel,list_kind", VARIANTS)
@@ -260,7 +260,7 @@ def test_cfg1_trajectory_fp64_100_steps():
     assert _fp64_force_err(f, fo) < 1e-12
 
 
-@pytest.mark.parametrize("kernel,list_kind", [(1, 0), (2, 0), (3, 0), (4, 0), (1, 1)])
+@pytest.mark.parametrize("kernel,list_kind", [(1, 0), (2, 0), (3, 0), (4, 0), (5, 0), (1, 1)])
 def test_run_in_pieces_equals_run_at_once_and_snapshots_match(kernel, list_kind):
     w = wl.make(1, n_override=7)
     a = md.from_workload(w, precision=md.MD_FP64, kernel=kernel, list_kind=list_kind)
@@ -413,7 +413,7 @@ def test_autotune_picks_a_variant_and_stays_correct():
     ms = s.md_autotune(2)
     assert all(v > 0 for v in ms.values())
     st = s.md_get_stats()
-    assert st["kernel_variant"] in (1, 2, 3)
+    assert st["kernel_variant"] in (1, 2, 3, 5)
     f = np.zeros((w.natoms, 3))
     s.md_compute_forces(f)
     assert _rel_rms(f, oracle.forces_brute(x, w.box, w.style, w.params, w.rc)[0]) < 1e-5
