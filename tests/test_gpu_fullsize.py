@@ -108,3 +108,34 @@ def test_full_size_list_rows_match_full_scan(cfg):
     assert bool((rows == int(ids[k])).any(dim=1).all().item())
     del nn, nb
     s.close()
+
+
+@pytest.mark.parametrize("cfg,kernel,list_kind,steps", [
+    (5, 4, 0, 8),      # direct cell-list kernel at 4,000,000 atoms
+    (5, 1, 1, 8),      # half list, atomic scatter
+    (5, 5, 0, 8),      # 4 lanes per atom
+    (3, 3, 0, 8),      # warp per atom at rc = 5 sigma (the paper's BpA regime)
+    (4, 2, 0, 12),     # EAM, 8 lanes per atom
+])
+def test_full_size_other_variants_match_oracle(cfg, kernel, list_kind, steps):
+    """Every kernel variant at full size: a short run crossing a rebuild, then the oracle recomputes forces and
+    energy from the GPU's own positions (same-input snapshot) and sampled atoms by full scans."""
+    from paper_1009_4330_b200 import md
+    w = wl.make(cfg)
+    N = w.natoms
+    s = md.from_workload(w, kernel=kernel, list_kind=list_kind)
+    s.md_run(steps, w.dt)
+    x = np.zeros((N, 3)); f_run = np.zeros((N, 3))
+    s.md_get_positions(x); s.md_get_forces(f_run)
+    f = np.zeros((N, 3))
+    E, _ = s.md_compute_forces(f, energy=True)
+    st = s.md_get_stats()
+    assert st["kernel_variant"] == kernel and st["nsteps_total"] == steps
+    fo, Eo, _, _, _ = oracle.forces(x, w.box, w.style, w.params, w.rc)
+    assert _rel_rms(f, fo) < 1e-5 and _rel_rms(f_run, fo) < 1e-5
+    assert abs(E - Eo) < 1e-6 * abs(Eo)
+    ids = _sample_ids(N, w.seed + 2)[:16]
+    fs, _ = oracle.forces_sample(x, w.box, w.style, w.params, w.rc, ids)
+    scale = np.sqrt((fo ** 2).sum(axis=1).mean())
+    assert np.abs(f[ids] - fs).max() < 3e-5 * scale
+    s.close()
