@@ -290,6 +290,16 @@ def run_ours(args, rk) -> None:
         "binding_resource_measured": "shared-memory data pipe (random 128-bit gathers of staged neighbor positions), "
                                      "see profiles/ and DESIGN.md 6",
     }
+    # the resource ncu shows saturated: one LDS.128 gather per list entry (two passes for EAM); a warp gather moves
+    # 32 x 16 B = 4 wavefronts at best, ~9 with the bank conflicts of random slots; 148 SMs x 1 wavefront per clock
+    passes = 2 if w.style == wl.PAIR_EAM else 1
+    gathers_per_s = passes * w.natoms * st["mean_neighbors"] / (ms_force * 1e-3) if ms_force > 0 else 0.0
+    sm_clock = 1.965e9
+    roofline["smem_gather"] = {
+        "achieved": gathers_per_s / 1e9, "unit": "G gathered entries/s",
+        "peak_conflict_free": 148 * sm_clock * 32 / 4 / 1e9,
+        "frac_of_conflict_free": gathers_per_s / (148 * sm_clock * 32 / 4),
+        "note": "DESIGN.md 6: ncu l1tex__data_pipe_lsu_wavefronts 84 % of peak at ~9 wavefronts per warp gather"}
     if not rk.is_root:
         return
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")    # written by hand from an ncu --set full capture
