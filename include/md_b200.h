@@ -91,7 +91,7 @@ typedef struct md_stats {
   int32_t max_tile_atoms;      /* largest staged count seen at the last build */
   int32_t max_neighbors;       /* longest list row at the last build */
   int32_t row_capacity;        /* list row capacity (entries) */
-  int32_t reserved_;
+  int32_t list_balanced;       /* 1: the current list's rows have been permuted for conflict-free gathers (long-lived lists only) */
   double mean_neighbors;       /* mean list row length at the last build */
   double kinetic_energy;       /* 1/2 sum m v^2 mvv2e at the time of the call */
   double ms_build;             /* device time of the last list build (bin+sort+build), CUDA events */

@@ -51,6 +51,9 @@ struct md_system_impl {
   int xcur = 0;   // buffer of x (flips at every build and at every fused kick+drift step)
   int force_threads = 256, batch = 8;
   bool force_timing_pending = false;
+  bool list_balanced = false;
+  int64_t steps_since_build = 0;
+  bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
   int brick_forced = 0;   // tile width in cells fixed by the autotuner (0: the planner's choice)
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
   void* xr[2] = {nullptr, nullptr};   // packed cell-relative positions (Vec4<T>, 32 B per atom reserved), buffer index = xcur
@@ -177,6 +180,11 @@ void fill_geom_for_b(const md_system* s, int b, Geom& g) {
       g.h[d] = std::ldexp(std::nearbyint(std::ldexp(m, bits)), e - bits);
     }
     g.b[d] = std::min(b, g.nc[d]);
+    if (const char* e = getenv("MD_B200_BRICK_XYZ")) {   // tuning experiments: "bx,by,bz"
+      int v[3] = {b, b, b};
+      sscanf(e, "%d,%d,%d", &v[0], &v[1], &v[2]);
+      g.b[d] = std::min(std::max(v[d], 1), g.nc[d]);
+    }
     g.nb[d] = (g.nc[d] + g.b[d] - 1) / g.b[d];
     g.ncell *= g.nc[d];
   }
@@ -332,6 +340,30 @@ int build_list_only(md_system* s) {
   return MD_OK;
 }
 
+// Row balancing (md_kernels.cuh): permutes every list row in place for conflict-free shared-memory gathers.  It
+// costs about as much as a few force evaluations and makes one 4-20 % faster, so it pays only for a list that
+// lives long: md_run applies it once a list has survived BALANCE_AFTER steps (a cold solid such as cfg 4 keeps
+// its list for hundreds of steps; a hot liquid rebuilds every ~6 and never gets there).
+constexpr int BALANCE_AFTER = 48;
+int balance_rows(md_system* s) {
+  const Geom& g = s->g;
+  if (s->no_balance || s->list_balanced || !s->list_valid || !s->list_built_for_export) return MD_OK;
+  BalanceArgs R{};
+  R.g = g; R.tab = s->tab; R.list = s->list; R.numneigh = s->numneigh;
+  R.row_bytes = g.row_cap * 2 + 16;
+  if ((R.row_bytes / 16) % 2 == 0) R.row_bytes += 16;
+  int threads = (int)std::min<size_t>(256, (160 * 1024) / (size_t)R.row_bytes) / 32 * 32;
+  if (threads >= 32) {
+    const size_t bsm = (size_t)threads * R.row_bytes;
+    if (g.K == 1) CK(launch(s, k_balance_rows<0>, g.ntiles, threads, bsm, R));
+    else if (g.K == 4) CK(launch(s, k_balance_rows<2>, g.ntiles, threads, bsm, R));
+    else if (g.K == 8) CK(launch(s, k_balance_rows<3>, g.ntiles, threads, bsm, R));
+    else CK(launch(s, k_balance_rows<5>, g.ntiles, threads, bsm, R));
+  }
+  s->list_balanced = true;
+  return MD_OK;
+}
+
 int build(md_system* s, bool need_list) {
   if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set before building");
   for (int attempt = 0; attempt < 6; ++attempt) {
@@ -386,6 +418,8 @@ int build(md_system* s, bool need_list) {
     s->mean_row = (double)F.sum_rows / (double)s->N;
     s->list_valid = true;
     s->list_built_for_export = do_list;
+    s->list_balanced = false;
+    s->steps_since_build = 0;
     return MD_OK;
   }
   return fail(s, MD_ERR_OVERFLOW, "tile or neighbor-row capacity still exceeded after re-planning");
@@ -579,6 +613,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   for (int t = 0; t < ntypes; ++t)
     if (!(mass[t] > 0.0)) return fail(nullptr, MD_ERR_BAD_ARGUMENT, "md_create: masses must be positive");
   s = new md_system();
+  if (const char* e = getenv("MD_B200_NO_BALANCE")) s->no_balance = atoi(e) != 0;
   auto bail = [&](int code) { std::string e = s->err; md_destroy(s); g_create_error = e; return code; };
   s->N = N;
   s->ld = ((size_t)N + 31) & ~(size_t)31;
@@ -791,6 +826,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
       const int flips = final_ran ? done - 1 : done;   // kick+drift launches that ran
       s->xcur ^= (flips & 1);
       s->nsteps_total += done;
+      s->steps_since_build += done;
       remaining -= done;
       parity = (parity + done) & 1;
       s->nforce -= (m - done);
@@ -802,6 +838,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         s->ms_build_in_run += s->ms_build;
         parity = 0;
       } else if (remaining > 0) {
+        if (s->steps_since_build >= BALANCE_AFTER && s->kernel_eff != MD_KERNEL_CELL) { rc = balance_rows(s); if (rc) return rc; }
         CK(cudaMemsetAsync(&s->flags_d->steps_done, 0, sizeof(int), s->stream));
         if (done == s->batch) s->batch = std::min(32, s->batch + 2);
       }
@@ -895,6 +932,7 @@ int md_get_stats(md_system* s, md_stats* out) {
     for (int d = 0; d < 3; ++d) { out->ncells[d] = s->g.nc[d]; out->brick[d] = s->g.b[d]; }
     out->ntiles = s->g.ntiles; out->tile_capacity = s->g.tile_cap; out->row_capacity = s->g.row_cap;
   }
+  out->list_balanced = s->list_balanced ? 1 : 0;
   out->max_tile_atoms = s->max_tile_atoms; out->max_neighbors = s->max_row; out->mean_neighbors = s->mean_row;
   CK(cudaMemsetAsync(s->scalars_d + 8, 0, sizeof(double), s->stream));
   CK(launch(s, k_kinetic, std::min<unsigned>(blocks_for(s->N, 256), 1184u), 256, 0, (int)s->N, s->ld, (const double*)s->v[s->cur],

@@ -887,6 +887,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_BLOCKS) k_build_list(
         nwords = before;   // count below from complete words + rem
       }
       const int n = nwords * 8 + rem;
+      if (!act && r0 + lane < pad4(c)) A.numneigh[(size_t)tile * g.interior_cap + tt.rstart[t] + r0 + lane] = 0;   // pad row
       if (act) {
         const int stored = n < g.row_cap ? n : g.row_cap;
         A.numneigh[(size_t)tile * g.interior_cap + a] = stored;
@@ -903,6 +904,90 @@ __global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_BLOCKS) k_build_list(
     atomicMax(&A.flags->max_row, my_max);
     if (my_max > g.row_cap) atomicMax(&A.flags->need_row_cap, my_max);
     atomicAdd(&A.flags->sum_rows, my_sum);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Row balancing (after every list build).  The force kernels fetch a neighbor with one 128-bit shared-memory load
+// per lane; the hardware serves such a load a quarter warp (8 threads) at a time, and two of the 8 threads
+// collide when their records fall into the same 16-byte bank group, i.e. when their slots agree mod 8 (measured:
+// ~9 wavefronts per warp gather on random slots against 4 without collisions -- the force kernels' bound).
+// The order of the entries within a row is free, so this kernel permutes every row such that, wherever
+// possible, position u of word q holds an entry with  slot mod 8 == (u + thread index of (row, q)) mod 8:
+// the 8 threads of a quarter warp, which walk their words in lockstep, then read 8 different bank groups.
+// Residue classes are never perfectly even, so the surplus of the longer classes fills the holes of the
+// shorter ones (those entries may collide), and the remaining holes name the dummy slot.
+// One thread per row; its output row is assembled in a private stripe of shared memory (row_bytes).
+// ---------------------------------------------------------------------------------------------------
+struct BalanceArgs {
+  Geom g;
+  const int* tab;
+  uint4* list;
+  const int* numneigh;
+  int row_bytes;      // shared-memory stripe per thread: row_cap * 2 + 16 (an odd number of 16-byte units)
+};
+
+template <int LOGK>
+__global__ void __launch_bounds__(256) k_balance_rows(BalanceArgs A) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const Geom& g = A.g;
+  constexpr int K = 1 << LOGK;
+  const int tile = blockIdx.x;
+  const int* __restrict__ h = A.tab + (size_t)tile * tile_tab_stride(g);
+  const int n_rows = h[0], n_slots = h[1];
+  if (n_slots > g.tile_cap || n_rows > g.interior_cap) return;
+  const int shift = g.code_shift;
+  const unsigned dummy = (unsigned)n_slots << shift;
+  const size_t slots_cap = (size_t)g.interior_cap << LOGK;
+  uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
+  unsigned short* out = reinterpret_cast<unsigned short*>(smem_raw + (size_t)threadIdx.x * A.row_bytes);
+  for (int a = threadIdx.x; a < n_rows; a += blockDim.x) {
+    const int n = min(A.numneigh[(size_t)tile * g.interior_cap + a], g.row_cap);
+    if (n <= 0) continue;
+    const int W = (n + 7) >> 3;
+    auto word_ptr = [&](int q) { return tlist + (size_t)(q >> LOGK) * slots_cap + ((size_t)a << LOGK) + (q & (K - 1)); };
+    auto tix = [&](int q) { return (a * K + (q & (K - 1))) & 7; };   // thread index mod 8 of the thread that reads word q
+    // pass A: entries per residue class (16-bit counters, four to a 64-bit register)
+    unsigned long long cnt[2] = {0ull, 0ull};
+    for (int q = 0; q < W; ++q) {
+      const uint4 w = *word_ptr(q);
+      const unsigned ww[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        const unsigned code = (e & 1) ? (ww[e >> 1] >> 16) : (ww[e >> 1] & 0xffffu);
+        if (q * 8 + e < n) {            // the build leaves the real entries in the first n positions
+          const unsigned rho = (code >> shift) & 7u;
+          cnt[rho >> 2] += 1ull << (16 * (rho & 3u));
+        }
+      }
+    }
+    auto count_of = [&](unsigned rho) { return (int)((cnt[rho >> 2] >> (16 * (rho & 3u))) & 0xffffu); };
+    // pass B: the k-th entry of class rho goes to word k, position (rho - tix(k)) & 7, while k < W; later ones fill holes
+    unsigned long long cur[2] = {0ull, 0ull};
+    int hr = 0, hk = min(count_of(0), W);     // hole cursor: class hr, word hk
+    auto next_hole = [&]() {
+      while (hr < 8 && hk >= W) { ++hr; hk = hr < 8 ? min(count_of((unsigned)hr), W) : 0; }
+      const int pos = hk * 8 + ((hr - tix(hk)) & 7);
+      ++hk;
+      return pos;
+    };
+    for (int q = 0; q < W; ++q) {
+      const uint4 w = *word_ptr(q);
+      const unsigned ww[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        const unsigned code = (e & 1) ? (ww[e >> 1] >> 16) : (ww[e >> 1] & 0xffffu);
+        if (q * 8 + e < n) {
+          const unsigned rho = (code >> shift) & 7u;
+          const int k = (int)((cur[rho >> 2] >> (16 * (rho & 3u))) & 0xffffu);
+          cur[rho >> 2] += 1ull << (16 * (rho & 3u));
+          const int pos = k < W ? k * 8 + (((int)rho - tix(k)) & 7) : next_hole();
+          out[pos] = (unsigned short)code;
+        }
+      }
+    }
+    for (int left = 8 * W - n; left > 0; --left) out[next_hole()] = (unsigned short)dummy;
+    for (int q = 0; q < W; ++q) *word_ptr(q) = *reinterpret_cast<const uint4*>(out + 8 * q);
   }
 }
 
@@ -925,12 +1010,16 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_export_list(Geom g, const int
     for (int k = threadIdx.x; k < tt.cnt[t]; k += blockDim.x) {
       const int a = tt.rstart[t] + k, n = numneigh[(size_t)tile * g.interior_cap + a], io = sid[tt.start[t] + k];
       nn_out[io] = n;
-      for (int e = 0; e < n && e < stride; ++e) {
+      // the row's n entries sit somewhere in its ceil(n/8) words; the other positions name the dummy slot
+      int m = 0;
+      for (int e = 0; e < ((n + 7) & ~7); ++e) {
         int q = e >> 3, s = q % K, c = q / K;
         uint4 w = tlist[(size_t)c * slots_cap + (size_t)a * K + s];
         unsigned word = (&w.x)[(e & 7) >> 1];
         unsigned code = (e & 1) ? (word >> 16) : (word & 0xffffu);
-        neigh_out[(long long)io * stride + e] = sid[code >> g.code_shift];
+        if ((int)(code >> g.code_shift) == tt.n_slots) continue;
+        if (m < stride) neigh_out[(long long)io * stride + m] = sid[code >> g.code_shift];
+        ++m;
       }
     }
   }

@@ -37,7 +37,7 @@ class md_stats(ctypes.Structure):
         ("precision", ctypes.c_int32), ("lanes_per_atom", ctypes.c_int32), ("ncells", ctypes.c_int32 * 3),
         ("brick", ctypes.c_int32 * 3), ("ntiles", ctypes.c_int32), ("tile_capacity", ctypes.c_int32),
         ("max_tile_atoms", ctypes.c_int32), ("max_neighbors", ctypes.c_int32), ("row_capacity", ctypes.c_int32),
-        ("reserved_", ctypes.c_int32), ("mean_neighbors", ctypes.c_double), ("kinetic_energy", ctypes.c_double),
+        ("list_balanced", ctypes.c_int32), ("mean_neighbors", ctypes.c_double), ("kinetic_energy", ctypes.c_double),
         ("ms_build", ctypes.c_double), ("ms_force", ctypes.c_double), ("ms_run", ctypes.c_double),
         ("launches_last_run", ctypes.c_int64), ("launches_total", ctypes.c_int64),
         ("ms_force_sampled", ctypes.c_double), ("nforce_sampled", ctypes.c_int64),

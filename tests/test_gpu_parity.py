@@ -311,6 +311,34 @@ def test_mixed_run_conserves_energy_and_momentum_cfg2_small():
     assert _rel_rms(f, fo) < 1e-5 and abs(E1 - Eo) < 1e-6 * abs(Eo)
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("kernel", [1, 5, 2, 3])
+def test_long_lived_list_is_balanced_and_stays_correct(kernel, precision):
+    """A cold solid keeps its list for hundreds of steps; after 48 steps md_run permutes the rows for conflict-free
+    shared-memory gathers (a pure reordering within each row).  Forces, energy and the pair set must not change."""
+    w = wl.make(4, n_override=6)
+    s = md.from_workload(w, precision=precision, kernel=kernel)
+    s.md_run(40, w.dt)
+    assert s.md_get_stats()["list_balanced"] == 0
+    nn0, nb0 = _gpu_rows(s, w.natoms, 160)
+    s.md_run(40, w.dt)
+    st = s.md_get_stats()
+    assert st["list_balanced"] == 1 and st["nbuilds"] == 1
+    nn1, nb1 = _gpu_rows(s, w.natoms, 160)
+    assert np.array_equal(nn0, nn1)
+    for i in range(w.natoms):
+        assert sorted(nb0[i, :nn0[i]].tolist()) == sorted(nb1[i, :nn1[i]].tolist())
+    x, f = np.zeros((w.natoms, 3)), np.zeros((w.natoms, 3))
+    s.md_get_positions(x)
+    E, W = s.md_compute_forces(f, energy=True, virial=True)
+    fo, Eo, Wo, _, _ = oracle.forces(x, w.box, w.style, w.params, w.rc)
+    if precision == md.MD_FP64:
+        assert _fp64_force_err(f, fo) < 1e-12 and abs(E - Eo) < 1e-12 * abs(Eo)
+    else:
+        assert _rel_rms(f, fo) < 1e-5 and abs(E - Eo) < 1e-6 * abs(Eo)
+    s.close()
+
+
 def test_eam_metal_units_run_matches_oracle():
     w = wl.make(4, n_override=6)
     s = md.from_workload(w, precision=md.MD_FP64)
