@@ -54,7 +54,8 @@ struct md_system_impl {
   bool list_balanced = false;
   int64_t steps_since_build = 0;
   bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
-  int brick_forced = 0;   // tile width in cells fixed by the autotuner (0: the planner's choice)
+  int brick_forced = 0;   // 9 + offset: the autotuner's step away from the planner's tile shape in the candidate list (0: none)
+  int shape_index = 0, shape_count = 0, build_threads = 256;
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
   void* xr[2] = {nullptr, nullptr};   // packed cell-relative positions (Vec4<T>, 32 B per atom reserved), buffer index = xcur
   int* tab = nullptr;                 // per-tile tables of the last build
@@ -158,12 +159,21 @@ size_t force_smem(const md_system* s, const Geom& g, bool half) {
          (size_t)((tile_tab_quads(g) + 7) & ~7) * 2 + (half ? (size_t)capA_of(g) * 4 : 0) + 16;
 }
 size_t cell_smem(const md_system* s, const Geom& g) { return sizeof(TileTables) + 4 * (size_t)capA_of(g) * elem_size(s) + 16; }
-size_t build_smem(const Geom& g) {
-  return sizeof(TileTables) + (size_t)tile_tab_cells(g) * 16 + BUILD_TASK_INTS * sizeof(int) + 3 * (size_t)capA_of(g) * sizeof(float) + (size_t)BUILD_THREADS * RING_STRIDE + 16;
+size_t build_smem(const Geom& g, int threads) {
+  return sizeof(TileTables) + (size_t)tile_tab_cells(g) * 16 + BUILD_TASK_INTS * sizeof(int) + 3 * (size_t)capA_of(g) * sizeof(float) +
+         (size_t)threads * RING_STRIDE + 16;
+}
+// threads per block of the list build: 256 when three such blocks fit an SM's shared memory, else 384 (two blocks):
+// 24 warps per SM either way
+int build_threads(const Geom& g) {
+  const size_t sm_total = 227 * 1024, reserve = 1024 + 512;
+  if (3 * (build_smem(g, BUILD_THREADS) + reserve) <= sm_total) return BUILD_THREADS;
+  if (2 * (build_smem(g, BUILD_MAX_THREADS) + reserve) <= sm_total) return BUILD_MAX_THREADS;
+  return BUILD_THREADS;
 }
 size_t export_smem(const Geom& g) { return sizeof(TileTables) + (size_t)capA_of(g) * sizeof(int) + 16; }
 
-void fill_geom_for_b(const md_system* s, int b, Geom& g) {
+void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   double rl = s->rc + s->skin;
   g.ncell = 1;
   for (int d = 0; d < 3; ++d) {
@@ -179,12 +189,7 @@ void fill_geom_for_b(const md_system* s, int b, Geom& g) {
       const double m = std::frexp(g.edge[d], &e);                 // edge = m 2^e, m in [0.5, 1)
       g.h[d] = std::ldexp(std::nearbyint(std::ldexp(m, bits)), e - bits);
     }
-    g.b[d] = std::min(b, g.nc[d]);
-    if (const char* e = getenv("MD_B200_BRICK_XYZ")) {   // tuning experiments: "bx,by,bz"
-      int v[3] = {b, b, b};
-      sscanf(e, "%d,%d,%d", &v[0], &v[1], &v[2]);
-      g.b[d] = std::min(std::max(v[d], 1), g.nc[d]);
-    }
+    g.b[d] = std::min(shape[d], g.nc[d]);
     g.nb[d] = (g.nc[d] + g.b[d] - 1) / g.b[d];
     g.ncell *= g.nc[d];
   }
@@ -207,40 +212,63 @@ void fill_geom_for_b(const md_system* s, int b, Geom& g) {
   g.chunk_cap = g.row_cap / unit;
 }
 
+// Candidate tile shapes (cells per tile edge, bx >= by >= bz, (bx+2)(by+2)(bz+2) <= MAX_TILE_CELLS), largest first.
+struct TileShape { int b[3]; };
+int tile_shapes(TileShape* out) {
+  int n = 0;
+  for (int cells = 64; cells >= 1; --cells)
+    for (int bx = 4; bx >= 1; --bx)
+      for (int by = bx; by >= 1; --by)
+        for (int bz = by; bz >= 1; --bz)
+          if (bx * by * bz == cells && (bx + 2) * (by + 2) * (bz + 2) <= MAX_TILE_CELLS) out[n++] = TileShape{{bx, by, bz}};
+  return n;
+}
+
 int plan(md_system* s) {
   double rl = s->rc + s->skin;
   for (int d = 0; d < 3; ++d)
     if (s->box[d] < 3.0 * rl) return fail(s, MD_ERR_BOX_TOO_SMALL, "box edge %d = %g < 3 (rc+skin) = %g", d, s->box[d], 3.0 * rl);
-  int forced = s->brick_forced;
-  if (const char* e = getenv("MD_B200_BRICK")) forced = atoi(e);
   double vol = s->box[0] * s->box[1] * s->box[2];
   double lscale = std::cbrt(vol / (double)s->N);   // ~ nearest-neighbor distance
-  int best = 0;
   Geom g{};
-  const size_t smem_soft = 100 * 1024, smem_hard = 200 * 1024;
+  const size_t smem_hard = 200 * 1024;
+  // three force blocks per SM: their phases (staging, list loop, epilogue) overlap better than those of two bigger ones
+  const size_t smem_three = (227 * 1024) / 3 - 1536 - 3200;
   const int code_shift = s->precision == MD_FP64 ? 4 : 3;
-  for (int pass = 0; pass < 3 && !best; ++pass) {
-    // pass 0: all preferences; pass 1: drop the tile-count preference; pass 2: only hard limits
-    for (int b = 6; b >= 1; --b) {
-      if (forced && b != forced) continue;
-      fill_geom_for_b(s, b, g);
-      if ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) > MAX_TILE_CELLS) continue;
-      if (g.tile_cap > (65535 >> code_shift)) continue;       // 16-bit slot codes
-      size_t sm = std::max(std::max(force_smem(s, g, g.half), build_smem(g)), cell_smem(s, g));
-      if (sm > smem_hard) continue;
-      if (!forced && pass < 2) {
-        if (sm > smem_soft) continue;
+  TileShape shapes[64];
+  const int nshapes = tile_shapes(shapes);
+  // feasible[]: shapes within the hard limits, largest first; `pick`: the first one that also meets the preferences
+  // of pass 0 (all), pass 1 (all but the tile count) or pass 2 (none)
+  int feasible[64], nfeas = 0, pick = -1;
+  int forced_shape[3] = {0, 0, 0};
+  if (const char* e = getenv("MD_B200_BRICK_XYZ")) sscanf(e, "%d,%d,%d", &forced_shape[0], &forced_shape[1], &forced_shape[2]);
+  for (int i = 0; i < nshapes; ++i) {
+    fill_geom_for_b(s, shapes[i].b, g);
+    if (g.b[0] != shapes[i].b[0] || g.b[1] != shapes[i].b[1] || g.b[2] != shapes[i].b[2]) continue;   // wider than the box
+    if (g.tile_cap > (65535 >> code_shift)) continue;       // 16-bit slot codes
+    size_t sm = std::max(std::max(force_smem(s, g, g.half), build_smem(g, build_threads(g))), cell_smem(s, g));
+    if (sm > smem_hard) continue;
+    if (forced_shape[0] && (forced_shape[0] != g.b[0] || forced_shape[1] != g.b[1] || forced_shape[2] != g.b[2])) continue;
+    feasible[nfeas++] = i;
+  }
+  if (!nfeas) return fail(s, MD_ERR_OVERFLOW, "no tile shape fits shared memory or the 16-bit slot codes (too many atoms per cell of edge rc+skin)");
+  for (int pass = 0; pass < 3 && pick < 0; ++pass) {
+    for (int f = 0; f < nfeas && pick < 0; ++f) {
+      fill_geom_for_b(s, shapes[feasible[f]].b, g);
+      if (pass < 2) {
+        if (force_smem(s, g, g.half) > smem_three) continue;
         double half_extent = 0;
         for (int d = 0; d < 3; ++d) half_extent = std::max(half_extent, 0.5 * (g.b[d] + 2) * g.edge[d]);
-        if (s->precision == MD_MIXED && half_extent > 9.0 * lscale && b > 1) continue;   // fp32 tile coordinates
+        if (s->precision == MD_MIXED && half_extent > 9.0 * lscale && g.b[0] > 1) continue;   // fp32 tile coordinates
         if (pass == 0 && g.ntiles < 2 * 148) continue;
       }
-      best = b;
-      break;
+      pick = f;
     }
   }
-  if (!best) return fail(s, MD_ERR_OVERFLOW, "no tile width fits shared memory (density too high for cells of edge rc+skin)");
-  fill_geom_for_b(s, best, g);
+  // the autotuner may step away from the planner's pick: brick_forced = 1 + offset + 8 (0: none)
+  if (s->brick_forced) pick = std::min(std::max(pick + (s->brick_forced - 9), 0), nfeas - 1);
+  s->shape_index = pick; s->shape_count = nfeas;
+  fill_geom_for_b(s, shapes[feasible[pick]].b, g);
   s->g = g;
   // block size of the list force kernels: the tile's rows should fill whole rounds of the block
   {
@@ -320,22 +348,23 @@ int build_list_only(md_system* s) {
   B.rl2_hi = B.rl2_mid + B.rl2_bw;      // the same fp32 sum the kernel's accept test and band test are consistent with
   B.list = s->list; B.numneigh = s->numneigh; B.flags = s->flags_d;
   const bool s4 = g.code_shift == 4;
-  const size_t sm = build_smem(g);
+  const int bt = build_threads(g);
+  const size_t sm = build_smem(g, bt);
   if (g.half) {
-    if (s4) CK(launch(s, k_build_list<true, 0, 4>, g.ntiles, BUILD_THREADS, sm, B));
-    else CK(launch(s, k_build_list<true, 0, 3>, g.ntiles, BUILD_THREADS, sm, B));
+    if (s4) CK(launch(s, k_build_list<true, 0, 4>, g.ntiles, bt, sm, B));
+    else CK(launch(s, k_build_list<true, 0, 3>, g.ntiles, bt, sm, B));
   } else if (g.K == 1) {
-    if (s4) CK(launch(s, k_build_list<false, 0, 4>, g.ntiles, BUILD_THREADS, sm, B));
-    else CK(launch(s, k_build_list<false, 0, 3>, g.ntiles, BUILD_THREADS, sm, B));
+    if (s4) CK(launch(s, k_build_list<false, 0, 4>, g.ntiles, bt, sm, B));
+    else CK(launch(s, k_build_list<false, 0, 3>, g.ntiles, bt, sm, B));
   } else if (g.K == 4) {
-    if (s4) CK(launch(s, k_build_list<false, 2, 4>, g.ntiles, BUILD_THREADS, sm, B));
-    else CK(launch(s, k_build_list<false, 2, 3>, g.ntiles, BUILD_THREADS, sm, B));
+    if (s4) CK(launch(s, k_build_list<false, 2, 4>, g.ntiles, bt, sm, B));
+    else CK(launch(s, k_build_list<false, 2, 3>, g.ntiles, bt, sm, B));
   } else if (g.K == 8) {
-    if (s4) CK(launch(s, k_build_list<false, 3, 4>, g.ntiles, BUILD_THREADS, sm, B));
-    else CK(launch(s, k_build_list<false, 3, 3>, g.ntiles, BUILD_THREADS, sm, B));
+    if (s4) CK(launch(s, k_build_list<false, 3, 4>, g.ntiles, bt, sm, B));
+    else CK(launch(s, k_build_list<false, 3, 3>, g.ntiles, bt, sm, B));
   } else {
-    if (s4) CK(launch(s, k_build_list<false, 5, 4>, g.ntiles, BUILD_THREADS, sm, B));
-    else CK(launch(s, k_build_list<false, 5, 3>, g.ntiles, BUILD_THREADS, sm, B));
+    if (s4) CK(launch(s, k_build_list<false, 5, 4>, g.ntiles, bt, sm, B));
+    else CK(launch(s, k_build_list<false, 5, 3>, g.ntiles, bt, sm, B));
   }
   return MD_OK;
 }
@@ -535,20 +564,21 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   s->planned = false;
   int rc = plan(s);
   if (rc) return rc;
-  const int b0 = std::max(s->g.b[0], std::max(s->g.b[1], s->g.b[2]));
   double best_score = 1e300;
   int best = MD_KERNEL_TPA, best_b = 0;
   if (ms_out) for (int k = 0; k < 4; ++k) ms_out[k] = 1e300;
-  // with thousands of tiles the planner's (shared-memory driven) width is right and the SMs are full either way;
-  // the width matters when the box yields few tiles
-  const bool sweep_b = s->g.ntiles < 2048;
-  for (int b = sweep_b ? std::max(1, b0 - 1) : b0; b <= (sweep_b ? std::min(4, b0 + 1) : b0); ++b) {
+  // with thousands of tiles the planner's pick is right and the SMs are full either way; the tile shape matters when
+  // the box yields few tiles: then its neighbours in the candidate list (two larger, two smaller) are timed too
+  const bool sweep = s->g.ntiles < 2048;
+  const int i0 = s->shape_index, nfeas = s->shape_count;
+  for (int off = sweep ? -2 : 0; off <= (sweep ? 2 : 0); ++off) {
+    if (i0 + off < 0 || i0 + off >= nfeas) continue;
     for (int k = 0; k < 4; ++k) {
       s->kernel_eff = cand[k];
-      s->brick_forced = b == b0 ? 0 : b;
+      s->brick_forced = off == 0 ? 0 : 9 + off;
       s->planned = false;
       rc = build(s, true);
-      if (rc == MD_ERR_OVERFLOW && b != b0) continue;   // this width does not fit shared memory
+      if (rc == MD_ERR_OVERFLOW && off != 0) continue;   // this shape does not fit with this many lanes per atom
       if (rc) return rc;
       const double ms_build = s->ms_build;
       rc = compute_forces_device(s, false);   // warm-up

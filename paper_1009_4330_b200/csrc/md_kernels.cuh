@@ -19,13 +19,14 @@
 namespace mdk {
 
 constexpr int MAX_TILE_CELLS = 216;    // (b+2)^3 <= 216  =>  b <= 4
-constexpr int BUILD_THREADS = 256;     // threads per block of the list-build and cell-list kernels
+constexpr int BUILD_THREADS = 256;     // threads per block of the list-build (when three blocks fit an SM) and cell-list kernels
+constexpr int BUILD_MAX_THREADS = 384; // list build: block size when only two blocks fit an SM
 constexpr int FORCE_MAX_THREADS = 640; // upper bound of the force kernels' block size (runtime choice)
 constexpr int FORCE_MIN_BLOCKS = 2;    // resident blocks per SM the mixed-precision force kernels are compiled for (<= 48 registers)
 #ifndef MDK_BUILD_MIN_BLOCKS
-#define MDK_BUILD_MIN_BLOCKS 3
+#define MDK_BUILD_MIN_BLOCKS 2
 #endif
-constexpr int BUILD_MIN_BLOCKS = MDK_BUILD_MIN_BLOCKS;    // resident blocks per SM the list-build kernel is compiled for (<= 85 registers)
+constexpr int BUILD_MIN_BLOCKS = MDK_BUILD_MIN_BLOCKS;    // with BUILD_MAX_THREADS: <= 85 registers, i.e. three 256-thread or two 384-thread blocks per SM
 constexpr int BUILD_TASK_INTS = 72;     // list-build: room for the first-task table of <= 64 interior cells (+1), 16-byte multiple
 constexpr int RING = 48;               // list-build: pending entries a lane can hold in shared memory (>= 32 + 8)
 constexpr int RING_STRIDE = RING * 2 + 16;   // bytes between the rings of neighbouring lanes (odd * 16)
@@ -720,7 +721,7 @@ __device__ __forceinline__ void build_scan_fast(unsigned& rp, float& m, unsigned
 
 // Shared memory: TileTables | offs[tile cells] float4 | xs[capA] ys[capA] zs[capA] floats | rings[nwarps*32*RING_STRIDE].
 template <bool HALF, int LOGK, int SHIFT>
-__global__ void __launch_bounds__(BUILD_THREADS, BUILD_MIN_BLOCKS) k_build_list(BuildArgs A) {
+__global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_list(BuildArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
   const Geom& g = A.g;
