@@ -24,6 +24,9 @@ def main() -> None:
     ap.add_argument("--rc", default="2.0,2.5,3.0,3.5,4.0,4.5,5.0,5.5,6.0")
     ap.add_argument("--melt", type=int, default=60)
     ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--nsweep", default="", help="also: whole-path throughput against system size (the shape of Fig. 7, L182-192): "
+                    "comma-separated fcc cells per edge, e.g. 6,8,10,14,20,28,40,56,80,100")
+    ap.add_argument("--nsteps", type=int, default=200)
     args = ap.parse_args()
     import torch
     if not torch.cuda.is_available():
@@ -39,7 +42,22 @@ def main() -> None:
           % (args.cells, args.rc, args.melt, args.reps, torch.cuda.get_device_name(0)))
     print("Times are ms per force evaluation (device time, best of %d); `build` is ms per list build with the thread-per-atom "
           "layout; `G entries/s` = N x list entries / best full-list time.\n" % args.reps)
-    for n in [int(c) for c in args.cells.split(",")]:
+    if args.nsweep:
+        print("## Whole path (md_run: builds + forces + integration) against system size, rc = 2.5, %d steps, MD_KERNEL_AUTO\n" % args.nsteps)
+        print("| atoms | tile shape | tiles | variant | builds | ms per step | atom-steps/s |")
+        print("|---|---|---|---|---|---|---|")
+        for n in [int(c) for c in args.nsweep.split(",")]:
+            w = wl.make(2, n_override=n)
+            s = md.from_workload(w, kernel=md.MD_KERNEL_AUTO)
+            s.md_run(args.nsteps, w.dt)                      # melts the lattice; selects variant and tile shape
+            s.md_run(args.nsteps, w.dt)
+            st = s.md_get_stats()
+            print("| %d | %s | %d | %s | %d | %.4f | %.3e |" % (w.natoms, "x".join(str(b) for b in st["brick"]), st["ntiles"],
+                  md.KERNEL_NAMES[st["kernel_variant"]], st["nbuilds_in_run"], st["ms_run"] / args.nsteps,
+                  w.natoms * args.nsteps / (st["ms_run"] * 1e-3)), flush=True)
+            s.close()
+        print()
+    for n in [int(c) for c in args.cells.split(",") if c]:
         base = wl.make(2, n_override=n)
         # melt once with the default cutoff so that every cutoff sees the same liquid snapshot
         s = md.from_workload(base, kernel=md.MD_KERNEL_TPA)
