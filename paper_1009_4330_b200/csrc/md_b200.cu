@@ -53,6 +53,7 @@ struct md_system_impl {
   bool force_timing_pending = false;
   bool list_balanced = false;
   int64_t steps_since_build = 0;
+  int balance_after = 0;     // BALANCE_AFTER, or MD_B200_BALANCE_AFTER (tuning experiments)
   bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
   int brick_forced = 0;   // 9 + offset: the autotuner's step away from the planner's tile shape in the candidate list (0: none)
   int shape_index = 0, shape_count = 0, build_threads = 256;
@@ -169,7 +170,8 @@ int build_threads(const Geom& g) {
   const size_t sm_total = 227 * 1024, reserve = 1024 + 512;
   if (3 * (build_smem(g, BUILD_THREADS) + reserve) <= sm_total) return BUILD_THREADS;
   if (2 * (build_smem(g, BUILD_MAX_THREADS) + reserve) <= sm_total) return BUILD_MAX_THREADS;
-  return BUILD_THREADS;
+  if (2 * (build_smem(g, BUILD_THREADS) + reserve) <= sm_total) return BUILD_THREADS;
+  return BUILD_MAX_THREADS;   // one block per SM: as many warps as the kernel is compiled for
 }
 size_t export_smem(const Geom& g) { return sizeof(TileTables) + (size_t)capA_of(g) * sizeof(int) + 16; }
 
@@ -414,7 +416,7 @@ int build(md_system* s, bool need_list) {
     }
     CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
               s->perm));
-    CK(launch(s, k_sort_cells, blocks_for(g.ncell, 128), 128, 0, g.ncell, (const int*)s->cell_start, s->perm));
+    CK(launch(s, k_sort_cells, blocks_for(g.ncell, 8), 256, 0, g.ncell, (const int*)s->cell_start, s->perm));   // a warp per cell
     if (s->precision == MD_FP64)
       CK(launch(s, k_permute<double>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
                 (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (double4*)s->xr[xo], s->ld));
@@ -449,6 +451,7 @@ int build(md_system* s, bool need_list) {
     s->list_built_for_export = do_list;
     s->list_balanced = false;
     s->steps_since_build = 0;
+    if (s->balance_after <= 0 && do_list) { int rcb = balance_rows(s); if (rcb) return rcb; }   // tuning experiments only
     return MD_OK;
   }
   return fail(s, MD_ERR_OVERFLOW, "tile or neighbor-row capacity still exceeded after re-planning");
@@ -644,6 +647,8 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
     if (!(mass[t] > 0.0)) return fail(nullptr, MD_ERR_BAD_ARGUMENT, "md_create: masses must be positive");
   s = new md_system();
   if (const char* e = getenv("MD_B200_NO_BALANCE")) s->no_balance = atoi(e) != 0;
+  s->balance_after = BALANCE_AFTER;
+  if (const char* e = getenv("MD_B200_BALANCE_AFTER")) s->balance_after = atoi(e);
   auto bail = [&](int code) { std::string e = s->err; md_destroy(s); g_create_error = e; return code; };
   s->N = N;
   s->ld = ((size_t)N + 31) & ~(size_t)31;
@@ -868,7 +873,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         s->ms_build_in_run += s->ms_build;
         parity = 0;
       } else if (remaining > 0) {
-        if (s->steps_since_build >= BALANCE_AFTER && s->kernel_eff != MD_KERNEL_CELL) { rc = balance_rows(s); if (rc) return rc; }
+        if (s->steps_since_build >= s->balance_after && s->kernel_eff != MD_KERNEL_CELL) { rc = balance_rows(s); if (rc) return rc; }
         CK(cudaMemsetAsync(&s->flags_d->steps_done, 0, sizeof(int), s->stream));
         if (done == s->batch) s->batch = std::min(32, s->batch + 2);
       }

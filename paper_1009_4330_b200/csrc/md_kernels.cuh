@@ -503,16 +503,50 @@ __global__ void k_fill_perm(int N, const int* __restrict__ cell_of, const int* _
 }
 
 // The atomic ranks of k_bin are not reproducible; sorting each cell's slice of perm by previous index
-// makes the whole order (and so every later summation order) deterministic.
-__global__ void k_sort_cells(int ncell, const int* __restrict__ cell_start, int* __restrict__ perm) {
-  int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= ncell) return;
-  int lo = cell_start[c], hi = cell_start[c + 1];
-  for (int a = lo + 1; a < hi; ++a) {
-    int key = perm[a], b = a - 1;
-    while (b >= lo && perm[b] > key) { perm[b + 1] = perm[b]; --b; }
-    perm[b + 1] = key;
+// makes the whole order (and so every later summation order) deterministic.  One warp per cell, rank sort:
+// every lane keeps up to SORT_PER of the cell's keys, each key's rank is the number of smaller keys (the keys
+// of a cell are distinct), broadcast lane by lane with shuffles: c * ceil(c/32) steps instead of the c^2 of a
+// serial insertion sort (a cell holds ~20 atoms at rc = 2.5 sigma, ~150 at rc = 5 sigma).
+constexpr int SORT_PER = 16;   // cells of up to 512 atoms; larger ones fall back to a serial sort by lane 0
+template <int PER>
+__device__ __forceinline__ void sort_cell_by_warp(int lo, int n, int lane, int* __restrict__ perm) {
+  int key[PER], rank[PER];
+#pragma unroll
+  for (int i = 0; i < PER; ++i) {
+    key[i] = lane + 32 * i < n ? perm[lo + lane + 32 * i] : 0x7fffffff;
+    rank[i] = 0;
   }
+#pragma unroll
+  for (int j = 0; j < PER; ++j) {          // the keys held in register j of every lane
+    const int cnt = min(32, n - 32 * j);
+    for (int l = 0; l < cnt; ++l) {
+      const int other = __shfl_sync(0xffffffffu, key[j], l);
+#pragma unroll
+      for (int i = 0; i < PER; ++i) rank[i] += other < key[i] ? 1 : 0;
+    }
+  }
+  __syncwarp();
+#pragma unroll
+  for (int i = 0; i < PER; ++i)
+    if (lane + 32 * i < n) perm[lo + rank[i]] = key[i];
+}
+__global__ void __launch_bounds__(256) k_sort_cells(int ncell, const int* __restrict__ cell_start, int* __restrict__ perm) {
+  const int lane = threadIdx.x & 31;
+  const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (c >= ncell) return;
+  const int lo = cell_start[c], n = cell_start[c + 1] - lo;
+  if (n <= 1) return;
+  if (n <= 32) sort_cell_by_warp<1>(lo, n, lane, perm);
+  else if (n <= 64) sort_cell_by_warp<2>(lo, n, lane, perm);
+  else if (n <= 128) sort_cell_by_warp<4>(lo, n, lane, perm);
+  else if (n <= 256) sort_cell_by_warp<8>(lo, n, lane, perm);
+  else if (n <= 32 * SORT_PER) sort_cell_by_warp<SORT_PER>(lo, n, lane, perm);
+  else if (lane == 0)
+    for (int a = lo + 1; a < lo + n; ++a) {
+      int key = perm[a], b = a - 1;
+      while (b >= lo && perm[b] > key) { perm[b + 1] = perm[b]; --b; }
+      perm[b + 1] = key;
+    }
 }
 
 // a2: spatial reorder of the per-atom arrays; x0 := x (reference for the displacement test)
