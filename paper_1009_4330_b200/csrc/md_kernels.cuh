@@ -1195,25 +1195,37 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
     A.f[gi] = tot[0]; A.f[ld + gi] = tot[1]; A.f[2 * ld + gi] = tot[2];
     return 0.0;
   }
+  // all loads first: the arrays may alias as far as the compiler knows, so a store between two loads would
+  // serialise three memory round trips
+  double vv[3], xx[3] = {0.0, 0.0, 0.0}, x0v[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) vv[d] = A.v[d * ld + gi];
+  if (A.epi == EPI_KICK_DRIFT) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { xx[d] = A.x[d * ld + gi]; x0v[d] = A.x0[d * ld + gi]; }
+  }
   const double dtf = A.half_dt_ftm2v / A.mass[A.type[gi]];
   double d2 = 0.0;
   T r[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    double vv = A.v[d * ld + gi] + dtf * tot[d];          // second half kick of this step
+    vv[d] += dtf * tot[d];                                  // second half kick of this step
     if (A.epi == EPI_KICK_DRIFT) {
-      vv += dtf * tot[d];                                 // first half kick of the next step
-      const double xx = A.x[d * ld + gi] + A.dt * vv;     // drift
-      A.x_new[d * ld + gi] = xx;
-      r[d] = (T)(xx - cc[d]);
-      const double dd = xx - A.x0[d * ld + gi];
+      vv[d] += dtf * tot[d];                                // first half kick of the next step
+      xx[d] += A.dt * vv[d];                                // drift
+      r[d] = (T)(xx[d] - cc[d]);
+      const double dd = xx[d] - x0v[d];
       d2 += dd * dd;
-    } else {
-      A.f[d * ld + gi] = tot[d];
     }
-    A.v[d * ld + gi] = vv;
   }
-  if (A.epi == EPI_KICK_DRIFT) reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(r[0], r[1], r[2], (T)0);
+  if (A.epi == EPI_KICK_DRIFT) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { A.x_new[d * ld + gi] = xx[d]; A.v[d * ld + gi] = vv[d]; }
+    reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(r[0], r[1], r[2], (T)0);
+  } else {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { A.f[d * ld + gi] = tot[d]; A.v[d * ld + gi] = vv[d]; }
+  }
   return d2;
 }
 
