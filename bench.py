@@ -300,6 +300,19 @@ def run_ours(args, rk) -> None:
         "peak_conflict_free": 148 * sm_clock * 32 / 4 / 1e9,
         "frac_of_conflict_free": gathers_per_s / (148 * sm_clock * 32 / 4),
         "note": "DESIGN.md 6: ncu l1tex__data_pipe_lsu_wavefronts 84 % of peak at ~9 wavefronts per warp gather"}
+    # the other heavy kernel: the list build, ALU-bound.  Tests = N x 27 x atoms per cell; peak = fp32
+    # lanes x clock / 5 lane-instructions per test (3 packed sub/fma pairs = 3, compare, emit), 148 SMs x 128 lanes
+    ncell = float(st["ncells"][0] * st["ncells"][1] * st["ncells"][2])
+    tests = 27.0 * w.natoms * w.natoms / ncell
+    ms_build = st["ms_build_in_run"] / max(1, st["nbuilds_in_run"])
+    peak_tests = 148 * 128 * 1.965e9 / 5.0
+    roofline_build = {
+        "kernel": "k_build_list (+ bin, sort, reorder, tables: the whole build)", "bound": "alu",
+        "achieved": tests / (ms_build * 1e-3) / 1e12 if ms_build > 0 else 0.0, "peak": peak_tests / 1e12, "unit": "T distance tests/s",
+        "frac": tests / (ms_build * 1e-3) / peak_tests if ms_build > 0 else 0.0, "ms_per_build": ms_build,
+        "builds_per_step": st["nbuilds_in_run"], "tests_per_build": tests,
+        "note": "peak counts 5 fp32 lane-instructions per candidate test at 148 SMs x 128 lanes x 1.965 GHz; a cell holds "
+                "~20 atoms for 32 lanes and each accepted entry costs a store and a pointer update (DESIGN.md 6)"}
     if not rk.is_root:
         return
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")    # written by hand from an ncu --set full capture
@@ -350,7 +363,7 @@ def run_ours(args, rk) -> None:
                    "parallelism": "replicas x%d (no collective)" % rk.world,
                    "l2": "L2 flushed between passes (2x126 MB write)" if dev_run["flushed_l2"] else
                          "inputs larger than L2 (state + list >> 126 MB)"},
-        "clocks": clocks, "roofline": roofline,
+        "clocks": clocks, "roofline": roofline, "roofline_build": roofline_build,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * 24 * w.natoms, "d2h_bytes_per_step": 24 * w.natoms + 8,
                 "ms_per_step": sum(e2e_run["wall_ms"]) / nruns},
         "gpu_launches": int(launches),
