@@ -408,6 +408,50 @@ def test_sparse_gas_empty_cells_and_zero_steps():
             assert abs(E - Eo) <= (1e-12 if prec == md.MD_FP64 else 2e-6) * max(abs(Eo), 1e-300)
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("kernel,list_kind", [(0, 0), (1, 0), (5, 0), (2, 0), (3, 0), (4, 0), (1, 1)])
+def test_non_cubic_box_ragged_tiles(kernel, list_kind, precision):
+    """A box with 5 x 4 x 3 cells: tile shapes are clipped to the box, the last tile of a dimension is narrower
+    than the others, every tile sees periodic images.  Pair set, forces, energy and virial against brute force."""
+    a = wl.LJ_A
+    nx, ny, nz = 9, 7, 6
+    base = np.array([[0, 0, 0], [.5, .5, 0], [.5, 0, .5], [0, .5, .5]])
+    g = np.stack(np.meshgrid(np.arange(nx), np.arange(ny), np.arange(nz), indexing="ij"), axis=-1).reshape(-1, 1, 3)
+    x = ((g + base[None]) * a).reshape(-1, 3)
+    box = np.array([nx, ny, nz]) * a
+    N = x.shape[0]
+    x = x + wl.uniform_displacements(5, np.arange(N, dtype=np.uint64), 0.15)
+    x -= np.floor(x / box) * box
+    rc, skin = 2.5, 0.3
+    s = md.System(box, N, np.zeros(N, np.int32), np.array([1.0]))
+    s.md_set_precision(precision)
+    s.md_set_neighbor(list_kind, kernel)
+    s.md_set_pair(md.MD_PAIR_LJ126, (1.0, 1.0), rc, skin)
+    s.md_set_positions(x)
+    s.md_build_neighbors()
+    st = s.md_get_stats()
+    assert st["ncells"] == [5, 4, 3]
+    nn, nb = _gpu_rows(s, N, 160)
+    got = {(min(i, int(j)), max(i, int(j))) for i in range(N) for j in nb[i, :nn[i]]}
+    sure, fuzzy = _oracle_pairs(x, box, rc + skin)
+    assert sure <= got and got <= (sure | fuzzy)
+    assert int(nn.sum()) == (len(got) if list_kind else 2 * len(got))
+    f = np.zeros((N, 3))
+    E, W = s.md_compute_forces(f, energy=True, virial=True)
+    fo, Eo, Wo, _, _ = oracle.forces_brute(x, box, oracle.PAIR_LJ, (1.0, 1.0), rc)
+    if precision == md.MD_FP64:
+        assert _fp64_force_err(f, fo) < 1e-12 and abs(E - Eo) < 1e-12 * abs(Eo)
+        assert np.abs(W - Wo).max() < 1e-11 * np.abs(Wo).max()
+    else:
+        assert _rel_rms(f, fo) < 1e-5 and abs(E - Eo) < 1e-6 * abs(Eo)
+    s.md_set_velocities(np.zeros((N, 3)))
+    s.md_run(30, 0.004)                       # crosses rebuilds as the perturbed lattice relaxes
+    xg = np.zeros((N, 3)); s.md_get_positions(xg); s.md_get_forces(f)
+    fo = oracle.forces(xg, box, oracle.PAIR_LJ, (1.0, 1.0), rc)[0]
+    assert (_fp64_force_err(f, fo) < 1e-12) if precision == md.MD_FP64 else (_rel_rms(f, fo) < 1e-5)
+    s.close()
+
+
 def test_two_types_select_masses():
     w = wl.make(1, n_override=6)
     types = (np.arange(w.natoms) % 2).astype(np.int32)
