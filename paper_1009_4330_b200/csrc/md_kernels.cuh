@@ -1,16 +1,16 @@
 // md_kernels.cuh -- device code of the B200-native MD hot path (sm_100a).
 //
 // Design in one paragraph (details in DESIGN.md).  Atoms are counting-sorted into cells of edge
-// >= rc+skin, the cells themselves ordered TILE-major: a tile ("brick") is a box of b^3 cells whose
-// atoms are contiguous in memory.  Every heavy kernel is one thread block per tile: it stages the tile's
-// interior cells plus a one-cell halo (periodic images resolved while staging) into shared memory as
-// TILE-CENTRED coordinates -- fp32 in mixed mode, which is what makes fp32 pair math accurate enough in
-// a 168-sigma box -- and then runs the paper's neighbor-list loop against shared
-// memory: the "random access" load of atom j (L100) is two LDS.64, not a texture/L1 gather, and the list
-// holds 16-bit tile-local slot codes, eight to a 128-bit word, so the index stream is half the classic
-// 4 B/entry.  One template covers thread-per-atom (K=1), sub-warp (K=8) and warp-per-atom (K=32, the
-// paper's BpA with a shuffle reduction instead of a block reduction).  The force kernel's epilogue can
-// also do the velocity-Verlet kick and drift, so a time step between rebuilds is ONE launch.
+// >= rc+skin, the cells themselves ordered TILE-major: a tile is a box of bx x by x bz cells whose atoms
+// are contiguous in memory.  Every heavy kernel is one thread block per tile: it stages the tile's cells
+// plus a one-cell halo (periodic images resolved while staging) into shared memory as TILE-CENTRED
+// coordinates -- fp32 in mixed mode, which is what makes fp32 pair math accurate enough in a 168-sigma
+// box -- and then runs the paper's neighbor-list loop against shared memory: the
+// "random access" load of atom j (L100) is one 128-bit shared-memory load, not a texture/L1 gather, and
+// the list holds 16-bit tile-local slot codes, eight to a 128-bit word, so the index stream is half the
+// classic 4 B/entry.  One template covers thread-per-atom (K=1), sub-warp (K=4, 8) and warp-per-atom
+// (K=32, the paper's BpA with a shuffle reduction instead of a block reduction).  The force kernel's
+// epilogue also does the velocity-Verlet kick and drift, so a time step between rebuilds is ONE launch.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -18,11 +18,11 @@
 
 namespace mdk {
 
-constexpr int MAX_TILE_CELLS = 216;    // (b+2)^3 <= 216  =>  b <= 4
+constexpr int MAX_TILE_CELLS = 216;    // (bx+2)(by+2)(bz+2) <= 216, each of bx, by, bz <= 4
 constexpr int BUILD_THREADS = 256;     // threads per block of the list-build (when three blocks fit an SM) and cell-list kernels
 constexpr int BUILD_MAX_THREADS = 384; // list build: block size when only two blocks fit an SM
 constexpr int FORCE_MAX_THREADS = 640; // upper bound of the force kernels' block size (runtime choice)
-constexpr int FORCE_MIN_BLOCKS = 2;    // resident blocks per SM the mixed-precision force kernels are compiled for (<= 48 registers)
+constexpr int FORCE_MIN_BLOCKS = 2;    // the mixed-precision force kernels are compiled for <= 48 registers: two 640-thread or three 416-thread blocks per SM
 #ifndef MDK_BUILD_MIN_BLOCKS
 #define MDK_BUILD_MIN_BLOCKS 2
 #endif
