@@ -101,3 +101,15 @@ def test_bench_reference_arm_other_ranks_do_no_work():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"], env=env,
                          capture_output=True, text=True, timeout=120)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_sweep_module_fails_loudly_without_a_gpu():
+    """The measurement helper has no CPU fallback either."""
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("needs a box without a GPU")
+    r = subprocess.run([sys.executable, "-m", "paper_1009_4330_b200.sweep", "--cells", "6", "--rc", "2.5"], capture_output=True, text=True,
+                       cwd=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    assert r.returncode != 0 and "no CUDA device" in (r.stderr + r.stdout)
