@@ -299,7 +299,7 @@ def run_ours(args, rk) -> None:
         "achieved": gathers_per_s / 1e9, "unit": "G gathered entries/s",
         "peak_conflict_free": 148 * sm_clock * 32 / 4 / 1e9,
         "frac_of_conflict_free": gathers_per_s / (148 * sm_clock * 32 / 4),
-        "note": "DESIGN.md 6: ncu l1tex__data_pipe_lsu_wavefronts 84 % of peak at ~9 wavefronts per warp gather"}
+        "note": "DESIGN.md 6: ncu l1tex__data_pipe_lsu_wavefronts 89 % of peak at ~9 wavefronts per warp gather (cfg 5)"}
     # the other heavy kernel: the list build, ALU-bound.  Tests = N x 27 x atoms per cell; peak = fp32
     # lanes x clock / 5 lane-instructions per test (3 packed sub/fma pairs = 3, compare, emit), 148 SMs x 128 lanes
     ncell = float(st["ncells"][0] * st["ncells"][1] * st["ncells"][2])
@@ -355,7 +355,10 @@ def run_ours(args, rk) -> None:
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": rk.world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32 pair math, f64 accumulate/integrate" if w.precision == wl.PREC_MIXED else "f64", "data": "synthetic",
+        "dtype": "f32" if w.precision == wl.PREC_MIXED else "f64",
+        "dtype_detail": ("pair terms in f32 on tile-centred coordinates; per-atom force, energy and virial accumulators, positions, "
+                         "velocities, integration and the list's distance decisions in f64 (BASELINE.json: fp32 compute / fp64 accumulate)")
+                        if w.precision == wl.PREC_MIXED else "everything in f64", "data": "synthetic",
         "config": {"workload": "cfg%d: %s" % (args.cfg, w.name), "natoms": w.natoms, "time_steps_per_step": w.nsteps,
                    "rc": w.rc, "skin": w.skin, "dt": w.dt, "list": "half" if args.half else "full",
                    "variant": md.KERNEL_NAMES[st["kernel_variant"]], "mean_neighbors": st["mean_neighbors"],
