@@ -199,7 +199,10 @@ void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   double per_cell = (double)s->N / g.ncell + 1.5;   // cells are padded to multiples of 4 slots
   double staged = per_cell * (g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2);
   double interior = per_cell * g.b[0] * g.b[1] * g.b[2];
-  g.tile_cap = (int)(staged * 1.2 * s->cap_scale_tile + 64);
+  // slack over the mean: five standard deviations of a Poisson count (a liquid fluctuates less), i.e. 7 % for the
+  // ~5000 staged atoms of an rc = 5 sigma tile and 9 % at cfg 5, where a flat 20 % would cost a resident block;
+  // an overflow is detected by the kernels and re-planned with a larger factor
+  g.tile_cap = (int)(staged * (1.0 + 5.0 / std::sqrt(std::max(staged, 1.0))) * s->cap_scale_tile + 64);
   g.tile_cap = (g.tile_cap + 7) & ~7;
   g.interior_cap = (int)(interior * 1.25 * s->cap_scale_int + 32);
   g.interior_cap = (g.interior_cap + 31) & ~31;
@@ -579,6 +582,7 @@ int autotune(md_system* s, int nrep, double* ms_out) {
     for (int k = 0; k < 4; ++k) {
       s->kernel_eff = cand[k];
       s->brick_forced = off == 0 ? 0 : 9 + off;
+      s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;   // an overflow of one shape must not inflate the next
       s->planned = false;
       rc = build(s, true);
       if (rc == MD_ERR_OVERFLOW && off != 0) continue;   // this shape does not fit with this many lanes per atom
@@ -599,6 +603,7 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   }
   s->kernel_eff = best;
   s->brick_forced = best_b;
+  s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;
   s->autotuned = true;
   s->planned = false;
   s->list_valid = false;
