@@ -721,11 +721,12 @@ __device__ __noinline__ unsigned build_scan_careful(const Geom& gs, const TileTa
 // The fast scan of nq quads of candidates (staged slots off/4 ..) for one lane: packed fp32 distance test, accepted
 // codes to the lane's ring, m = min |r2 - rl2| (the guard-band detector).  SELF: the candidates are the lane's own
 // cell, skip the code `self`.
-template <bool SELF, int SHIFT>
+template <bool SELF, int SHIFT, int FIXED>
 __device__ __forceinline__ void build_scan_fast(unsigned& rp, float& m, unsigned xs_a, unsigned ys_a, unsigned zs_a, unsigned off,
                                                 unsigned code, int nq, f32x2 xi2, f32x2 yi2, f32x2 zi2, f32x2 mid2, float hi,
                                                 unsigned self) {
-#pragma unroll 2
+  if constexpr (FIXED > 0) nq = FIXED;   // the common full piece: a constant trip count, no loop bookkeeping
+#pragma unroll 4
   for (int q = 0; q < nq; ++q) {
     f32x2 X01, X23, Y01, Y23, Z01, Z23;
     lds_2x2(xs_a + off, X01, X23);
@@ -902,8 +903,9 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
           }
           const unsigned rp_seg = rp;
           float m = 1e30f;
-          if (own) build_scan_fast<true, SHIFT>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
-          else build_scan_fast<false, SHIFT>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
+          if (own) build_scan_fast<true, SHIFT, 0>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
+          else if (nq == 8) build_scan_fast<false, SHIFT, 8>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
+          else build_scan_fast<false, SHIFT, 0>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
           if (__builtin_expect(m <= bw, 0)) {
             // some candidate of this piece lies in the guard band of the fp32 test: redo the piece, deciding the
             // in-band candidates in fp64 from the global positions (the pair set is exactly the fp64 one)
