@@ -452,6 +452,53 @@ def test_non_cubic_box_ragged_tiles(kernel, list_kind, precision):
     s.close()
 
 
+@pytest.mark.parametrize("seed", list(range(16)))
+def test_randomised_boxes_densities_cutoffs(seed):
+    """Seeded random geometry: orthogonal boxes with unequal edges, densities from a dilute gas to a dense fluid
+    (a jittered simple-cubic lattice with random vacancies, so no two atoms overlap), cutoffs and skins that move
+    the cell grid from 3 to 6 cells per edge, every variant and both precisions in turn.  Pair set against the
+    brute-force enumeration; forces, energy, virial against the O(N^2) definition."""
+    rs = np.random.RandomState(1000 + seed)
+    rc = float(rs.uniform(1.6, 2.6)); skin = float(rs.uniform(0.0, 0.5)); rl = rc + skin
+    edges = rl * rs.uniform(3.02, 6.3, size=3)
+    a = float(rs.uniform(0.95, 1.6))                                    # lattice spacing: density a^-3 x occupancy
+    n = np.maximum(np.floor(edges / a).astype(int), 1)
+    box = n * a
+    box = np.maximum(box, 3.001 * rl)
+    g = np.stack(np.meshgrid(*[np.arange(k) for k in n], indexing="ij"), axis=-1).reshape(-1, 3).astype(float)
+    keep = rs.uniform(size=len(g)) < rs.uniform(0.25, 1.0)
+    x = (g[keep] + 0.5) * (box / n) + rs.uniform(-0.12, 0.12, size=(int(keep.sum()), 3)) * a
+    x += box * rs.randint(-2, 3, size=x.shape)                          # any periodic image on input
+    N = x.shape[0]
+    kernel, list_kind = [(0, 0), (1, 0), (5, 0), (2, 0), (3, 0), (4, 0), (1, 1), (0, 0)][seed % 8]
+    precision = (seed // 8) % 2
+    s = md.System(box, N, np.zeros(N, np.int32), np.array([1.0]))
+    s.md_set_precision(precision)
+    s.md_set_neighbor(list_kind, kernel)
+    s.md_set_pair(md.MD_PAIR_LJ126, (1.0, 1.0), rc, skin)
+    s.md_set_positions(x)
+    s.md_build_neighbors()
+    nn, nb = _gpu_rows(s, N, 256)
+    got = {(min(i, int(j)), max(i, int(j))) for i in range(N) for j in nb[i, :nn[i]]}
+    xw = x - np.floor(x / box) * box
+    sure, fuzzy = _oracle_pairs(xw, box, rl)
+    assert sure <= got and got <= (sure | fuzzy)
+    assert int(nn.sum()) == (len(got) if list_kind else 2 * len(got))
+    f = np.zeros((N, 3))
+    E, W = s.md_compute_forces(f, energy=True, virial=True)
+    fo, Eo, Wo, _, _ = oracle.forces_brute(xw, box, oracle.PAIR_LJ, (1.0, 1.0), rc)
+    if precision == md.MD_FP64:
+        assert _fp64_force_err(f, fo) < 1e-12
+        assert abs(E - Eo) < 1e-12 * max(abs(Eo), 1.0) and np.abs(W - Wo).max() < 1e-11 * max(np.abs(Wo).max(), 1.0)
+    else:
+        # a random dense configuration has large repulsive and attractive terms that cancel in E; the fp32 pair terms
+        # are accurate to 1e-6 of the terms themselves, so the energy is judged against sum |u_pair|
+        _, _, r2 = oracle.pairs_brute(xw, box, rc, with_r2=True)
+        uabs = float(np.abs(4.0 * (r2 ** -6 - r2 ** -3)).sum())
+        assert _rel_rms(f, fo) < 1e-5 and abs(E - Eo) < 1e-6 * max(uabs, 1.0)
+    s.close()
+
+
 def test_two_types_select_masses():
     w = wl.make(1, n_override=6)
     types = (np.arange(w.natoms) % 2).astype(np.int32)
