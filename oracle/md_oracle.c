@@ -143,7 +143,7 @@ void orc_forces_brute(int64_t N, const double* x, const double* box, const orc_p
         }
       }
   } else {
-    double* rho = (double*)calloc((size_t)N, sizeof(double));
+    double* rho = (double*)calloc(N > 0 ? (size_t)N : 1, sizeof(double));
     for (int64_t i = 0; i < N; ++i)
       for (int64_t j = i + 1; j < N; ++j) {
         double r2 = 0.0;
