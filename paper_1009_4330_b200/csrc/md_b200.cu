@@ -161,7 +161,7 @@ size_t force_smem(const md_system* s, const Geom& g, bool half) {
 }
 size_t cell_smem(const md_system* s, const Geom& g) { return sizeof(TileTables) + 4 * (size_t)capA_of(g) * elem_size(s) + 16; }
 size_t build_smem(const Geom& g, int threads) {
-  return sizeof(TileTables) + (size_t)tile_tab_cells(g) * 16 + BUILD_TASK_INTS * sizeof(int) + 3 * (size_t)capA_of(g) * sizeof(float) +
+  return sizeof(TileTables) + (size_t)tile_tab_cells(g) * 16 + (size_t)build_rowcell_len(g) * 2 + 3 * (size_t)capA_of(g) * sizeof(float) +
          (size_t)threads * RING_STRIDE + 16;
 }
 // threads per block of the list build: 256 when three such blocks fit an SM's shared memory, else 384 (two blocks):

@@ -27,7 +27,6 @@ constexpr int FORCE_MIN_BLOCKS = 2;    // the mixed-precision force kernels are 
 #define MDK_BUILD_MIN_BLOCKS 2
 #endif
 constexpr int BUILD_MIN_BLOCKS = MDK_BUILD_MIN_BLOCKS;    // with BUILD_MAX_THREADS: <= 85 registers, i.e. three 256-thread or two 384-thread blocks per SM
-constexpr int BUILD_TASK_INTS = 72;     // list-build: room for the first-task table of <= 64 interior cells (+1), 16-byte multiple
 constexpr int RING = 48;               // list-build: pending entries a lane can hold in shared memory (>= 32 + 8)
 constexpr int RING_STRIDE = RING * 2 + 16;   // bytes between the rings of neighbouring lanes (odd * 16)
 
@@ -621,6 +620,7 @@ struct BuildArgs {
 };
 
 __device__ __forceinline__ int build_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
+__host__ __device__ inline int build_rowcell_len(const Geom& g) { return ((g.interior_cap >> 2) + 15) & ~7; }   // u16 entries, 16-byte multiple
 
 __device__ __noinline__ bool confirm_pair_fp64(const Geom& g, const TileTables& tt, const double* __restrict__ x, size_t ld,
                                                int gi, int ti, int gj, int tj, double rl2) {
@@ -754,7 +754,43 @@ __device__ __forceinline__ void build_scan_fast(unsigned& rp, float& m, unsigned
   }
 }
 
-// Shared memory: TileTables | offs[tile cells] float4 | xs[capA] ys[capA] zs[capA] floats | rings[nwarps*32*RING_STRIDE].
+// The same when the lanes of the warp hold different numbers of quads (their atoms belong to different cells): the
+// warp runs nqmax rounds; a lane that has used up its nq quads reads the far-away dummy quad at off_dummy instead.
+template <bool SELF, int SHIFT>
+__device__ __forceinline__ void build_scan_ragged(unsigned& rp, float& m, unsigned xs_a, unsigned ys_a, unsigned zs_a, unsigned off,
+                                                  unsigned code, int nq, int nqmax, unsigned off_dummy, f32x2 xi2, f32x2 yi2, f32x2 zi2,
+                                                  f32x2 mid2, float hi, unsigned self) {
+#pragma unroll 2
+  for (int q = 0; q < nqmax; ++q) {
+    const unsigned o = q < nq ? off : off_dummy;
+    f32x2 X01, X23, Y01, Y23, Z01, Z23;
+    lds_2x2(xs_a + o, X01, X23);
+    lds_2x2(ys_a + o, Y01, Y23);
+    lds_2x2(zs_a + o, Z01, Z23);
+    const f32x2 dx01 = sub2(xi2, X01), dx23 = sub2(xi2, X23);
+    const f32x2 dy01 = sub2(yi2, Y01), dy23 = sub2(yi2, Y23);
+    const f32x2 dz01 = sub2(zi2, Z01), dz23 = sub2(zi2, Z23);
+    const f32x2 q01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
+    const f32x2 q23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
+    float e0, e1, e2, e3;
+    unpack2(sub2(q01, mid2), e0, e1);
+    unpack2(sub2(q23, mid2), e2, e3);
+    m = fminf(fminf(m, fabsf(e0)), fabsf(e1));
+    m = fminf(fminf(m, fabsf(e2)), fabsf(e3));
+    if constexpr (SELF) {
+      ring_push2_self(rp, code, code + (1u << SHIFT), q01, hi, self);
+      ring_push2_self(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi, self);
+    } else {
+      ring_push2(rp, code, code + (1u << SHIFT), q01, hi);
+      ring_push2(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi);
+    }
+    off += 16;
+    code += 4u << SHIFT;
+  }
+}
+
+// Shared memory: TileTables | offs[tile cells] float4 | rowcell[interior_cap/4 + 8] u16 | xs[capA] ys[capA] zs[capA] floats |
+// rings[nwarps*32*RING_STRIDE].
 template <bool HALF, int LOGK, int SHIFT>
 __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_list(BuildArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -763,8 +799,8 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
   constexpr int K = 1 << LOGK;
   const int capA = build_capA(g);
   float4* offs = reinterpret_cast<float4*>(smem_raw + sizeof(TileTables));
-  int* task0 = reinterpret_cast<int*>(offs + tile_tab_cells(g));   // [nic + 1] first task of each interior cell
-  float* xs = reinterpret_cast<float*>(task0 + BUILD_TASK_INTS);
+  unsigned short* rowcell = reinterpret_cast<unsigned short*>(offs + tile_tab_cells(g));   // tile cell of every quad of list rows
+  float* xs = reinterpret_cast<float*>(rowcell + build_rowcell_len(g));
   float* ys = xs + capA;
   float* zs = ys + capA;
   unsigned char* rings = reinterpret_cast<unsigned char*>(zs + capA);
@@ -778,12 +814,13 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
     soff[threadIdx.x] = (dz * tt.tc[1] + dy) * tt.tc[0] + dx;
   }
   if (tt.n_slots > g.tile_cap || tt.n_int_slots > g.interior_cap) return;   // host re-plans and rebuilds
-  // a task = 32 consecutive rows (atoms) of one interior cell; tasks are dealt to the warps round robin, so a tile
-  // of one big cell (rc = 5 sigma: ~150 atoms per cell) still keeps several warps busy
-  if (threadIdx.x == 0) {
-    int run = 0;
-    for (int ic = 0; ic < tt.nic; ++ic) { task0[ic] = run; run += (tt.cnt[interior_tile_cell(tt, ic)] + 31) >> 5; }
-    task0[tt.nic] = run;
+  // A task = 8 consecutive quads of list rows = 32 lanes, one atom each.  Rows are padded per cell to multiples of 4,
+  // so a quad belongs to one cell, but the 8 quads of a task may belong to different cells (a cell of ~20 atoms fills
+  // 5 quads): the lanes of a warp then walk different candidate runs of about the same length, in lockstep.  Tasks
+  // are dealt to the warps round robin, so a tile of one big cell (rc = 5 sigma: ~150 atoms) still keeps several busy.
+  for (int ic = threadIdx.x; ic < tt.nic; ic += blockDim.x) {
+    const int t = interior_tile_cell(tt, ic);
+    for (int i = 0; i < pad4(tt.cnt[t]) >> 2; ++i) rowcell[(tt.rstart[t] >> 2) + i] = (unsigned short)t;
   }
   // staging: tile-centred fp32 coordinates = packed cell-relative coordinate + the cell's offset (the same values the
   // force kernels stage), one thread per quad of slots, SoA so that four candidates are one broadcast 128-bit load
@@ -820,7 +857,9 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
       *reinterpret_cast<float4*>(ys + 4 * q) = make_float4(yv[0], yv[1], yv[2], yv[3]);
       *reinterpret_cast<float4*>(zs + 4 * q) = make_float4(zv[0], zv[1], zv[2], zv[3]);
     }
-    if (threadIdx.x == 0) { xs[tt.n_slots] = 1e15f; ys[tt.n_slots] = 1e15f; zs[tt.n_slots] = 1e15f; }   // the dummy slot
+    if (threadIdx.x < 4) {   // the dummy quad (its first slot is the dummy slot the list's padding names)
+      xs[tt.n_slots + threadIdx.x] = 1e15f; ys[tt.n_slots + threadIdx.x] = 1e15f; zs[tt.n_slots + threadIdx.x] = 1e15f;
+    }
   }
   __syncthreads();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -836,20 +875,20 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
   int my_max = 0;
   unsigned long long my_sum = 0;
 
-  const int ntasks = task0[tt.nic];
-  int ic = 0;
+  const int nrq = tt.n_int_slots >> 2;                 // quads of list rows in use
+  const unsigned off_dummy = 4u * (unsigned)tt.n_slots;
 #pragma unroll 1
-  for (int task = wid; task < ntasks; task += nw) {
-    while (task0[ic + 1] <= task) ++ic;
-    const int t = interior_tile_cell(tt, ic);
+  for (int task = wid; task * 8 < nrq; task += nw) {
+    const int rq = task * 8 + (lane >> 2);             // this lane's quad of rows
+    const bool haveq = rq < nrq;
+    const int t = rowcell[haveq ? rq : 0];             // its tile cell
     const int c = tt.cnt[t], g_lo = tt.gstart[t];
     {
-      const int r0 = (task - task0[ic]) << 5;
-      const bool act = r0 + lane < c;
-      const int kin = act ? r0 + lane : 0;
-      const int a = tt.rstart[t] + kin;             // list row
-      const int aslot = tt.start[t] + kin;          // staged slot
-      const int gi = g_lo + r0 + lane;
+      const int kin = haveq ? 4 * rq - tt.rstart[t] + (lane & 3) : c;   // index of the atom within its cell
+      const bool act = kin < c;
+      const int a = 4 * (haveq ? rq : 0) + (lane & 3);                  // list row
+      const int aslot = tt.start[t] + (act ? kin : 0);                  // staged slot
+      const int gi = g_lo + kin;
       // an idle lane sits far away from everything, pad slots (+1e15) included: it accepts nothing
       const float xi = act ? xs[aslot] : -1e15f, yi = act ? ys[aslot] : -1e15f, zi = act ? zs[aslot] : -1e15f;
       const f32x2 xi2 = pack2(xi, xi), yi2 = pack2(yi, yi), zi2 = pack2(zi, zi);
@@ -876,15 +915,15 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
 #pragma unroll 1
       for (int sc = 0; sc < NRUN; ++sc) {
         int tfirst, s0, s1;
-        bool own;
+        bool own;                                        // the run holds the atom's own cell (the same for all lanes)
         if constexpr (HALF) {
           tfirst = t + soff[sc];
-          own = tfirst == t;
-          // keep (i, j) iff j follows i in the sorted order; a cell is a contiguous range of that order, so for
-          // another cell the answer is the same for all of its atoms
-          if (!own && tt.gstart[tfirst] < g_lo) continue;
+          own = sc == 13;
           s0 = tt.start[tfirst];
           s1 = s0 + pad4(tt.cnt[tfirst]);
+          // keep (i, j) iff j follows i in the sorted order; a cell is a contiguous range of that order, so for
+          // another cell the answer is the same for all of its atoms
+          if (!own && tt.gstart[tfirst] < g_lo) s1 = s0;
         } else {
           const int tc = t + soff[3 * sc + 1];
           tfirst = tc - 1;
@@ -892,21 +931,32 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
           s0 = tt.start[tc - 1];
           s1 = tt.start[tc + 1] + pad4(tt.cnt[tc + 1]);
         }
+        // (a lane without an atom scans its quad's runs like the others, so that full pieces stay uniform; it sits
+        // far away and accepts nothing)
+        const int npieces = (int)__reduce_max_sync(0xffffffffu, (unsigned)((s1 - s0 + 31) >> 5));
 #pragma unroll 1
-        for (int j0 = s0; j0 < s1; j0 += 32) {   // pieces of <= 32 slots: what the ring is guaranteed to take
+        for (int pc = 0; pc < npieces; ++pc) {   // pieces of <= 32 slots: what the ring is guaranteed to take
+          const int j0 = s0 + 32 * pc;
+          const int nq = max(0, min(8, (s1 - j0) >> 2));
           if ((int)(rp - rbase) > 2 * (RING - 32)) flush();
-          const int nq = min(8, (s1 - j0) >> 2);
           if (HALF && own) {
             // own cell: slot order is the sorted order
-            rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, aslot, aslot, rp, j0, 4 * nq, tfirst, SHIFT);
+            if (nq > 0)
+              rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, aslot, aslot, rp, j0, 4 * nq, tfirst, SHIFT);
             continue;
           }
           const unsigned rp_seg = rp;
           float m = 1e30f;
-          if (own) build_scan_fast<true, SHIFT, 0>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
-          else if (nq == 8) build_scan_fast<false, SHIFT, 8>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
-          else build_scan_fast<false, SHIFT, 0>(rp, m, xs_a, ys_a, zs_a, 4u * (unsigned)j0, (unsigned)j0 << SHIFT, nq, xi2, yi2, zi2, mid2, hi, selfcode);
-          if (__builtin_expect(m <= bw, 0)) {
+          const unsigned off = 4u * (unsigned)j0, code = (unsigned)j0 << SHIFT;
+          if (__all_sync(0xffffffffu, nq == 8)) {
+            if (own) build_scan_fast<true, SHIFT, 8>(rp, m, xs_a, ys_a, zs_a, off, code, 8, xi2, yi2, zi2, mid2, hi, selfcode);
+            else build_scan_fast<false, SHIFT, 8>(rp, m, xs_a, ys_a, zs_a, off, code, 8, xi2, yi2, zi2, mid2, hi, selfcode);
+          } else {
+            const int nqmax = (int)__reduce_max_sync(0xffffffffu, (unsigned)nq);
+            if (own) build_scan_ragged<true, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, nqmax, off_dummy, xi2, yi2, zi2, mid2, hi, selfcode);
+            else build_scan_ragged<false, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, nqmax, off_dummy, xi2, yi2, zi2, mid2, hi, selfcode);
+          }
+          if (__builtin_expect(m <= bw && nq > 0, 0)) {
             // some candidate of this piece lies in the guard band of the fp32 test: redo the piece, deciding the
             // in-band candidates in fp64 from the global positions (the pair set is exactly the fp64 one)
             rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, own ? aslot : -1, -1, rp_seg, j0, 4 * nq,
@@ -924,7 +974,7 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
         nwords = before;   // count below from complete words + rem
       }
       const int n = nwords * 8 + rem;
-      if (!act && r0 + lane < pad4(c)) A.numneigh[(size_t)tile * g.interior_cap + tt.rstart[t] + r0 + lane] = 0;   // pad row
+      if (!act && haveq) A.numneigh[(size_t)tile * g.interior_cap + a] = 0;   // pad row
       if (act) {
         const int stored = n < g.row_cap ? n : g.row_cap;
         A.numneigh[(size_t)tile * g.interior_cap + a] = stored;
