@@ -419,7 +419,8 @@ int build(md_system* s, bool need_list) {
     }
     CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
               s->perm));
-    CK(launch(s, k_sort_cells, blocks_for(g.ncell, 8), 256, 0, g.ncell, (const int*)s->cell_start, s->perm));   // a warp per cell
+    CK(launch(s, k_sort_cells, std::min<unsigned>(blocks_for(g.ncell, 8), 148u * 8u), 256, 0, g.ncell, (const int*)s->cell_start,
+              s->perm));   // a warp per cell, grid-stride
     if (s->precision == MD_FP64)
       CK(launch(s, k_permute<double>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
                 (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (double4*)s->xr[xo], s->ld));

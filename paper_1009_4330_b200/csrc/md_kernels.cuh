@@ -531,21 +531,23 @@ __device__ __forceinline__ void sort_cell_by_warp(int lo, int n, int lane, int* 
 }
 __global__ void __launch_bounds__(256) k_sort_cells(int ncell, const int* __restrict__ cell_start, int* __restrict__ perm) {
   const int lane = threadIdx.x & 31;
-  const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (c >= ncell) return;
-  const int lo = cell_start[c], n = cell_start[c + 1] - lo;
-  if (n <= 1) return;
-  if (n <= 32) sort_cell_by_warp<1>(lo, n, lane, perm);
-  else if (n <= 64) sort_cell_by_warp<2>(lo, n, lane, perm);
-  else if (n <= 128) sort_cell_by_warp<4>(lo, n, lane, perm);
-  else if (n <= 256) sort_cell_by_warp<8>(lo, n, lane, perm);
-  else if (n <= 32 * SORT_PER) sort_cell_by_warp<SORT_PER>(lo, n, lane, perm);
-  else if (lane == 0)
-    for (int a = lo + 1; a < lo + n; ++a) {
-      int key = perm[a], b = a - 1;
-      while (b >= lo && perm[b] > key) { perm[b + 1] = perm[b]; --b; }
-      perm[b + 1] = key;
-    }
+  const int nwarps = gridDim.x * (blockDim.x >> 5);
+  for (int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); c < ncell; c += nwarps) {   // a warp per cell, grid-stride
+    const int lo = cell_start[c], n = cell_start[c + 1] - lo;
+    if (n <= 1) continue;
+    if (n <= 32) sort_cell_by_warp<1>(lo, n, lane, perm);
+    else if (n <= 64) sort_cell_by_warp<2>(lo, n, lane, perm);
+    else if (n <= 128) sort_cell_by_warp<4>(lo, n, lane, perm);
+    else if (n <= 256) sort_cell_by_warp<8>(lo, n, lane, perm);
+    else if (n <= 32 * SORT_PER) sort_cell_by_warp<SORT_PER>(lo, n, lane, perm);
+    else if (lane == 0)
+      for (int a = lo + 1; a < lo + n; ++a) {
+        int key = perm[a], b = a - 1;
+        while (b >= lo && perm[b] > key) { perm[b + 1] = perm[b]; --b; }
+        perm[b + 1] = key;
+      }
+    __syncwarp();
+  }
 }
 
 // a2: spatial reorder of the per-atom arrays; x0 := x (reference for the displacement test)
