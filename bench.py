@@ -210,7 +210,6 @@ def time_workload(torch, md, w, stream, steps: int, warmup: int, kernel: int, li
             if scratch is not None:
                 _flush_l2(torch, scratch)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            l0 = s.md_get_stats()["launches_total"]
             stream.synchronize()
             t0 = time.perf_counter()
             e0.record(stream)
@@ -219,14 +218,16 @@ def time_workload(torch, md, w, stream, steps: int, warmup: int, kernel: int, li
             s.md_run(w.nsteps, w.dt)
             if host_io:
                 s.md_get_positions(x_out)
-                ke = s.md_get_stats()["kinetic_energy"]
+                ke = s.md_kinetic_energy()
             e1.record(stream)
             stream.synchronize()
             t1 = time.perf_counter()
             if it >= warmup:
                 times.append(e0.elapsed_time(e1)); wall.append(1e3 * (t1 - t0))
                 st = s.md_get_stats()
-                launches += st["launches_total"] - l0 - 1     # minus the k_kinetic of this trailing stats call
+                # the library's own launches inside the timed region: md_run's, the two scatter kernels of
+                # md_set_positions / md_set_velocities and, with host buffers, the gather + kinetic-energy kernels
+                launches += st["launches_last_run"] + 2 + (2 if host_io else 0)
         if st is None:
             st = s.md_get_stats()
         s.close()

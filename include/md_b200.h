@@ -89,10 +89,10 @@ typedef struct md_stats {
   int32_t ntiles;              /* thread blocks per force launch */
   int32_t tile_capacity;       /* staged atoms a tile can hold */
   int32_t max_tile_atoms;      /* largest staged count seen at the last build */
-  int32_t max_neighbors;       /* longest list row at the last build */
+  int32_t max_neighbors;       /* most neighbors of any atom in the current list (exact fp64 pair set, counted on demand) */
   int32_t row_capacity;        /* list row capacity (entries) */
   int32_t list_balanced;       /* 1: the current list's rows have been permuted for conflict-free gathers (long-lived lists only) */
-  double mean_neighbors;       /* mean list row length at the last build */
+  double mean_neighbors;       /* mean neighbors per atom in the current list (exact fp64 pair set, counted on demand) */
   double kinetic_energy;       /* 1/2 sum m v^2 mvv2e at the time of the call */
   double ms_build;             /* device time of the last list build (bin+sort+build), CUDA events */
   double ms_force;             /* device time of the last md_compute_forces */
@@ -104,6 +104,11 @@ typedef struct md_stats {
   int64_t nforce_sampled;      /* how many steps were sampled (every ceil(nsteps/128)-th) */
   double ms_build_in_run;      /* summed device time of the list builds (bin+sort+reorder+build) */
   int64_t nbuilds_in_run;      /* list builds inside the last md_run */
+  /* the STORED rows: one per pair of consecutive atoms of a cell, holding the union of the two atoms' neighbors
+   * (a superset of the fp64 pair set, see md_get_neighbor_rows) */
+  int32_t max_row;             /* longest stored row at the last build */
+  int32_t reserved0;
+  double mean_row;             /* mean stored row length at the last build (entries per pair of atoms) */
 } md_stats;
 
 /* Creates a system: orthogonal periodic box [0,Lx) x [0,Ly) x [0,Lz), N atoms with type ids in
@@ -154,6 +159,19 @@ int md_get_forces(md_system* s, double* f);
  * (host or device int32 buffers).  Rows longer than stride are truncated (numneigh still holds the true
  * length).  Half lists hold each unordered pair in exactly one of the two rows. */
 int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride);
+
+/* The STORED list rows as they are, for checking the build itself (north_star (2)).
+ * The library keeps one row per PAIR of consecutive atoms of a cell: the union of the two atoms' neighbors by a
+ * conservative fp32 test (r^2 < (rc+skin)^2 (1 + band)), without the two atoms themselves; it is a superset of the
+ * fp64 pair sets that md_get_neighbors returns.  All three outputs are indexed by caller atom id (host or device
+ * int32 buffers): row_owner[i] = id of the first atom of i's pair (i itself if i is the first); numrow[i] =
+ * entries of the row if i is a first atom, else 0; entries[i x stride ..] = the row in caller ids (first atoms
+ * only; rows longer than stride are truncated, numrow still holds the true length). */
+int md_get_neighbor_rows(md_system* s, int32_t* row_owner, int32_t* numrow, int32_t* entries, int64_t stride);
+
+/* Kinetic energy 1/2 sum m v^2 mvv2e of the current velocities (host double; synchronises the stream).
+ * (NVE; the metric a time-stepping caller reads back.) */
+int md_kinetic_energy(md_system* s, double* ke_out);
 
 /* Setup-time mini benchmark of PAPER.md L137: on the current positions, builds the list and times nrep
  * force evaluations with each of TPA, SUBWARP, WARP and SUBWARP4, at the planner's tile width and its two

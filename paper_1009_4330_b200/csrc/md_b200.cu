@@ -13,6 +13,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <type_traits>
 #include <string>
 
@@ -61,7 +62,13 @@ struct md_system_impl {
   void* xr[2] = {nullptr, nullptr};   // packed cell-relative positions (Vec4<T>, 32 B per atom reserved), buffer index = xcur
   int* tab = nullptr;                 // per-tile tables of the last build
   size_t tab_alloc = 0;
-  int *cell_of = nullptr, *rank = nullptr, *perm = nullptr, *numneigh = nullptr;
+  int *cell_of = nullptr, *rank = nullptr, *perm = nullptr, *mkey = nullptr, *numneigh = nullptr;
+  int* nstat_d = nullptr;            // 4 ints: exact neighbor statistics of k_export_list (max; sum as 64 bits at [2])
+  int* export_buf = nullptr;         // staging for md_get_neighbors / md_get_neighbor_rows into host buffers
+  size_t export_alloc = 0;
+  bool counts_valid = false;         // max_nb_exact / mean_nb_exact belong to the current list
+  int max_nb_exact = 0;
+  double mean_nb_exact = 0;
   size_t numneigh_alloc = 0;
   int *cell_count = nullptr, *cell_start = nullptr;
   size_t cell_alloc = 0;
@@ -84,7 +91,7 @@ struct md_system_impl {
 
   // stats
   int64_t nsteps_total = 0, nbuilds = 0, nforce = 0, launches = 0, launches_last_run = 0;
-  int max_tile_atoms = 0, max_row = 0;
+  int max_tile_atoms = 0, max_row = 0;   // max_row / mean_row: the stored PAIR rows (union of the two atoms' neighbors)
   double mean_row = 0;
   double ms_build = 0, ms_force = 0, ms_run = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr, ev3 = nullptr;
@@ -93,7 +100,6 @@ struct md_system_impl {
   double ms_force_sampled = 0, ms_build_in_run = 0;
   int64_t nforce_sampled = 0, nbuilds_in_run = 0, nforce_sampled_acc = 0;
 
-  std::map<const void*, size_t> smem_set;
   std::string err;
 };
 
@@ -119,19 +125,40 @@ int fail(md_system* s, int code, const char* fmt, ...) {
     if (e_ != cudaSuccess) return fail(s, MD_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
   } while (0)
 
+// Kernels that need more than the default 48 KB of dynamic shared memory are opted in ONCE per process to the
+// device's maximum: the attribute belongs to the kernel (per context), not to a handle, so it must never be
+// lowered by another handle with a smaller tile geometry.
+std::mutex g_attr_mutex;
+std::map<const void*, int> g_attr_set;
+template <class Kern>
+cudaError_t opt_in_smem(Kern kern) {
+  const void* key = reinterpret_cast<const void*>(kern);
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(g_attr_mutex);
+  auto it = g_attr_set.find(key);
+  if (it != g_attr_set.end() && (it->second >> dev & 1)) return cudaSuccess;
+  int optin = 0;
+  e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return e;
+  cudaFuncAttributes fa;
+  e = cudaFuncGetAttributes(&fa, kern);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
+  if (e != cudaSuccess) return e;
+  g_attr_set[key] |= 1 << (dev & 31);
+  return cudaSuccess;
+}
+
 template <class Kern, class... Args>
 cudaError_t launch(md_system* s, Kern kern, unsigned grid, unsigned block, size_t smem, Args... args) {
   if (grid == 0) return cudaSuccess;
   if (smem > 40 * 1024) {   // static shared memory (reduction scratch) counts against the 48 KB default too
-    const void* key = reinterpret_cast<const void*>(kern);
-    auto it = s->smem_set.find(key);
-    if (it == s->smem_set.end() || it->second < smem) {
-      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-      if (e != cudaSuccess) return e;
-      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared);
-      if (e != cudaSuccess) return e;
-      s->smem_set[key] = smem;
-    }
+    cudaError_t e = opt_in_smem(kern);
+    if (e != cudaSuccess) return e;
   }
   kern<<<grid, block, smem, s->stream>>>(args...);
   s->launches++;
@@ -173,7 +200,7 @@ int build_threads(const Geom& g) {
   if (2 * (build_smem(g, BUILD_THREADS) + reserve) <= sm_total) return BUILD_THREADS;
   return BUILD_MAX_THREADS;   // one block per SM: as many warps as the kernel is compiled for
 }
-size_t export_smem(const Geom& g) { return sizeof(TileTables) + (size_t)capA_of(g) * sizeof(int) + 16; }
+size_t export_smem(const Geom& g) { return sizeof(TileTables) + (size_t)capA_of(g) * (2 * sizeof(int) + 2) + 16; }
 
 void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   double rl = s->rc + s->skin;
@@ -212,7 +239,9 @@ void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   double vol = s->box[0] * s->box[1] * s->box[2];
   double mean_nb = 4.0 / 3.0 * M_PI * rl * rl * rl * s->N / vol * (g.half ? 0.5 : 1.0);
   int unit = 8 * g.K;
-  g.row_cap = (int)(mean_nb * 1.5 * s->cap_scale_row + 24);
+  // a stored row is the union of the neighbors of two atoms ~1.4 sigma apart: ~1.4 x the single-atom mean (measured
+  // 1.38 in the LJ liquid), times the same 1.5 x slack over the mean as before
+  g.row_cap = (int)(mean_nb * 1.4 * 1.5 * s->cap_scale_row + 24);
   g.row_cap = ((g.row_cap + unit - 1) / unit) * unit;
   g.chunk_cap = g.row_cap / unit;
 }
@@ -275,16 +304,17 @@ int plan(md_system* s) {
   s->shape_index = pick; s->shape_count = nfeas;
   fill_geom_for_b(s, shapes[feasible[pick]].b, g);
   s->g = g;
-  // block size of the list force kernels: the tile's rows should fill whole rounds of the block
+  // block size of the list force kernels: the tile's pair rows should fill whole rounds of the block
   {
-    double rows = ((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.06 + 8.0;
+    double rows = 0.5 * (((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.06 + 8.0);
     double lanes = rows * g.K;
-    int tmax = FORCE_MAX_THREADS;
+    int tmax = s->precision == MD_FP64 ? FORCE_MAX_THREADS_WIDE : FORCE_MAX_THREADS;
+    if (force_smem(s, g, g.half) <= smem_three) tmax = std::min(tmax, 384);   // three resident blocks of <= 56 registers
     int rounds = (int)std::ceil(lanes / tmax);
     int t = (int)std::ceil(lanes / std::max(rounds, 1));
     t = ((t + 31) / 32) * 32;
     s->force_threads = std::min(std::max(t, 32), tmax);
-    if (const char* e = getenv("MD_B200_THREADS")) s->force_threads = std::min(std::max(atoi(e) / 32 * 32, 32), FORCE_MAX_THREADS);
+    if (const char* e = getenv("MD_B200_THREADS")) s->force_threads = std::min(std::max(atoi(e) / 32 * 32, 32), tmax);
   }
   // pair constants
   PairParams& P = s->P;
@@ -298,6 +328,7 @@ int plan(md_system* s) {
     P.A = s->params[0]; P.p = s->params[1]; P.B = s->params[2]; P.q = s->params[3];
     P.inv_r0 = 1.0 / s->params[4]; P.p_r0 = P.p * P.inv_r0; P.q_r0 = P.q * P.inv_r0;
   }
+  P.fill_float_copies();
   // (re)allocate what depends on the geometry
   if ((size_t)g.ncell + 1 > s->cell_alloc) {
     cudaFree(s->cell_count); cudaFree(s->cell_start);
@@ -305,14 +336,14 @@ int plan(md_system* s) {
     CK(dalloc(&s->cell_count, s->cell_alloc + s->cell_alloc / SCAN_BLOCK + 2));   // + the scan's block sums
     CK(dalloc(&s->cell_start, s->cell_alloc));
   }
-  size_t words = (size_t)g.ntiles * g.chunk_cap * g.interior_cap * g.K;
+  size_t words = (size_t)g.ntiles * g.chunk_cap * prow_cap(g) * g.K;
   if (words > s->list_words) {
     cudaFree(s->list);
     s->list = nullptr; s->list_words = 0;
     CK(dalloc(&s->list, words));
     s->list_words = words;
   }
-  size_t rows = (size_t)g.ntiles * g.interior_cap;
+  size_t rows = (size_t)g.ntiles * prow_cap(g);
   if (rows > s->numneigh_alloc) {
     cudaFree(s->numneigh);
     s->numneigh = nullptr; s->numneigh_alloc = 0;
@@ -341,16 +372,15 @@ int build_list_only(md_system* s) {
   const Geom& g = s->g;
   double rl = s->rc + s->skin;
   BuildArgs B{};
-  B.g = g; B.cell_start = s->cell_start; B.tab = s->tab; B.x = s->x[s->xcur]; B.ld = s->ld; B.rl2 = rl * rl;
+  B.g = g; B.tab = s->tab;
   B.xr = s->xr[s->xcur]; B.xr_double = s->precision == MD_FP64 ? 1 : 0;
   // guard band of the fp32 distance test: tile-centred coordinates up to E are
   // rounded to fp32, so r^2 carries a relative error of about (7 E / rl + 3) 2^-24; four times that is used.
+  // The stored rows are a superset of the fp64 pair set: everything with fp32 r^2 < rl^2 (1 + band).
   double E = 0;
   for (int d = 0; d < 3; ++d) E = std::max(E, 0.5 * (g.b[d] + 2) * g.edge[d] + s->skin);
   double band = 4.0 * (7.0 * E / rl + 3.0) * std::ldexp(1.0, -24);
-  B.rl2_mid = (float)(rl * rl);
-  B.rl2_bw = std::nextafterf((float)(rl * rl * band), INFINITY);
-  B.rl2_hi = B.rl2_mid + B.rl2_bw;      // the same fp32 sum the kernel's accept test and band test are consistent with
+  B.rl2_hi = std::nextafterf((float)(rl * rl * (1.0 + band)), INFINITY);
   B.list = s->list; B.numneigh = s->numneigh; B.flags = s->flags_d;
   const bool s4 = g.code_shift == 4;
   const int bt = build_threads(g);
@@ -400,6 +430,8 @@ int balance_rows(md_system* s) {
 
 int build(md_system* s, bool need_list) {
   if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set before building");
+  // nothing of the previous list survives a build, successful or not
+  s->list_valid = false; s->forces_valid = false; s->list_built_for_export = false; s->counts_valid = false;
   for (int attempt = 0; attempt < 6; ++attempt) {
     if (!s->planned) { int rc = plan(s); if (rc) return rc; }
     const Geom& g = s->g;
@@ -418,9 +450,9 @@ int build(md_system* s, bool need_list) {
       CK(launch(s, k_scan_cells, nblk, 1024, 0, g.ncell, (const int*)s->cell_count, (const int*)bsum, s->cell_start));
     }
     CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
-              s->perm));
+              s->perm, s->mkey));
     CK(launch(s, k_sort_cells, std::min<unsigned>(blocks_for(g.ncell, 8), 148u * 8u), 256, 0, g.ncell, (const int*)s->cell_start,
-              s->perm));   // a warp per cell, grid-stride
+              s->perm, s->mkey));   // a warp per cell, grid-stride
     if (s->precision == MD_FP64)
       CK(launch(s, k_permute<double>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
                 (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (double4*)s->xr[xo], s->ld));
@@ -450,7 +482,7 @@ int build(md_system* s, bool need_list) {
     if (again) { s->planned = false; continue; }
     s->max_tile_atoms = F.max_tile_atoms;
     s->max_row = F.max_row;
-    s->mean_row = (double)F.sum_rows / (double)s->N;
+    s->mean_row = (double)F.sum_rows / (0.5 * (double)s->N);   // entries per stored pair row
     s->list_valid = true;
     s->list_built_for_export = do_list;
     s->list_balanced = false;
@@ -476,23 +508,23 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
   using Body = BodyT<T, EV>;
   const Geom& g = s->g;
   const bool half = g.half != 0;
+  // the energy/virial and fp64 instantiations are compiled for more registers, hence smaller blocks
+  const int threads = (EV || sizeof(T) == 8) ? std::min(s->force_threads, FORCE_MAX_THREADS_WIDE) : s->force_threads;
   if (s->kernel_eff == MD_KERNEL_CELL) {
     CK(launch(s, k_cell_force<T, Body, MODE, EV>, g.ntiles, BUILD_THREADS, cell_smem(s, g), A));
   } else if (half) {
-    if constexpr (MODE == 0 && std::is_same<Body, LJBody<T, EV>>::value) {
-      CK(cudaMemsetAsync(A.f, 0, 3 * s->ld * sizeof(double), s->stream));
-      CK(launch(s, k_tile_force<T, Body, 1, 0, EV, true>, g.ntiles, s->force_threads, force_smem(s, g, true), A));
-    } else {
-      return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
-    }
+    // each pair once: the term of the row's atoms in registers, the term of j scattered with fp64 atomics
+    if (MODE == 0) CK(cudaMemsetAsync(A.f, 0, 3 * s->ld * sizeof(double), s->stream));
+    else CK(cudaMemsetAsync(A.rho, 0, s->ld * sizeof(double), s->stream));
+    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, true>, g.ntiles, threads, force_smem(s, g, true), A));
   } else if (g.K == 1) {
-    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
+    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
   } else if (g.K == 4) {
-    CK(launch(s, k_tile_force<T, Body, 4, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
+    CK(launch(s, k_tile_force<T, Body, 4, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
   } else if (g.K == 8) {
-    CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
+    CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
   } else {
-    CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false>, g.ntiles, s->force_threads, force_smem(s, g, false), A));
+    CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
   }
   return MD_OK;
 }
@@ -515,6 +547,9 @@ int launch_force_T(md_system* s, const StepMode& M) {
     int rc = launch_force_variant<T, EamDensityBody, 1, EV>(s, A);   // pass 1: rho, F'(rho), sum F(rho)
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
+    if (g.half && s->kernel_eff != MD_KERNEL_CELL)   // half list: rho was scattered with atomics, so F'(rho) needs its own pass
+      CK(launch(s, k_eam_embed<T>, blocks_for(s->N, 256), 256, 0, (int)s->N, s->P.B, (const double*)s->rho, s->fp, (T*)s->xr[xb],
+                EV ? s->scalars_d : (double*)nullptr));
     A.fp_in = s->fp;
     rc = launch_force_variant<T, EamForceBody, 0, EV>(s, A);          // pass 2: forces
     if (rc) return rc;
@@ -675,7 +710,8 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   }
   CKC(dalloc(&s->f, 3 * s->ld)); CKC(dalloc(&s->x0, 3 * s->ld)); CKC(dalloc(&s->rho, s->ld)); CKC(dalloc(&s->fp, s->ld));
   CKC(cudaMemsetAsync(s->f, 0, 3 * s->ld * sizeof(double), s->stream));
-  CKC(dalloc(&s->cell_of, s->ld)); CKC(dalloc(&s->rank, s->ld)); CKC(dalloc(&s->perm, s->ld));
+  CKC(dalloc(&s->cell_of, s->ld)); CKC(dalloc(&s->rank, s->ld)); CKC(dalloc(&s->perm, s->ld)); CKC(dalloc(&s->mkey, s->ld));
+  CKC(dalloc(&s->nstat_d, (size_t)4));
   CKC(dalloc(&s->mass_d, (size_t)ntypes)); CKC(dalloc(&s->scalars_d, 16)); CKC(dalloc(&s->io_d, 3 * s->ld));
   CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
@@ -687,7 +723,16 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   CKC(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
   CKC(launch(s, k_iota, blocks_for(N, 256), 256, 0, (int)N, s->id[0]));
   CKC(cudaMemcpyAsync(s->type[0], s->types_caller, (size_t)N * sizeof(int), cudaMemcpyDeviceToDevice, s->stream));
+  {   // type ids index the mass table on the device: refuse anything outside 0..ntypes-1
+    CKC(cudaMemsetAsync(s->nstat_d, 0, 4 * sizeof(int), s->stream));
+    CKC(launch(s, k_check_types, blocks_for(N, 256), 256, 0, (int)N, (const int*)s->types_caller, ntypes, s->nstat_d));
+    CKC(cudaMemcpyAsync(s->flags_h, s->nstat_d, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  }
   CKC(cudaStreamSynchronize(s->stream));
+  if (*reinterpret_cast<const int*>(s->flags_h) != 0) {
+    fail(s, MD_ERR_BAD_ARGUMENT, "md_create: type ids must lie in 0..ntypes-1");
+    return bail(MD_ERR_BAD_ARGUMENT);
+  }
 #undef CKC
   *out = s;
   return MD_OK;
@@ -697,7 +742,8 @@ void md_destroy(md_system* s) {
   if (!s) return;
   for (int k = 0; k < 2; ++k) { cudaFree(s->x[k]); cudaFree(s->v[k]); cudaFree(s->id[k]); cudaFree(s->type[k]); cudaFree(s->xr[k]); }
   cudaFree(s->tab);
-  cudaFree(s->f); cudaFree(s->x0); cudaFree(s->rho); cudaFree(s->fp); cudaFree(s->cell_of); cudaFree(s->rank); cudaFree(s->perm);
+  cudaFree(s->f); cudaFree(s->x0); cudaFree(s->rho); cudaFree(s->fp); cudaFree(s->cell_of); cudaFree(s->rank); cudaFree(s->perm); cudaFree(s->mkey);
+  cudaFree(s->nstat_d); cudaFree(s->export_buf);
   cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d);
   cudaFree(s->ev_partials); cudaFree(s->scalars_d); cudaFree(s->io_d); cudaFree(s->io_i); cudaFree(s->types_caller); cudaFree(s->flags_d);
   if (s->flags_h) cudaFreeHost(s->flags_h);
@@ -746,7 +792,6 @@ int md_set_pair(md_system* s, int style, const double* params, int nparams, doub
   for (int k = 0; k < need; ++k)
     if (!std::isfinite(params[k])) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: non-finite parameter");
   if (style == MD_PAIR_EAM_FS && !(params[4] > 0.0)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: r0 must be positive");
-  if (style == MD_PAIR_EAM_FS && s->list_kind == MD_LIST_HALF) return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
   for (int d = 0; d < 3; ++d)
     if (s->box[d] < 3.0 * (rc + skin))
       return fail(s, MD_ERR_BOX_TOO_SMALL, "box edge %d = %g < 3 (rc+skin) = %g", d, s->box[d], 3.0 * (rc + skin));
@@ -763,7 +808,6 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel) {
   if (kernel < MD_KERNEL_AUTO || kernel > MD_KERNEL_SUBWARP4) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown kernel");
   if (list_kind == MD_LIST_HALF && !(kernel == MD_KERNEL_TPA || kernel == MD_KERNEL_AUTO))
     return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: a half list needs MD_KERNEL_TPA");
-  if (list_kind == MD_LIST_HALF && s->style == MD_PAIR_EAM_FS) return fail(s, MD_ERR_BAD_ARGUMENT, "EAM with a half list is not supported");
   s->list_kind = list_kind;
   s->kernel_req = kernel;
   s->kernel_eff = kernel == MD_KERNEL_AUTO ? MD_KERNEL_TPA : kernel;
@@ -812,12 +856,15 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   int64_t launches0 = s->launches, builds0 = s->nbuilds;
   s->force_timing_pending = false;   // ev0 / ev1 are reused below
   s->ms_build_in_run = 0;
-  CK(cudaEventRecord(s->ev0, s->stream));
+  // ms_run covers the time stepping proper: variant selection (autotune, which reuses ev0 / ev1) and a first list
+  // build that the call may have to do come before the first event; that build is reported in ms_build_in_run
   const bool had_list = s->list_valid;
   int rc = ensure_list(s);
   if (rc) return rc;
   if (!had_list) s->ms_build_in_run += s->ms_build;
+  CK(cudaEventRecord(s->ev0, s->stream));
   if (!s->forces_valid) { rc = compute_forces_device(s, false); if (rc) return rc; }
+  if (nsteps > 0) s->counts_valid = false;
   const int N = (int)s->N;
   const double trigger = 0.25 * s->skin * s->skin;
   const double hdtf = 0.5 * dt * s->ftm2v;
@@ -859,9 +906,10 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
       const int done = s->flags_h->steps_done;
       const bool stopped = s->flags_h->stop != 0;
       if (done < 0 || done > m || (!stopped && done != m)) return fail(s, MD_ERR_CUDA, "md_run: inconsistent step count from the device (%d of %d)", done, m);
-      for (int k = 0; k < m; ++k) {   // timings of the launches that really ran
+      for (int k = 0; k < m; ++k) {   // timings of the launches that really ran; a sampled launch that was skipped gives its slot back
         if (sample_slot[k] < 0) continue;
         if (k < done) { float t = 0; CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev[2 * sample_slot[k] + 1])); s->ms_force_sampled += t; s->nforce_sampled_acc++; }
+        else nsampled = std::min(nsampled, sample_slot[k]);
       }
       const bool final_ran = done == m && (int64_t)m == remaining;
       const int flips = final_ran ? done - 1 : done;   // kick+drift launches that ran
@@ -942,24 +990,83 @@ int md_get_forces(md_system* s, double* f) {
   return get_vec3(s, s->f, f);
 }
 
-int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride) {
-  if (!s || !numneigh || !neigh || stride <= 0) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_neighbors: bad argument") : MD_ERR_BAD_ARGUMENT;
+// one launch of k_export_list; device buffers only
+static int export_launch(md_system* s, int mode, int* nn, int* neigh, int* owner, int64_t stride, int* stat) {
+  const Geom& g = s->g;
+  const double rl = s->rc + s->skin;
+  ExportArgs E{};
+  E.g = g; E.tab = s->tab; E.id = s->id[s->cur]; E.x = s->x[s->xcur]; E.ld = s->ld; E.list = s->list; E.numneigh = s->numneigh;
+  E.rl2 = rl * rl; E.mode = mode; E.nn_out = nn; E.neigh_out = neigh; E.owner_out = owner; E.stride = (long long)stride; E.stat = stat;
+  CK(launch(s, k_export_list, g.ntiles, BUILD_THREADS, export_smem(g), E));
+  return MD_OK;
+}
+
+// Exact per-atom neighbor statistics of the current list (the stored rows are per pair of atoms and a superset):
+// counted by the export kernel with the fp64 test, once per list.  Positions must be those of the build for the
+// counts to be the build-time pair set; after time steps they describe the current positions.
+static int exact_counts(md_system* s) {
+  if (s->counts_valid) return MD_OK;
+  if (!s->list_valid || !s->list_built_for_export) { s->max_nb_exact = 0; s->mean_nb_exact = 0; return MD_OK; }
+  CK(cudaMemsetAsync(s->nstat_d, 0, 4 * sizeof(int), s->stream));
+  int rc = export_launch(s, EXPORT_EXACT, s->io_i, nullptr, nullptr, 0, s->nstat_d);
+  if (rc) return rc;
+  int h[4];
+  CK(cudaMemcpyAsync(h, s->nstat_d, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  unsigned long long sum;
+  memcpy(&sum, &h[2], sizeof sum);
+  s->max_nb_exact = h[0];
+  s->mean_nb_exact = (double)sum / (double)s->N;
+  s->counts_valid = true;
+  return MD_OK;
+}
+
+static int export_common(md_system* s, int mode, int32_t* numneigh, int32_t* neigh, int32_t* owner, int64_t stride) {
   int rc = ensure_list(s);
   if (rc) return rc;
   if (!s->list_built_for_export) { rc = build(s, true); if (rc) return rc; }
-  const Geom& g = s->g;
-  bool dev_n = is_device_ptr(numneigh), dev_l = is_device_ptr(neigh);
-  int *dn = numneigh, *dl = neigh;
-  if (!dev_n) dn = s->io_i;
-  if (!dev_l) CK(cudaMalloc((void**)&dl, (size_t)s->N * stride * sizeof(int)));
-  size_t smem = export_smem(g);
-  cudaError_t e = launch(s, k_export_list, g.ntiles, BUILD_THREADS, smem, g, (const int*)s->tab, (const int*)s->id[s->cur],
-                         (const uint4*)s->list, (const int*)s->numneigh, dn, dl, (long long)stride);
-  if (e == cudaSuccess && !dev_n) e = cudaMemcpyAsync(numneigh, dn, (size_t)s->N * sizeof(int), cudaMemcpyDeviceToHost, s->stream);
-  if (e == cudaSuccess && !dev_l) e = cudaMemcpyAsync(neigh, dl, (size_t)s->N * stride * sizeof(int), cudaMemcpyDeviceToHost, s->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
-  if (!dev_l) cudaFree(dl);
-  if (e != cudaSuccess) return fail(s, MD_ERR_CUDA, "md_get_neighbors: %s", cudaGetErrorString(e));
+  const size_t N = (size_t)s->N;
+  const bool dev_n = is_device_ptr(numneigh), dev_l = is_device_ptr(neigh), dev_o = owner ? is_device_ptr(owner) : true;
+  // host buffers are filled through one staging buffer of the handle: [neigh N*stride][numneigh N][owner N]
+  const size_t need = (dev_l ? 0 : N * (size_t)stride) + (dev_n ? 0 : N) + (dev_o ? 0 : N);
+  if (need > s->export_alloc) {
+    cudaFree(s->export_buf);
+    s->export_buf = nullptr; s->export_alloc = 0;
+    CK(dalloc(&s->export_buf, need));
+    s->export_alloc = need;
+  }
+  int* p = s->export_buf;
+  int* dl = dev_l ? neigh : p; if (!dev_l) p += N * (size_t)stride;
+  int* dn = dev_n ? numneigh : p; if (!dev_n) p += N;
+  int* dow = owner ? (dev_o ? owner : p) : nullptr;
+  rc = export_launch(s, mode, dn, dl, dow, stride, nullptr);
+  if (rc) return rc;
+  if (!dev_n) CK(cudaMemcpyAsync(numneigh, dn, N * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  if (!dev_l) CK(cudaMemcpyAsync(neigh, dl, N * (size_t)stride * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  if (owner && !dev_o) CK(cudaMemcpyAsync(owner, dow, N * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return MD_OK;
+}
+
+int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride) {
+  if (!s || !numneigh || !neigh || stride <= 0) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_neighbors: bad argument") : MD_ERR_BAD_ARGUMENT;
+  return export_common(s, EXPORT_EXACT, numneigh, neigh, nullptr, stride);
+}
+
+int md_get_neighbor_rows(md_system* s, int32_t* row_owner, int32_t* numrow, int32_t* entries, int64_t stride) {
+  if (!s || !row_owner || !numrow || !entries || stride <= 0)
+    return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_neighbor_rows: bad argument") : MD_ERR_BAD_ARGUMENT;
+  return export_common(s, EXPORT_RAW, numrow, entries, row_owner, stride);
+}
+
+int md_kinetic_energy(md_system* s, double* ke_out) {
+  if (!s || !ke_out) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_kinetic_energy: NULL") : MD_ERR_BAD_ARGUMENT;
+  CK(cudaMemsetAsync(s->scalars_d + 8, 0, sizeof(double), s->stream));
+  CK(launch(s, k_kinetic, std::min<unsigned>(blocks_for(s->N, 256), 1184u), 256, 0, (int)s->N, s->ld, (const double*)s->v[s->cur],
+            (const int*)s->type[s->cur], (const double*)s->mass_d, s->scalars_d + 8));
+  CK(cudaMemcpyAsync(s->scalars_h + 8, s->scalars_d + 8, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  *ke_out = s->scalars_h[8] * s->mvv2e;
   return MD_OK;
 }
 
@@ -974,13 +1081,16 @@ int md_get_stats(md_system* s, md_stats* out) {
     out->ntiles = s->g.ntiles; out->tile_capacity = s->g.tile_cap; out->row_capacity = s->g.row_cap;
   }
   out->list_balanced = s->list_balanced ? 1 : 0;
-  out->max_tile_atoms = s->max_tile_atoms; out->max_neighbors = s->max_row; out->mean_neighbors = s->mean_row;
-  CK(cudaMemsetAsync(s->scalars_d + 8, 0, sizeof(double), s->stream));
-  CK(launch(s, k_kinetic, std::min<unsigned>(blocks_for(s->N, 256), 1184u), 256, 0, (int)s->N, s->ld, (const double*)s->v[s->cur],
-            (const int*)s->type[s->cur], (const double*)s->mass_d, s->scalars_d + 8));
-  CK(cudaMemcpyAsync(s->scalars_h + 8, s->scalars_d + 8, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
-  CK(cudaStreamSynchronize(s->stream));
-  out->kinetic_energy = s->scalars_h[8] * s->mvv2e;
+  {
+    int rc = exact_counts(s);
+    if (rc) return rc;
+  }
+  out->max_tile_atoms = s->max_tile_atoms; out->max_neighbors = s->max_nb_exact; out->mean_neighbors = s->mean_nb_exact;
+  out->max_row = s->max_row; out->mean_row = s->mean_row;
+  {
+    int rc = md_kinetic_energy(s, &out->kinetic_energy);
+    if (rc) return rc;
+  }
   if (s->force_timing_pending) {
     float ms = 0;
     if (cudaEventElapsedTime(&ms, s->ev0, s->ev1) == cudaSuccess) s->ms_force = ms;

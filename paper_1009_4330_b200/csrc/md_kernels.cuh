@@ -21,8 +21,9 @@ namespace mdk {
 constexpr int MAX_TILE_CELLS = 216;    // (bx+2)(by+2)(bz+2) <= 216, each of bx, by, bz <= 4
 constexpr int BUILD_THREADS = 256;     // threads per block of the list-build (when three blocks fit an SM) and cell-list kernels
 constexpr int BUILD_MAX_THREADS = 384; // list build: block size when only two blocks fit an SM
-constexpr int FORCE_MAX_THREADS = 640; // upper bound of the force kernels' block size (runtime choice)
-constexpr int FORCE_MIN_BLOCKS = 2;    // the mixed-precision force kernels are compiled for <= 48 registers: two 640-thread or three 416-thread blocks per SM
+constexpr int FORCE_MAX_THREADS = 1024;     // upper bound of the force kernels' block size (runtime choice): the mixed-precision
+                                            // kernels are compiled for <= 56 registers (three 384-thread blocks per SM)
+constexpr int FORCE_MAX_THREADS_WIDE = 640; // the same for the fp64 and the energy/virial instantiations (<= 96 registers)
 #ifndef MDK_BUILD_MIN_BLOCKS
 #define MDK_BUILD_MIN_BLOCKS 2
 #endif
@@ -409,12 +410,22 @@ __device__ __forceinline__ void tile_stage(const Geom& g, const TileTables& tt, 
 // ---------------------------------------------------------------------------------------------------
 // a1: wrap + bin (north_star (1))
 // ---------------------------------------------------------------------------------------------------
+// It also packs, above the atom's arrival rank in its cell (bits 0..19), a 9-bit MORTON KEY of the atom's position
+// within its cell (3 bits per dimension, bits 20..28): k_sort_cells orders a cell's atoms by it, so that
+// consecutive atoms of a cell are spatial neighbours -- the list rows are per PAIR of consecutive atoms (below).
+__device__ __forceinline__ int morton3(int a, int b, int c) {   // interleave three 3-bit numbers
+  int m = 0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) m |= (((a >> k) & 1) << (3 * k)) | (((b >> k) & 1) << (3 * k + 1)) | (((c >> k) & 1) << (3 * k + 2));
+  return m;
+}
+constexpr int RANK_BITS = 20;
 __global__ void k_bin(Geom g, int N, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
                       int* __restrict__ cell_of, int* __restrict__ rank, int* __restrict__ cell_count, Flags* flags) {
   int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= N) return;
   double p[3] = {x[k], y[k], z[k]};
-  int c[3];
+  int c[3], sub[3];
   bool bad = false;
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
@@ -424,12 +435,14 @@ __global__ void k_bin(Geom g, int N, double* __restrict__ x, double* __restrict_
     if (w < 0.0) w = 0.0;
     p[d] = w;
     c[d] = cell_index_1d(g, d, w);
+    const int q = (int)((w * g.inv_edge[d] - (double)c[d]) * 8.0);
+    sub[d] = q < 0 ? 0 : (q > 7 ? 7 : q);
   }
   if (bad) atomicExch(&flags->nonfinite, 1);
-  x[k] = p[0]; y[k] = p[1]; z[k] = p[2];
+  else { x[k] = p[0]; y[k] = p[1]; z[k] = p[2]; }   // a non-finite coordinate is reported, not overwritten
   int oid = cell_order_id(g, c[0], c[1], c[2]);
   cell_of[k] = oid;
-  rank[k] = atomicAdd(&cell_count[oid], 1);
+  rank[k] = atomicAdd(&cell_count[oid], 1) | (morton3(sub[0], sub[1], sub[2]) << RANK_BITS);
 }
 
 // a2: exclusive scan of the cell counts in two launches: per-block sums of SCAN_BLOCK cells, then every block
@@ -496,30 +509,37 @@ __global__ void __launch_bounds__(1024) k_scan_cells(int ncell, const int* __res
 }
 
 __global__ void k_fill_perm(int N, const int* __restrict__ cell_of, const int* __restrict__ rank,
-                            const int* __restrict__ cell_start, int* __restrict__ perm) {
+                            const int* __restrict__ cell_start, int* __restrict__ perm, int* __restrict__ mkey) {
   int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k < N) perm[cell_start[cell_of[k]] + rank[k]] = k;
+  if (k >= N) return;
+  const int r = rank[k], pos = cell_start[cell_of[k]] + (r & ((1 << RANK_BITS) - 1));
+  perm[pos] = k;
+  mkey[pos] = r >> RANK_BITS;
 }
 
-// The atomic ranks of k_bin are not reproducible; sorting each cell's slice of perm by previous index
-// makes the whole order (and so every later summation order) deterministic.  One warp per cell, rank sort:
-// every lane keeps up to SORT_PER of the cell's keys, each key's rank is the number of smaller keys (the keys
-// of a cell are distinct), broadcast lane by lane with shuffles: c * ceil(c/32) steps instead of the c^2 of a
-// serial insertion sort (a cell holds ~20 atoms at rc = 2.5 sigma, ~150 at rc = 5 sigma).
+// The atomic ranks of k_bin are not reproducible; sorting each cell's slice of perm by (Morton key of the
+// position within the cell, previous index) makes the whole order (and so every later summation order)
+// deterministic AND spatially coherent within the cell.  One warp per cell, rank sort: every lane keeps up to
+// SORT_PER of the cell's keys, each key's rank is the number of smaller keys (the keys of a cell are distinct),
+// broadcast lane by lane with shuffles: c * ceil(c/32) steps instead of the c^2 of a serial insertion sort
+// (a cell holds ~20 atoms at rc = 2.5 sigma, ~150 at rc = 5 sigma).
 constexpr int SORT_PER = 16;   // cells of up to 512 atoms; larger ones fall back to a serial sort by lane 0
+typedef unsigned long long sortkey_t;
+__device__ __forceinline__ sortkey_t sort_key(int mk, int prev) { return ((sortkey_t)(unsigned)mk << 32) | (unsigned)prev; }
 template <int PER>
-__device__ __forceinline__ void sort_cell_by_warp(int lo, int n, int lane, int* __restrict__ perm) {
-  int key[PER], rank[PER];
+__device__ __forceinline__ void sort_cell_by_warp(int lo, int n, int lane, int* __restrict__ perm, const int* __restrict__ mkey) {
+  sortkey_t key[PER];
+  int rank[PER];
 #pragma unroll
   for (int i = 0; i < PER; ++i) {
-    key[i] = lane + 32 * i < n ? perm[lo + lane + 32 * i] : 0x7fffffff;
+    key[i] = lane + 32 * i < n ? sort_key(mkey[lo + lane + 32 * i], perm[lo + lane + 32 * i]) : ~0ull;
     rank[i] = 0;
   }
 #pragma unroll
   for (int j = 0; j < PER; ++j) {          // the keys held in register j of every lane
     const int cnt = min(32, n - 32 * j);
     for (int l = 0; l < cnt; ++l) {
-      const int other = __shfl_sync(0xffffffffu, key[j], l);
+      const sortkey_t other = __shfl_sync(0xffffffffu, key[j], l);
 #pragma unroll
       for (int i = 0; i < PER; ++i) rank[i] += other < key[i] ? 1 : 0;
     }
@@ -527,24 +547,27 @@ __device__ __forceinline__ void sort_cell_by_warp(int lo, int n, int lane, int* 
   __syncwarp();
 #pragma unroll
   for (int i = 0; i < PER; ++i)
-    if (lane + 32 * i < n) perm[lo + rank[i]] = key[i];
+    if (lane + 32 * i < n) perm[lo + rank[i]] = (int)(unsigned)key[i];
 }
-__global__ void __launch_bounds__(256) k_sort_cells(int ncell, const int* __restrict__ cell_start, int* __restrict__ perm) {
+__global__ void __launch_bounds__(256) k_sort_cells(int ncell, const int* __restrict__ cell_start, int* __restrict__ perm,
+                                                    int* __restrict__ mkey) {
   const int lane = threadIdx.x & 31;
   const int nwarps = gridDim.x * (blockDim.x >> 5);
   for (int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); c < ncell; c += nwarps) {   // a warp per cell, grid-stride
     const int lo = cell_start[c], n = cell_start[c + 1] - lo;
     if (n <= 1) continue;
-    if (n <= 32) sort_cell_by_warp<1>(lo, n, lane, perm);
-    else if (n <= 64) sort_cell_by_warp<2>(lo, n, lane, perm);
-    else if (n <= 128) sort_cell_by_warp<4>(lo, n, lane, perm);
-    else if (n <= 256) sort_cell_by_warp<8>(lo, n, lane, perm);
-    else if (n <= 32 * SORT_PER) sort_cell_by_warp<SORT_PER>(lo, n, lane, perm);
+    if (n <= 32) sort_cell_by_warp<1>(lo, n, lane, perm, mkey);
+    else if (n <= 64) sort_cell_by_warp<2>(lo, n, lane, perm, mkey);
+    else if (n <= 128) sort_cell_by_warp<4>(lo, n, lane, perm, mkey);
+    else if (n <= 256) sort_cell_by_warp<8>(lo, n, lane, perm, mkey);
+    else if (n <= 32 * SORT_PER) sort_cell_by_warp<SORT_PER>(lo, n, lane, perm, mkey);
     else if (lane == 0)
       for (int a = lo + 1; a < lo + n; ++a) {
-        int key = perm[a], b = a - 1;
-        while (b >= lo && perm[b] > key) { perm[b + 1] = perm[b]; --b; }
-        perm[b + 1] = key;
+        const int kp = perm[a], km = mkey[a];
+        const sortkey_t key = sort_key(km, kp);
+        int b = a - 1;
+        while (b >= lo && sort_key(mkey[b], perm[b]) > key) { perm[b + 1] = perm[b]; mkey[b + 1] = mkey[b]; --b; }
+        perm[b + 1] = kp; mkey[b + 1] = km;
       }
     __syncwarp();
   }
@@ -588,6 +611,10 @@ __global__ void k_gather_out(int N, const int* __restrict__ id, const double* __
   size_t o = 3 * (size_t)id[n];
   out[o] = in[n]; out[o + 1] = in[ld + n]; out[o + 2] = in[2 * ld + n];
 }
+__global__ void k_check_types(int N, const int* __restrict__ type, int ntypes, int* __restrict__ bad) {
+  int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n < N && (type[n] < 0 || type[n] >= ntypes)) atomicExch(bad, 1);
+}
 __global__ void k_iota(int N, int* __restrict__ a) {
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n < N) a[n] = n;
@@ -595,53 +622,55 @@ __global__ void k_iota(int N, int* __restrict__ a) {
 
 // ---------------------------------------------------------------------------------------------------
 // a3: Verlet list build from the 27-cell stencil of the staged tile (north_star (2)).
-// One WARP per interior cell, one LANE per atom of that cell: every lane walks the same candidate
-// sequence (the 27 cells' staged slots, four candidates per 128-bit broadcast load from SoA shared
-// memory), so there is no divergence in the test loop.  The distance test runs in fp32 on tile-centred
-// coordinates with a guard band: r2 < rl2_lo accepts, r2 >= rl2_hi rejects, and the rare candidate in
-// between is decided in fp64 from the global positions, so the pair set is exactly the fp64 one.
-// Accepted slot codes go to a small per-lane ring in shared memory (one predicated 16-bit store each)
-// and leave for global memory as complete 128-bit words.
-// Shared memory: TileTables | xs[capA] ys[capA] zs[capA] floats | rings[nwarps*32*RING_STRIDE].
-// List layout: 16-bit codes (slot << code_shift), 8 per uint4; entry e of row a sits in word
-//   q = e/8, lane s = q % K, chunk c = q / K  at  list[tile_base + c*slots_cap + a*K + s].
+//
+// PAIR ROWS.  A list row belongs to a PAIR of consecutive atoms of a cell (staged slots 2m, 2m+1; k_sort_cells
+// orders a cell's atoms along a Morton curve, so the two are ~1.4 sigma apart in the LJ liquid) and holds the
+// UNION of their neighbors: every staged atom j with |x_j - x_a|^2 < rl^2 for a = either atom of the pair,
+// except the two atoms themselves (their mutual term is added by the force kernels directly).  The force
+// kernel gathers each listed j ONCE and evaluates it against both atoms (packed f32x2 math), which cuts the
+// gathers, the index stream and the list-loop instructions per atom to ~0.69 (measured union size: 1.38 rows).
+//
+// SUPERSET SEMANTICS.  The distance test runs in fp32 on tile-centred coordinates and accepts r2 < rl2_hi,
+// rl2_hi = rl^2 (1 + band) with band four times the worst-case fp32 rounding of r2 (host: build_list_only), so a
+// row never misses a pair the fp64 definition contains; it may hold a few pairs beyond rl (in the band, or
+// within rl of the partner only), which the force kernels' r2 < rc2 test makes harmless.  The EXACT fp64 pair
+// set of an atom (north_star (2)) is the row's entries that pass |x_i - x_j|^2 < rl^2 in fp64 from the global
+// positions: md_get_neighbors (k_export_list) returns exactly that, md_get_neighbor_rows returns the raw rows.
+//
+// One LANE per pair row; a task = 32 consecutive pair rows (16 quads of slots).  Rows are padded per cell to
+// multiples of 4 slots, so a quad belongs to one cell, but the quads of a task may belong to different cells:
+// the lanes of a warp then walk different candidate runs of about the same length, in lockstep (ragged pieces
+// read a far-away dummy quad).  Four candidates per 128-bit broadcast load from SoA shared memory; accepted slot
+// codes go to a small per-lane ring in shared memory (one predicated 16-bit store + pointer add each) and
+// leave for global memory as complete 128-bit words.
+// Shared memory: TileTables | offs[tile cells] float4 | rowcell[interior_cap/4 + 8] u16 | xs[capA] ys[capA] zs[capA] floats |
+// rings[nwarps*32*RING_STRIDE].
+// List layout: 16-bit codes (slot << code_shift), 8 per uint4; entry e of pair row r sits in word
+//   q = e/8, lane s = q % K, chunk c = q / K  at  list[tile_base + c*slots_cap + r*K + s],  slots_cap = prow_cap * K.
 // Unused entries of the last word hold the dummy slot n_slots (a far-away point).
 // ---------------------------------------------------------------------------------------------------
 struct BuildArgs {
   Geom g;
-  const int* cell_start;
   const int* tab;          // per-tile tables (k_tile_tables)
-  const double* x; size_t ld;
-  const void* xr;          // packed cell-relative positions (float4, or double4 when xr_double) of the positions in x
+  const void* xr;          // packed cell-relative positions (float4, or double4 when xr_double)
   int xr_double;
-  double rl2;
-  float rl2_hi, rl2_mid, rl2_bw;   // fp32 test: accept r2 < hi = mid + bw; |r2 - mid| <= bw is decided in fp64 (mid = fl(rl2))
+  float rl2_hi;            // fp32 accept test: r2 < rl2_hi = rl^2 (1 + band)
   uint4* list;
-  int* numneigh;           // [ntiles][interior_cap]
+  int* numneigh;           // [ntiles][prow_cap]: entries of each pair row
   Flags* flags;
 };
 
+__host__ __device__ inline int prow_cap(const Geom& g) { return g.interior_cap >> 1; }   // pair rows a tile can hold
 __device__ __forceinline__ int build_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
 __host__ __device__ inline int build_rowcell_len(const Geom& g) { return ((g.interior_cap >> 2) + 15) & ~7; }   // u16 entries, 16-byte multiple
-
-__device__ __noinline__ bool confirm_pair_fp64(const Geom& g, const TileTables& tt, const double* __restrict__ x, size_t ld,
-                                               int gi, int ti, int gj, int tj, double rl2) {
-  double oi[3], oj[3];
-  tile_cell_offset(g, tt, ti, oi);
-  tile_cell_offset(g, tt, tj, oj);
-  double r2 = 0.0;
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    double dd = (x[d * ld + gi] + oi[d]) - (x[d * ld + gj] + oj[d]);
-    r2 += dd * dd;
-  }
-  return r2 < rl2;
-}
 
 // packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2: two lanes of math per issue slot)
 typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+// the same, never rematerialised: for loop invariants (ptxas otherwise rebuilds the pair with two moves at every use)
+__device__ __forceinline__ f32x2 pack2_once(float lo, float hi) { f32x2 r; asm volatile("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
@@ -650,149 +679,121 @@ __device__ __forceinline__ void lds_2x2(unsigned a, f32x2& p01, f32x2& p23) {
   asm volatile("ld.shared.v2.u64 {%0,%1}, [%2];" : "=l"(p01), "=l"(p23) : "r"(a));
 }
 
-// ring push of a candidate pair: for each half of r2 = {r2_a, r2_b}: if (r2 < hi) { ring[rp] = code (16 bit); rp += 2 }
-// The compare lives in the asm so that it feeds the two predicated instructions directly (FSETP, @P STS.U16, @P IADD).
-__device__ __forceinline__ void ring_push2(unsigned& rp, unsigned code_a, unsigned code_b, f32x2 r2, float hi) {
-  asm volatile(
-      "{ .reg .pred p; .reg .f32 a, b; .reg .b16 c, d;\n"
-      "  mov.b64 {a, b}, %3;\n"
-      "  mov.b32 {c, d}, %1;\n"
-      "  setp.lt.f32 p, a, %4;\n"
-      "  @p st.shared.u16 [%0], c;\n"
-      "  @p add.u32 %0, %0, 2;\n"
-      "  mov.b32 {c, d}, %2;\n"
-      "  setp.lt.f32 p, b, %4;\n"
-      "  @p st.shared.u16 [%0], c;\n"
-      "  @p add.u32 %0, %0, 2; }"
-      : "+r"(rp)
-      : "r"(code_a), "r"(code_b), "l"(r2), "f"(hi)
-      : "memory");
-}
-// the same with one more condition per candidate: its code differs from `self` (the lane's own atom)
-__device__ __forceinline__ void ring_push2_self(unsigned& rp, unsigned code_a, unsigned code_b, f32x2 r2, float hi, unsigned self) {
-  asm volatile(
-      "{ .reg .pred p; .reg .f32 a, b; .reg .b16 c, d;\n"
-      "  mov.b64 {a, b}, %3;\n"
-      "  mov.b32 {c, d}, %1;\n"
-      "  setp.lt.f32 p, a, %4;\n"
-      "  setp.ne.and.u32 p, %1, %5, p;\n"
-      "  @p st.shared.u16 [%0], c;\n"
-      "  @p add.u32 %0, %0, 2;\n"
-      "  mov.b32 {c, d}, %2;\n"
-      "  setp.lt.f32 p, b, %4;\n"
-      "  setp.ne.and.u32 p, %2, %5, p;\n"
-      "  @p st.shared.u16 [%0], c;\n"
-      "  @p add.u32 %0, %0, 2; }"
-      : "+r"(rp)
-      : "r"(code_a), "r"(code_b), "l"(r2), "f"(hi), "r"(self)
-      : "memory");
-}
-// predicated 16-bit store to the lane's ring + pointer advance (slow paths)
-__device__ __forceinline__ void ring_push(unsigned& rp, unsigned code, bool take) {
-  asm volatile("{ .reg .pred p; .reg .b16 c, d; mov.b32 {c, d}, %1; setp.ne.u32 p, %2, 0; @p st.shared.u16 [%0], c; @p add.u32 %0, %0, 2; }"
-               : "+r"(rp)
-               : "r"(code), "r"((unsigned)take)
-               : "memory");
-}
-
-// The careful scan of the `nslot` staged slots from j0 on (a piece of a run of consecutive tile cells; tc is a
-// cell at or before the one holding j0) for the lane's atom (tile-centred position xi, yi, zi; global index gi;
-// tile cell t; act: the lane holds an atom): the same fp32 accept test as the fast loop, plus the exclusions
-// (never slot jskip, only slots > jmin), plus an fp64 decision from the global positions for every candidate
-// inside the guard band.  Used for the own cell of a half list and to redo a piece in which the fast loop saw
-// an in-band candidate.  Everything is passed by value or lives in shared memory (gs: a shared copy of the
-// geometry), so the kernel keeps no stack frame for it.
-struct BuildBand { double rl2; float hi, mid, bw; };
-__device__ __noinline__ unsigned build_scan_careful(const Geom& gs, const TileTables& tt, const double* __restrict__ x, size_t ld,
-                                                    BuildBand bd, const float* xs, const float* ys, const float* zs, float xi, float yi,
-                                                    float zi, int act, int gi, int t, int jskip, int jmin, unsigned rp, int j0,
-                                                    int nslot, int tc, int shift) {
-  for (int j = j0; j < j0 + nslot; ++j) {
-    while (j >= tt.start[tc] + pad4(tt.cnt[tc])) ++tc;
-    const int k = j - tt.start[tc];
-    const float ex = xi - xs[j], ey = yi - ys[j], ez = zi - zs[j];
-    const float r2s = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
-    bool take = r2s < bd.hi && j != jskip && j > jmin;     // pad slots (k >= cnt) are far away: never taken
-    if (act && take && k < tt.cnt[tc] && fabsf(r2s - bd.mid) <= bd.bw)
-      take = confirm_pair_fp64(gs, tt, x, ld, gi, t, tt.gstart[tc] + k, tc, bd.rl2);
-    ring_push(rp, (unsigned)j << shift, take);
-  }
-  return rp;
-}
-
-// The fast scan of nq quads of candidates (staged slots off/4 ..) for one lane: packed fp32 distance test, accepted
-// codes to the lane's ring, m = min |r2 - rl2| (the guard-band detector).  SELF: the candidates are the lane's own
-// cell, skip the code `self`.
-template <bool SELF, int SHIFT, int FIXED>
-__device__ __forceinline__ void build_scan_fast(unsigned& rp, float& m, unsigned xs_a, unsigned ys_a, unsigned zs_a, unsigned off,
-                                                unsigned code, int nq, f32x2 xi2, f32x2 yi2, f32x2 zi2, f32x2 mid2, float hi,
-                                                unsigned self) {
-  if constexpr (FIXED > 0) nq = FIXED;   // the common full piece: a constant trip count, no loop bookkeeping
-#pragma unroll 4
-  for (int q = 0; q < nq; ++q) {
-    f32x2 X01, X23, Y01, Y23, Z01, Z23;
-    lds_2x2(xs_a + off, X01, X23);
-    lds_2x2(ys_a + off, Y01, Y23);
-    lds_2x2(zs_a + off, Z01, Z23);
-    const f32x2 dx01 = sub2(xi2, X01), dx23 = sub2(xi2, X23);
-    const f32x2 dy01 = sub2(yi2, Y01), dy23 = sub2(yi2, Y23);
-    const f32x2 dz01 = sub2(zi2, Z01), dz23 = sub2(zi2, Z23);
-    const f32x2 q01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
-    const f32x2 q23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
-    float e0, e1, e2, e3;
-    unpack2(sub2(q01, mid2), e0, e1);
-    unpack2(sub2(q23, mid2), e2, e3);
-    m = fminf(fminf(m, fabsf(e0)), fabsf(e1));
-    m = fminf(fminf(m, fabsf(e2)), fabsf(e3));
-    if constexpr (SELF) {
-      ring_push2_self(rp, code, code + (1u << SHIFT), q01, hi, self);
-      ring_push2_self(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi, self);
-    } else {
-      ring_push2(rp, code, code + (1u << SHIFT), q01, hi);
-      ring_push2(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi);
-    }
-    off += 16;
-    code += 4u << SHIFT;
+// ring push of two candidates for a PAIR of atoms: qa = r2 of atom 0 to {candidate a, candidate b}, qb = the same
+// for atom 1.  For each candidate: if (min(r2_0, r2_1) < hi) { ring[rp] = code (16 bit); rp += 2 }.  The compares
+// live in the asm so that they feed the two predicated instructions directly (FSETP, FSETP.OR, @P STS.U16, @P IADD).
+// SELF = 0: no exclusion (the candidates belong to another cell)
+// SELF = 1: own cell, full list: skip the pair's own two slots: (code - self0) as unsigned must exceed one slot
+// SELF = 2: own cell, half list: only slots after the pair's second atom: (code - self0) as signed must exceed one slot
+template <int SELF, int SHIFT>
+__device__ __forceinline__ void ring_push_pair(unsigned& rp, unsigned code_a, f32x2 qa, f32x2 qb, float hi, unsigned self0) {
+  if constexpr (SELF == 0) {
+    asm volatile(
+        "{ .reg .pred p; .reg .f32 a0, a1, b0, b1; .reg .b16 c, d; .reg .b32 cb;\n"
+        "  mov.b64 {a0, a1}, %2;\n"
+        "  mov.b64 {b0, b1}, %3;\n"
+        "  mov.b32 {c, d}, %1;\n"
+        "  setp.lt.f32 p, a0, %4;\n"
+        "  setp.lt.or.f32 p, b0, %4, p;\n"
+        "  @p st.shared.u16 [%0], c;\n"
+        "  @p add.u32 %0, %0, 2;\n"
+        "  add.u32 cb, %1, %5;\n"
+        "  mov.b32 {c, d}, cb;\n"
+        "  setp.lt.f32 p, a1, %4;\n"
+        "  setp.lt.or.f32 p, b1, %4, p;\n"
+        "  @p st.shared.u16 [%0], c;\n"
+        "  @p add.u32 %0, %0, 2; }"
+        : "+r"(rp)
+        : "r"(code_a), "l"(qa), "l"(qb), "f"(hi), "n"(1 << SHIFT)
+        : "memory");
+  } else if constexpr (SELF == 1) {
+    asm volatile(
+        "{ .reg .pred p; .reg .f32 a0, a1, b0, b1; .reg .b16 c, d; .reg .b32 cb, df;\n"
+        "  mov.b64 {a0, a1}, %2;\n"
+        "  mov.b64 {b0, b1}, %3;\n"
+        "  mov.b32 {c, d}, %1;\n"
+        "  sub.u32 df, %1, %6;\n"
+        "  setp.lt.f32 p, a0, %4;\n"
+        "  setp.lt.or.f32 p, b0, %4, p;\n"
+        "  setp.gt.and.u32 p, df, %5, p;\n"
+        "  @p st.shared.u16 [%0], c;\n"
+        "  @p add.u32 %0, %0, 2;\n"
+        "  add.u32 cb, %1, %5;\n"
+        "  mov.b32 {c, d}, cb;\n"
+        "  add.u32 df, df, %5;\n"
+        "  setp.lt.f32 p, a1, %4;\n"
+        "  setp.lt.or.f32 p, b1, %4, p;\n"
+        "  setp.gt.and.u32 p, df, %5, p;\n"
+        "  @p st.shared.u16 [%0], c;\n"
+        "  @p add.u32 %0, %0, 2; }"
+        : "+r"(rp)
+        : "r"(code_a), "l"(qa), "l"(qb), "f"(hi), "n"(1 << SHIFT), "r"(self0)
+        : "memory");
+  } else {
+    asm volatile(
+        "{ .reg .pred p; .reg .f32 a0, a1, b0, b1; .reg .b16 c, d; .reg .b32 cb, df;\n"
+        "  mov.b64 {a0, a1}, %2;\n"
+        "  mov.b64 {b0, b1}, %3;\n"
+        "  mov.b32 {c, d}, %1;\n"
+        "  sub.u32 df, %1, %6;\n"
+        "  setp.lt.f32 p, a0, %4;\n"
+        "  setp.lt.or.f32 p, b0, %4, p;\n"
+        "  setp.gt.and.s32 p, df, %5, p;\n"
+        "  @p st.shared.u16 [%0], c;\n"
+        "  @p add.u32 %0, %0, 2;\n"
+        "  add.u32 cb, %1, %5;\n"
+        "  mov.b32 {c, d}, cb;\n"
+        "  add.u32 df, df, %5;\n"
+        "  setp.lt.f32 p, a1, %4;\n"
+        "  setp.lt.or.f32 p, b1, %4, p;\n"
+        "  setp.gt.and.s32 p, df, %5, p;\n"
+        "  @p st.shared.u16 [%0], c;\n"
+        "  @p add.u32 %0, %0, 2; }"
+        : "+r"(rp)
+        : "r"(code_a), "l"(qa), "l"(qb), "f"(hi), "n"(1 << SHIFT), "r"(self0)
+        : "memory");
   }
 }
 
-// The same when the lanes of the warp hold different numbers of quads (their atoms belong to different cells): the
-// warp runs nqmax rounds; a lane that has used up its nq quads reads the far-away dummy quad at off_dummy instead.
-template <bool SELF, int SHIFT>
-__device__ __forceinline__ void build_scan_ragged(unsigned& rp, float& m, unsigned xs_a, unsigned ys_a, unsigned zs_a, unsigned off,
-                                                  unsigned code, int nq, int nqmax, unsigned off_dummy, f32x2 xi2, f32x2 yi2, f32x2 zi2,
-                                                  f32x2 mid2, float hi, unsigned self) {
+// The scan of nq quads of candidates (staged slots off/4 ..) for one lane = one pair of atoms: packed fp32 distance
+// test of both atoms against four candidates per iteration, accepted codes to the lane's ring.
+// FIXED > 0: the common full piece, a constant trip count.  RAGGED: the lanes of the warp hold different numbers of
+// quads (their pairs belong to different cells): the warp runs nqmax rounds; a lane that has used up its nq quads
+// reads the far-away dummy quad at off_dummy instead.
+struct PairPos { f32x2 x0, y0, z0, x1, y1, z1; };   // each coordinate of an atom duplicated into both halves
+template <int SELF, int SHIFT, int FIXED, bool RAGGED>
+__device__ __forceinline__ void build_scan(unsigned& rp, unsigned xs_a, unsigned ys_a, unsigned zs_a, unsigned off, unsigned code, int nq,
+                                           int nqmax, unsigned off_dummy, const PairPos& P, float hi, unsigned self0) {
+  const int trips = FIXED > 0 ? FIXED : (RAGGED ? nqmax : nq);
 #pragma unroll 2
-  for (int q = 0; q < nqmax; ++q) {
-    const unsigned o = q < nq ? off : off_dummy;
+  for (int q = 0; q < trips; ++q) {
+    const unsigned o = (RAGGED && q >= nq) ? off_dummy : off;
     f32x2 X01, X23, Y01, Y23, Z01, Z23;
     lds_2x2(xs_a + o, X01, X23);
     lds_2x2(ys_a + o, Y01, Y23);
     lds_2x2(zs_a + o, Z01, Z23);
-    const f32x2 dx01 = sub2(xi2, X01), dx23 = sub2(xi2, X23);
-    const f32x2 dy01 = sub2(yi2, Y01), dy23 = sub2(yi2, Y23);
-    const f32x2 dz01 = sub2(zi2, Z01), dz23 = sub2(zi2, Z23);
-    const f32x2 q01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
-    const f32x2 q23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
-    float e0, e1, e2, e3;
-    unpack2(sub2(q01, mid2), e0, e1);
-    unpack2(sub2(q23, mid2), e2, e3);
-    m = fminf(fminf(m, fabsf(e0)), fabsf(e1));
-    m = fminf(fminf(m, fabsf(e2)), fabsf(e3));
-    if constexpr (SELF) {
-      ring_push2_self(rp, code, code + (1u << SHIFT), q01, hi, self);
-      ring_push2_self(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi, self);
-    } else {
-      ring_push2(rp, code, code + (1u << SHIFT), q01, hi);
-      ring_push2(rp, code + (2u << SHIFT), code + (3u << SHIFT), q23, hi);
+    f32x2 qa01, qa23, qb01, qb23;
+    {
+      const f32x2 dx01 = sub2(P.x0, X01), dx23 = sub2(P.x0, X23);
+      const f32x2 dy01 = sub2(P.y0, Y01), dy23 = sub2(P.y0, Y23);
+      const f32x2 dz01 = sub2(P.z0, Z01), dz23 = sub2(P.z0, Z23);
+      qa01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
+      qa23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
     }
+    {
+      const f32x2 dx01 = sub2(P.x1, X01), dx23 = sub2(P.x1, X23);
+      const f32x2 dy01 = sub2(P.y1, Y01), dy23 = sub2(P.y1, Y23);
+      const f32x2 dz01 = sub2(P.z1, Z01), dz23 = sub2(P.z1, Z23);
+      qb01 = fma2(dz01, dz01, fma2(dy01, dy01, mul2(dx01, dx01)));
+      qb23 = fma2(dz23, dz23, fma2(dy23, dy23, mul2(dx23, dx23)));
+    }
+    ring_push_pair<SELF, SHIFT>(rp, code, qa01, qb01, hi, self0);
+    ring_push_pair<SELF, SHIFT>(rp, code + (2u << SHIFT), qa23, qb23, hi, self0);
     off += 16;
     code += 4u << SHIFT;
   }
 }
 
-// Shared memory: TileTables | offs[tile cells] float4 | rowcell[interior_cap/4 + 8] u16 | xs[capA] ys[capA] zs[capA] floats |
-// rings[nwarps*32*RING_STRIDE].
 template <bool HALF, int LOGK, int SHIFT>
 __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_list(BuildArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -801,25 +802,19 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
   constexpr int K = 1 << LOGK;
   const int capA = build_capA(g);
   float4* offs = reinterpret_cast<float4*>(smem_raw + sizeof(TileTables));
-  unsigned short* rowcell = reinterpret_cast<unsigned short*>(offs + tile_tab_cells(g));   // tile cell of every quad of list rows
+  unsigned short* rowcell = reinterpret_cast<unsigned short*>(offs + tile_tab_cells(g));   // tile cell of every quad of interior slots
   float* xs = reinterpret_cast<float*>(rowcell + build_rowcell_len(g));
   float* ys = xs + capA;
   float* zs = ys + capA;
   unsigned char* rings = reinterpret_cast<unsigned char*>(zs + capA);
   const int tile = blockIdx.x;
-  __shared__ Geom gs;   // for the slow paths: a reference to kernel parameters would cost a stack copy
   __shared__ int soff[27];   // tile-cell index offsets of the 27-cell stencil (the same for every cell of the tile)
-  if (threadIdx.x == 0) gs = A.g;
   tile_load(g, tile, A.tab, tt);
   if (threadIdx.x < 27) {
     const int dx = (int)threadIdx.x % 3 - 1, dy = ((int)threadIdx.x / 3) % 3 - 1, dz = (int)threadIdx.x / 9 - 1;
     soff[threadIdx.x] = (dz * tt.tc[1] + dy) * tt.tc[0] + dx;
   }
   if (tt.n_slots > g.tile_cap || tt.n_int_slots > g.interior_cap) return;   // host re-plans and rebuilds
-  // A task = 8 consecutive quads of list rows = 32 lanes, one atom each.  Rows are padded per cell to multiples of 4,
-  // so a quad belongs to one cell, but the 8 quads of a task may belong to different cells (a cell of ~20 atoms fills
-  // 5 quads): the lanes of a warp then walk different candidate runs of about the same length, in lockstep.  Tasks
-  // are dealt to the warps round robin, so a tile of one big cell (rc = 5 sigma: ~150 atoms) still keeps several busy.
   for (int ic = threadIdx.x; ic < tt.nic; ic += blockDim.x) {
     const int t = interior_tile_cell(tt, ic);
     for (int i = 0; i < pad4(tt.cnt[t]) >> 2; ++i) rowcell[(tt.rstart[t] >> 2) + i] = (unsigned short)t;
@@ -866,120 +861,107 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
   __syncthreads();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const unsigned rbase = smem_addr(rings) + (unsigned)(wid * 32 + lane) * RING_STRIDE;
-  const size_t slots_cap = (size_t)g.interior_cap << LOGK;
+  const size_t slots_cap = (size_t)prow_cap(g) << LOGK;
   uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
   const int max_words = g.chunk_cap << LOGK;
   const unsigned dummy = (unsigned)tt.n_slots << SHIFT;
-  const float hi = A.rl2_hi, bw = A.rl2_bw;
-  const BuildBand bd = {A.rl2, A.rl2_hi, A.rl2_mid, A.rl2_bw};
-  const f32x2 mid2 = pack2(A.rl2_mid, A.rl2_mid);
+  const float hi = A.rl2_hi;
   const unsigned xs_a = smem_addr(xs), ys_a = smem_addr(ys), zs_a = smem_addr(zs);
   int my_max = 0;
   unsigned long long my_sum = 0;
 
-  const int nrq = tt.n_int_slots >> 2;                 // quads of list rows in use
+  const int nrq = tt.n_int_slots >> 2;                 // quads of interior slots in use
   const unsigned off_dummy = 4u * (unsigned)tt.n_slots;
 #pragma unroll 1
-  for (int task = wid; task * 8 < nrq; task += nw) {
-    const int rq = task * 8 + (lane >> 2);             // this lane's quad of rows
+  for (int task = wid; task * 16 < nrq; task += nw) {
+    const int rq = task * 16 + (lane >> 1);            // this lane's quad of slots; the lane owns its pair (lane & 1)
     const bool haveq = rq < nrq;
     const int t = rowcell[haveq ? rq : 0];             // its tile cell
     const int c = tt.cnt[t], g_lo = tt.gstart[t];
+    const int kin0 = haveq ? 4 * rq - tt.rstart[t] + 2 * (lane & 1) : c;   // index of the pair's first atom within its cell
+    const bool act0 = kin0 < c, act1 = kin0 + 1 < c;
+    const int prow = 2 * (haveq ? rq : 0) + (lane & 1);                  // pair row
+    const int aslot0 = tt.start[t] + (act0 ? kin0 : 0);                  // staged slot of the first atom
+    PairPos P;
     {
-      const int kin = haveq ? 4 * rq - tt.rstart[t] + (lane & 3) : c;   // index of the atom within its cell
-      const bool act = kin < c;
-      const int a = 4 * (haveq ? rq : 0) + (lane & 3);                  // list row
-      const int aslot = tt.start[t] + (act ? kin : 0);                  // staged slot
-      const int gi = g_lo + kin;
-      // an idle lane sits far away from everything, pad slots (+1e15) included: it accepts nothing
-      const float xi = act ? xs[aslot] : -1e15f, yi = act ? ys[aslot] : -1e15f, zi = act ? zs[aslot] : -1e15f;
-      const f32x2 xi2 = pack2(xi, xi), yi2 = pack2(yi, yi), zi2 = pack2(zi, zi);
-      const unsigned selfcode = (unsigned)aslot << SHIFT;
-      unsigned rp = rbase;
-      int nwords = 0;
-      auto store_word = [&](uint4 v) {
-        if (nwords < max_words) {
-          const int s = nwords & (K - 1), cch = nwords >> LOGK;
-          st_stream(tlist + (size_t)cch * slots_cap + ((size_t)a << LOGK) + s, v);
-        }
-        ++nwords;
-      };
-      auto flush = [&]() {   // complete words leave; the remainder moves to the ring start
-        const int pend = (int)(rp - rbase) >> 1, full = pend >> 3;
-        for (int w = 0; w < full; ++w) store_word(lds_u4(rbase + 16 * w));
-        if (full) sts_u4(rbase, lds_u4(rbase + 16 * full));
-        rp = rbase + 2 * (pend & 7);
-      };
-      // Full list: 9 runs, one per (dy, dz): the cells x-1, x, x+1 are consecutive tile cells, hence one contiguous
-      // range of staged slots (pad slots in between are far away and never taken).  Half list: 27 one-cell runs,
-      // because a whole cell is kept or dropped (below).
-      constexpr int NRUN = HALF ? 27 : 9;
+      // an idle atom sits far away from everything, pad slots (+1e15) included: it accepts nothing
+      const float x0 = act0 ? xs[aslot0] : -1e15f, y0 = act0 ? ys[aslot0] : -1e15f, z0 = act0 ? zs[aslot0] : -1e15f;
+      const float x1 = act1 ? xs[aslot0 + 1] : -1e15f, y1 = act1 ? ys[aslot0 + 1] : -1e15f, z1 = act1 ? zs[aslot0 + 1] : -1e15f;
+      P.x0 = pack2(x0, x0); P.y0 = pack2(y0, y0); P.z0 = pack2(z0, z0);
+      P.x1 = pack2(x1, x1); P.y1 = pack2(y1, y1); P.z1 = pack2(z1, z1);
+    }
+    const unsigned self0 = (unsigned)aslot0 << SHIFT;
+    unsigned rp = rbase;
+    int nwords = 0;
+    auto store_word = [&](uint4 v) {
+      if (nwords < max_words) {
+        const int s = nwords & (K - 1), cch = nwords >> LOGK;
+        st_stream(tlist + (size_t)cch * slots_cap + ((size_t)prow << LOGK) + s, v);
+      }
+      ++nwords;
+    };
+    auto flush = [&]() {   // complete words leave; the remainder moves to the ring start
+      const int pend = (int)(rp - rbase) >> 1, full = pend >> 3;
+      for (int w = 0; w < full; ++w) store_word(lds_u4(rbase + 16 * w));
+      if (full) sts_u4(rbase, lds_u4(rbase + 16 * full));
+      rp = rbase + 2 * (pend & 7);
+    };
+    // Full list: 9 runs, one per (dy, dz): the cells x-1, x, x+1 are consecutive tile cells, hence one contiguous
+    // range of staged slots (pad slots in between are far away and never taken).  Half list: 27 one-cell runs,
+    // because a whole cell is kept or dropped (below).
+    constexpr int NRUN = HALF ? 27 : 9;
 #pragma unroll 1
-      for (int sc = 0; sc < NRUN; ++sc) {
-        int tfirst, s0, s1;
-        bool own;                                        // the run holds the atom's own cell (the same for all lanes)
-        if constexpr (HALF) {
-          tfirst = t + soff[sc];
-          own = sc == 13;
-          s0 = tt.start[tfirst];
-          s1 = s0 + pad4(tt.cnt[tfirst]);
-          // keep (i, j) iff j follows i in the sorted order; a cell is a contiguous range of that order, so for
-          // another cell the answer is the same for all of its atoms
-          if (!own && tt.gstart[tfirst] < g_lo) s1 = s0;
+    for (int sc = 0; sc < NRUN; ++sc) {
+      int s0, s1;
+      bool own;                                        // the run holds the pair's own cell (the same for all lanes)
+      if constexpr (HALF) {
+        const int tfirst = t + soff[sc];
+        own = sc == 13;
+        s0 = tt.start[tfirst];
+        s1 = s0 + pad4(tt.cnt[tfirst]);
+        // keep (i, j) iff j follows i in the sorted order; a cell is a contiguous range of that order, so for
+        // another cell the answer is the same for all of its atoms; the own cell keeps the slots after the pair
+        if (!own && tt.gstart[tfirst] < g_lo) s1 = s0;
+      } else {
+        const int tc = t + soff[3 * sc + 1];
+        own = sc == 4;
+        s0 = tt.start[tc - 1];
+        s1 = tt.start[tc + 1] + pad4(tt.cnt[tc + 1]);
+      }
+      // (a lane without atoms scans its quad's runs like the others, so that full pieces stay uniform; it sits
+      // far away and accepts nothing)
+      const int npieces = (int)__reduce_max_sync(0xffffffffu, (unsigned)((s1 - s0 + 31) >> 5));
+#pragma unroll 1
+      for (int pc = 0; pc < npieces; ++pc) {   // pieces of <= 32 slots: what the ring is guaranteed to take
+        const int j0 = s0 + 32 * pc;
+        const int nq = max(0, min(8, (s1 - j0) >> 2));
+        if ((int)(rp - rbase) > 2 * (RING - 32)) flush();
+        const unsigned off = 4u * (unsigned)j0, code = (unsigned)j0 << SHIFT;
+        constexpr int SELF = HALF ? 2 : 1;
+        if (__all_sync(0xffffffffu, nq == 8)) {
+          if (own) build_scan<SELF, SHIFT, 8, false>(rp, xs_a, ys_a, zs_a, off, code, 8, 8, off_dummy, P, hi, self0);
+          else build_scan<0, SHIFT, 8, false>(rp, xs_a, ys_a, zs_a, off, code, 8, 8, off_dummy, P, hi, self0);
         } else {
-          const int tc = t + soff[3 * sc + 1];
-          tfirst = tc - 1;
-          own = sc == 4;
-          s0 = tt.start[tc - 1];
-          s1 = tt.start[tc + 1] + pad4(tt.cnt[tc + 1]);
-        }
-        // (a lane without an atom scans its quad's runs like the others, so that full pieces stay uniform; it sits
-        // far away and accepts nothing)
-        const int npieces = (int)__reduce_max_sync(0xffffffffu, (unsigned)((s1 - s0 + 31) >> 5));
-#pragma unroll 1
-        for (int pc = 0; pc < npieces; ++pc) {   // pieces of <= 32 slots: what the ring is guaranteed to take
-          const int j0 = s0 + 32 * pc;
-          const int nq = max(0, min(8, (s1 - j0) >> 2));
-          if ((int)(rp - rbase) > 2 * (RING - 32)) flush();
-          if (HALF && own) {
-            // own cell: slot order is the sorted order
-            if (nq > 0)
-              rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, aslot, aslot, rp, j0, 4 * nq, tfirst, SHIFT);
-            continue;
-          }
-          const unsigned rp_seg = rp;
-          float m = 1e30f;
-          const unsigned off = 4u * (unsigned)j0, code = (unsigned)j0 << SHIFT;
-          if (__all_sync(0xffffffffu, nq == 8)) {
-            if (own) build_scan_fast<true, SHIFT, 8>(rp, m, xs_a, ys_a, zs_a, off, code, 8, xi2, yi2, zi2, mid2, hi, selfcode);
-            else build_scan_fast<false, SHIFT, 8>(rp, m, xs_a, ys_a, zs_a, off, code, 8, xi2, yi2, zi2, mid2, hi, selfcode);
-          } else {
-            const int nqmax = (int)__reduce_max_sync(0xffffffffu, (unsigned)nq);
-            if (own) build_scan_ragged<true, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, nqmax, off_dummy, xi2, yi2, zi2, mid2, hi, selfcode);
-            else build_scan_ragged<false, SHIFT>(rp, m, xs_a, ys_a, zs_a, off, code, nq, nqmax, off_dummy, xi2, yi2, zi2, mid2, hi, selfcode);
-          }
-          if (__builtin_expect(m <= bw && nq > 0, 0)) {
-            // some candidate of this piece lies in the guard band of the fp32 test: redo the piece, deciding the
-            // in-band candidates in fp64 from the global positions (the pair set is exactly the fp64 one)
-            rp = build_scan_careful(gs, tt, A.x, A.ld, bd, xs, ys, zs, xi, yi, zi, act, gi, t, own ? aslot : -1, -1, rp_seg, j0, 4 * nq,
-                                    tfirst, SHIFT);
-          }
+          const int nqmax = (int)__reduce_max_sync(0xffffffffu, (unsigned)nq);
+          if (own) build_scan<SELF, SHIFT, 0, true>(rp, xs_a, ys_a, zs_a, off, code, nq, nqmax, off_dummy, P, hi, self0);
+          else build_scan<0, SHIFT, 0, true>(rp, xs_a, ys_a, zs_a, off, code, nq, nqmax, off_dummy, P, hi, self0);
         }
       }
-      // last words: complete ones, then the partial one padded with the dummy code
-      flush();
-      const int rem = (int)(rp - rbase) >> 1;   // 0..7
-      if (rem) {
-        for (int p = rem; p < 8; ++p) sts_u16(rbase + 2 * p, dummy);
-        const int before = nwords;
-        store_word(lds_u4(rbase));
-        nwords = before;   // count below from complete words + rem
-      }
-      const int n = nwords * 8 + rem;
-      if (!act && haveq) A.numneigh[(size_t)tile * g.interior_cap + a] = 0;   // pad row
-      if (act) {
-        const int stored = n < g.row_cap ? n : g.row_cap;
-        A.numneigh[(size_t)tile * g.interior_cap + a] = stored;
+    }
+    // last words: complete ones, then the partial one padded with the dummy code
+    flush();
+    const int rem = (int)(rp - rbase) >> 1;   // 0..7
+    if (rem) {
+      for (int p = rem; p < 8; ++p) sts_u16(rbase + 2 * p, dummy);
+      const int before = nwords;
+      store_word(lds_u4(rbase));
+      nwords = before;   // count below from complete words + rem
+    }
+    const int n = nwords * 8 + rem;
+    if (haveq) {
+      const int stored = act0 ? (n < g.row_cap ? n : g.row_cap) : 0;   // a pad pair row is empty
+      A.numneigh[(size_t)tile * prow_cap(g) + prow] = stored;
+      if (act0) {
         my_max = max(my_max, n);
         my_sum += (unsigned long long)stored;
       }
@@ -1006,7 +988,7 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
 // the 8 threads of a quarter warp, which walk their words in lockstep, then read 8 different bank groups.
 // Residue classes are never perfectly even, so the surplus of the longer classes fills the holes of the
 // shorter ones (those entries may collide), and the remaining holes name the dummy slot.
-// One thread per row; its output row is assembled in a private stripe of shared memory (row_bytes).
+// One thread per (pair) row; its output row is assembled in a private stripe of shared memory (row_bytes).
 // ---------------------------------------------------------------------------------------------------
 struct BalanceArgs {
   Geom g;
@@ -1023,15 +1005,15 @@ __global__ void __launch_bounds__(256) k_balance_rows(BalanceArgs A) {
   constexpr int K = 1 << LOGK;
   const int tile = blockIdx.x;
   const int* __restrict__ h = A.tab + (size_t)tile * tile_tab_stride(g);
-  const int n_rows = h[0], n_slots = h[1];
-  if (n_slots > g.tile_cap || n_rows > g.interior_cap) return;
+  const int n_rows = h[0] >> 1, n_slots = h[1];   // pair rows
+  if (n_slots > g.tile_cap || h[0] > g.interior_cap) return;
   const int shift = g.code_shift;
   const unsigned dummy = (unsigned)n_slots << shift;
-  const size_t slots_cap = (size_t)g.interior_cap << LOGK;
+  const size_t slots_cap = (size_t)prow_cap(g) << LOGK;
   uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
   unsigned short* out = reinterpret_cast<unsigned short*>(smem_raw + (size_t)threadIdx.x * A.row_bytes);
   for (int a = threadIdx.x; a < n_rows; a += blockDim.x) {
-    const int n = min(A.numneigh[(size_t)tile * g.interior_cap + a], g.row_cap);
+    const int n = min(A.numneigh[(size_t)tile * prow_cap(g) + a], g.row_cap);
     if (n <= 0) continue;
     const int W = (n + 7) >> 3;
     auto word_ptr = [&](int q) { return tlist + (size_t)(q >> LOGK) * slots_cap + ((size_t)a << LOGK) + (q & (K - 1)); };
@@ -1080,43 +1062,114 @@ __global__ void __launch_bounds__(256) k_balance_rows(BalanceArgs A) {
   }
 }
 
-// list export in caller ids (pair-set parity).  Shared memory: TileTables | sid[tile_cap+4] ints.
-__global__ void __launch_bounds__(BUILD_THREADS) k_export_list(Geom g, const int* __restrict__ tab, const int* __restrict__ id,
-                                                               const uint4* __restrict__ list, const int* __restrict__ numneigh,
-                                                               int* __restrict__ nn_out, int* __restrict__ neigh_out, long long stride) {
+// fp64 decision of the pair-set definition (north_star (2)): |x_i - x_j|^2 < rl^2 from the global positions, atom gi
+// of tile cell ti against atom gj of tile cell tj (their periodic images are the ones the tile stages).
+__device__ __forceinline__ bool pair_in_list_fp64(const Geom& g, const TileTables& tt, const double* __restrict__ x, size_t ld,
+                                                  int gi, int ti, int gj, int tj, double rl2) {
+  double oi[3], oj[3];
+  tile_cell_offset(g, tt, ti, oi);
+  tile_cell_offset(g, tt, tj, oj);
+  double r2 = 0.0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    double dd = (x[d * ld + gi] + oi[d]) - (x[d * ld + gj] + oj[d]);
+    r2 += dd * dd;
+  }
+  return r2 < rl2;
+}
+
+// List export in caller ids (pair-set parity; test / diagnostic path, one thread per interior atom).
+//   EXPORT_EXACT: nn_out[i], neigh_out[i][..] = the exact fp64 neighbor set of atom i: the entries of its pair's row
+//                 (plus its partner) that pass the fp64 test; neigh_out may be NULL (counts only);
+//                 stat[0] = max count (int), stat[2..3] = sum of counts (unsigned long long) when stat != NULL.
+//   EXPORT_RAW:   the stored rows as they are: nn_out[i] = row length and neigh_out[i][..] = the row's entries for
+//                 the FIRST atom of a pair (0 for the second); owner_out[i] = caller id of the pair's first atom.
+// Shared memory: TileTables | sid[capA] | sgi[capA] ints | scl[capA] u16.
+constexpr int EXPORT_EXACT = 0, EXPORT_RAW = 1;
+struct ExportArgs {
+  Geom g;
+  const int* tab; const int* id; const double* x; size_t ld;
+  const uint4* list; const int* numneigh;
+  double rl2;
+  int mode;
+  int* nn_out; int* neigh_out; int* owner_out; long long stride;
+  int* stat;
+};
+__global__ void __launch_bounds__(BUILD_THREADS) k_export_list(ExportArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
+  const Geom& g = A.g;
+  const int capA = (g.tile_cap + 8) & ~3;
   int* sid = reinterpret_cast<int*>(smem_raw + sizeof(TileTables));
+  int* sgi = sid + capA;
+  unsigned short* scl = reinterpret_cast<unsigned short*>(sgi + capA);
   const int tile = blockIdx.x;
-  tile_load(g, tile, tab, tt);
-  tile_stage(g, tt, g.tile_cap, [&](int slot, int gi, const double*, int) { sid[slot] = id[gi]; }, [&](int slot) { sid[slot] = -1; });
+  tile_load(g, tile, A.tab, tt);
+  tile_stage(g, tt, g.tile_cap, [&](int slot, int gi, const double*, int t) { sid[slot] = A.id[gi]; sgi[slot] = gi; scl[slot] = (unsigned short)t; },
+             [&](int slot) { sid[slot] = -1; sgi[slot] = 0; scl[slot] = 0; });
   __syncthreads();
   const int K = g.K;
-  const size_t slots_cap = (size_t)g.interior_cap * K;
-  const uint4* tlist = list + (size_t)tile * g.chunk_cap * slots_cap;
+  const size_t slots_cap = (size_t)prow_cap(g) * K;
+  const uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
+  int my_max = 0;
+  unsigned long long my_sum = 0;
   for (int ic = 0; ic < tt.nic; ++ic) {
     const int t = interior_tile_cell(tt, ic);
-    for (int k = threadIdx.x; k < tt.cnt[t]; k += blockDim.x) {
-      const int a = tt.rstart[t] + k, n = numneigh[(size_t)tile * g.interior_cap + a], io = sid[tt.start[t] + k];
-      nn_out[io] = n;
-      // the row's n entries sit somewhere in its ceil(n/8) words; the other positions name the dummy slot
-      int m = 0;
-      for (int e = 0; e < ((n + 7) & ~7); ++e) {
-        int q = e >> 3, s = q % K, c = q / K;
-        uint4 w = tlist[(size_t)c * slots_cap + (size_t)a * K + s];
-        unsigned word = (&w.x)[(e & 7) >> 1];
-        unsigned code = (e & 1) ? (word >> 16) : (word & 0xffffu);
-        if ((int)(code >> g.code_shift) == tt.n_slots) continue;
-        if (m < stride) neigh_out[(long long)io * stride + m] = sid[code >> g.code_shift];
-        ++m;
+    const int c = tt.cnt[t];
+    for (int k = threadIdx.x; k < c; k += blockDim.x) {
+      const int prow = (tt.rstart[t] + k) >> 1, which = k & 1;
+      const int n = A.numneigh[(size_t)tile * prow_cap(g) + prow];
+      const int slot = tt.start[t] + k, io = sid[slot], gi = sgi[slot];
+      const int pslot = slot ^ 1;                      // the partner's slot (cells start at multiples of 4)
+      const bool have_partner = (k ^ 1) < c;
+      if (A.mode == EXPORT_RAW) {
+        A.owner_out[io] = which ? sid[pslot] : io;
+        if (which) { A.nn_out[io] = 0; continue; }
       }
+      int m = 0;
+      auto emit = [&](int jo) {
+        if (A.neigh_out && m < A.stride) A.neigh_out[(long long)io * A.stride + m] = jo;
+        ++m;
+      };
+      // the partner: never stored in the row (the force kernels add the pair's mutual term directly)
+      if (A.mode == EXPORT_EXACT && have_partner && (!g.half || which == 0) &&
+          pair_in_list_fp64(g, tt, A.x, A.ld, gi, t, sgi[pslot], t, A.rl2))
+        emit(sid[pslot]);
+      // the row's n entries sit somewhere in its ceil(n/8) words; the other positions name the dummy slot
+      for (int e = 0; e < ((n + 7) & ~7); ++e) {
+        const int q = e >> 3, sl = q % K, ch = q / K;
+        const uint4 w = tlist[(size_t)ch * slots_cap + (size_t)prow * K + sl];
+        const unsigned word = (&w.x)[(e & 7) >> 1];
+        const unsigned code = (e & 1) ? (word >> 16) : (word & 0xffffu);
+        const int js = (int)(code >> g.code_shift);
+        if (js == tt.n_slots) continue;
+        if (A.mode == EXPORT_RAW || pair_in_list_fp64(g, tt, A.x, A.ld, gi, t, sgi[js], scl[js], A.rl2)) emit(sid[js]);
+      }
+      A.nn_out[io] = m;
+      my_max = max(my_max, m);
+      my_sum += (unsigned long long)m;
+    }
+  }
+  if (A.stat) {
+    for (int o = 16; o > 0; o >>= 1) {
+      my_max = max(my_max, __shfl_xor_sync(0xffffffffu, my_max, o));
+      my_sum += __shfl_xor_sync(0xffffffffu, my_sum, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+      atomicMax(&A.stat[0], my_max);
+      atomicAdd(reinterpret_cast<unsigned long long*>(A.stat + 2), my_sum);
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------------
 // pair styles.  T = double (MD_FP64) or float (MD_MIXED pair math).
-// A Body accumulates per-word partial sums in T; the kernels add them to per-atom totals in double.
+// A Body has two entry points:
+//   pair  -- one (i, j) term on scalars (the direct cell-list kernel);
+//   pair2 -- the terms (i0, j) and (i1, j) of the two atoms of a PAIR ROW against one gathered j, on two-wide
+//            values Pk<T>: for float a packed f32x2 register pair (FADD2 / FMUL2 / FFMA2: two lanes of math per
+//            issue slot), for double a plain struct of two doubles.
+// Both accumulate per-word partial sums in T; the kernels add them to per-atom totals in double.
 // Bodies are branch-free: out-of-range partners contribute an exact zero through a select.
 // ---------------------------------------------------------------------------------------------------
 template <typename T> struct Vec2;
@@ -1126,11 +1179,44 @@ template <typename T> __device__ __forceinline__ typename Vec2<T>::type lds_v2(u
 template <> __device__ __forceinline__ float2 lds_v2<float>(unsigned a) { return lds_f2(a); }
 template <> __device__ __forceinline__ double2 lds_v2<double>(unsigned a) { return lds_d2(a); }
 
+struct d64x2 { double a, b; };
+template <typename T> struct Pk;
+template <> struct Pk<float> { using type = f32x2; };
+template <> struct Pk<double> { using type = d64x2; };
+__device__ __forceinline__ f32x2 pk_make(float a, float b) { return pack2(a, b); }
+__device__ __forceinline__ d64x2 pk_make(double a, double b) { return d64x2{a, b}; }
+__device__ __forceinline__ f32x2 pk_make_once(float a, float b) { return pack2_once(a, b); }
+__device__ __forceinline__ d64x2 pk_make_once(double a, double b) { return d64x2{a, b}; }
+__device__ __forceinline__ float pk_lo(f32x2 v) { float a, b; unpack2(v, a, b); return a; }
+__device__ __forceinline__ float pk_hi(f32x2 v) { float a, b; unpack2(v, a, b); return b; }
+__device__ __forceinline__ double pk_lo(d64x2 v) { return v.a; }
+__device__ __forceinline__ double pk_hi(d64x2 v) { return v.b; }
+__device__ __forceinline__ f32x2 pk_add(f32x2 x, f32x2 y) { return add2(x, y); }
+__device__ __forceinline__ f32x2 pk_sub(f32x2 x, f32x2 y) { return sub2(x, y); }
+__device__ __forceinline__ f32x2 pk_mul(f32x2 x, f32x2 y) { return mul2(x, y); }
+__device__ __forceinline__ f32x2 pk_fma(f32x2 x, f32x2 y, f32x2 z) { return fma2(x, y, z); }
+__device__ __forceinline__ d64x2 pk_add(d64x2 x, d64x2 y) { return d64x2{x.a + y.a, x.b + y.b}; }
+__device__ __forceinline__ d64x2 pk_sub(d64x2 x, d64x2 y) { return d64x2{x.a - y.a, x.b - y.b}; }
+__device__ __forceinline__ d64x2 pk_mul(d64x2 x, d64x2 y) { return d64x2{x.a * y.a, x.b * y.b}; }
+__device__ __forceinline__ d64x2 pk_fma(d64x2 x, d64x2 y, d64x2 z) { return d64x2{fma(x.a, y.a, z.a), fma(x.b, y.b, z.b)}; }
+template <typename T> __device__ __forceinline__ typename Pk<T>::type pk_splat(T a) { return pk_make(a, a); }
+
 struct PairParams {    // host-prepared constants, in double; kernels convert once
   double rc2;
   double lj1, lj2, lj3, lj4;             // 48 eps s^12, 24 eps s^6, 4 eps s^12, 4 eps s^6
   double A, p_r0, B, q_r0, inv_r0, p, q; // EAM: A, p/r0, B, q/r0, 1/r0, p, q
+  // the same rounded to fp32 once on the host (fill_float_copies): the mixed-precision bodies read these straight
+  // from the constant bank instead of converting the doubles inside the list loop
+  float f_rc2, f_lj1, f_lj2, f_lj3, f_lj4, f_A, f_p_r0, f_q_r0, f_p, f_q;
+  __host__ void fill_float_copies() {
+    f_rc2 = (float)rc2; f_lj1 = (float)lj1; f_lj2 = (float)lj2; f_lj3 = (float)lj3; f_lj4 = (float)lj4;
+    f_A = (float)A; f_p_r0 = (float)p_r0; f_q_r0 = (float)q_r0; f_p = (float)p; f_q = (float)q;
+  }
 };
+template <typename T> __device__ __forceinline__ T pp_pick(double d, float f);
+template <> __device__ __forceinline__ float pp_pick<float>(double, float f) { return f; }
+template <> __device__ __forceinline__ double pp_pick<double>(double d, float) { return d; }
+#define MDK_PP(name) pp_pick<T>(P.name, P.f_##name)
 
 template <typename T> __device__ __forceinline__ T t_rcp(T x);
 template <> __device__ __forceinline__ float t_rcp<float>(float x) { return rcp_approx(x); }
@@ -1142,12 +1228,21 @@ template <typename T> __device__ __forceinline__ T t_exp(T x);
 template <> __device__ __forceinline__ float t_exp<float>(float x) { return ex2_approx(x * 1.4426950408889634f); }
 template <> __device__ __forceinline__ double t_exp<double>(double x) { return exp(x); }
 
+// the six virial products of one term, accumulated two-wide: p[4..9] += {dx dx, dy dy, dz dz, dx dy, dx dz, dy dz} fp
+template <class PK>
+__device__ __forceinline__ void virial2(PK dx, PK dy, PK dz, PK fp, PK* p) {
+  const PK fx = pk_mul(fp, dx), fy = pk_mul(fp, dy), fz = pk_mul(fp, dz);
+  p[4] = pk_fma(dx, fx, p[4]); p[5] = pk_fma(dy, fy, p[5]); p[6] = pk_fma(dz, fz, p[6]);
+  p[7] = pk_fma(dx, fy, p[7]); p[8] = pk_fma(dx, fz, p[8]); p[9] = pk_fma(dy, fz, p[9]);
+}
+
 // LJ 12-6 force (+ energy, virial when EV).  PAPER.md L102 calcPairForce, App. A L256.
 template <typename T, bool EV>
 struct LJBody {
   static constexpr int NT = EV ? 10 : 3;   // fx fy fz [e wxx wyy wzz wxy wxz wyz]
+  using PK = typename Pk<T>::type;
   T rc2, lj1, lj2, lj3, lj4;
-  __device__ explicit LJBody(const PairParams& P) : rc2((T)P.rc2), lj1((T)P.lj1), lj2((T)P.lj2), lj3((T)P.lj3), lj4((T)P.lj4) {}
+  __device__ explicit LJBody(const PairParams& P) : rc2(MDK_PP(rc2)), lj1(MDK_PP(lj1)), lj2(MDK_PP(lj2)), lj3(MDK_PP(lj3)), lj4(MDK_PP(lj4)) {}
   __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T, bool ok, T (&p)[NT]) const {
     const bool in = ok && r2 < rc2;
     T r2i = t_rcp<T>(r2);
@@ -1160,18 +1255,39 @@ struct LJBody {
       p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
     }
   }
+  // 1/r^2 := 0 beyond the cutoff: r^-6, the force factor and the energy term are then exact zeros
+  __device__ __forceinline__ void pair2(PK dx, PK dy, PK dz, PK r2, PK, PK (&p)[NT]) const {
+    const T ra = pk_lo(r2), rb = pk_hi(r2);
+    const T ia = ra < rc2 ? t_rcp<T>(ra) : (T)0, ib = rb < rc2 ? t_rcp<T>(rb) : (T)0;
+    const PK r2i = pk_make(ia, ib);
+    const PK r6 = pk_mul(pk_mul(r2i, r2i), r2i);
+    const PK fp = pk_mul(pk_mul(r6, pk_fma(pk_splat<T>(lj1), r6, pk_splat<T>(-lj2))), r2i);
+    p[0] = pk_fma(fp, dx, p[0]); p[1] = pk_fma(fp, dy, p[1]); p[2] = pk_fma(fp, dz, p[2]);
+    if constexpr (EV) {
+      p[3] = pk_fma(r6, pk_fma(pk_splat<T>(lj3), r6, pk_splat<T>(-lj4)), p[3]);
+      virial2(dx, dy, dz, fp, p);
+    }
+  }
 };
 
 // EAM pass 1: rho_i = sum_j exp(-q (r/r0 - 1))            (a6)
 template <typename T, bool EV>
 struct EamDensityBody {
   static constexpr int NT = 1;
+  using PK = typename Pk<T>::type;
   T rc2, q_r0, q;
-  __device__ explicit EamDensityBody(const PairParams& P) : rc2((T)P.rc2), q_r0((T)P.q_r0), q((T)P.q) {}
+  __device__ explicit EamDensityBody(const PairParams& P) : rc2(MDK_PP(rc2)), q_r0(MDK_PP(q_r0)), q(MDK_PP(q)) {}
   __device__ __forceinline__ void pair(T, T, T, T r2, T, bool ok, T (&p)[NT]) const {
     const bool in = ok && r2 < rc2;
     T r = r2 * t_rsqrt<T>(r2);
     p[0] += in ? t_exp<T>(q - q_r0 * r) : (T)0;
+  }
+  __device__ __forceinline__ void pair2(PK, PK, PK, PK r2, PK, PK (&p)[NT]) const {
+    const T ra = pk_lo(r2), rb = pk_hi(r2);
+    const PK r = pk_mul(r2, pk_make(t_rsqrt<T>(ra), t_rsqrt<T>(rb)));
+    const PK arg = pk_fma(pk_splat<T>(-q_r0), r, pk_splat<T>(q));
+    const T ea = ra < rc2 ? t_exp<T>(pk_lo(arg)) : (T)0, eb = rb < rc2 ? t_exp<T>(pk_hi(arg)) : (T)0;
+    p[0] = pk_add(p[0], pk_make(ea, eb));
   }
 };
 
@@ -1179,9 +1295,10 @@ struct EamDensityBody {
 template <typename T, bool EV>
 struct EamForceBody {
   static constexpr int NT = EV ? 10 : 3;
+  using PK = typename Pk<T>::type;
   T rc2, q_r0, q, p_r0, pp, A;
   __device__ explicit EamForceBody(const PairParams& P)
-      : rc2((T)P.rc2), q_r0((T)P.q_r0), q((T)P.q), p_r0((T)P.p_r0), pp((T)P.p), A((T)P.A) {}
+      : rc2(MDK_PP(rc2)), q_r0(MDK_PP(q_r0)), q(MDK_PP(q)), p_r0(MDK_PP(p_r0)), pp(MDK_PP(p)), A(MDK_PP(A)) {}
   __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T wsum, bool ok, T (&p)[NT]) const {
     const bool in = ok && r2 < rc2;
     T rinv = t_rsqrt<T>(r2);
@@ -1195,6 +1312,24 @@ struct EamForceBody {
       p[3] += in ? phi : (T)0;
       p[4] += dx * dx * fp; p[5] += dy * dy * fp; p[6] += dz * dz * fp;
       p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
+    }
+  }
+  // 1/r := 0 and phi := 0 beyond the cutoff zero the force factor and the energy term
+  __device__ __forceinline__ void pair2(PK dx, PK dy, PK dz, PK r2, PK wsum, PK (&p)[NT]) const {
+    const T ra = pk_lo(r2), rb = pk_hi(r2);
+    const T ia = t_rsqrt<T>(ra), ib = t_rsqrt<T>(rb);
+    const PK r = pk_mul(r2, pk_make(ia, ib));
+    const PK arho = pk_fma(pk_splat<T>(-q_r0), r, pk_splat<T>(q));
+    const PK aphi = pk_fma(pk_splat<T>(-p_r0), r, pk_splat<T>(pp));
+    const bool ina = ra < rc2, inb = rb < rc2;
+    const PK rho = pk_make(t_exp<T>(pk_lo(arho)), t_exp<T>(pk_hi(arho)));
+    const PK phi = pk_make(ina ? A * t_exp<T>(pk_lo(aphi)) : (T)0, inb ? A * t_exp<T>(pk_hi(aphi)) : (T)0);
+    const PK rinv = pk_make(ina ? ia : (T)0, inb ? ib : (T)0);
+    const PK fp = pk_mul(pk_fma(pk_mul(wsum, pk_splat<T>(q_r0)), rho, pk_mul(pk_splat<T>(p_r0), phi)), rinv);
+    p[0] = pk_fma(fp, dx, p[0]); p[1] = pk_fma(fp, dy, p[1]); p[2] = pk_fma(fp, dz, p[2]);
+    if constexpr (EV) {
+      p[3] = pk_add(p[3], phi);
+      virial2(dx, dy, dz, fp, p);
     }
   }
 };
@@ -1283,6 +1418,16 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
   return d2;
 }
 
+// per-pair epilogue: the two atoms gi and gi + 1 (the second only if act1), one after the other (both at once
+// would need 36 more live registers than the list loop leaves); returns max |x'-x0|^2 for EPI_KICK_DRIFT (else 0).
+template <typename T>
+__device__ __forceinline__ double atom_epilogue2(const ForceArgs& A, int gi, bool act1, const double (&ta)[3], const double (&tb)[3],
+                                                 const double (&cc)[3]) {
+  double d2 = atom_epilogue<T>(A, gi, ta, cc);
+  if (act1) d2 = fmax(d2, atom_epilogue<T>(A, gi + 1, tb, cc));
+  return d2;
+}
+
 // ---------------------------------------------------------------------------------------------------
 // staged-tile gathers: the "random access" load of atom j is ONE 128-bit shared-memory
 // load (two for fp64) of {x, y, z, w} in tile-centred coordinates; w holds -F'(rho_j) in EAM pass 2.
@@ -1301,6 +1446,20 @@ template <> __device__ __forceinline__ double4 lds_v4<double>(unsigned a) {
   asm volatile("ld.shared.v2.f64 {%0,%1}, [%2+16];" : "=d"(r.z), "=d"(r.w) : "r"(a));
   return r;
 }
+
+// One staged record loaded component by component (four scalar loads): for the row's OWN two atoms, whose
+// coordinates are then free to sit in whatever registers the packed pairs {x0, x1}, {y0, y1}, {z0, z1} need
+// (after a 128-bit load they are pinned to an aligned quad, and ptxas rebuilds each pair with two moves per use).
+template <typename T> __device__ __forceinline__ typename Vec4<T>::type lds_v4_scalars(unsigned a);
+template <> __device__ __forceinline__ float4 lds_v4_scalars<float>(unsigned a) {
+  float4 r;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r.x) : "r"(a));
+  asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(r.y) : "r"(a));
+  asm volatile("ld.shared.f32 %0, [%1+8];" : "=f"(r.z) : "r"(a));
+  asm volatile("ld.shared.f32 %0, [%1+12];" : "=f"(r.w) : "r"(a));
+  return r;
+}
+template <> __device__ __forceinline__ double4 lds_v4_scalars<double>(unsigned a) { return lds_v4<double>(a); }
 
 // TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP)
 __device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count) {
@@ -1325,27 +1484,28 @@ __device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// the neighbor-list loop of PAPER.md L88-122 for one (atom, lane): walks this lane's 128-bit words,
+// the neighbor-list loop of PAPER.md L88-122 for one (pair row, lane): walks this lane's 128-bit words,
 // 8 entries each; each entry is a slot code (slot << code_shift; the staged record sits at
-// st_base + 2 * code).  w of the staged atoms holds -F'(rho_j) for EAM pass 2, so pw - jw = F'_i + F'_j.
+// st_base + 2 * code) and is evaluated against BOTH atoms of the pair (pi0, pi1) with two-wide math.
+// w of the staged atoms holds -F'(rho_j) for EAM pass 2, so pw - jw = F'_i + F'_j.
 // ---------------------------------------------------------------------------------------------------
 template <typename T, class Body>
 __device__ __forceinline__ void list_loop(const Body& body, unsigned st_base, const uint4* __restrict__ words, size_t word_stride,
-                                          int nwords, typename Vec4<T>::type pi, double (&tot)[Body::NT], uint4 w0, bool have_w0) {
+                                          int nwords, typename Vec4<T>::type pi0, typename Vec4<T>::type pi1, double (&tot0)[Body::NT],
+                                          double (&tot1)[Body::NT], uint4 w0, bool have_w0) {
   constexpr int NT = Body::NT;
+  using PK = typename Pk<T>::type;
   if (nwords <= 0) return;
-  // two words in flight ahead of the one being processed: a word is ~200 issue slots of work for the warp,
-  // less than one DRAM round trip when the SM is busy with other warps
+  // one word in flight ahead of the one being processed: a word is 8 gathers x 2 atoms = ~250 issue slots of work
+  // for the warp, i.e. more than a DRAM round trip once the SM's other warps take their turns
   uint4 w = have_w0 ? w0 : ld_stream(words);
-  uint4 wn = w;
-  if (nwords > 1) wn = ld_stream(words + word_stride);
+  const PK xi = pk_make_once(pi0.x, pi1.x), yi = pk_make_once(pi0.y, pi1.y), zi = pk_make_once(pi0.z, pi1.z), wi = pk_make(pi0.w, pi1.w);
   for (int c = 0; c < nwords; ++c) {
     const uint4 cur = w;
-    w = wn;
-    if (c + 2 < nwords) wn = ld_stream(words + (size_t)(c + 2) * word_stride);
-    T p[NT];
+    if (c + 1 < nwords) w = ld_stream(words + (size_t)(c + 1) * word_stride);
+    PK p[NT];
 #pragma unroll
-    for (int k = 0; k < NT; ++k) p[k] = (T)0;
+    for (int k = 0; k < NT; ++k) p[k] = pk_splat<T>((T)0);
     const unsigned ww[4] = {cur.x, cur.y, cur.z, cur.w};
 #pragma unroll
     for (int h = 0; h < 4; ++h) {
@@ -1353,33 +1513,36 @@ __device__ __forceinline__ void list_loop(const Body& body, unsigned st_base, co
       for (int u = 0; u < 2; ++u) {
         const unsigned code = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
         const typename Vec4<T>::type pj = lds_v4<T>(st_base + 2u * code);
-        const T dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-        const T r2 = dx * dx + dy * dy + dz * dz;
-        body.pair(dx, dy, dz, r2, pi.w - pj.w, true, p);
+        const PK dx = pk_sub(xi, pk_splat<T>(pj.x)), dy = pk_sub(yi, pk_splat<T>(pj.y)), dz = pk_sub(zi, pk_splat<T>(pj.z));
+        const PK r2 = pk_fma(dz, dz, pk_fma(dy, dy, pk_mul(dx, dx)));
+        body.pair2(dx, dy, dz, r2, pk_sub(wi, pk_splat<T>(pj.w)), p);
       }
     }
 #pragma unroll
-    for (int k = 0; k < NT; ++k) tot[k] += (double)p[k];
+    for (int k = 0; k < NT; ++k) { tot0[k] += (double)pk_lo(p[k]); tot1[k] += (double)pk_hi(p[k]); }
   }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a5/a6/a7: the tile force kernel over the Verlet list.
+// a5/a6/a7: the tile force kernel over the Verlet list of PAIR ROWS.
 //   MODE 0: forces (LJ or EAM pass 2) + epilogue A.epi (+ per-block energy/virial partials when EV)
 //   MODE 1: EAM pass 1 -> rho[N], fp[N] = F'(rho), packed w = -F'(rho) (+ embedding energy partial when EV)
-//   HALF (MODE 0 only, K = 1, EPI_FORCES only): each pair once, -F scattered to f[j] with fp64 atomics.
-// Thread <-> (interior slot a = list row, lane s of K).  Block size is chosen by the host so that the
+//   HALF (K = 1): each pair once, the term on j scattered with fp64 atomics (forces -F; density: the same rho term);
+//         EPI_FORCES only, the unfused integrator kernels do the time stepping.
+// Thread <-> (pair row r = interior slots 2r, 2r+1; lane s of K).  Block size is chosen by the host so that the
 // tile's rows fill whole rounds of the block.
 // Staging: the tile's cells (interior + one-cell halo) are contiguous runs of the packed array, so each
-// is ONE TMA bulk copy (cp.async.bulk, <= 125 per tile, all in flight at once, one mbarrier); a second
+// is ONE TMA bulk copy (cp.async.bulk, <= 216 per tile, all in flight at once, one mbarrier); a second
 // pass in shared memory adds each cell's offset from the tile centre (periodic image included).
 // Shared memory: TileTables | st[capA] Vec4<T> | offs[tile cells] Vec4<T> | scell[interior_cap] u16 | qcell[quads] u16 | (HALF: sgid[capA] int)
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int force_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
+constexpr int FORCE_MAX_REGS = 56;   // three 384-thread blocks (or one 1024-thread block) per SM
 
 template <typename T, class Body, int K, int MODE, bool EV, bool HALF>
-__global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 : FORCE_MIN_BLOCKS) k_tile_force(ForceArgs A) {
+__global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile_force(ForceArgs A) {
   using V4 = typename Vec4<T>::type;
+  using PK = typename Pk<T>::type;
   constexpr int NT = Body::NT;
   if (list_is_stale(A)) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1397,7 +1560,7 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
   const int tileid = blockIdx.x;
   if (threadIdx.x == 0) mbar_init(mbar, 1);
   tile_load(g, tileid, A.tab, tt);
-  const int icap = g.interior_cap;
+  const int pcap = prow_cap(g);
   const unsigned st_base = smem_addr(st);
   int n_first = 0;
   uint4 w_first = make_uint4(0, 0, 0, 0);
@@ -1414,9 +1577,9 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
     }
     // while the bulk copies fly: this thread's row length and first list word of the first round, ...
     if constexpr (!HALF) {
-      if ((int)threadIdx.x < icap * K) {
-        n_first = A.numneigh[(size_t)tileid * icap + threadIdx.x / K];
-        w_first = ld_stream(A.list + (size_t)tileid * g.chunk_cap * ((size_t)icap * K) + threadIdx.x);
+      if ((int)threadIdx.x < pcap * K) {
+        n_first = A.numneigh[(size_t)tileid * pcap + threadIdx.x / K];
+        w_first = ld_stream(A.list + (size_t)tileid * g.chunk_cap * ((size_t)pcap * K) + threadIdx.x);
       }
     }
     // ... and the quad -> tile cell map of this tile
@@ -1448,37 +1611,55 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
         }
         if constexpr (HALF) sgid[slot] = k0 + u < c ? tt.gstart[t] + k0 + u : 0;
       }
-      if (interior) *reinterpret_cast<uint2*>(scell + tt.rstart[t] + k0) = make_uint2(sc[0], sc[1]);   // indexed by list row
+      if (interior) *reinterpret_cast<uint2*>(scell + tt.rstart[t] + k0) = make_uint2(sc[0], sc[1]);   // indexed by interior slot
     }
     if (threadIdx.x == 0) st[tt.n_slots] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);   // the dummy slot
   }
   __syncthreads();
   const Body body(A.P);
   const size_t ld = A.ld;
-  const size_t slots_cap = (size_t)icap * K;
+  const size_t slots_cap = (size_t)pcap * K;
   const uint4* tlist = A.list + (size_t)tileid * g.chunk_cap * slots_cap;
   double ev[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   double d2max = 0.0;
-  const int nslots = tt.n_int_slots * K;
-  for (int base = 0; base < nslots; base += blockDim.x) {   // uniform trip count: the shuffles below need full groups
+  const int nlanes = (tt.n_int_slots >> 1) * K;
+  for (int base = 0; base < nlanes; base += blockDim.x) {   // uniform trip count: the shuffles below need full groups
     const int sidx = base + threadIdx.x;
-    const int a = sidx / K, s = sidx % K;
-    unsigned cell = 0xffffu;
-    if (sidx < nslots) cell = scell[a];
-    const bool active = cell != 0xffffu;
-    const int kin = active ? a - tt.rstart[cell] : 0;       // index of the atom within its cell
-    const int gi = active ? tt.gstart[cell] + kin : 0;
-    double tot[NT];
+    const int r = sidx / K, s = sidx % K;                   // pair row, lane of the row
+    unsigned cells = 0xffffffffu;
+    if (sidx < nlanes) cells = reinterpret_cast<const unsigned*>(scell)[r];
+    const unsigned cell = cells & 0xffffu;
+    const bool act0 = cell != 0xffffu, act1 = (cells >> 16) != 0xffffu;   // the pair's atoms (act1 implies act0)
+    const int kin = act0 ? 2 * r - tt.rstart[cell] : 0;     // index of the first atom within its cell
+    const int gi = act0 ? tt.gstart[cell] + kin : 0;        // the second atom is gi + 1
+    double tot0[NT], tot1[NT];
 #pragma unroll
-    for (int k = 0; k < NT; ++k) tot[k] = 0.0;
-    if (active) {
-      V4 pi = st[tt.start[cell] + kin];
-      pi.w = -pi.w;
-      const int n = (!HALF && base == 0) ? n_first : A.numneigh[(size_t)tileid * icap + a];
-      const int nq = (n + 7) >> 3;                          // words of this atom
+    for (int k = 0; k < NT; ++k) { tot0[k] = 0.0; tot1[k] = 0.0; }
+    if (act0) {
+      const int slot0 = tt.start[cell] + kin;
+      V4 pi0 = lds_v4_scalars<T>(st_base + (unsigned)slot0 * (unsigned)sizeof(V4));
+      V4 pi1 = lds_v4_scalars<T>(st_base + (unsigned)(slot0 + 1) * (unsigned)sizeof(V4));   // a pad slot if there is no partner: far from everything
+      if (!act1) { pi1.x = (T)-1e15; pi1.y = (T)-1e15; pi1.z = (T)-1e15; pi1.w = (T)0; }    // ... and from the dummy slot too
+      pi0.w = -pi0.w; pi1.w = -pi1.w;
+      const int n = (!HALF && base == 0) ? n_first : A.numneigh[(size_t)tileid * pcap + r];
+      const int nq = (n + 7) >> 3;                          // words of this row
+      if (act1 && s == 0) {
+        // the pair's mutual term (the two atoms are never entries of their own row)
+        PK p[NT];
+#pragma unroll
+        for (int k = 0; k < NT; ++k) p[k] = pk_splat<T>((T)0);
+        const T ex = pi0.x - pi1.x, ey = pi0.y - pi1.y, ez = pi0.z - pi1.z;
+        const T r2 = ex * ex + ey * ey + ez * ez;
+        body.pair2(pk_make(ex, -ex), pk_make(ey, -ey), pk_make(ez, -ez), pk_splat<T>(r2), pk_splat<T>(pi0.w + pi1.w), p);
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+          tot0[k] += (double)pk_lo(p[k]);
+          if (!(HALF && MODE == 0 && k >= 3)) tot1[k] += (double)pk_hi(p[k]);   // a half list counts the pair's energy and virial once
+        }
+      }
       if constexpr (!HALF) {
         if constexpr (MODE == 0) {
-          if (A.epi != EPI_FORCES) {   // the epilogue's operands: start them towards L2 now
+          if (A.epi != EPI_FORCES) {   // the epilogue's operands: start them towards L2 now (a 32-byte sector holds both atoms')
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + gi));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + ld + gi));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + 2 * ld + gi));
@@ -1493,9 +1674,9 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
           }
         }
         const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
-        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi, tot, w_first, base == 0);
+        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi0, pi1, tot0, tot1, w_first, base == 0);
       } else {
-        // half list: each in-range pair once; +F to i (registers), -F to j (atomics)
+        // half list: each in-range pair once; the term of i (registers), the term of j (atomics)
         for (int c = 0; c < nq; ++c) {
           const uint4 cur = tlist[(size_t)c * slots_cap + sidx];
           const unsigned ww[4] = {cur.x, cur.y, cur.z, cur.w};
@@ -1505,34 +1686,40 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
             for (int u = 0; u < 2; ++u) {
               const unsigned code = u ? (ww[h] >> 16) : (ww[h] & 0xffffu);
               const V4 pj = lds_v4<T>(st_base + 2u * code);
-              const T dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-              const T r2 = dx * dx + dy * dy + dz * dz;
-              T p[NT];
+              const PK dx = pk_make(pi0.x - pj.x, pi1.x - pj.x), dy = pk_make(pi0.y - pj.y, pi1.y - pj.y), dz = pk_make(pi0.z - pj.z, pi1.z - pj.z);
+              const PK r2 = pk_fma(dz, dz, pk_fma(dy, dy, pk_mul(dx, dx)));
+              PK p[NT];
 #pragma unroll
-              for (int k = 0; k < NT; ++k) p[k] = (T)0;
-              body.pair(dx, dy, dz, r2, pi.w - pj.w, true, p);
-              if (p[0] != (T)0 || p[1] != (T)0 || p[2] != (T)0) {
-                const int gj = sgid[code >> g.code_shift];
-                atomicAdd(&A.f[gj], -(double)p[0]);
-                atomicAdd(&A.f[ld + gj], -(double)p[1]);
-                atomicAdd(&A.f[2 * ld + gj], -(double)p[2]);
+              for (int k = 0; k < NT; ++k) p[k] = pk_splat<T>((T)0);
+              body.pair2(dx, dy, dz, r2, pk_make(pi0.w - pj.w, pi1.w - pj.w), p);
+              const int gj = sgid[code >> g.code_shift];
+              if constexpr (MODE == 0) {
+                const T sx = pk_lo(p[0]) + pk_hi(p[0]), sy = pk_lo(p[1]) + pk_hi(p[1]), sz = pk_lo(p[2]) + pk_hi(p[2]);
+                if (sx != (T)0 || sy != (T)0 || sz != (T)0) {
+                  atomicAdd(&A.f[gj], -(double)sx);
+                  atomicAdd(&A.f[ld + gj], -(double)sy);
+                  atomicAdd(&A.f[2 * ld + gj], -(double)sz);
+                }
+              } else {
+                const T sr = pk_lo(p[0]) + pk_hi(p[0]);     // rho is symmetric: j receives what i0 and i1 receive
+                if (sr != (T)0) atomicAdd(&A.rho[gj], (double)sr);
               }
 #pragma unroll
-              for (int k = 0; k < NT; ++k) tot[k] += (double)p[k];
+              for (int k = 0; k < NT; ++k) { tot0[k] += (double)pk_lo(p[k]); tot1[k] += (double)pk_hi(p[k]); }
             }
         }
       }
     }
     if constexpr (K > 1) {
 #pragma unroll
-      for (int k = 0; k < NT; ++k) tot[k] = group_sum<K>(tot[k]);
+      for (int k = 0; k < NT; ++k) { tot0[k] = group_sum<K>(tot0[k]); tot1[k] = group_sum<K>(tot1[k]); }
     }
-    if (active && s == 0) {
+    if (act0 && s == 0) {
       if constexpr (MODE == 0) {
         if constexpr (HALF) {
-          atomicAdd(&A.f[gi], tot[0]); atomicAdd(&A.f[ld + gi], tot[1]); atomicAdd(&A.f[2 * ld + gi], tot[2]);
+          atomicAdd(&A.f[gi], tot0[0]); atomicAdd(&A.f[ld + gi], tot0[1]); atomicAdd(&A.f[2 * ld + gi], tot0[2]);
+          if (act1) { atomicAdd(&A.f[gi + 1], tot1[0]); atomicAdd(&A.f[ld + gi + 1], tot1[1]); atomicAdd(&A.f[2 * ld + gi + 1], tot1[2]); }
         } else {
-          const double t3[3] = {tot[0], tot[1], tot[2]};
           double cc[3] = {0.0, 0.0, 0.0};
           if (A.epi == EPI_KICK_DRIFT) {
             const int m = tt.meta[cell];
@@ -1540,21 +1727,31 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
 #pragma unroll
             for (int d = 0; d < 3; ++d) cc[d] = cell_anchor_1d(g, d, tt.c0[d] + tq[d] - 1);
           }
-          d2max = fmax(d2max, atom_epilogue<T>(A, gi, t3, cc));
+          const double ta[3] = {tot0[0], tot0[1], tot0[2]}, tb[3] = {tot1[0], tot1[1], tot1[2]};
+          d2max = fmax(d2max, atom_epilogue2<T>(A, gi, act1, ta, tb, cc));
         }
         if constexpr (EV) {
           const double wgt = HALF ? 1.0 : 0.5;   // a full list visits every pair twice
 #pragma unroll
-          for (int k = 0; k < 7; ++k) ev[k] += wgt * tot[3 + k];
+          for (int k = 0; k < 7; ++k) ev[k] += wgt * (tot0[3 + k] + (act1 ? tot1[3 + k] : 0.0));
         }
       } else {
-        const double rho = tot[0];
-        const double sq = sqrt(rho);
-        const double fpv = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
-        A.rho[gi] = rho;
-        A.fp_out[gi] = fpv;
-        reinterpret_cast<T*>(const_cast<void*>(A.xr))[4 * (size_t)gi + 3] = (T)(-fpv);   // read back as pj.w by pass 2
-        if constexpr (EV) ev[0] += -A.P.B * sq;                  // embedding energy F(rho_i)
+        if constexpr (HALF) {
+          atomicAdd(&A.rho[gi], tot0[0]);
+          if (act1) atomicAdd(&A.rho[gi + 1], tot1[0]);
+        } else {
+#pragma unroll
+          for (int a = 0; a < 2; ++a) {
+            if (a == 1 && !act1) break;
+            const double rho = a ? tot1[0] : tot0[0];
+            const double sq = sqrt(rho);
+            const double fpv = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
+            A.rho[gi + a] = rho;
+            A.fp_out[gi + a] = fpv;
+            reinterpret_cast<T*>(const_cast<void*>(A.xr))[4 * (size_t)(gi + a) + 3] = (T)(-fpv);   // read back as pj.w by pass 2
+            if constexpr (EV) ev[0] += -A.P.B * sq;                  // embedding energy F(rho_i)
+          }
+        }
       }
     }
   }
@@ -1572,6 +1769,27 @@ __global__ void __launch_bounds__(FORCE_MAX_THREADS, (EV || sizeof(T) == 8) ? 1 
       if ((threadIdx.x & 31) == 0 && d2max > A.trigger) atomic_max_double_bits(&A.flags->max_disp2_bits[1 - A.parity], d2max);
     }
     if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
+  }
+}
+
+// EAM with a half list, between the two passes: rho (accumulated with atomics by pass 1) -> F'(rho), the packed
+// w = -F'(rho) that pass 2 gathers, and the embedding energy (one partial per block, added to ev_partials[.][0]).
+template <typename T>
+__global__ void __launch_bounds__(256) k_eam_embed(int N, double B, const double* __restrict__ rho, double* __restrict__ fp, T* __restrict__ xr4,
+                                                   double* __restrict__ ev_out) {
+  __shared__ double red[32];
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  double e[1] = {0.0};
+  if (n < N) {
+    const double r = rho[n], sq = sqrt(r);
+    const double fpv = r > 0.0 ? -B / (2.0 * sq) : 0.0;
+    fp[n] = fpv;
+    xr4[4 * (size_t)n + 3] = (T)(-fpv);
+    e[0] = -B * sq;
+  }
+  if (ev_out) {
+    block_sum<1>(e, red);
+    if (threadIdx.x == 0) atomicAdd(ev_out, e[0]);
   }
 }
 

@@ -26,7 +26,8 @@ KERNEL_NAMES = {0: "auto", 1: "tpa", 2: "subwarp8", 3: "warp", 4: "cell", 5: "su
 EXPORTS = [
     "md_create", "md_destroy", "md_set_units", "md_set_precision", "md_set_positions", "md_set_velocities",
     "md_set_pair", "md_set_neighbor", "md_build_neighbors", "md_compute_forces", "md_run", "md_get_positions",
-    "md_get_velocities", "md_get_forces", "md_get_neighbors", "md_autotune", "md_get_stats", "md_last_error",
+    "md_get_velocities", "md_get_forces", "md_get_neighbors", "md_get_neighbor_rows", "md_kinetic_energy", "md_autotune",
+    "md_get_stats", "md_last_error",
 ]
 
 
@@ -42,6 +43,7 @@ class md_stats(ctypes.Structure):
         ("launches_last_run", ctypes.c_int64), ("launches_total", ctypes.c_int64),
         ("ms_force_sampled", ctypes.c_double), ("nforce_sampled", ctypes.c_int64),
         ("ms_build_in_run", ctypes.c_double), ("nbuilds_in_run", ctypes.c_int64),
+        ("max_row", ctypes.c_int32), ("reserved0", ctypes.c_int32), ("mean_row", ctypes.c_double),
     ]
 
     def as_dict(self) -> dict:
@@ -83,6 +85,8 @@ def _load():
     L.md_get_velocities.argtypes = [vp, dp]
     L.md_get_forces.argtypes = [vp, dp]
     L.md_get_neighbors.argtypes = [vp, ip, ip, ctypes.c_int64]
+    L.md_get_neighbor_rows.argtypes = [vp, ip, ip, ip, ctypes.c_int64]
+    L.md_kinetic_energy.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.md_autotune.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     L.md_get_stats.argtypes = [vp, ctypes.POINTER(md_stats)]
     L.md_last_error.argtypes = [vp]
@@ -196,6 +200,15 @@ class System:
     def md_get_neighbors(self, numneigh, neigh, stride: int):
         self._ck(lib.md_get_neighbors(self._h, _addr(numneigh, np.int32, self.natoms),
                                       _addr(neigh, np.int32, self.natoms * stride), stride))
+
+    def md_get_neighbor_rows(self, row_owner, numrow, entries, stride: int):
+        self._ck(lib.md_get_neighbor_rows(self._h, _addr(row_owner, np.int32, self.natoms), _addr(numrow, np.int32, self.natoms),
+                                          _addr(entries, np.int32, self.natoms * stride), stride))
+
+    def md_kinetic_energy(self) -> float:
+        ke = ctypes.c_double(0.0)
+        self._ck(lib.md_kinetic_energy(self._h, ctypes.byref(ke)))
+        return ke.value
 
     def md_autotune(self, nrep: int = 3):
         ms = (ctypes.c_double * 4)()

@@ -86,8 +86,8 @@ def test_full_list_pair_set_matches_brute_force(cfg, n, amp, kernel):
 @pytest.mark.parametrize("precision", [0, 1])
 @pytest.mark.parametrize("kernel,list_kind", [(1, 0), (2, 0), (1, 1)])
 def test_pairs_at_the_list_radius_are_decided_in_fp64(kernel, list_kind, precision):
-    """The build's distance test runs in fp32 with a guard band; every candidate inside the band must be decided
-    in fp64.  Dimers are planted at r = rl (1 +- d) with d from 1e-5 down to 3e-9 (far inside the fp32 band,
+    """The build's distance test runs in fp32 and accepts everything up to a guard band beyond rl (the stored rows
+    are a superset); the pair set the library reports is decided in fp64.  Dimers are planted at r = rl (1 +- d) with d from 1e-5 down to 3e-9 (far inside the fp32 band,
     outside the 1e-9 exclusion of the comparison), in random orientations, all over a periodic box, so that the
     partner sits in any of the 27 stencil cells and across the periodic boundary."""
     rc, skin = 2.5, 0.3
@@ -124,6 +124,55 @@ def test_pairs_at_the_list_radius_are_decided_in_fp64(kernel, list_kind, precisi
     s.close()
 
 
+@pytest.mark.parametrize("cfg,n,amp,kernel,list_kind,precision", [
+    (1, 6, 0.15, 1, 0, 0), (2, 8, 0.15, 1, 0, 1), (1, 7, 0.15, 2, 0, 1), (4, 6, 0.2, 1, 0, 1), (1, 7, 0.15, 1, 1, 1),
+])
+def test_stored_rows_are_a_tight_superset(cfg, n, amp, kernel, list_kind, precision):
+    """What the build kernel itself writes (md_get_neighbor_rows): one row per pair of consecutive atoms of a cell,
+    holding the union of the two atoms' neighbors without the two atoms themselves.  Every row must contain all
+    fp64 neighbors of both atoms (nothing missed) and nothing beyond the fp32 guard band around rl (no junk);
+    for a half list the same with 'neighbors' = the partners the exact export assigns to the two atoms."""
+    w, x, s = _system(cfg, n, amp, precision, kernel, list_kind)
+    s.md_build_neighbors()
+    N = w.natoms
+    rl = w.rc + w.skin
+    st = s.md_get_stats()
+    stride = int(st["max_row"]) + 8
+    owner = np.zeros(N, np.int32); nrow = np.zeros(N, np.int32); ent = np.full(N * stride, -1, np.int32)
+    s.md_get_neighbor_rows(owner, nrow, ent, stride)
+    ent = ent.reshape(N, stride)
+    nn, nb = _gpu_rows(s, N, 1024 if cfg != 4 else 256)
+    exact = [set(nb[i, :nn[i]].tolist()) for i in range(N)]
+    pi, pj, _ = oracle.pairs_brute(x, w.box, rl * (1.0 + 2e-5), with_r2=True)
+    loose = [set() for _ in range(N)]
+    for a, b in zip(pi.tolist(), pj.tolist()):
+        loose[a].add(b); loose[b].add(a)
+    firsts = np.nonzero(owner == np.arange(N))[0]
+    seconds = np.nonzero(owner != np.arange(N))[0]
+    assert len(firsts) + len(seconds) == N and len(seconds) <= len(firsts)
+    assert np.all(owner[owner[seconds]] == owner[seconds]) and np.all(nrow[seconds] == 0)
+    assert len(set(owner[seconds].tolist())) == len(seconds), "an atom is the partner of two first atoms"
+    partner = {int(owner[j]): int(j) for j in seconds}
+    assert nrow[firsts].max() == st["max_row"]
+    assert nrow[firsts].sum() / (0.5 * N) == pytest.approx(st["mean_row"], rel=1e-12)
+    total_exact = 0
+    for i0 in firsts.tolist():
+        row = ent[i0, :nrow[i0]].tolist()
+        have = set(row)
+        assert len(have) == len(row), "duplicate entry in a stored row"
+        pair = {i0} | ({partner[i0]} if i0 in partner else set())
+        assert not (have & pair), "a pair's own atoms must not be entries of its row"
+        need = set().union(*(exact[a] for a in pair)) - pair
+        allow = set().union(*(loose[a] for a in pair))
+        assert need <= have <= allow
+        total_exact += sum(len(exact[a]) for a in pair)
+    assert total_exact == nn.sum()
+    # the union costs less than 1.6 single rows in these dense systems (the point of pairing spatial neighbours)
+    if list_kind == 0:
+        assert st["mean_row"] < 1.6 * st["mean_neighbors"]
+    s.close()
+
+
 def test_half_list_holds_each_pair_once():
     w, x, s = _system(1, 7, 0.15, md.MD_FP64, md.MD_KERNEL_TPA, list_kind=md.MD_LIST_HALF)
     s.md_build_neighbors()
@@ -143,8 +192,6 @@ VARIANTS = [("tpa", 1, 0), ("subwarp4", 5, 0), ("subwarp8", 2, 0), ("warp", 3, 0
 @pytest.mark.parametrize("name,kernel,list_kind", VARIANTS)
 @pytest.mark.parametrize("cfg,n,amp", [(1, 6, 0.12), (1, 9, 0.12), (4, 5, 0.25), (4, 8, 0.25)])
 def test_fp64_forces_energy_virial(cfg, n, amp, name, kernel, list_kind):
-    if cfg == 4 and list_kind == 1:
-        pytest.skip("EAM with a half list is not supported (documented)")
     w, x, s = _system(cfg, n, amp, md.MD_FP64, kernel, list_kind)
     fo, Eo, Wo, npairs, _ = oracle.forces_brute(x, w.box, w.style, w.params, w.rc)
     f = np.zeros((w.natoms, 3))
@@ -161,8 +208,6 @@ def test_fp64_forces_energy_virial(cfg, n, amp, name, kernel, list_kind):
 @pytest.mark.parametrize("name,kernel,list_kind", VARIANTS)
 @pytest.mark.parametrize("cfg,n,amp", [(2, 8, 0.12), (4, 8, 0.25)])
 def test_mixed_forces_energy_virial(cfg, n, amp, name, kernel, list_kind):
-    if cfg == 4 and list_kind == 1:
-        pytest.skip("EAM with a half list is not supported (documented)")
     w, x, s = _system(cfg, n, amp, md.MD_MIXED, kernel, list_kind)
     fo, Eo, Wo, _, _ = oracle.forces_brute(x, w.box, w.style, w.params, w.rc)
     f = np.zeros((w.natoms, 3))
@@ -315,19 +360,27 @@ def test_mixed_run_conserves_energy_and_momentum_cfg2_small():
 @pytest.mark.parametrize("kernel", [1, 5, 2, 3])
 def test_long_lived_list_is_balanced_and_stays_correct(kernel, precision):
     """A cold solid keeps its list for hundreds of steps; after 48 steps md_run permutes the rows for conflict-free
-    shared-memory gathers (a pure reordering within each row).  Forces, energy and the pair set must not change."""
+    shared-memory gathers (a pure reordering within each stored row).  Forces, energy and the stored rows (as sets)
+    must not change."""
     w = wl.make(4, n_override=6)
     s = md.from_workload(w, precision=precision, kernel=kernel)
+    N = w.natoms
+
+    def stored_rows():
+        owner = np.zeros(N, np.int32); nrow = np.zeros(N, np.int32); ent = np.full(N * 192, -1, np.int32)
+        s.md_get_neighbor_rows(owner, nrow, ent, 192)
+        return owner, nrow, ent.reshape(N, 192)
+
     s.md_run(40, w.dt)
     assert s.md_get_stats()["list_balanced"] == 0
-    nn0, nb0 = _gpu_rows(s, w.natoms, 160)
+    o0, n0, e0 = stored_rows()
     s.md_run(40, w.dt)
     st = s.md_get_stats()
     assert st["list_balanced"] == 1 and st["nbuilds"] == 1
-    nn1, nb1 = _gpu_rows(s, w.natoms, 160)
-    assert np.array_equal(nn0, nn1)
-    for i in range(w.natoms):
-        assert sorted(nb0[i, :nn0[i]].tolist()) == sorted(nb1[i, :nn1[i]].tolist())
+    o1, n1, e1 = stored_rows()
+    assert np.array_equal(o0, o1) and np.array_equal(n0, n1)
+    for i in range(N):
+        assert sorted(e0[i, :n0[i]].tolist()) == sorted(e1[i, :n1[i]].tolist())
     x, f = np.zeros((w.natoms, 3)), np.zeros((w.natoms, 3))
     s.md_get_positions(x)
     E, W = s.md_compute_forces(f, energy=True, virial=True)
