@@ -16,6 +16,7 @@
 #include <mutex>
 #include <type_traits>
 #include <string>
+#include <vector>
 
 #include "md_kernels.cuh"
 
@@ -51,11 +52,14 @@ struct md_system_impl {
   int cur = 0;    // buffer of v, id, type (flips at every build)
   int xcur = 0;   // buffer of x (flips at every build and at every fused kick+drift step)
   int force_threads = 256, batch = 8;
+  int num_sms = 148;
   bool force_timing_pending = false;
   bool list_balanced = false;
   int64_t steps_since_build = 0;
   int balance_after = 0;     // BALANCE_AFTER, or MD_B200_BALANCE_AFTER (tuning experiments)
   bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
+  int p_groups = 2;             // consumer groups of the persistent force kernel (MD_B200_PGROUPS)
+  bool no_persistent = false;   // MD_B200_NO_PERSISTENT=1: run k_tile_force where k_tile_force_p would be used (A/B measurements)
   int brick_forced = 0;   // 9 + offset: the autotuner's step away from the planner's tile shape in the candidate list (0: none)
   int shape_index = 0, shape_count = 0, build_threads = 256;
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
@@ -75,6 +79,8 @@ struct md_system_impl {
   uint4* list = nullptr;
   size_t list_words = 0;
   double* mass_d = nullptr;
+  double* dtf_d = nullptr;       // [ntypes]: dt/2 ftm2v / mass of the current md_run
+  std::vector<double> mass_h;
   double* ev_partials = nullptr;
   size_t ev_tiles_alloc = 0;
   double* scalars_d = nullptr;   // 16 doubles: [0..7] energy/virial, [8] kinetic
@@ -202,6 +208,17 @@ int build_threads(const Geom& g) {
 }
 size_t export_smem(const Geom& g) { return sizeof(TileTables) + (size_t)capA_of(g) * (2 * sizeof(int) + 2) + 16; }
 
+// The persistent, warp-specialised force kernel (k_tile_force_p) serves the mixed-precision full-list variants; it
+// needs three tile buffers in shared memory.  Everything else (fp64, energy/virial, half list) runs k_tile_force.
+constexpr size_t SMEM_OPTIN_BUDGET = 227 * 1024 - 1024;
+bool persistent_eligible(const md_system* s) {
+  return s->precision == MD_MIXED && s->list_kind == MD_LIST_FULL && s->kernel_eff != MD_KERNEL_CELL && !s->no_persistent;
+}
+int p_groups(const md_system* s) { return s->p_groups; }               // consumer groups per block (1 or 2)
+int p_nbuf(const md_system* s) { return s->p_groups + 1; }             // tile buffers: one per group + one being loaded
+int p_max_group_threads(const md_system* s) { return ((FORCE_P_MAX_THREADS - 32) / s->p_groups) / 32 * 32; }
+bool use_persistent(const md_system* s, const Geom& g) { return persistent_eligible(s) && force_p_smem(g, p_nbuf(s)) <= SMEM_OPTIN_BUDGET; }
+
 void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   double rl = s->rc + s->skin;
   g.ncell = 1;
@@ -290,11 +307,16 @@ int plan(md_system* s) {
     for (int f = 0; f < nfeas && pick < 0; ++f) {
       fill_geom_for_b(s, shapes[feasible[f]].b, g);
       if (pass < 2) {
-        if (force_smem(s, g, g.half) > smem_three) continue;
+        const bool pers = persistent_eligible(s);
+        if (pers ? force_p_smem(g, p_nbuf(s)) > SMEM_OPTIN_BUDGET : force_smem(s, g, g.half) > smem_three) continue;
         double half_extent = 0;
         for (int d = 0; d < 3; ++d) half_extent = std::max(half_extent, 0.5 * (g.b[d] + 2) * g.edge[d]);
         if (s->precision == MD_MIXED && half_extent > 9.0 * lscale && g.b[0] > 1) continue;   // fp32 tile coordinates
         if (pass == 0 && g.ntiles < 2 * 148) continue;
+        // thread-per-row: the tile's pair rows (+ 5 % for the fullest tiles) should fit ONE round of a block small
+        // enough for three resident blocks (384 threads of <= 56 registers); a second, nearly empty round costs
+        // more than the smaller tile does
+        if (g.K == 1 && 0.5 * ((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.05 > (pers ? (double)p_max_group_threads(s) : 384.0)) continue;
       }
       pick = f;
     }
@@ -306,10 +328,11 @@ int plan(md_system* s) {
   s->g = g;
   // block size of the list force kernels: the tile's pair rows should fill whole rounds of the block
   {
-    double rows = 0.5 * (((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.06 + 8.0);
+    double rows = 0.5 * ((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.05;
     double lanes = rows * g.K;
     int tmax = s->precision == MD_FP64 ? FORCE_MAX_THREADS_WIDE : FORCE_MAX_THREADS;
-    if (force_smem(s, g, g.half) <= smem_three) tmax = std::min(tmax, 384);   // three resident blocks of <= 56 registers
+    if (use_persistent(s, g)) tmax = p_max_group_threads(s);                       // threads of ONE consumer group
+    else if (force_smem(s, g, g.half) <= smem_three) tmax = std::min(tmax, 384);   // three resident blocks of <= 56 registers
     int rounds = (int)std::ceil(lanes / tmax);
     int t = (int)std::ceil(lanes / std::max(rounds, 1));
     t = ((t + 31) / 32) * 32;
@@ -517,14 +540,26 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
     if (MODE == 0) CK(cudaMemsetAsync(A.f, 0, 3 * s->ld * sizeof(double), s->stream));
     else CK(cudaMemsetAsync(A.rho, 0, s->ld * sizeof(double), s->stream));
     CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, true>, g.ntiles, threads, force_smem(s, g, true), A));
-  } else if (g.K == 1) {
-    CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
-  } else if (g.K == 4) {
-    CK(launch(s, k_tile_force<T, Body, 4, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
-  } else if (g.K == 8) {
-    CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
   } else {
-    CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
+    if constexpr (std::is_same<T, float>::value && !EV) {
+      if (use_persistent(s, g)) {
+        // persistent, warp-specialised path: one block per SM, two consumer groups of `threads` + one producer warp
+        const int ng = p_groups(s), nb = p_nbuf(s);
+        const int gth = std::min(threads, p_max_group_threads(s));
+        const unsigned grid = (unsigned)std::min(g.ntiles, s->num_sms);
+        const unsigned block = (unsigned)(ng * gth + 32);
+        const size_t sm = force_p_smem(g, nb);
+        if (g.K == 1) CK(launch(s, k_tile_force_p<Body, 1, MODE>, grid, block, sm, A, gth, ng, nb));
+        else if (g.K == 4) CK(launch(s, k_tile_force_p<Body, 4, MODE>, grid, block, sm, A, gth, ng, nb));
+        else if (g.K == 8) CK(launch(s, k_tile_force_p<Body, 8, MODE>, grid, block, sm, A, gth, ng, nb));
+        else CK(launch(s, k_tile_force_p<Body, 32, MODE>, grid, block, sm, A, gth, ng, nb));
+        return MD_OK;
+      }
+    }
+    if (g.K == 1) CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
+    else if (g.K == 4) CK(launch(s, k_tile_force<T, Body, 4, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
+    else if (g.K == 8) CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
+    else CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
   }
   return MD_OK;
 }
@@ -538,6 +573,7 @@ int launch_force_T(md_system* s, const StepMode& M) {
   A.numneigh = s->numneigh; A.fp_in = nullptr; A.f = s->f; A.rho = s->rho; A.fp_out = s->fp; A.ev_partials = s->ev_partials;
   A.epi = M.epi; A.in_run = M.in_run; A.parity = M.parity;
   A.v = s->v[s->cur]; A.x_new = s->x[xb ^ 1]; A.xr_new = s->xr[xb ^ 1]; A.x0 = s->x0; A.type = s->type[s->cur]; A.mass = s->mass_d;
+  A.dtf_type = s->dtf_d;
   A.dt = M.dt; A.half_dt_ftm2v = M.hdtf; A.trigger = M.trigger; A.flags = s->flags_d;
   if (s->style == MD_PAIR_LJ126) {
     int rc = launch_force_variant<T, LJBody, 0, EV>(s, A);
@@ -688,9 +724,15 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
     if (!(mass[t] > 0.0)) return fail(nullptr, MD_ERR_BAD_ARGUMENT, "md_create: masses must be positive");
   s = new md_system();
   if (const char* e = getenv("MD_B200_NO_BALANCE")) s->no_balance = atoi(e) != 0;
+  if (const char* e = getenv("MD_B200_NO_PERSISTENT")) s->no_persistent = atoi(e) != 0;
+  if (const char* e = getenv("MD_B200_PGROUPS")) s->p_groups = atoi(e) == 1 ? 1 : 2;
   s->balance_after = BALANCE_AFTER;
   if (const char* e = getenv("MD_B200_BALANCE_AFTER")) s->balance_after = atoi(e);
   auto bail = [&](int code) { std::string e = s->err; md_destroy(s); g_create_error = e; return code; };
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) s->num_sms = sms;
+  }
   s->N = N;
   s->ld = ((size_t)N + 31) & ~(size_t)31;
   s->stream = (cudaStream_t)cuda_stream;
@@ -712,7 +754,8 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   CKC(cudaMemsetAsync(s->f, 0, 3 * s->ld * sizeof(double), s->stream));
   CKC(dalloc(&s->cell_of, s->ld)); CKC(dalloc(&s->rank, s->ld)); CKC(dalloc(&s->perm, s->ld)); CKC(dalloc(&s->mkey, s->ld));
   CKC(dalloc(&s->nstat_d, (size_t)4));
-  CKC(dalloc(&s->mass_d, (size_t)ntypes)); CKC(dalloc(&s->scalars_d, 16)); CKC(dalloc(&s->io_d, 3 * s->ld));
+  CKC(dalloc(&s->mass_d, (size_t)ntypes)); CKC(dalloc(&s->dtf_d, (size_t)ntypes));
+  s->mass_h.assign(mass, mass + ntypes); CKC(dalloc(&s->scalars_d, 16)); CKC(dalloc(&s->io_d, 3 * s->ld));
   CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
   CKC(cudaEventCreate(&s->ev0)); CKC(cudaEventCreate(&s->ev1)); CKC(cudaEventCreate(&s->ev2)); CKC(cudaEventCreate(&s->ev3));
@@ -744,7 +787,7 @@ void md_destroy(md_system* s) {
   cudaFree(s->tab);
   cudaFree(s->f); cudaFree(s->x0); cudaFree(s->rho); cudaFree(s->fp); cudaFree(s->cell_of); cudaFree(s->rank); cudaFree(s->perm); cudaFree(s->mkey);
   cudaFree(s->nstat_d); cudaFree(s->export_buf);
-  cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d);
+  cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d); cudaFree(s->dtf_d);
   cudaFree(s->ev_partials); cudaFree(s->scalars_d); cudaFree(s->io_d); cudaFree(s->io_i); cudaFree(s->types_caller); cudaFree(s->flags_d);
   if (s->flags_h) cudaFreeHost(s->flags_h);
   if (s->scalars_h) cudaFreeHost(s->scalars_h);
@@ -868,6 +911,12 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   const int N = (int)s->N;
   const double trigger = 0.25 * s->skin * s->skin;
   const double hdtf = 0.5 * dt * s->ftm2v;
+  {   // per-type kick factor of the fused epilogue (same expression as the integrator kernels: hdtf / m)
+    std::vector<double> dtf(s->mass_h.size());
+    for (size_t t = 0; t < dtf.size(); ++t) dtf[t] = hdtf / s->mass_h[t];
+    CK(cudaMemcpyAsync(s->dtf_d, dtf.data(), dtf.size() * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    CK(cudaStreamSynchronize(s->stream));   // dtf is a stack object
+  }
   const int64_t sample_every = (nsteps + md_system_impl::NSAMPLE - 1) / md_system_impl::NSAMPLE;
   int nsampled = 0;
   s->ms_force_sampled = 0;

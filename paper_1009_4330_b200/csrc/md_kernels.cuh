@@ -276,14 +276,15 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
 // (TILE_HDR ints of header + four ints {gstart, start<<16 | cnt, meta, rstart} per tile cell); every tile kernel
 // launched between two builds only loads them (tile_load: one coalesced read, one barrier).
 // ---------------------------------------------------------------------------------------------------
-constexpr int TILE_CELL_INTS = 4;   // ints per tile cell in the table
+constexpr int TILE_CELL_INTS = 7;   // ints per tile cell in the table: gstart, start<<16|cnt, meta, rstart, and the fp32 offset
+                                    // (x, y, z) of the cell's packed coordinates from the tile centre (tile_cell_offset_rel)
 constexpr int TILE_HDR = 8;   // n_int_slots, n_slots, n_int_atoms, brick_start, n_staged_atoms, pad x3
 __host__ __device__ inline int tile_tab_cells(const Geom& g) { return ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) + 3) & ~3; }
 // after the per-cell ints: one u16 per QUAD of staged slots (cells are padded to 4 slots, so a quad belongs to
 // one tile cell) = the tile cell of that quad; lets the force kernel post-process the staged tile slot-parallel
 __host__ __device__ inline int tile_tab_quads(const Geom& g) { return (g.tile_cap >> 2) + 2; }
 __host__ __device__ inline int tile_tab_stride(const Geom& g) {
-  return TILE_HDR + TILE_CELL_INTS * tile_tab_cells(g) + ((tile_tab_quads(g) + 1) >> 1);
+  return (TILE_HDR + TILE_CELL_INTS * tile_tab_cells(g) + ((tile_tab_quads(g) + 1) >> 1) + 3) & ~3;   // a multiple of 16 bytes: one bulk copy
 }
 
 __device__ __forceinline__ void tile_dims(const Geom& g, int tile, int c0[3], int w[3]) {
@@ -334,6 +335,15 @@ __global__ void __launch_bounds__(128) k_tile_tables(Geom g, const int* __restri
     h[TILE_HDR + tcs + t] = (int)(((unsigned)tt.start[t] << 16) | ((unsigned)tt.cnt[t] & 0xffffu));
     h[TILE_HDR + 2 * tcs + t] = tx | ty << 8 | tz << 16 | (tile_cell_is_interior(tt, t) ? 1 << 24 : 0);
     h[TILE_HDR + 3 * tcs + t] = tt.rstart[t];
+    {
+      const int tq[3] = {tx, ty, tz};
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {   // the same expression as tile_cell_offset_rel
+        const int u = tt.c0[d] + tq[d] - 1;
+        const double wrap = u < 0 ? g.nc[d] * g.h[d] - g.L[d] : (u >= g.nc[d] ? g.L[d] - g.nc[d] * g.h[d] : 0.0);
+        h[TILE_HDR + (4 + d) * tcs + t] = __float_as_int((float)((2 * (u - tt.c0[d]) + 1 - tt.w[d]) * (0.5 * g.h[d]) + wrap));
+      }
+    }
     staged += tt.cnt[t];
     unsigned short* qc = reinterpret_cast<unsigned short*>(h + TILE_HDR + TILE_CELL_INTS * tcs);
     const int q0 = tt.start[t] >> 2, q1 = min((tt.start[t] + pad4(tt.cnt[t])) >> 2, tile_tab_quads(g));
@@ -1361,6 +1371,7 @@ struct ForceArgs {
   int parity;              // reads max_disp2_bits[parity], writes max_disp2_bits[1-parity]
   double* v; double* x_new; const double* x0;
   const int* type; const double* mass;
+  const double* dtf_type;  // [ntypes]: half_dt_ftm2v / mass[t] (host-prepared per md_run)
   double dt, half_dt_ftm2v, trigger;
   Flags* flags;
 };
@@ -1393,7 +1404,7 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
 #pragma unroll
     for (int d = 0; d < 3; ++d) { xx[d] = A.x[d * ld + gi]; x0v[d] = A.x0[d * ld + gi]; }
   }
-  const double dtf = A.half_dt_ftm2v / A.mass[A.type[gi]];
+  const double dtf = A.dtf_type[A.type[gi]];   // dt/2 ftm2v / m of the atom's type (a tiny table, L1-resident)
   double d2 = 0.0;
   T r[3];
 #pragma unroll
@@ -1496,13 +1507,17 @@ __device__ __forceinline__ void list_loop(const Body& body, unsigned st_base, co
   constexpr int NT = Body::NT;
   using PK = typename Pk<T>::type;
   if (nwords <= 0) return;
-  // one word in flight ahead of the one being processed: a word is 8 gathers x 2 atoms = ~250 issue slots of work
-  // for the warp, i.e. more than a DRAM round trip once the SM's other warps take their turns
+  // two words in flight ahead of the one being processed: a word is 8 gathers x 2 atoms = ~230 issue slots of work
+  // for the warp, but with only a few of the SM's warps inside this loop at a time that is less than a DRAM round
+  // trip (measured: with one word ahead, 16 % of the loop's stall samples wait for the next word)
   uint4 w = have_w0 ? w0 : ld_stream(words);
+  uint4 wn = w;
+  if (nwords > 1) wn = ld_stream(words + word_stride);
   const PK xi = pk_make_once(pi0.x, pi1.x), yi = pk_make_once(pi0.y, pi1.y), zi = pk_make_once(pi0.z, pi1.z), wi = pk_make(pi0.w, pi1.w);
   for (int c = 0; c < nwords; ++c) {
     const uint4 cur = w;
-    if (c + 1 < nwords) w = ld_stream(words + (size_t)(c + 1) * word_stride);
+    w = wn;
+    if (c + 2 < nwords) wn = ld_stream(words + (size_t)(c + 2) * word_stride);
     PK p[NT];
 #pragma unroll
     for (int k = 0; k < NT; ++k) p[k] = pk_splat<T>((T)0);
@@ -1660,6 +1675,7 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
       if constexpr (!HALF) {
         if constexpr (MODE == 0) {
           if (A.epi != EPI_FORCES) {   // the epilogue's operands: start them towards L2 now (a 32-byte sector holds both atoms')
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.type + gi));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + gi));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + ld + gi));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + 2 * ld + gi));
@@ -1673,7 +1689,11 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
             }
           }
         }
+#ifdef MDK_SKIP_LOOP   // timing experiment: everything but the list loop
+        const int mine = 0;
+#else
         const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
+#endif
         list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi0, pi1, tot0, tot1, w_first, base == 0);
       } else {
         // half list: each in-range pair once; the term of i (registers), the term of j (atomics)
@@ -1790,6 +1810,280 @@ __global__ void __launch_bounds__(256) k_eam_embed(int N, double B, const double
   if (ev_out) {
     block_sum<1>(e, red);
     if (threadIdx.x == 0) atomicAdd(ev_out, e[0]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a5/a6/a7, the mixed-precision production path: the SAME list loop, bodies and epilogue as k_tile_force, in a
+// PERSISTENT, warp-specialised kernel (one block per SM) that takes the tile prologue off the critical path.
+// Measured on B200 at cfg 5: the prologue of k_tile_force (table loads -> barrier -> ~140 small bulk copies ->
+// mbarrier wait -> offset pass -> barrier) is a chain of dependent round trips worth 0.16 ms of a 0.51 ms
+// launch, with a third of the resident warps waiting in it at any time.  Here
+//   * one PRODUCER warp walks the block's tiles ahead of the others: one bulk copy brings the tile's table
+//     (k_tile_tables: cell starts, counts, offsets, quad map) into shared memory, then one bulk copy per tile
+//     cell stages the packed coordinates, all counted on the buffer's `full` mbarrier;
+//   * two CONSUMER groups of `gthreads` threads each take the block's tiles alternately; a group waits for its
+//     buffer, adds the cell offsets in place (shared memory only), runs the list loop and the fused epilogue,
+//     and hands the buffer back through the `empty` mbarrier;
+//   * three tile buffers: two being computed on, one being loaded.
+// Tiles of a block: blockIdx.x + k gridDim.x; tile k uses buffer k % 3 and group k % 2.
+// Shared memory: mbarriers (128 B) | 3 x { table[tile_tab_stride] ints | st[capA] float4 | scell[interior_cap] u16 }.
+// ---------------------------------------------------------------------------------------------------
+constexpr int FORCE_P_MAX_NBUF = 3;               // tile buffers: ngroups being computed on + one being loaded
+constexpr int FORCE_P_MAX_REGS = 72;              // up to 896 threads per block
+constexpr int FORCE_P_MAX_THREADS = 896;          // consumer threads + one producer warp
+__host__ __device__ inline size_t force_p_buf_bytes(const Geom& g) {
+  return (size_t)tile_tab_stride(g) * 4 + (size_t)force_capA(g) * 16 + (((size_t)g.interior_cap * 2 + 15) & ~(size_t)15);
+}
+__host__ __device__ inline size_t force_p_smem(const Geom& g, int nbuf) { return 128 + (size_t)nbuf * force_p_buf_bytes(g); }
+__host__ __device__ inline int force_p_chunks(const Geom& g) { return ((g.tile_cap >> 2) + 1 + 31) >> 5; }   // chunks of 32 quads of slots
+
+__device__ __forceinline__ void mbar_arrive(unsigned mbar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar) : "memory");
+}
+__device__ __forceinline__ void group_barrier(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// the per-tile table as it lies in shared memory (k_tile_tables' layout)
+struct TileView {
+  const int* h;
+  int tcs;
+  __device__ __forceinline__ int n_int_slots() const { return h[0]; }
+  __device__ __forceinline__ int n_slots() const { return h[1]; }
+  __device__ __forceinline__ int n_staged() const { return h[4]; }
+  __device__ __forceinline__ int gstart(int t) const { return h[TILE_HDR + t]; }
+  __device__ __forceinline__ int start(int t) const { return (int)((unsigned)h[TILE_HDR + tcs + t] >> 16); }
+  __device__ __forceinline__ int cnt(int t) const { return h[TILE_HDR + tcs + t] & 0xffff; }
+  __device__ __forceinline__ int meta(int t) const { return h[TILE_HDR + 2 * tcs + t]; }
+  __device__ __forceinline__ int rstart(int t) const { return h[TILE_HDR + 3 * tcs + t]; }
+  __device__ __forceinline__ float off(int d, int t) const { return __int_as_float(h[TILE_HDR + (4 + d) * tcs + t]); }
+  __device__ __forceinline__ const unsigned short* qc() const { return reinterpret_cast<const unsigned short*>(h + TILE_HDR + TILE_CELL_INTS * tcs); }
+};
+
+template <class Body, int K, int MODE>
+__global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gthreads, int NG, int NB) {
+  using T = float;
+  using V4 = float4;
+  constexpr int NT = Body::NT;
+  if (list_is_stale(A)) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const Geom& g = A.g;
+  const int capA = force_capA(g), tcs = tile_tab_cells(g), tab_ints = tile_tab_stride(g);
+  const unsigned buf_bytes = (unsigned)force_p_buf_bytes(g);
+  const unsigned smem0 = smem_addr(smem_raw);
+  // per buffer: `tabfull` (the table has landed), `full` (the coordinates have landed), `ready` (the cell offsets
+  // have been added: the list loop may start), `empty` (the consumers are done: the producer may refill), and a
+  // work counter `ctr` for the post-processing chunks
+  constexpr int MB = FORCE_P_MAX_NBUF;
+  auto full = [&](int b) { return smem0 + 8u * (unsigned)b; };
+  auto tabfull = [&](int b) { return smem0 + 8u * (unsigned)(MB + b); };
+  auto empty = [&](int b) { return smem0 + 8u * (unsigned)(2 * MB + b); };
+  auto ready = [&](int b) { return smem0 + 8u * (unsigned)(3 * MB + b); };
+  int* ctr = reinterpret_cast<int*>(smem_raw + 8 * 4 * MB);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int gwarps = gthreads >> 5;
+  const int nchunks = force_p_chunks(g);
+  if (threadIdx.x == 0) {
+    for (int b = 0; b < NB; ++b) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(full(b)), "r"(1) : "memory");
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tabfull(b)), "r"(1) : "memory");
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(empty(b)), "r"(gwarps) : "memory");
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(ready(b)), "r"(nchunks) : "memory");
+      ctr[b] = 0;
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int ntl = ((int)g.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this block
+  const int pcap = prow_cap(g);
+
+  if (wid >= NG * gwarps) {
+    // ---------------- producer warp: walks ALL tiles of the block in order ----------------
+    if (wid > NG * gwarps) return;
+    const V4* __restrict__ xr = reinterpret_cast<const V4*>(A.xr);
+    for (int k = 0; k < ntl; ++k) {
+      const int b = k % NB, j = k / NB;
+      const int tile = (int)blockIdx.x + k * (int)gridDim.x;
+      unsigned char* bufp = smem_raw + 128 + (size_t)b * buf_bytes;
+      const unsigned buf = smem0 + 128u + (unsigned)b * buf_bytes;
+      TileView tv{reinterpret_cast<const int*>(bufp), tcs};
+      if (j > 0) mbar_wait(empty(b), (unsigned)((j - 1) & 1));
+      if (lane == 0) {
+        ctr[b] = 0;
+        mbar_expect_tx(tabfull(b), (unsigned)tab_ints * 4u);
+        bulk_g2s(buf, A.tab + (size_t)tile * tab_ints, (unsigned)tab_ints * 4u, tabfull(b));
+      }
+      mbar_wait(tabfull(b), (unsigned)(j & 1));
+      int c0[3], w[3];
+      tile_dims(g, tile, c0, w);
+      const int ntc = (w[0] + 2) * (w[1] + 2) * (w[2] + 2);
+      if (lane == 0) mbar_expect_tx(full(b), (unsigned)tv.n_staged() * 16u);
+      __syncwarp();
+      const unsigned st_a = buf + (unsigned)tab_ints * 4u;
+      for (int t = lane; t < ntc; t += 32) {
+        const int c = tv.cnt(t);
+        if (c > 0) bulk_g2s(st_a + (unsigned)tv.start(t) * 16u, xr + tv.gstart(t), (unsigned)c * 16u, full(b));
+      }
+    }
+    return;
+  }
+
+  // ---------------- consumer groups ----------------
+  const int grp = wid / gwarps, gt = (int)threadIdx.x - grp * gthreads;
+  const Body body(A.P);
+  const size_t ld = A.ld;
+  const size_t slots_cap = (size_t)pcap * K;
+  double d2max = 0.0;
+  for (int k = grp; k < ntl; k += NG) {
+    const int b = k % NB, j = k / NB;
+    const int tile = (int)blockIdx.x + k * (int)gridDim.x;
+    const uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
+    // while the tile lands: this thread's row length and first list word of the first round
+    int n_first = 0;
+    uint4 w_first = make_uint4(0, 0, 0, 0);
+    if (gt < pcap * K) {
+      n_first = A.numneigh[(size_t)tile * pcap + gt / K];
+      w_first = ld_stream(tlist + gt);
+    }
+    unsigned char* bufp = smem_raw + 128 + (size_t)b * buf_bytes;
+    TileView tv{reinterpret_cast<const int*>(bufp), tcs};
+    V4* st = reinterpret_cast<V4*>(bufp + (size_t)tab_ints * 4);
+    unsigned short* scell = reinterpret_cast<unsigned short*>(st + capA);
+    const unsigned st_base = smem_addr(st);
+    mbar_wait(tabfull(b), (unsigned)(j & 1));
+    mbar_wait(full(b), (unsigned)(j & 1));
+    {
+      // offsets, pad slots, slot -> cell map, in chunks of 32 quads of slots dealt to whichever warps of the group
+      // get here first (the warps of a group finish their previous tile at different times: no group barrier)
+      const int nq = tv.n_slots() >> 2;
+      const unsigned short* qc = tv.qc();
+      for (;;) {
+        int ch = 0;
+        if (lane == 0) ch = atomicAdd(&ctr[b], 1);
+        ch = __shfl_sync(0xffffffffu, ch, 0);
+        if (ch >= nchunks) break;
+        const int q = ch * 32 + lane;
+        if (q < nq) {
+          const int t = qc[q];
+          const int c = tv.cnt(t), k0 = 4 * q - tv.start(t);
+          const float ox = tv.off(0, t), oy = tv.off(1, t), oz = tv.off(2, t);
+          const bool interior = (tv.meta(t) >> 24) != 0;
+          unsigned sc[2] = {0xffffffffu, 0xffffffffu};
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int slot = 4 * q + u;
+            if (k0 + u < c) {
+              V4 v = st[slot];
+              v.x += ox; v.y += oy; v.z += oz;
+              st[slot] = v;
+              sc[u >> 1] = (u & 1) ? ((sc[u >> 1] & 0xffffu) | ((unsigned)t << 16)) : ((sc[u >> 1] & 0xffff0000u) | (unsigned)t);
+            } else {
+              st[slot] = make_float4(1e15f, 1e15f, 1e15f, 0.f);
+            }
+          }
+          if (interior) *reinterpret_cast<uint2*>(scell + tv.rstart(t) + k0) = make_uint2(sc[0], sc[1]);   // indexed by interior slot
+        } else if (q == nq) {
+          st[tv.n_slots()] = make_float4(1e15f, 1e15f, 1e15f, 0.f);   // the dummy slot
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(ready(b));   // release: the waits below acquire the chunk
+      }
+    }
+    mbar_wait(ready(b), (unsigned)(j & 1));
+    int c0[3], wdt[3];
+    tile_dims(g, tile, c0, wdt);
+    const int nlanes = (tv.n_int_slots() >> 1) * K;
+    for (int base = 0; base < nlanes; base += gthreads) {   // uniform trip count: the shuffles below need full groups
+      const int sidx = base + gt;
+      const int r = sidx / K, s = sidx % K;                   // pair row, lane of the row
+      unsigned cells = 0xffffffffu;
+      if (sidx < nlanes) cells = reinterpret_cast<const unsigned*>(scell)[r];
+      const unsigned cell = cells & 0xffffu;
+      const bool act0 = cell != 0xffffu, act1 = (cells >> 16) != 0xffffu;   // the pair's atoms (act1 implies act0)
+      const int kin = act0 ? 2 * r - tv.rstart(cell) : 0;     // index of the first atom within its cell
+      const int gi = act0 ? tv.gstart(cell) + kin : 0;        // the second atom is gi + 1
+      double tot0[NT], tot1[NT];
+#pragma unroll
+      for (int q = 0; q < NT; ++q) { tot0[q] = 0.0; tot1[q] = 0.0; }
+      if (act0) {
+        const int slot0 = tv.start(cell) + kin;
+        V4 pi0 = lds_v4_scalars<T>(st_base + (unsigned)slot0 * 16u);
+        V4 pi1 = lds_v4_scalars<T>(st_base + (unsigned)(slot0 + 1) * 16u);   // a pad slot if there is no partner
+        if (!act1) { pi1.x = -1e15f; pi1.y = -1e15f; pi1.z = -1e15f; pi1.w = 0.f; }
+        pi0.w = -pi0.w; pi1.w = -pi1.w;
+        const int n = base == 0 ? n_first : A.numneigh[(size_t)tile * pcap + r];
+        const int nq = (n + 7) >> 3;                          // words of this row
+        if (act1 && s == 0) {
+          // the pair's mutual term (the two atoms are never entries of their own row)
+          typename Pk<T>::type p[NT];
+#pragma unroll
+          for (int q = 0; q < NT; ++q) p[q] = pk_splat<T>(0.f);
+          const T ex = pi0.x - pi1.x, ey = pi0.y - pi1.y, ez = pi0.z - pi1.z;
+          const T r2 = ex * ex + ey * ey + ez * ez;
+          body.pair2(pk_make(ex, -ex), pk_make(ey, -ey), pk_make(ez, -ez), pk_splat<T>(r2), pk_splat<T>(pi0.w + pi1.w), p);
+#pragma unroll
+          for (int q = 0; q < NT; ++q) { tot0[q] += (double)pk_lo(p[q]); tot1[q] += (double)pk_hi(p[q]); }
+        }
+        if constexpr (MODE == 0) {
+          if (A.epi != EPI_FORCES) {   // the epilogue's operands: start them towards L2 now (a 32-byte sector holds both atoms')
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.type + gi));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + gi));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + ld + gi));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.v + 2 * ld + gi));
+            if (A.epi == EPI_KICK_DRIFT) {
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x + ld + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x + 2 * ld + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x0 + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x0 + ld + gi));
+              asm volatile("prefetch.global.L2 [%0];" ::"l"(A.x0 + 2 * ld + gi));
+            }
+          }
+        }
+        const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
+        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi0, pi1, tot0, tot1, w_first, base == 0);
+      }
+      if constexpr (K > 1) {
+#pragma unroll
+        for (int q = 0; q < NT; ++q) { tot0[q] = group_sum<K>(tot0[q]); tot1[q] = group_sum<K>(tot1[q]); }
+      }
+      if (act0 && s == 0) {
+        if constexpr (MODE == 0) {
+          double cc[3] = {0.0, 0.0, 0.0};
+          if (A.epi == EPI_KICK_DRIFT) {
+            const int m = tv.meta(cell);
+            const int tq[3] = {m & 0xff, (m >> 8) & 0xff, (m >> 16) & 0xff};
+#pragma unroll
+            for (int d = 0; d < 3; ++d) cc[d] = cell_anchor_1d(g, d, c0[d] + tq[d] - 1);
+          }
+          const double ta[3] = {tot0[0], tot0[1], tot0[2]}, tb[3] = {tot1[0], tot1[1], tot1[2]};
+          d2max = fmax(d2max, atom_epilogue2<T>(A, gi, act1, ta, tb, cc));
+        } else {
+#pragma unroll
+          for (int a = 0; a < 2; ++a) {
+            if (a == 1 && !act1) break;
+            const double rho = a ? tot1[0] : tot0[0];
+            const double sq = sqrt(rho);
+            const double fpv = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
+            A.rho[gi + a] = rho;
+            A.fp_out[gi + a] = fpv;
+            reinterpret_cast<T*>(const_cast<void*>(A.xr))[4 * (size_t)(gi + a) + 3] = (T)(-fpv);   // read back as pj.w by pass 2
+          }
+        }
+      }
+    }
+    // the group is done with this buffer: hand it back to the producer (its next writes are bulk copies)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty(b));
+  }
+  if constexpr (MODE == 0) {
+    if (A.epi == EPI_KICK_DRIFT) {   // a4: device-side max-displacement reduction (see k_tile_force)
+      for (int o = 16; o > 0; o >>= 1) d2max = fmax(d2max, __shfl_xor_sync(0xffffffffu, d2max, o));
+      if (lane == 0 && d2max > A.trigger) atomic_max_double_bits(&A.flags->max_disp2_bits[1 - A.parity], d2max);
+    }
+    if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
   }
 }
 
