@@ -244,7 +244,7 @@ def run_ours(args, rk) -> None:
     stream = torch.cuda.Stream()
     hbm_gbs, peak_src = measured_peaks()
     kernel = {"auto": md.MD_KERNEL_AUTO, "tpa": md.MD_KERNEL_TPA, "subwarp8": md.MD_KERNEL_SUBWARP, "warp": md.MD_KERNEL_WARP,
-              "cell": md.MD_KERNEL_CELL, "subwarp4": md.MD_KERNEL_SUBWARP4}[args.kernel]
+              "cell": md.MD_KERNEL_CELL, "subwarp4": md.MD_KERNEL_SUBWARP4, "subwarp2": md.MD_KERNEL_SUBWARP2}[args.kernel]
     list_kind = md.MD_LIST_HALF if args.half else md.MD_LIST_FULL
 
     w = wl.make(args.cfg, seed_offset=mdist.replica_seed_offset(rk))
@@ -386,7 +386,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--cfg", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "tpa", "subwarp4", "subwarp8", "warp", "cell"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "tpa", "subwarp2", "subwarp4", "subwarp8", "warp", "cell"])
     ap.add_argument("--half", action="store_true", help="half list (Newton's third law, atomics); TPA only")
     ap.add_argument("--all-configs", dest="all_configs", action="store_true", default=True)
     ap.add_argument("--no-all-configs", dest="all_configs", action="store_false")

@@ -68,12 +68,13 @@ typedef struct md_system md_system; /* opaque */
 #define MD_LIST_HALF 1    /* each pair once; -F scattered to j with atomics (Newton's third law, L76) */
 
 /* force-kernel variants */
-#define MD_KERNEL_AUTO 0     /* setup-time mini benchmark picks among TPA / SUBWARP4 / SUBWARP / WARP (L137) */
+#define MD_KERNEL_AUTO 0     /* setup-time mini benchmark picks among TPA / SUBWARP2 / SUBWARP4 / SUBWARP / WARP (L137) */
 #define MD_KERNEL_TPA 1      /* one thread per atom (L88-104) */
 #define MD_KERNEL_SUBWARP 2  /* 8 lanes per atom, shuffle reduction */
 #define MD_KERNEL_WARP 3     /* 32 lanes per atom, shuffle reduction (the paper's BpA, L105-122) */
 #define MD_KERNEL_CELL 4     /* no list: every atom scans the 27-cell stencil of its tile (L64-82) */
 #define MD_KERNEL_SUBWARP4 5 /* 4 lanes per atom, shuffle reduction: fills the SM when a tile holds few atoms with long rows */
+#define MD_KERNEL_SUBWARP2 6 /* 2 lanes per list row, shuffle reduction */
 
 typedef struct md_stats {
   int64_t natoms;
@@ -174,11 +175,11 @@ int md_get_neighbor_rows(md_system* s, int32_t* row_owner, int32_t* numrow, int3
 int md_kinetic_energy(md_system* s, double* ke_out);
 
 /* Setup-time mini benchmark of PAPER.md L137: on the current positions, builds the list and times nrep
- * force evaluations with each of TPA, SUBWARP, WARP and SUBWARP4, at the planner's tile width and its two
+ * force evaluations with each of TPA, SUBWARP, WARP, SUBWARP4 and SUBWARP2, at the planner's tile width and its two
  * neighbours; keeps the combination with the lowest (force evaluation + 1/8 list build) time, and
  * reports the best force time of each variant (ms per evaluation, in the order TPA, SUBWARP, WARP,
- * SUBWARP4) if ms_out is not NULL.  MD_KERNEL_AUTO runs it once before the first build. */
-int md_autotune(md_system* s, int nrep, double ms_out[4]);
+ * SUBWARP4, SUBWARP2) if ms_out is not NULL.  MD_KERNEL_AUTO runs it once before the first build. */
+int md_autotune(md_system* s, int nrep, double ms_out[5]);
 
 int md_get_stats(md_system* s, md_stats* out);
 const char* md_last_error(const md_system* s); /* s may be NULL: error of a failed md_create */

@@ -58,6 +58,7 @@ struct md_system_impl {
   int64_t steps_since_build = 0;
   int balance_after = 0;     // BALANCE_AFTER, or MD_B200_BALANCE_AFTER (tuning experiments)
   bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
+  int p_min_tiles_per_sm = 8;   // k_tile_force_p is used from this many tiles per SM on (MD_B200_PMIN)
   int p_groups = 2;             // consumer groups of the persistent force kernel (MD_B200_PGROUPS)
   bool no_persistent = false;   // MD_B200_NO_PERSISTENT=1: run k_tile_force where k_tile_force_p would be used (A/B measurements)
   int brick_forced = 0;   // 9 + offset: the autotuner's step away from the planner's tile shape in the candidate list (0: none)
@@ -183,7 +184,9 @@ bool is_device_ptr(const void* p) {
 template <class T>
 cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T)); }
 
-int lanes_for(int kernel) { return kernel == MD_KERNEL_SUBWARP ? 8 : (kernel == MD_KERNEL_WARP ? 32 : (kernel == MD_KERNEL_SUBWARP4 ? 4 : 1)); }
+int lanes_for(int kernel) {
+  return kernel == MD_KERNEL_SUBWARP ? 8 : (kernel == MD_KERNEL_WARP ? 32 : (kernel == MD_KERNEL_SUBWARP4 ? 4 : (kernel == MD_KERNEL_SUBWARP2 ? 2 : 1)));
+}
 
 // ---- planning: cell grid, tile width, capacities -----------------------------------------------------
 size_t elem_size(const md_system* s) { return s->precision == MD_FP64 ? sizeof(double) : sizeof(float); }
@@ -216,8 +219,12 @@ bool persistent_eligible(const md_system* s) {
 }
 int p_groups(const md_system* s) { return s->p_groups; }               // consumer groups per block (1 or 2)
 int p_nbuf(const md_system* s) { return s->p_groups + 1; }             // tile buffers: one per group + one being loaded
-int p_max_group_threads(const md_system* s) { return ((FORCE_P_MAX_THREADS - 32) / s->p_groups) / 32 * 32; }
-bool use_persistent(const md_system* s, const Geom& g) { return persistent_eligible(s) && force_p_smem(g, p_nbuf(s)) <= SMEM_OPTIN_BUDGET; }
+int p_max_group_threads(const md_system* s) { return ((FORCE_P_MAX_THREADS - 32 * FORCE_P_NPROD) / s->p_groups) / 32 * 32; }
+// ... and enough tiles per SM for the producer to run ahead (with a few tiles per block the static tile assignment
+// quantises badly: 2 or 3 tiles per block at 256,000 atoms)
+bool use_persistent(const md_system* s, const Geom& g) {
+  return persistent_eligible(s) && g.ntiles >= s->p_min_tiles_per_sm * s->num_sms && force_p_smem(g, p_nbuf(s)) <= SMEM_OPTIN_BUDGET;
+}
 
 void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   double rl = s->rc + s->skin;
@@ -242,7 +249,7 @@ void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   g.ntiles = g.nb[0] * g.nb[1] * g.nb[2];
   double per_cell = (double)s->N / g.ncell + 1.5;   // cells are padded to multiples of 4 slots
   double staged = per_cell * (g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2);
-  double interior = per_cell * g.b[0] * g.b[1] * g.b[2];
+  double interior = (per_cell - 1.0) * g.b[0] * g.b[1] * g.b[2];   // list rows: cells padded to multiples of 2
   // slack over the mean: five standard deviations of a Poisson count (a liquid fluctuates less), i.e. 7 % for the
   // ~5000 staged atoms of an rc = 5 sigma tile and 9 % at cfg 5, where a flat 20 % would cost a resident block;
   // an overflow is detected by the kernels and re-planned with a larger factor
@@ -307,7 +314,7 @@ int plan(md_system* s) {
     for (int f = 0; f < nfeas && pick < 0; ++f) {
       fill_geom_for_b(s, shapes[feasible[f]].b, g);
       if (pass < 2) {
-        const bool pers = persistent_eligible(s);
+        const bool pers = persistent_eligible(s) && g.ntiles >= s->p_min_tiles_per_sm * s->num_sms;
         if (pers ? force_p_smem(g, p_nbuf(s)) > SMEM_OPTIN_BUDGET : force_smem(s, g, g.half) > smem_three) continue;
         double half_extent = 0;
         for (int d = 0; d < 3; ++d) half_extent = std::max(half_extent, 0.5 * (g.b[d] + 2) * g.edge[d]);
@@ -316,7 +323,7 @@ int plan(md_system* s) {
         // thread-per-row: the tile's pair rows (+ 5 % for the fullest tiles) should fit ONE round of a block small
         // enough for three resident blocks (384 threads of <= 56 registers); a second, nearly empty round costs
         // more than the smaller tile does
-        if (g.K == 1 && 0.5 * ((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.05 > (pers ? (double)p_max_group_threads(s) : 384.0)) continue;
+        if (g.K == 1 && 0.5 * ((double)s->N / g.ncell + 0.5) * g.b[0] * g.b[1] * g.b[2] * 1.05 > (pers ? (double)p_max_group_threads(s) : 384.0)) continue;
       }
       pick = f;
     }
@@ -328,7 +335,7 @@ int plan(md_system* s) {
   s->g = g;
   // block size of the list force kernels: the tile's pair rows should fill whole rounds of the block
   {
-    double rows = 0.5 * ((double)s->N / g.ncell + 1.5) * g.b[0] * g.b[1] * g.b[2] * 1.05;
+    double rows = 0.5 * ((double)s->N / g.ncell + 0.5) * g.b[0] * g.b[1] * g.b[2] * 1.05;
     double lanes = rows * g.K;
     int tmax = s->precision == MD_FP64 ? FORCE_MAX_THREADS_WIDE : FORCE_MAX_THREADS;
     if (use_persistent(s, g)) tmax = p_max_group_threads(s);                       // threads of ONE consumer group
@@ -414,6 +421,9 @@ int build_list_only(md_system* s) {
   } else if (g.K == 1) {
     if (s4) CK(launch(s, k_build_list<false, 0, 4>, g.ntiles, bt, sm, B));
     else CK(launch(s, k_build_list<false, 0, 3>, g.ntiles, bt, sm, B));
+  } else if (g.K == 2) {
+    if (s4) CK(launch(s, k_build_list<false, 1, 4>, g.ntiles, bt, sm, B));
+    else CK(launch(s, k_build_list<false, 1, 3>, g.ntiles, bt, sm, B));
   } else if (g.K == 4) {
     if (s4) CK(launch(s, k_build_list<false, 2, 4>, g.ntiles, bt, sm, B));
     else CK(launch(s, k_build_list<false, 2, 3>, g.ntiles, bt, sm, B));
@@ -443,6 +453,7 @@ int balance_rows(md_system* s) {
   if (threads >= 32) {
     const size_t bsm = (size_t)threads * R.row_bytes;
     if (g.K == 1) CK(launch(s, k_balance_rows<0>, g.ntiles, threads, bsm, R));
+    else if (g.K == 2) CK(launch(s, k_balance_rows<1>, g.ntiles, threads, bsm, R));
     else if (g.K == 4) CK(launch(s, k_balance_rows<2>, g.ntiles, threads, bsm, R));
     else if (g.K == 8) CK(launch(s, k_balance_rows<3>, g.ntiles, threads, bsm, R));
     else CK(launch(s, k_balance_rows<5>, g.ntiles, threads, bsm, R));
@@ -547,9 +558,10 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
         const int ng = p_groups(s), nb = p_nbuf(s);
         const int gth = std::min(threads, p_max_group_threads(s));
         const unsigned grid = (unsigned)std::min(g.ntiles, s->num_sms);
-        const unsigned block = (unsigned)(ng * gth + 32);
+        const unsigned block = (unsigned)(ng * gth + 32 * FORCE_P_NPROD);
         const size_t sm = force_p_smem(g, nb);
         if (g.K == 1) CK(launch(s, k_tile_force_p<Body, 1, MODE>, grid, block, sm, A, gth, ng, nb));
+        else if (g.K == 2) CK(launch(s, k_tile_force_p<Body, 2, MODE>, grid, block, sm, A, gth, ng, nb));
         else if (g.K == 4) CK(launch(s, k_tile_force_p<Body, 4, MODE>, grid, block, sm, A, gth, ng, nb));
         else if (g.K == 8) CK(launch(s, k_tile_force_p<Body, 8, MODE>, grid, block, sm, A, gth, ng, nb));
         else CK(launch(s, k_tile_force_p<Body, 32, MODE>, grid, block, sm, A, gth, ng, nb));
@@ -557,6 +569,7 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
       }
     }
     if (g.K == 1) CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
+    else if (g.K == 2) CK(launch(s, k_tile_force<T, Body, 2, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
     else if (g.K == 4) CK(launch(s, k_tile_force<T, Body, 4, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
     else if (g.K == 8) CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
     else CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
@@ -635,7 +648,7 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   // The setup-time mini benchmark of PAPER.md L137, over lanes per atom (1, 8, 32) and, because the best tile
   // width depends on how many tiles the box yields, over the planner's width and its two neighbours.  Score of a
   // candidate: one force evaluation plus an eighth of a list build (a typical rebuild interval).
-  const int cand[4] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_SUBWARP4};
+  const int cand[5] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2};
   s->force_timing_pending = false;   // ev0 / ev1 are reused below
   s->brick_forced = 0;
   s->kernel_eff = MD_KERNEL_TPA;
@@ -644,14 +657,14 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   if (rc) return rc;
   double best_score = 1e300;
   int best = MD_KERNEL_TPA, best_b = 0;
-  if (ms_out) for (int k = 0; k < 4; ++k) ms_out[k] = 1e300;
+  if (ms_out) for (int k = 0; k < 5; ++k) ms_out[k] = 1e300;
   // with thousands of tiles the planner's pick is right and the SMs are full either way; the tile shape matters when
   // the box yields few tiles: then its neighbours in the candidate list (two larger, two smaller) are timed too
   const bool sweep = s->g.ntiles < 2048;
   const int i0 = s->shape_index, nfeas = s->shape_count;
   for (int off = sweep ? -2 : 0; off <= (sweep ? 2 : 0); ++off) {
     if (i0 + off < 0 || i0 + off >= nfeas) continue;
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < 5; ++k) {
       s->kernel_eff = cand[k];
       s->brick_forced = off == 0 ? 0 : 9 + off;
       s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;   // an overflow of one shape must not inflate the next
@@ -726,6 +739,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   if (const char* e = getenv("MD_B200_NO_BALANCE")) s->no_balance = atoi(e) != 0;
   if (const char* e = getenv("MD_B200_NO_PERSISTENT")) s->no_persistent = atoi(e) != 0;
   if (const char* e = getenv("MD_B200_PGROUPS")) s->p_groups = atoi(e) == 1 ? 1 : 2;
+  if (const char* e = getenv("MD_B200_PMIN")) s->p_min_tiles_per_sm = std::max(0, atoi(e));
   s->balance_after = BALANCE_AFTER;
   if (const char* e = getenv("MD_B200_BALANCE_AFTER")) s->balance_after = atoi(e);
   auto bail = [&](int code) { std::string e = s->err; md_destroy(s); g_create_error = e; return code; };
@@ -848,7 +862,7 @@ int md_set_pair(md_system* s, int style, const double* params, int nparams, doub
 int md_set_neighbor(md_system* s, int list_kind, int kernel) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (list_kind != MD_LIST_FULL && list_kind != MD_LIST_HALF) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown list kind");
-  if (kernel < MD_KERNEL_AUTO || kernel > MD_KERNEL_SUBWARP4) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown kernel");
+  if (kernel < MD_KERNEL_AUTO || kernel > MD_KERNEL_SUBWARP2) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown kernel");
   if (list_kind == MD_LIST_HALF && !(kernel == MD_KERNEL_TPA || kernel == MD_KERNEL_AUTO))
     return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: a half list needs MD_KERNEL_TPA");
   s->list_kind = list_kind;
@@ -868,7 +882,7 @@ int md_build_neighbors(md_system* s) {
   return build(s, false);
 }
 
-int md_autotune(md_system* s, int nrep, double ms_out[4]) {
+int md_autotune(md_system* s, int nrep, double ms_out[5]) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   return autotune(s, nrep, ms_out);
 }

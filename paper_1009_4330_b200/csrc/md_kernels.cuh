@@ -185,7 +185,8 @@ __device__ __forceinline__ void block_max_to_flag(double v, double* red, unsigne
 // Staged slot order: the tile's cells (interior + halo) in tile scan order, x fastest; every cell is padded to a
 // multiple of 4 slots (pad slots hold a far-away point), so that a cell's coordinates can be read four at a time
 // with aligned 128-bit loads, and the three x-neighbours of a stencil row are ONE contiguous run of slots.
-// List rows number the interior atoms only (same cell order, same padding): row = rstart[t] + k for atom k of
+// List rows number the interior atoms only (same cell order, every cell padded to a multiple of 2: a list row
+// belongs to a PAIR of atoms): interior slot = rstart[t] + k, pair row = (rstart[t] + k) / 2 for atom k of
 // interior tile cell t, whose staged slot is start[t] + k.
 // ---------------------------------------------------------------------------------------------------
 struct alignas(16) TileTables {   // lives in shared memory
@@ -193,7 +194,7 @@ struct alignas(16) TileTables {   // lives in shared memory
   int gstart[MAX_TILE_CELLS]; // global (sorted) index of the first atom of tile cell t
   int cnt[MAX_TILE_CELLS];    // atoms in tile cell t
   int meta[MAX_TILE_CELLS];   // tx | ty << 8 | tz << 16 | interior << 24   (filled by tile_load only)
-  int rstart[MAX_TILE_CELLS]; // interior cells: list row of the cell's first atom (multiple of 4); rows number the
+  int rstart[MAX_TILE_CELLS]; // interior cells: interior slot of the cell's first atom (multiple of 2); rows number the
                               // interior atoms only, in the same cell order
   int c0[3], w[3], tc[3];     // first interior cell, interior width, tile width (w+2)
   int ntc;                    // tc[0]*tc[1]*tc[2]
@@ -205,6 +206,7 @@ struct alignas(16) TileTables {   // lives in shared memory
 };
 
 __device__ __forceinline__ int pad4(int c) { return (c + 3) & ~3; }
+__device__ __forceinline__ int pad2(int c) { return (c + 1) & ~1; }
 __device__ __forceinline__ int interior_tile_cell(const TileTables& tt, int ic) {
   int lx = ic % tt.w[0], ly = (ic / tt.w[0]) % tt.w[1], lz = ic / (tt.w[0] * tt.w[1]);
   return ((lz + 1) * tt.tc[1] + (ly + 1)) * tt.tc[0] + (lx + 1);
@@ -251,7 +253,7 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
     for (int t = lo; t < hi; ++t) {
       const int c4 = pad4(tt.cnt[t]);
       sum += c4;
-      if (tile_cell_is_interior(tt, t)) isum += c4;
+      if (tile_cell_is_interior(tt, t)) isum += pad2(tt.cnt[t]);
     }
     int incl = sum, iincl = isum;
 #pragma unroll
@@ -264,7 +266,7 @@ __device__ inline void tile_setup(const Geom& g, int tile, const int* __restrict
       const int c4 = pad4(tt.cnt[t]);
       tt.start[t] = run;
       run += c4;
-      if (tile_cell_is_interior(tt, t)) { tt.rstart[t] = irun; irun += c4; } else tt.rstart[t] = 0;
+      if (tile_cell_is_interior(tt, t)) { tt.rstart[t] = irun; irun += pad2(tt.cnt[t]); } else tt.rstart[t] = 0;
     }
     if (tid == 31) { tt.n_int_slots = iincl; tt.n_slots = incl; }
   }
@@ -647,8 +649,7 @@ __global__ void k_iota(int N, int* __restrict__ a) {
 // set of an atom (north_star (2)) is the row's entries that pass |x_i - x_j|^2 < rl^2 in fp64 from the global
 // positions: md_get_neighbors (k_export_list) returns exactly that, md_get_neighbor_rows returns the raw rows.
 //
-// One LANE per pair row; a task = 32 consecutive pair rows (16 quads of slots).  Rows are padded per cell to
-// multiples of 4 slots, so a quad belongs to one cell, but the quads of a task may belong to different cells:
+// One LANE per pair row; a task = 32 consecutive pair rows, which may belong to different cells:
 // the lanes of a warp then walk different candidate runs of about the same length, in lockstep (ragged pieces
 // read a far-away dummy quad).  Four candidates per 128-bit broadcast load from SoA shared memory; accepted slot
 // codes go to a small per-lane ring in shared memory (one predicated 16-bit store + pointer add each) and
@@ -672,7 +673,7 @@ struct BuildArgs {
 
 __host__ __device__ inline int prow_cap(const Geom& g) { return g.interior_cap >> 1; }   // pair rows a tile can hold
 __device__ __forceinline__ int build_capA(const Geom& g) { return (g.tile_cap + 8) & ~3; }
-__host__ __device__ inline int build_rowcell_len(const Geom& g) { return ((g.interior_cap >> 2) + 15) & ~7; }   // u16 entries, 16-byte multiple
+__host__ __device__ inline int build_rowcell_len(const Geom& g) { return ((g.interior_cap >> 1) + 15) & ~7; }   // u16 entries (one per pair row), 16-byte multiple
 
 // packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2: two lanes of math per issue slot)
 typedef unsigned long long f32x2;
@@ -827,7 +828,7 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
   if (tt.n_slots > g.tile_cap || tt.n_int_slots > g.interior_cap) return;   // host re-plans and rebuilds
   for (int ic = threadIdx.x; ic < tt.nic; ic += blockDim.x) {
     const int t = interior_tile_cell(tt, ic);
-    for (int i = 0; i < pad4(tt.cnt[t]) >> 2; ++i) rowcell[(tt.rstart[t] >> 2) + i] = (unsigned short)t;
+    for (int i = 0; i < pad2(tt.cnt[t]) >> 1; ++i) rowcell[(tt.rstart[t] >> 1) + i] = (unsigned short)t;
   }
   // staging: tile-centred fp32 coordinates = packed cell-relative coordinate + the cell's offset (the same values the
   // force kernels stage), one thread per quad of slots, SoA so that four candidates are one broadcast 128-bit load
@@ -880,17 +881,16 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
   int my_max = 0;
   unsigned long long my_sum = 0;
 
-  const int nrq = tt.n_int_slots >> 2;                 // quads of interior slots in use
+  const int nrp = tt.n_int_slots >> 1;                 // pair rows in use
   const unsigned off_dummy = 4u * (unsigned)tt.n_slots;
 #pragma unroll 1
-  for (int task = wid; task * 16 < nrq; task += nw) {
-    const int rq = task * 16 + (lane >> 1);            // this lane's quad of slots; the lane owns its pair (lane & 1)
-    const bool haveq = rq < nrq;
-    const int t = rowcell[haveq ? rq : 0];             // its tile cell
+  for (int task = wid; task * 32 < nrp; task += nw) {
+    const int prow = task * 32 + lane;                 // this lane's pair row
+    const bool havep = prow < nrp;
+    const int t = rowcell[havep ? prow : 0];           // its tile cell
     const int c = tt.cnt[t], g_lo = tt.gstart[t];
-    const int kin0 = haveq ? 4 * rq - tt.rstart[t] + 2 * (lane & 1) : c;   // index of the pair's first atom within its cell
+    const int kin0 = havep ? 2 * prow - tt.rstart[t] : c;   // index of the pair's first atom within its cell
     const bool act0 = kin0 < c, act1 = kin0 + 1 < c;
-    const int prow = 2 * (haveq ? rq : 0) + (lane & 1);                  // pair row
     const int aslot0 = tt.start[t] + (act0 ? kin0 : 0);                  // staged slot of the first atom
     PairPos P;
     {
@@ -968,8 +968,8 @@ __global__ void __launch_bounds__(BUILD_MAX_THREADS, BUILD_MIN_BLOCKS) k_build_l
       nwords = before;   // count below from complete words + rem
     }
     const int n = nwords * 8 + rem;
-    if (haveq) {
-      const int stored = act0 ? (n < g.row_cap ? n : g.row_cap) : 0;   // a pad pair row is empty
+    if (havep) {
+      const int stored = act0 ? (n < g.row_cap ? n : g.row_cap) : 0;
       A.numneigh[(size_t)tile * prow_cap(g) + prow] = stored;
       if (act0) {
         my_max = max(my_max, n);
@@ -1429,14 +1429,73 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
   return d2;
 }
 
-// per-pair epilogue: the two atoms gi and gi + 1 (the second only if act1), one after the other (both at once
-// would need 36 more live registers than the list loop leaves); returns max |x'-x0|^2 for EPI_KICK_DRIFT (else 0).
-template <typename T>
+// per-pair epilogue: the two atoms gi and gi + 1 (the second only if act1); returns max |x'-x0|^2 for
+// EPI_KICK_DRIFT (else 0).  WIDE = false: one atom after the other (both at once would need 36 more live registers
+// than the 56-register kernels have); WIDE = true (k_tile_force_p, 72 registers): all loads of both atoms first.
+template <typename T, bool WIDE>
 __device__ __forceinline__ double atom_epilogue2(const ForceArgs& A, int gi, bool act1, const double (&ta)[3], const double (&tb)[3],
                                                  const double (&cc)[3]) {
-  double d2 = atom_epilogue<T>(A, gi, ta, cc);
-  if (act1) d2 = fmax(d2, atom_epilogue<T>(A, gi + 1, tb, cc));
-  return d2;
+  if constexpr (!WIDE) {
+    double d2 = atom_epilogue<T>(A, gi, ta, cc);
+    if (act1) d2 = fmax(d2, atom_epilogue<T>(A, gi + 1, tb, cc));
+    return d2;
+  } else {
+    const size_t ld = A.ld;
+    if (A.epi == EPI_FORCES) {
+      A.f[gi] = ta[0]; A.f[ld + gi] = ta[1]; A.f[2 * ld + gi] = ta[2];
+      if (act1) { A.f[gi + 1] = tb[0]; A.f[ld + gi + 1] = tb[1]; A.f[2 * ld + gi + 1] = tb[2]; }
+      return 0.0;
+    }
+    const int g1 = act1 ? gi + 1 : gi;
+    double va[3], vb[3], xa[3] = {0.0, 0.0, 0.0}, xb[3] = {0.0, 0.0, 0.0}, x0a[3] = {0.0, 0.0, 0.0}, x0b[3] = {0.0, 0.0, 0.0};
+    const int tya = A.type[gi], tyb = A.type[g1];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { va[d] = A.v[d * ld + gi]; vb[d] = A.v[d * ld + g1]; }
+    if (A.epi == EPI_KICK_DRIFT) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        xa[d] = A.x[d * ld + gi]; xb[d] = A.x[d * ld + g1];
+        x0a[d] = A.x0[d * ld + gi]; x0b[d] = A.x0[d * ld + g1];
+      }
+    }
+    const double dtfa = A.dtf_type[tya], dtfb = A.dtf_type[tyb];
+    double d2a = 0.0, d2b = 0.0;
+    T ra[3], rb[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      va[d] += dtfa * ta[d];                                  // second half kick of this step
+      vb[d] += dtfb * tb[d];
+      if (A.epi == EPI_KICK_DRIFT) {
+        va[d] += dtfa * ta[d];                                // first half kick of the next step
+        vb[d] += dtfb * tb[d];
+        xa[d] += A.dt * va[d];                                // drift
+        xb[d] += A.dt * vb[d];
+        ra[d] = (T)(xa[d] - cc[d]);
+        rb[d] = (T)(xb[d] - cc[d]);
+        const double da = xa[d] - x0a[d], db = xb[d] - x0b[d];
+        d2a += da * da;
+        d2b += db * db;
+      }
+    }
+    if (A.epi == EPI_KICK_DRIFT) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { A.x_new[d * ld + gi] = xa[d]; A.v[d * ld + gi] = va[d]; }
+      reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(ra[0], ra[1], ra[2], (T)0);
+      if (act1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { A.x_new[d * ld + gi + 1] = xb[d]; A.v[d * ld + gi + 1] = vb[d]; }
+        reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi + 1] = make_v4<T>(rb[0], rb[1], rb[2], (T)0);
+      }
+    } else {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { A.f[d * ld + gi] = ta[d]; A.v[d * ld + gi] = va[d]; }
+      if (act1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { A.f[d * ld + gi + 1] = tb[d]; A.v[d * ld + gi + 1] = vb[d]; }
+      }
+    }
+    return act1 ? fmax(d2a, d2b) : d2a;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1626,7 +1685,11 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
         }
         if constexpr (HALF) sgid[slot] = k0 + u < c ? tt.gstart[t] + k0 + u : 0;
       }
-      if (interior) *reinterpret_cast<uint2*>(scell + tt.rstart[t] + k0) = make_uint2(sc[0], sc[1]);   // indexed by interior slot
+      if (interior) {   // indexed by interior slot; a pair of slots is one list row (the cell's rows are padded to 2, not 4)
+        unsigned* sp = reinterpret_cast<unsigned*>(scell + tt.rstart[t] + k0);
+        if (k0 < c) sp[0] = sc[0];
+        if (k0 + 2 < c) sp[1] = sc[1];
+      }
     }
     if (threadIdx.x == 0) st[tt.n_slots] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);   // the dummy slot
   }
@@ -1748,7 +1811,7 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
             for (int d = 0; d < 3; ++d) cc[d] = cell_anchor_1d(g, d, tt.c0[d] + tq[d] - 1);
           }
           const double ta[3] = {tot0[0], tot0[1], tot0[2]}, tb[3] = {tot1[0], tot1[1], tot1[2]};
-          d2max = fmax(d2max, atom_epilogue2<T>(A, gi, act1, ta, tb, cc));
+          d2max = fmax(d2max, atom_epilogue2<T, false>(A, gi, act1, ta, tb, cc));
         }
         if constexpr (EV) {
           const double wgt = HALF ? 1.0 : 0.5;   // a full list visits every pair twice
@@ -1831,7 +1894,8 @@ __global__ void __launch_bounds__(256) k_eam_embed(int N, double B, const double
 // ---------------------------------------------------------------------------------------------------
 constexpr int FORCE_P_MAX_NBUF = 3;               // tile buffers: ngroups being computed on + one being loaded
 constexpr int FORCE_P_MAX_REGS = 72;              // up to 896 threads per block
-constexpr int FORCE_P_MAX_THREADS = 896;          // consumer threads + one producer warp
+constexpr int FORCE_P_MAX_THREADS = 896;          // consumer threads + the producer warps
+constexpr int FORCE_P_NPROD = 4;                  // producer warps
 __host__ __device__ inline size_t force_p_buf_bytes(const Geom& g) {
   return (size_t)tile_tab_stride(g) * 4 + (size_t)force_capA(g) * 16 + (((size_t)g.interior_cap * 2 + 15) & ~(size_t)15);
 }
@@ -1863,6 +1927,7 @@ struct TileView {
 
 template <class Body, int K, int MODE>
 __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gthreads, int NG, int NB) {
+  constexpr int NP = FORCE_P_NPROD;
   using T = float;
   using V4 = float4;
   constexpr int NT = Body::NT;
@@ -1899,8 +1964,11 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   const int pcap = prow_cap(g);
 
   if (wid >= NG * gwarps) {
-    // ---------------- producer warp: walks ALL tiles of the block in order ----------------
-    if (wid > NG * gwarps) return;
+    // ---------------- producer warps: they walk ALL tiles of the block in order, sharing each tile's copies ----------------
+    // (issuing ~150 small bulk copies takes one warp several microseconds; measured with one producer warp, the
+    // staging pipeline alone took 0.2 ms per launch at cfg 5 and the consumers waited for it)
+    const int pw = wid - NG * gwarps;
+    if (pw >= NP) return;
     const V4* __restrict__ xr = reinterpret_cast<const V4*>(A.xr);
     for (int k = 0; k < ntl; ++k) {
       const int b = k % NB, j = k / NB;
@@ -1909,7 +1977,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
       const unsigned buf = smem0 + 128u + (unsigned)b * buf_bytes;
       TileView tv{reinterpret_cast<const int*>(bufp), tcs};
       if (j > 0) mbar_wait(empty(b), (unsigned)((j - 1) & 1));
-      if (lane == 0) {
+      if (pw == 0 && lane == 0) {
         ctr[b] = 0;
         mbar_expect_tx(tabfull(b), (unsigned)tab_ints * 4u);
         bulk_g2s(buf, A.tab + (size_t)tile * tab_ints, (unsigned)tab_ints * 4u, tabfull(b));
@@ -1918,10 +1986,10 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
       int c0[3], w[3];
       tile_dims(g, tile, c0, w);
       const int ntc = (w[0] + 2) * (w[1] + 2) * (w[2] + 2);
-      if (lane == 0) mbar_expect_tx(full(b), (unsigned)tv.n_staged() * 16u);
-      __syncwarp();
+      if (pw == 0 && lane == 0) mbar_expect_tx(full(b), (unsigned)tv.n_staged() * 16u);
+      group_barrier(3, 32 * NP);   // the byte count is posted before any of the tile's copies can complete
       const unsigned st_a = buf + (unsigned)tab_ints * 4u;
-      for (int t = lane; t < ntc; t += 32) {
+      for (int t = pw * 32 + lane; t < ntc; t += 32 * NP) {
         const int c = tv.cnt(t);
         if (c > 0) bulk_g2s(st_a + (unsigned)tv.start(t) * 16u, xr + tv.gstart(t), (unsigned)c * 16u, full(b));
       }
@@ -1982,7 +2050,11 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
               st[slot] = make_float4(1e15f, 1e15f, 1e15f, 0.f);
             }
           }
-          if (interior) *reinterpret_cast<uint2*>(scell + tv.rstart(t) + k0) = make_uint2(sc[0], sc[1]);   // indexed by interior slot
+          if (interior) {   // indexed by interior slot; a pair of slots is one list row (the cell's rows are padded to 2, not 4)
+          unsigned* sp = reinterpret_cast<unsigned*>(scell + tv.rstart(t) + k0);
+          if (k0 < c) sp[0] = sc[0];
+          if (k0 + 2 < c) sp[1] = sc[1];
+        }
         } else if (q == nq) {
           st[tv.n_slots()] = make_float4(1e15f, 1e15f, 1e15f, 0.f);   // the dummy slot
         }
@@ -2041,7 +2113,11 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
             }
           }
         }
+#ifdef MDK_SKIP_LOOP   // timing experiment: everything but the list loop
+        const int mine = 0;
+#else
         const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
+#endif
         list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi0, pi1, tot0, tot1, w_first, base == 0);
       }
       if constexpr (K > 1) {
@@ -2058,7 +2134,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
             for (int d = 0; d < 3; ++d) cc[d] = cell_anchor_1d(g, d, c0[d] + tq[d] - 1);
           }
           const double ta[3] = {tot0[0], tot0[1], tot0[2]}, tb[3] = {tot1[0], tot1[1], tot1[2]};
-          d2max = fmax(d2max, atom_epilogue2<T>(A, gi, act1, ta, tb, cc));
+          d2max = fmax(d2max, atom_epilogue2<T, false>(A, gi, act1, ta, tb, cc));
         } else {
 #pragma unroll
           for (int a = 0; a < 2; ++a) {

@@ -20,8 +20,8 @@ MD_ERR_BAD_ARGUMENT, MD_ERR_BOX_TOO_SMALL, MD_ERR_CUDA, MD_ERR_OVERFLOW, MD_ERR_
 MD_FP64, MD_MIXED = 0, 1
 MD_PAIR_LJ126, MD_PAIR_EAM_FS = 1, 2
 MD_LIST_FULL, MD_LIST_HALF = 0, 1
-MD_KERNEL_AUTO, MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_CELL, MD_KERNEL_SUBWARP4 = 0, 1, 2, 3, 4, 5
-KERNEL_NAMES = {0: "auto", 1: "tpa", 2: "subwarp8", 3: "warp", 4: "cell", 5: "subwarp4"}
+MD_KERNEL_AUTO, MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_CELL, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2 = 0, 1, 2, 3, 4, 5, 6
+KERNEL_NAMES = {0: "auto", 1: "tpa", 2: "subwarp8", 3: "warp", 4: "cell", 5: "subwarp4", 6: "subwarp2"}
 
 EXPORTS = [
     "md_create", "md_destroy", "md_set_units", "md_set_precision", "md_set_positions", "md_set_velocities",
@@ -211,9 +211,9 @@ class System:
         return ke.value
 
     def md_autotune(self, nrep: int = 3):
-        ms = (ctypes.c_double * 4)()
+        ms = (ctypes.c_double * 5)()
         self._ck(lib.md_autotune(self._h, nrep, ms))
-        return {"tpa": ms[0], "subwarp8": ms[1], "warp": ms[2], "subwarp4": ms[3]}
+        return {"tpa": ms[0], "subwarp8": ms[1], "warp": ms[2], "subwarp4": ms[3], "subwarp2": ms[4]}
 
     def md_get_stats(self) -> dict:
         st = md_stats()

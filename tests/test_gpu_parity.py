@@ -186,7 +186,7 @@ def test_half_list_holds_each_pair_once():
 
 # ---- forces, energy, virial: small boxes, every kernel variant, against the O(N^2) definition --------------
 
-VARIANTS = [("tpa", 1, 0), ("subwarp4", 5, 0), ("subwarp8", 2, 0), ("warp", 3, 0), ("cell", 4, 0), ("half", 1, 1)]
+VARIANTS = [("tpa", 1, 0), ("subwarp2", 6, 0), ("subwarp4", 5, 0), ("subwarp8", 2, 0), ("warp", 3, 0), ("cell", 4, 0), ("half", 1, 1)]
 
 
 @pytest.mark.parametrize("name,kernel,list_kind", VARIANTS)
