@@ -41,6 +41,8 @@ struct md_system_impl {
   int kernel_req = MD_KERNEL_TPA;
   int kernel_eff = MD_KERNEL_TPA;
   bool autotuned = false;
+  int tune_stage = 0;            // 1: variant chosen on the caller's positions at setup; 2: confirmed on evolved positions (md_run)
+  int64_t tune_step = 0;         // nsteps_total at the setup-time choice
   bool have_x = false, pair_set = false, planned = false, list_valid = false, forces_valid = false;
   bool list_built_for_export = false;
 
@@ -101,7 +103,7 @@ struct md_system_impl {
   int max_tile_atoms = 0, max_row = 0;   // max_row / mean_row: the stored PAIR rows (union of the two atoms' neighbors)
   double mean_row = 0;
   double ms_build = 0, ms_force = 0, ms_run = 0;
-  cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr, ev3 = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr, ev3 = nullptr, ev4 = nullptr, ev5 = nullptr;   // run, build, autotune
   static constexpr int NSAMPLE = 128;          // sampled force timings per md_run
   cudaEvent_t pev[2 * NSAMPLE] = {};
   double ms_force_sampled = 0, ms_build_in_run = 0;
@@ -219,7 +221,7 @@ bool persistent_eligible(const md_system* s) {
 }
 int p_groups(const md_system* s) { return s->p_groups; }               // consumer groups per block (1 or 2)
 int p_nbuf(const md_system* s) { return s->p_groups + 1; }             // tile buffers: one per group + one being loaded
-int p_max_group_threads(const md_system* s) { return ((FORCE_P_MAX_THREADS - 32 * FORCE_P_NPROD) / s->p_groups) / 32 * 32; }
+int p_max_group_threads(const md_system* s) { return ((FORCE_P_MAX_THREADS - 32 * FORCE_P_NPROD) / s->p_groups) / 128 * 128; }   // whole warpgroups (register split)
 // ... and enough tiles per SM for the producer to run ahead (with a few tiles per block the static tile assignment
 // quantises badly: 2 or 3 tiles per block at 256,000 atoms)
 bool use_persistent(const md_system* s, const Geom& g) {
@@ -556,7 +558,7 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
       if (use_persistent(s, g)) {
         // persistent, warp-specialised path: one block per SM, two consumer groups of `threads` + one producer warp
         const int ng = p_groups(s), nb = p_nbuf(s);
-        const int gth = std::min(threads, p_max_group_threads(s));
+        const int gth = std::min((threads + 127) / 128 * 128, p_max_group_threads(s));   // whole warpgroups
         const unsigned grid = (unsigned)std::min(g.ntiles, s->num_sms);
         const unsigned block = (unsigned)(ng * gth + 32 * FORCE_P_NPROD);
         const size_t sm = force_p_smem(g, nb);
@@ -649,7 +651,6 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   // width depends on how many tiles the box yields, over the planner's width and its two neighbours.  Score of a
   // candidate: one force evaluation plus an eighth of a list build (a typical rebuild interval).
   const int cand[5] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2};
-  s->force_timing_pending = false;   // ev0 / ev1 are reused below
   s->brick_forced = 0;
   s->kernel_eff = MD_KERNEL_TPA;
   s->planned = false;
@@ -664,7 +665,9 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   const int i0 = s->shape_index, nfeas = s->shape_count;
   for (int off = sweep ? -2 : 0; off <= (sweep ? 2 : 0); ++off) {
     if (i0 + off < 0 || i0 + off >= nfeas) continue;
-    for (int k = 0; k < 5; ++k) {
+    for (int kk = 0; kk < 5; ++kk) {
+      static const int by_lanes[5] = {0, 4, 3, 1, 2};   // cand[] in the order 1, 2, 4, 8, 32 lanes per row
+      const int k = by_lanes[kk];
       s->kernel_eff = cand[k];
       s->brick_forced = off == 0 ? 0 : 9 + off;
       s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;   // an overflow of one shape must not inflate the next
@@ -675,21 +678,27 @@ int autotune(md_system* s, int nrep, double* ms_out) {
       const double ms_build = s->ms_build;
       rc = compute_forces_device(s, false);   // warm-up
       if (rc) return rc;
-      CK(cudaEventRecord(s->ev0, s->stream));
+      CK(cudaEventRecord(s->ev4, s->stream));
       for (int r = 0; r < nrep; ++r) { rc = compute_forces_device(s, false); if (rc) return rc; }
-      CK(cudaEventRecord(s->ev1, s->stream));
+      CK(cudaEventRecord(s->ev5, s->stream));
       CK(cudaStreamSynchronize(s->stream));
       float ms = 0;
-      cudaEventElapsedTime(&ms, s->ev0, s->ev1);
+      cudaEventElapsedTime(&ms, s->ev4, s->ev5);
       const double per = ms / nrep, score = per + ms_build / 8.0;
       if (ms_out && per < ms_out[k]) ms_out[k] = per;
-      if (score < best_score) { best_score = score; best = cand[k]; best_b = s->brick_forced; }
+      // more lanes per row must win by 5 %: the timing here is of plain force evaluations on the positions of the moment
+      // (often the initial lattice), and near a tie the variant with fewer lanes has the cheaper fused epilogue
+      if (score < (best_score < 1e299 && lanes_for(cand[k]) > lanes_for(best) ? 0.95 * best_score : best_score)) {
+        best_score = score; best = cand[k]; best_b = s->brick_forced;
+      }
     }
   }
   s->kernel_eff = best;
   s->brick_forced = best_b;
   s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;
   s->autotuned = true;
+  s->tune_stage = s->tune_stage == 0 ? 1 : 2;
+  s->tune_step = s->nsteps_total;
   s->planned = false;
   s->list_valid = false;
   return MD_OK;
@@ -772,7 +781,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   s->mass_h.assign(mass, mass + ntypes); CKC(dalloc(&s->scalars_d, 16)); CKC(dalloc(&s->io_d, 3 * s->ld));
   CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
-  CKC(cudaEventCreate(&s->ev0)); CKC(cudaEventCreate(&s->ev1)); CKC(cudaEventCreate(&s->ev2)); CKC(cudaEventCreate(&s->ev3));
+  CKC(cudaEventCreate(&s->ev0)); CKC(cudaEventCreate(&s->ev1)); CKC(cudaEventCreate(&s->ev2)); CKC(cudaEventCreate(&s->ev3)); CKC(cudaEventCreate(&s->ev4)); CKC(cudaEventCreate(&s->ev5));
   for (int k = 0; k < 2 * md_system_impl::NSAMPLE; ++k) CKC(cudaEventCreate(&s->pev[k]));
   CKC(cudaMemcpyAsync(s->mass_d, mass, ntypes * sizeof(double), cudaMemcpyHostToDevice, s->stream));
   CKC(cudaMemcpyAsync(s->types_caller, types, (size_t)N * sizeof(int), is_device_ptr(types) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
@@ -809,6 +818,8 @@ void md_destroy(md_system* s) {
   if (s->ev1) cudaEventDestroy(s->ev1);
   if (s->ev2) cudaEventDestroy(s->ev2);
   if (s->ev3) cudaEventDestroy(s->ev3);
+  if (s->ev4) cudaEventDestroy(s->ev4);
+  if (s->ev5) cudaEventDestroy(s->ev5);
   for (cudaEvent_t e : s->pev) if (e) cudaEventDestroy(e);
   delete s;
 }
@@ -823,7 +834,7 @@ int md_set_units(md_system* s, double ftm2v, double mvv2e) {
 int md_set_precision(md_system* s, int mode) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (mode != MD_FP64 && mode != MD_MIXED) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_precision: unknown mode %d", mode);
-  if (mode != s->precision) { s->precision = mode; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->brick_forced = 0; }
+  if (mode != s->precision) { s->precision = mode; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->tune_stage = 0; s->brick_forced = 0; }
   return MD_OK;
 }
 
@@ -855,7 +866,7 @@ int md_set_pair(md_system* s, int style, const double* params, int nparams, doub
   s->style = style;
   for (int k = 0; k < 5; ++k) s->params[k] = k < need ? params[k] : 0.0;
   s->rc = rc; s->skin = skin;
-  s->pair_set = true; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->brick_forced = 0;
+  s->pair_set = true; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->tune_stage = 0; s->brick_forced = 0;
   return MD_OK;
 }
 
@@ -868,7 +879,7 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel) {
   s->list_kind = list_kind;
   s->kernel_req = kernel;
   s->kernel_eff = kernel == MD_KERNEL_AUTO ? MD_KERNEL_TPA : kernel;
-  s->autotuned = false; s->brick_forced = 0;
+  s->autotuned = false; s->tune_stage = 0; s->brick_forced = 0;
   s->planned = false; s->list_valid = false; s->forces_valid = false;
   return MD_OK;
 }
@@ -985,6 +996,13 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
       if (final_ran) s->forces_valid = true;
       if (stopped) {
         s->batch = std::min(32, std::max(2, done + 2));
+        // MD_KERNEL_AUTO: the setup-time choice was made on the caller's positions, often a perfect
+        // lattice, whose rows all have one length; it is confirmed ONCE on evolved positions, at the first rebuild
+        // that comes 20 or more time steps later (the timing builds its own lists; the state is left as a build leaves it)
+        if (s->kernel_req == MD_KERNEL_AUTO && s->tune_stage == 1 && s->nsteps_total - s->tune_step >= 20) {
+          rc = autotune(s, 3, nullptr);
+          if (rc) return rc;
+        }
         rc = build(s, false);   // also clears the flags
         if (rc) return rc;
         s->ms_build_in_run += s->ms_build;

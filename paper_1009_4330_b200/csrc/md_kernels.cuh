@@ -1893,8 +1893,9 @@ __global__ void __launch_bounds__(256) k_eam_embed(int N, double B, const double
 // Shared memory: mbarriers (128 B) | 3 x { table[tile_tab_stride] ints | st[capA] float4 | scell[interior_cap] u16 }.
 // ---------------------------------------------------------------------------------------------------
 constexpr int FORCE_P_MAX_NBUF = 3;               // tile buffers: ngroups being computed on + one being loaded
-constexpr int FORCE_P_MAX_REGS = 72;              // up to 896 threads per block
+constexpr int FORCE_P_MAX_REGS = 72;              // registers per thread at launch: up to 896 threads per block
 constexpr int FORCE_P_MAX_THREADS = 896;          // consumer threads + the producer warps
+constexpr int FORCE_P_CONSUMER_REGS = 80;         // after the register split below: (896 x 72 - 128 x 24) / 768
 constexpr int FORCE_P_NPROD = 4;                  // producer warps
 __host__ __device__ inline size_t force_p_buf_bytes(const Geom& g) {
   return (size_t)tile_tab_stride(g) * 4 + (size_t)force_capA(g) * 16 + (((size_t)g.interior_cap * 2 + 15) & ~(size_t)15);
@@ -1963,7 +1964,12 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   const int ntl = ((int)g.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this block
   const int pcap = prow_cap(g);
 
+  // Register split (setmaxnreg): the block is launched with FORCE_P_MAX_REGS registers per thread; the producer
+  // warpgroup keeps 24 and hands the rest to the consumer warpgroups, which grow to FORCE_P_CONSUMER_REGS (the list
+  // loop spills 68 bytes at 72 registers, 16 at 80; measured -3 % at cfg 5).  Hence groups are whole warpgroups
+  // (gthreads % 128 == 0) and the producers are the last four warps of the block.
   if (wid >= NG * gwarps) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
     // ---------------- producer warps: they walk ALL tiles of the block in order, sharing each tile's copies ----------------
     // (issuing ~150 small bulk copies takes one warp several microseconds; measured with one producer warp, the
     // staging pipeline alone took 0.2 ms per launch at cfg 5 and the consumers waited for it)
@@ -1998,6 +2004,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   }
 
   // ---------------- consumer groups ----------------
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(FORCE_P_CONSUMER_REGS));
   const int grp = wid / gwarps, gt = (int)threadIdx.x - grp * gthreads;
   const Body body(A.P);
   const size_t ld = A.ld;
