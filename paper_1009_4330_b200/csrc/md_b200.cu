@@ -653,6 +653,7 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   const int cand[5] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2};
   s->brick_forced = 0;
   s->kernel_eff = MD_KERNEL_TPA;
+  s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;   // the candidate list below must be the one the loop plans with
   s->planned = false;
   int rc = plan(s);
   if (rc) return rc;
@@ -673,6 +674,8 @@ int autotune(md_system* s, int nrep, double* ms_out) {
       s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;   // an overflow of one shape must not inflate the next
       s->planned = false;
       rc = build(s, true);
+      if (rc && getenv("MD_B200_TUNE_VERBOSE"))
+        fprintf(stderr, "autotune: K=%d off %d shape %dx%dx%d: build failed (%d) %s\n", lanes_for(cand[k]), off, s->g.b[0], s->g.b[1], s->g.b[2], rc, s->err.c_str());
       if (rc == MD_ERR_OVERFLOW && off != 0) continue;   // this shape does not fit with this many lanes per atom
       if (rc) return rc;
       const double ms_build = s->ms_build;
@@ -685,6 +688,9 @@ int autotune(md_system* s, int nrep, double* ms_out) {
       float ms = 0;
       cudaEventElapsedTime(&ms, s->ev4, s->ev5);
       const double per = ms / nrep, score = per + ms_build / 8.0;
+      if (getenv("MD_B200_TUNE_VERBOSE"))
+        fprintf(stderr, "autotune: off %d i0 %d nfeas %d K=%d shape %dx%dx%d tiles %d threads %d force %.4f ms build %.4f ms score %.4f\n", off, i0, nfeas, lanes_for(cand[k]), s->g.b[0],
+                s->g.b[1], s->g.b[2], s->g.ntiles, s->force_threads, per, ms_build, score);
       if (ms_out && per < ms_out[k]) ms_out[k] = per;
       // more lanes per row must win by 5 %: the timing here is of plain force evaluations on the positions of the moment
       // (often the initial lattice), and near a tie the variant with fewer lanes has the cheaper fused epilogue

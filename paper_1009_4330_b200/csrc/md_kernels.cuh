@@ -1926,6 +1926,42 @@ struct TileView {
   __device__ __forceinline__ const unsigned short* qc() const { return reinterpret_cast<const unsigned short*>(h + TILE_HDR + TILE_CELL_INTS * tcs); }
 };
 
+// post-processing of one chunk (32 quads of staged slots) of a landed tile: cell offsets added in place, pad slots and
+// the dummy slot set far away, pair row -> cells map.  One warp per chunk.
+__device__ __forceinline__ void force_p_post_chunk(const TileView& tv, float4* st, unsigned short* scell, int ch, int lane) {
+  const int nq = tv.n_slots() >> 2;
+  const int q = ch * 32 + lane;
+  if (q < nq) {
+    const int t = tv.qc()[q];
+    const int c = tv.cnt(t), k0 = 4 * q - tv.start(t);
+    const float ox = tv.off(0, t), oy = tv.off(1, t), oz = tv.off(2, t);
+    const bool interior = (tv.meta(t) >> 24) != 0;
+    unsigned sc[2] = {0xffffffffu, 0xffffffffu};
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int slot = 4 * q + u;
+      if (k0 + u < c) {
+        float4 v = st[slot];
+        v.x += ox; v.y += oy; v.z += oz;
+        st[slot] = v;
+        sc[u >> 1] = (u & 1) ? ((sc[u >> 1] & 0xffffu) | ((unsigned)t << 16)) : ((sc[u >> 1] & 0xffff0000u) | (unsigned)t);
+      } else {
+        st[slot] = make_float4(1e15f, 1e15f, 1e15f, 0.f);
+      }
+    }
+    if (interior) {   // indexed by interior slot; a pair of slots is one list row (the cell's rows are padded to 2, not 4)
+      unsigned* sp = reinterpret_cast<unsigned*>(scell + tv.rstart(t) + k0);
+      if (k0 < c) sp[0] = sc[0];
+      if (k0 + 2 < c) sp[1] = sc[1];
+    }
+  } else if (q == nq) {
+    st[tv.n_slots()] = make_float4(1e15f, 1e15f, 1e15f, 0.f);   // the dummy slot
+  }
+}
+
+#ifndef MDK_FORCE_P_PRODUCER_POST
+#define MDK_FORCE_P_PRODUCER_POST 1   // 1: the producer warps post-process the landed tile; 0: the consumer warps do (chunks dealt on arrival)
+#endif
 template <class Body, int K, int MODE>
 __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gthreads, int NG, int NB) {
   constexpr int NP = FORCE_P_NPROD;
@@ -1999,6 +2035,21 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
         const int c = tv.cnt(t);
         if (c > 0) bulk_g2s(st_a + (unsigned)tv.start(t) * 16u, xr + tv.gstart(t), (unsigned)c * 16u, full(b));
       }
+#if MDK_FORCE_P_PRODUCER_POST
+      // the tile's post-processing, off the consumers' critical path (7 % of their time when they did it themselves):
+      // the producers run a tile ahead of the consumers, so they can afford to wait for the copies here
+      mbar_wait(full(b), (unsigned)(j & 1));
+      {
+        float4* stp = reinterpret_cast<float4*>(bufp + (size_t)tab_ints * 4);
+        unsigned short* scp = reinterpret_cast<unsigned short*>(stp + capA);
+        for (int ch = pw; ch < nchunks; ch += NP) {
+          force_p_post_chunk(tv, stp, scp, ch, lane);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(ready(b));   // release: the consumers' wait acquires the chunk
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // these generic stores precede the buffer's next bulk copies
+      }
+#endif
     }
     return;
   }
@@ -2026,49 +2077,21 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
     V4* st = reinterpret_cast<V4*>(bufp + (size_t)tab_ints * 4);
     unsigned short* scell = reinterpret_cast<unsigned short*>(st + capA);
     const unsigned st_base = smem_addr(st);
+#if !MDK_FORCE_P_PRODUCER_POST
     mbar_wait(tabfull(b), (unsigned)(j & 1));
     mbar_wait(full(b), (unsigned)(j & 1));
-    {
-      // offsets, pad slots, slot -> cell map, in chunks of 32 quads of slots dealt to whichever warps of the group
-      // get here first (the warps of a group finish their previous tile at different times: no group barrier)
-      const int nq = tv.n_slots() >> 2;
-      const unsigned short* qc = tv.qc();
-      for (;;) {
-        int ch = 0;
-        if (lane == 0) ch = atomicAdd(&ctr[b], 1);
-        ch = __shfl_sync(0xffffffffu, ch, 0);
-        if (ch >= nchunks) break;
-        const int q = ch * 32 + lane;
-        if (q < nq) {
-          const int t = qc[q];
-          const int c = tv.cnt(t), k0 = 4 * q - tv.start(t);
-          const float ox = tv.off(0, t), oy = tv.off(1, t), oz = tv.off(2, t);
-          const bool interior = (tv.meta(t) >> 24) != 0;
-          unsigned sc[2] = {0xffffffffu, 0xffffffffu};
-#pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const int slot = 4 * q + u;
-            if (k0 + u < c) {
-              V4 v = st[slot];
-              v.x += ox; v.y += oy; v.z += oz;
-              st[slot] = v;
-              sc[u >> 1] = (u & 1) ? ((sc[u >> 1] & 0xffffu) | ((unsigned)t << 16)) : ((sc[u >> 1] & 0xffff0000u) | (unsigned)t);
-            } else {
-              st[slot] = make_float4(1e15f, 1e15f, 1e15f, 0.f);
-            }
-          }
-          if (interior) {   // indexed by interior slot; a pair of slots is one list row (the cell's rows are padded to 2, not 4)
-          unsigned* sp = reinterpret_cast<unsigned*>(scell + tv.rstart(t) + k0);
-          if (k0 < c) sp[0] = sc[0];
-          if (k0 + 2 < c) sp[1] = sc[1];
-        }
-        } else if (q == nq) {
-          st[tv.n_slots()] = make_float4(1e15f, 1e15f, 1e15f, 0.f);   // the dummy slot
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(ready(b));   // release: the waits below acquire the chunk
-      }
+    // chunks of 32 quads of slots dealt to whichever warps of the group get here first (the warps of a group finish
+    // their previous tile at different times: no group barrier)
+    for (;;) {
+      int ch = 0;
+      if (lane == 0) ch = atomicAdd(&ctr[b], 1);
+      ch = __shfl_sync(0xffffffffu, ch, 0);
+      if (ch >= nchunks) break;
+      force_p_post_chunk(tv, st, scell, ch, lane);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ready(b));   // release: the waits below acquire the chunk
     }
+#endif
     mbar_wait(ready(b), (unsigned)(j & 1));
     int c0[3], wdt[3];
     tile_dims(g, tile, c0, wdt);
