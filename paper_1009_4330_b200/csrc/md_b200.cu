@@ -60,7 +60,7 @@ struct md_system_impl {
   int64_t steps_since_build = 0;
   int balance_after = 0;     // BALANCE_AFTER, or MD_B200_BALANCE_AFTER (tuning experiments)
   bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
-  int p_min_tiles_per_sm = 8;   // k_tile_force_p is used from this many tiles per SM on (MD_B200_PMIN)
+  int p_min_tiles_per_sm = 1;   // k_tile_force_p is used from this many tiles per SM on (MD_B200_PMIN; measured: cfg 4 -4 % at 2-3 tiles per SM)
   int p_groups = 2;             // consumer groups of the persistent force kernel (MD_B200_PGROUPS)
   bool no_persistent = false;   // MD_B200_NO_PERSISTENT=1: run k_tile_force where k_tile_force_p would be used (A/B measurements)
   int brick_forced = 0;   // 9 + offset: the autotuner's step away from the planner's tile shape in the candidate list (0: none)
@@ -263,7 +263,9 @@ void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
   g.half = s->list_kind == MD_LIST_HALF ? 1 : 0;
   g.code_shift = s->precision == MD_FP64 ? 4 : 3;
   double vol = s->box[0] * s->box[1] * s->box[2];
-  double mean_nb = 4.0 / 3.0 * M_PI * rl * rl * rl * s->N / vol * (g.half ? 0.5 : 1.0);
+  // (a half list keeps or drops another cell whole, so its rows range from empty to nearly the full neighborhood:
+  // the row capacity is that of the full list)
+  double mean_nb = 4.0 / 3.0 * M_PI * rl * rl * rl * s->N / vol;
   int unit = 8 * g.K;
   // a stored row is the union of the neighbors of two atoms ~1.4 sigma apart: ~1.4 x the single-atom mean (measured
   // 1.38 in the LJ liquid), times the same 1.5 x slack over the mean as before
@@ -620,16 +622,17 @@ int compute_forces_device(md_system* s, bool ev, const StepMode& M = StepMode())
 
 int autotune(md_system* s, int nrep, double* ms_out);
 
-int initial_integrate(md_system* s, double dt, double hdtf) {
+int initial_integrate(md_system* s, double dt, double hdtf, bool in_run = false) {
+  const Flags* rf = in_run ? s->flags_d : nullptr;
   const int N = (int)s->N;
   if (s->precision == MD_FP64)
     CK(launch(s, k_initial_integrate<double>, blocks_for(N, 256), 256, 0, s->g, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
               (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, (double4*)s->xr[s->xcur], dt, hdtf,
-              &s->flags_d->max_disp2_bits[0]));
+              &s->flags_d->max_disp2_bits[0], rf));
   else
     CK(launch(s, k_initial_integrate<float>, blocks_for(N, 256), 256, 0, s->g, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
               (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, (float4*)s->xr[s->xcur], dt, hdtf,
-              &s->flags_d->max_disp2_bits[0]));
+              &s->flags_d->max_disp2_bits[0], rf));
   return MD_OK;
 }
 
@@ -1020,43 +1023,75 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
       }
     }
   } else {
-    // half list: the scatter kernel's forces are complete only when it has finished, so integrate separately
-    for (int64_t step = 0; step < nsteps; ++step) {
-      CK(cudaMemsetAsync(s->flags_d->max_disp2_bits, 0, 2 * sizeof(unsigned long long), s->stream));
-      rc = initial_integrate(s, dt, hdtf);
-      if (rc) return rc;
-      CK(cudaMemcpyAsync(&s->flags_h->max_disp2_bits[0], &s->flags_d->max_disp2_bits[0], sizeof(unsigned long long), cudaMemcpyDeviceToHost,
-                         s->stream));
-      CK(cudaStreamSynchronize(s->stream));
-      double d2;
-      memcpy(&d2, &s->flags_h->max_disp2_bits[0], sizeof d2);
-      if (d2 > trigger) { rc = build(s, false); if (rc) return rc; s->ms_build_in_run += s->ms_build; }
-      const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
-      if (sample) CK(cudaEventRecord(s->pev[2 * nsampled], s->stream));
-      rc = compute_forces_device(s, false);
-      if (rc) return rc;
-      if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
+    // half list: the scatter kernel's forces are complete only when it has finished, so a time step is three launches
+    // (kick + drift + displacement flag | forces | kick).  They are enqueued in batches like the fused path: the force
+    // kernel reads the flag the integrator has just written and, if the list is stale, does nothing and raises `stop`;
+    // every later kernel of the batch then does nothing either.  The host reads {steps_done, stop} once per batch; the
+    // step that stopped has had its first half (kick + drift) applied, so the host rebuilds, evaluates the forces and
+    // finishes it before it enqueues the next batch.
+    auto final_integrate = [&](bool in_run) -> int {
       CK(launch(s, k_final_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->v[s->cur], (const double*)s->f, (const int*)s->type[s->cur],
-                (const double*)s->mass_d, hdtf));
-      s->nsteps_total++;
+                (const double*)s->mass_d, hdtf, in_run ? s->flags_d : (Flags*)nullptr));
+      return MD_OK;
+    };
+    CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
+    int64_t remaining = nsteps;
+    while (remaining > 0) {
+      const int m = (int)std::min<int64_t>(s->batch, remaining);
+      int sample_slot[64];
+      for (int k = 0; k < m; ++k) {
+        rc = initial_integrate(s, dt, hdtf, true);
+        if (rc) return rc;
+        StepMode M;
+        M.epi = EPI_FORCES; M.in_run = 1; M.parity = 0; M.trigger = trigger;
+        const int64_t step = nsteps - remaining + k;
+        const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
+        sample_slot[k] = -1;
+        if (sample) { sample_slot[k] = nsampled; CK(cudaEventRecord(s->pev[2 * nsampled], s->stream)); }
+        rc = compute_forces_device(s, false, M);
+        if (rc) return rc;
+        if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
+        rc = final_integrate(true);
+        if (rc) return rc;
+      }
+      CK(cudaMemcpyAsync(s->flags_h, s->flags_d, sizeof(Flags), cudaMemcpyDeviceToHost, s->stream));
+      CK(cudaStreamSynchronize(s->stream));
+      const int done = s->flags_h->steps_done;
+      const bool stopped = s->flags_h->stop != 0;
+      if (done < 0 || done > m || (!stopped && done != m)) return fail(s, MD_ERR_CUDA, "md_run: inconsistent step count from the device (%d of %d)", done, m);
+      for (int k = 0; k < m; ++k) {
+        if (sample_slot[k] < 0) continue;
+        if (k < done) { float t = 0; CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev[2 * sample_slot[k] + 1])); s->ms_force_sampled += t; s->nforce_sampled_acc++; }
+        else nsampled = std::min(nsampled, sample_slot[k]);
+      }
+      s->nsteps_total += done;
+      s->steps_since_build += done;
+      remaining -= done;
+      s->nforce -= (m - done);
+      if (stopped) {
+        s->batch = std::min(32, std::max(2, done + 2));
+        rc = build(s, false);   // also clears the flags
+        if (rc) return rc;
+        s->ms_build_in_run += s->ms_build;
+        rc = compute_forces_device(s, false);
+        if (rc) return rc;
+        rc = final_integrate(false);
+        if (rc) return rc;
+        s->nsteps_total++; s->steps_since_build++; remaining--;
+      } else if (remaining > 0) {
+        CK(cudaMemsetAsync(&s->flags_d->steps_done, 0, sizeof(int), s->stream));
+        if (done == s->batch) s->batch = std::min(32, s->batch + 2);
+      }
     }
+    s->forces_valid = true;
   }
   CK(cudaEventRecord(s->ev1, s->stream));
   CK(cudaStreamSynchronize(s->stream));
   float ms = 0;
   cudaEventElapsedTime(&ms, s->ev0, s->ev1);
   s->ms_run = ms;
-  if (!fused) {
-    for (int k = 0; k < nsampled; ++k) {
-      float t = 0;
-      CK(cudaEventElapsedTime(&t, s->pev[2 * k], s->pev[2 * k + 1]));
-      s->ms_force_sampled += t;
-    }
-    s->nforce_sampled = nsampled;
-  } else {
-    s->nforce_sampled = s->nforce_sampled_acc;
-    s->nforce_sampled_acc = 0;
-  }
+  s->nforce_sampled = s->nforce_sampled_acc;
+  s->nforce_sampled_acc = 0;
   s->nbuilds_in_run = s->nbuilds - builds0;
   s->launches_last_run = s->launches - launches0;
   return MD_OK;

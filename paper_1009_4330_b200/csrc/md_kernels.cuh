@@ -2323,8 +2323,10 @@ __global__ void k_reduce_ev(int ntiles, const double* __restrict__ partials, dou
 template <typename T>
 __global__ void k_initial_integrate(Geom g, int N, size_t ld, double* __restrict__ x, double* __restrict__ v, const double* __restrict__ f,
                                     const double* __restrict__ x0, const int* __restrict__ type, const double* __restrict__ mass,
-                                    typename Vec4<T>::type* __restrict__ xr, double dt, double half_dt_ftm2v, unsigned long long* flag) {
+                                    typename Vec4<T>::type* __restrict__ xr, double dt, double half_dt_ftm2v, unsigned long long* flag,
+                                    const Flags* run_flags) {
   __shared__ double red[32];
+  if (run_flags && run_flags->stop) return;   // a batched step after the one that found the list stale: do nothing
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   double d2 = 0.0;
   if (n < N) {
@@ -2347,8 +2349,12 @@ __global__ void k_initial_integrate(Geom g, int N, size_t ld, double* __restrict
 }
 
 __global__ void k_final_integrate(int N, size_t ld, double* __restrict__ v, const double* __restrict__ f,
-                                  const int* __restrict__ type, const double* __restrict__ mass, double half_dt_ftm2v) {
+                                  const int* __restrict__ type, const double* __restrict__ mass, double half_dt_ftm2v, Flags* run_flags) {
   int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (run_flags) {   // batched stepping (half-list path): skipped once the list is stale; the step's last kernel counts it
+    if (run_flags->stop) return;
+    if (n == 0) atomicAdd(&run_flags->steps_done, 1);
+  }
   if (n >= N) return;
   double dtf = half_dt_ftm2v / mass[type[n]];
 #pragma unroll

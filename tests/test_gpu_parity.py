@@ -406,6 +406,28 @@ def test_eam_metal_units_run_matches_oracle():
     assert s.md_get_stats()["kinetic_energy"] == pytest.approx(ke, rel=1e-10)
 
 
+@pytest.mark.parametrize("cfg,n,nsteps", [(1, 7, 80), (4, 6, 40)])
+def test_half_list_run_matches_oracle_trajectory(cfg, n, nsteps):
+    """Half list (Newton's third law) through md_run: the batched three-launch time step (kick+drift |
+    scatter forces | kick) with the device-side stale flag must rebuild at the oracle's steps (+-1) and follow
+    its trajectory; LJ (hot liquid: several rebuilds inside the run) and two-pass EAM."""
+    w = wl.make(cfg, n_override=n)
+    s = md.from_workload(w, precision=md.MD_FP64, kernel=md.MD_KERNEL_TPA, list_kind=md.MD_LIST_HALF)
+    s.md_run(nsteps, w.dt)
+    x, v, f = (np.zeros((w.natoms, 3)) for _ in range(3))
+    s.md_get_positions(x); s.md_get_velocities(v); s.md_get_forces(f)
+    ref = oracle.run_nve(w.x, w.v, w.box, np.full(w.natoms, w.mass[0]), w.style, w.params, w.rc, w.skin, w.dt, nsteps,
+                         ftm2v=w.ftm2v, mvv2e=w.mvv2e)
+    assert np.abs(_minimg(x - ref["x"], w.box)).max() < 1e-9
+    assert np.abs(v - ref["v"]).max() < 1e-8 * max(1.0, np.abs(ref["v"]).max())
+    st = s.md_get_stats()
+    assert st["nsteps_total"] == nsteps
+    assert abs(st["nbuilds"] - ref["nbuild"]) <= 1
+    fo = oracle.forces(x, w.box, w.style, w.params, w.rc)[0]
+    assert _fp64_force_err(f, fo) < 1e-11
+    s.close()
+
+
 # ---- errors and degenerate inputs ------------------------------------------------------------------------------
 
 def test_error_paths():
