@@ -17,7 +17,7 @@ e2e       the same through the C ABI with HOST (pinned) buffers: H2D of x and v,
           final positions and the kinetic energy, every step, inside the timed region
 roofline  dominant kernel = the pair-force tile kernel; SURVEY.md 8(d)'s algorithmic bytes per launch / its
           mean launch duration (CUDA events on the library's stream inside md_run, sampled steps of the
-          timed region); traffic = measured DRAM bytes per launch from profiles/traffic.json
+          timed region); traffic = measured DRAM bytes per launch from the committed ncu summary profiles/r02_ncu_full_force_cfgN.md
 cpu_baseline   the oracle (oracle/md_oracle.c, as it stands) on the host cores, bounded sample
 
 N > 1: independent replicas, one per GPU, no data-path collective ("scaling": "weak").
@@ -42,6 +42,7 @@ if ROOT not in sys.path:
 
 from paper_1009_4330_b200 import dist as mdist          # noqa: E402
 from paper_1009_4330_b200 import workloads as wl        # noqa: E402
+from paper_1009_4330_b200 import ncu_summary            # noqa: E402  (text parsing only)
 
 METRIC = "atom-timesteps/s (force+neighbor+integrate)"
 UNIT = "atom-timesteps/s"
@@ -127,12 +128,53 @@ def survey_force_bytes(natoms: int, mean_neighbors: float, style: int) -> float:
     return per_atom * natoms
 
 
+# SURVEY.md 8(d) "optimistic ceilings": algorithmic HBM bytes of ONE atom-timestep of the whole path (index stream at
+# 4 B per list entry + per-atom state + fused integration; gathers charged to cache; list build excluded)
+PATH_BYTES = {1: 540.0, 2: 540.0, 3: 2330.0, 4: 880.0, 5: 540.0}
+PROFILE_MD = "profiles/r02_ncu_full_force_cfg%d.md"     # written by `python -m paper_1009_4330_b200.ncu_summary full ...`
+
+
+def roofline_block(cfg: int, w, st: dict, value: float, hbm_gbs: float, peak_src: str) -> dict:
+    """The `roofline` object of one configuration: dominant kernel = the pair-force kernel (both passes for EAM)."""
+    nf = max(1, st["nforce_sampled"])
+    ms_force = st["ms_force_sampled"] / nf
+    sbytes = survey_force_bytes(w.natoms, st["mean_neighbors"], w.style)
+    lbytes = layout_force_bytes(w.natoms, st["mean_row"], w.style)
+    achieved = sbytes / (ms_force * 1e-3) / 1e9 if ms_force > 0 else 0.0
+    persistent = w.precision == wl.PREC_MIXED
+    r = {
+        "bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+        "frac_of_nominal_8TBps": achieved / 8000.0, "traffic": None, "peak_source": peak_src,
+        "kernel": "%s<%s,K=%d>" % ("k_tile_force_p" if persistent else "k_tile_force", "LJ" if w.style == wl.PAIR_LJ else "EAM density+force",
+                                   st["lanes_per_atom"]),
+        "algorithmic_bytes_per_launch": sbytes,
+        "algorithmic_bytes_definition": "SURVEY.md 8(d): (4 B x exact list entries + 52 B) per atom (EAM: two passes), DESIGN.md 6",
+        "own_layout_bytes_per_launch": lbytes,
+        "ms_per_launch": ms_force, "launches_sampled": st["nforce_sampled"],
+        "path_bytes_per_atom_step": PATH_BYTES[cfg],
+        "path_frac": value / (hbm_gbs * 1e9 / PATH_BYTES[cfg]),
+        "note": "frac is SURVEY 8(d)'s ALGORITHMIC-bytes ceiling over the measured HBM copy rate, not the share of the binding "
+                "resource: the kernel moves fewer bytes than that (2-byte slot codes, one row per pair of atoms: "
+                "own_layout_bytes_per_launch) and ncu shows it bound by the FP32 (FMA) pipe and latency, DRAM at ~30 % "
+                "(profiles/, DESIGN.md 6)",
+    }
+    if w.style == wl.PAIR_EAM and ms_force > 0:
+        p1 = st["ms_force_pass1_sampled"] / nf
+        r["ms_pass1_density"] = p1
+        r["ms_pass2_force"] = ms_force - p1
+    t = ncu_summary.traffic(os.path.join(ROOT, PROFILE_MD % cfg))
+    if t is not None:
+        r["traffic"] = t
+        r["traffic_source"] = (PROFILE_MD % cfg) + " (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum; both passes summed for EAM)"
+    return r
+
+
 def layout_force_bytes(natoms: int, mean_neighbors: float, style: int) -> float:
     """The same with THIS library's list layout (16-bit tile-local slot codes: 2 B per entry) -- what the
     kernel itself must move; reported beside the SURVEY figure, never as ``achieved``."""
-    per_atom = 2.0 * mean_neighbors + 4 + 24 + 24
+    per_atom = 2.0 * (0.5 * mean_neighbors) + 2 + 24 + 24        # mean_neighbors here = entries per stored PAIR row (md_stats.mean_row)
     if style == wl.PAIR_EAM:
-        per_atom = 2 * (2.0 * mean_neighbors + 4 + 24) + 16 + 8 + 24
+        per_atom = 2 * (2.0 * (0.5 * mean_neighbors) + 2 + 24) + 16 + 8 + 24
     return per_atom * natoms
 
 
@@ -270,37 +312,23 @@ def run_ours(args, rk) -> None:
     # roofline of the dominant kernel: sampled force launches inside the timed md_run
     nf = max(1, st["nforce_sampled"])
     ms_force = st["ms_force_sampled"] / nf
-    sbytes = survey_force_bytes(w.natoms, st["mean_neighbors"], w.style)
-    lbytes = layout_force_bytes(w.natoms, st["mean_neighbors"], w.style)
-    achieved = sbytes / (ms_force * 1e-3) / 1e9 if ms_force > 0 else 0.0
     nruns = max(1, args.steps)
     ms_per_step = 1e3 * tmax / nruns
-    roofline = {
-        "bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
-        "frac_of_nominal_8TBps": achieved / 8000.0,
-        "traffic": None, "peak_source": peak_src,
-        "kernel": "k_tile_force<%s,%s,K=%d>" % ("float" if w.precision == wl.PREC_MIXED else "double",
-                                                 "LJ" if w.style == wl.PAIR_LJ else "EAM density+force", st["lanes_per_atom"]),
-        "algorithmic_bytes_per_launch": sbytes,
-        "algorithmic_bytes_definition": "SURVEY.md 8(d): (4 B x list entries + 52 B) per atom (EAM: two passes), DESIGN.md 6",
-        "own_layout_bytes_per_launch": lbytes,
-        "achieved_with_own_layout_bytes": lbytes / (ms_force * 1e-3) / 1e9 if ms_force > 0 else 0.0,
-        "ms_per_launch": ms_force, "launches_sampled": st["nforce_sampled"],
-        "share_of_step": {"force": ms_force * w.nsteps / (1e3 * tmax / nruns) if tmax > 0 else None,
-                          "build": st["ms_build_in_run"] / (1e3 * tmax / nruns) if tmax > 0 else None},
-        "binding_resource_measured": "shared-memory data pipe (random 128-bit gathers of staged neighbor positions), "
-                                     "see profiles/ and DESIGN.md 6",
-    }
-    # the resource ncu shows saturated: one LDS.128 gather per list entry (two passes for EAM); a warp gather moves
-    # 32 x 16 B = 4 wavefronts at best, ~9 with the bank conflicts of random slots; 148 SMs x 1 wavefront per clock
+    roofline = roofline_block(args.cfg, w, st, value, hbm_gbs, peak_src)
+    roofline["share_of_step"] = {"force": ms_force * w.nsteps / (1e3 * tmax / nruns) if tmax > 0 else None,
+                                 "build": st["ms_build_in_run"] / (1e3 * tmax / nruns) if tmax > 0 else None}
+    # the resource ncu shows busiest: the FP32 pipe.  A list entry costs 14 packed f32x2 operations for the two atoms of its
+    # row (3 sub, 3 for r^2, 5 for the LJ factor, 3 accumulate); a packed operation occupies the pipe for 2 cycles per warp
+    # (measured: DESIGN.md 6), so one launch needs entries/32 x 28 pipe cycles on 148 x 4 sub-cores at full lanes
     passes = 2 if w.style == wl.PAIR_EAM else 1
-    gathers_per_s = passes * w.natoms * st["mean_neighbors"] / (ms_force * 1e-3) if ms_force > 0 else 0.0
+    entries = passes * 0.5 * w.natoms * st["mean_row"]
     sm_clock = 1.965e9
-    roofline["smem_gather"] = {
-        "achieved": gathers_per_s / 1e9, "unit": "G gathered entries/s",
-        "peak_conflict_free": 148 * sm_clock * 32 / 4 / 1e9,
-        "frac_of_conflict_free": gathers_per_s / (148 * sm_clock * 32 / 4),
-        "note": "DESIGN.md 6: ncu l1tex__data_pipe_lsu_wavefronts 89 % of peak at ~9 wavefronts per warp gather (cfg 5)"}
+    fp32_floor_ms = entries / 32.0 * 28.0 / (148 * 4) / sm_clock * 1e3
+    roofline["fp32_pipe"] = {
+        "list_entries_per_launch": entries, "packed_ops_per_entry": 14, "pipe_cycles_per_packed_warp_op": 2,
+        "floor_ms_full_lanes": fp32_floor_ms, "frac_of_floor": fp32_floor_ms / ms_force if ms_force > 0 else None,
+        "note": "LJ count; the floor assumes every lane of every warp busy (the rows of a warp differ in length: ~25 % of the "
+                "lanes idle) and no prologue/epilogue; EAM bodies cost more per entry"}
     # the other heavy kernel: the list build, ALU-bound.  Tests = N x 27 x atoms per cell; peak = fp32
     # lanes x clock / 5 lane-instructions per test (3 packed sub/fma pairs = 3, compare, emit), 148 SMs x 128 lanes
     ncell = float(st["ncells"][0] * st["ncells"][1] * st["ncells"][2])
@@ -316,30 +344,28 @@ def run_ours(args, rk) -> None:
                 "~20 atoms for 32 lanes and each accepted entry costs a store and a pointer update (DESIGN.md 6)"}
     if not rk.is_root:
         return
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")    # written by hand from an ncu --set full capture
-    try:
-        with open(traffic_file) as fh:
-            roofline["traffic"] = json.load(fh).get("cfg%d" % args.cfg, {}).get("dram_bytes_per_launch")
-            roofline["traffic_source"] = "profiles/traffic.json (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)"
-    except Exception:
-        pass
     per_config = {}
     if args.all_configs and rk.world == 1:
+        sampler2 = ClockSampler(dev)
+        sampler2.start()
+        t_pc0 = time.perf_counter()
         for c in (1, 2, 3, 4, 5):
             if c == args.cfg:
                 continue
             wc = wl.make(c)
-            r = time_workload(torch, md, wc, stream, 3, 3, kernel if c != 3 else md.MD_KERNEL_AUTO, list_kind if wc.style == wl.PAIR_LJ else md.MD_LIST_FULL,
-                              host_io=False)
+            r = time_workload(torch, md, wc, stream, 5, 3, md.MD_KERNEL_AUTO if args.kernel == "auto" else kernel,
+                              list_kind if wc.style == wl.PAIR_LJ else md.MD_LIST_FULL, host_io=False)
             sc = r["stats"]
-            msf = sc["ms_force_sampled"] / max(1, sc["nforce_sampled"])
+            vc = wc.natoms * wc.nsteps * len(r["ms"]) / (sum(r["ms"]) * 1e-3)
             per_config["cfg%d" % c] = {
-                "workload": wc.name, "value": wc.natoms * wc.nsteps * len(r["ms"]) / (sum(r["ms"]) * 1e-3), "unit": UNIT,
+                "workload": wc.name, "value": vc, "unit": UNIT, "passes_timed": len(r["ms"]),
                 "ms_per_pass": sum(r["ms"]) / len(r["ms"]), "time_steps": wc.nsteps, "builds": sc["nbuilds_in_run"],
-                "variant": md.KERNEL_NAMES[sc["kernel_variant"]], "mean_neighbors": sc["mean_neighbors"],
-                "force_ms_per_launch": msf,
-                "force_GBps": survey_force_bytes(wc.natoms, sc["mean_neighbors"], wc.style) / (msf * 1e-3) / 1e9 if msf > 0 else None,
+                "ms_per_build": sc["ms_build_in_run"] / max(1, sc["nbuilds_in_run"]),
+                "variant": md.KERNEL_NAMES[sc["kernel_variant"]], "brick": sc["brick"], "tiles": sc["ntiles"],
+                "mean_neighbors": sc["mean_neighbors"], "mean_row": sc["mean_row"],
+                "roofline": roofline_block(c, wc, sc, vc, hbm_gbs, peak_src),
                 "l2_flushed_between_passes": r["flushed_l2"]}
+        per_config["clocks"] = sampler2.stop(t_pc0, time.perf_counter())
         # the paper's comparison (Eq. 1): neighbor-list kernel against the direct cell-list kernel, and
         # the half list (Newton's third law, atomics), on the bench workload itself
         for name, kv, lk in (("cell_list", md.MD_KERNEL_CELL, md.MD_LIST_FULL), ("half_list_tpa", md.MD_KERNEL_TPA, md.MD_LIST_HALF)):

@@ -110,6 +110,7 @@ typedef struct md_stats {
   int32_t max_row;             /* longest stored row at the last build */
   int32_t reserved0;
   double mean_row;             /* mean stored row length at the last build (entries per pair of atoms) */
+  double ms_force_pass1_sampled; /* EAM: the share of ms_force_sampled spent in pass 1 (density + embedding); 0 for LJ */
 } md_stats;
 
 /* Creates a system: orthogonal periodic box [0,Lx) x [0,Ly) x [0,Lz), N atoms with type ids in

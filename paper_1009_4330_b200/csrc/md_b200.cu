@@ -106,6 +106,9 @@ struct md_system_impl {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr, ev3 = nullptr, ev4 = nullptr, ev5 = nullptr;   // run, build, autotune
   static constexpr int NSAMPLE = 128;          // sampled force timings per md_run
   cudaEvent_t pev[2 * NSAMPLE] = {};
+  cudaEvent_t pev_mid[NSAMPLE] = {};           // EAM: between the two passes of a sampled force evaluation
+  cudaEvent_t mid_event = nullptr;             // recorded by the next EAM force evaluation after its first pass (md_run sets it)
+  double ms_pass1_sampled = 0;
   double ms_force_sampled = 0, ms_build_in_run = 0;
   int64_t nforce_sampled = 0, nbuilds_in_run = 0, nforce_sampled_acc = 0;
 
@@ -603,6 +606,7 @@ int launch_force_T(md_system* s, const StepMode& M) {
     if (g.half && s->kernel_eff != MD_KERNEL_CELL)   // half list: rho was scattered with atomics, so F'(rho) needs its own pass
       CK(launch(s, k_eam_embed<T>, blocks_for(s->N, 256), 256, 0, (int)s->N, s->P.B, (const double*)s->rho, s->fp, (T*)s->xr[xb],
                 EV ? s->scalars_d : (double*)nullptr));
+    if (s->mid_event) CK(cudaEventRecord(s->mid_event, s->stream));
     A.fp_in = s->fp;
     rc = launch_force_variant<T, EamForceBody, 0, EV>(s, A);          // pass 2: forces
     if (rc) return rc;
@@ -639,7 +643,7 @@ int initial_integrate(md_system* s, double dt, double hdtf, bool in_run = false)
 int ensure_list(md_system* s) {
   if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set first");
   if (s->kernel_req == MD_KERNEL_AUTO && !s->autotuned) {
-    int rc = autotune(s, 3, nullptr);
+    int rc = autotune(s, 5, nullptr);
     if (rc) return rc;
   }
   if (!s->list_valid) return build(s, false);
@@ -792,6 +796,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
   CKC(cudaEventCreate(&s->ev0)); CKC(cudaEventCreate(&s->ev1)); CKC(cudaEventCreate(&s->ev2)); CKC(cudaEventCreate(&s->ev3)); CKC(cudaEventCreate(&s->ev4)); CKC(cudaEventCreate(&s->ev5));
   for (int k = 0; k < 2 * md_system_impl::NSAMPLE; ++k) CKC(cudaEventCreate(&s->pev[k]));
+  for (int k = 0; k < md_system_impl::NSAMPLE; ++k) CKC(cudaEventCreate(&s->pev_mid[k]));
   CKC(cudaMemcpyAsync(s->mass_d, mass, ntypes * sizeof(double), cudaMemcpyHostToDevice, s->stream));
   CKC(cudaMemcpyAsync(s->types_caller, types, (size_t)N * sizeof(int), is_device_ptr(types) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
                       s->stream));
@@ -830,6 +835,7 @@ void md_destroy(md_system* s) {
   if (s->ev4) cudaEventDestroy(s->ev4);
   if (s->ev5) cudaEventDestroy(s->ev5);
   for (cudaEvent_t e : s->pev) if (e) cudaEventDestroy(e);
+  for (cudaEvent_t e : s->pev_mid) if (e) cudaEventDestroy(e);
   delete s;
 }
 
@@ -896,7 +902,7 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel) {
 int md_build_neighbors(md_system* s) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (s->kernel_req == MD_KERNEL_AUTO && !s->autotuned) {
-    int rc = autotune(s, 3, nullptr);
+    int rc = autotune(s, 5, nullptr);
     if (rc) return rc;
   }
   return build(s, false);
@@ -953,7 +959,8 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   }
   const int64_t sample_every = (nsteps + md_system_impl::NSAMPLE - 1) / md_system_impl::NSAMPLE;
   int nsampled = 0;
-  s->ms_force_sampled = 0;
+  s->ms_force_sampled = 0; s->ms_pass1_sampled = 0;
+  const bool eam = s->style == MD_PAIR_EAM_FS;
   const bool fused = s->list_kind != MD_LIST_HALF;
   if (nsteps > 0 && fused) {
     // Velocity Verlet with ONE launch per time step (two for EAM): the force kernel of step n also does the
@@ -979,8 +986,9 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         const int64_t step = nsteps - remaining + k;
         const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
         sample_slot[k] = -1;
-        if (sample) { sample_slot[k] = nsampled; CK(cudaEventRecord(s->pev[2 * nsampled], s->stream)); }
+        if (sample) { sample_slot[k] = nsampled; CK(cudaEventRecord(s->pev[2 * nsampled], s->stream)); if (eam) s->mid_event = s->pev_mid[nsampled]; }
         rc = compute_forces_device(s, false, M);
+        s->mid_event = nullptr;
         if (rc) return rc;
         if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
       }
@@ -991,7 +999,11 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
       if (done < 0 || done > m || (!stopped && done != m)) return fail(s, MD_ERR_CUDA, "md_run: inconsistent step count from the device (%d of %d)", done, m);
       for (int k = 0; k < m; ++k) {   // timings of the launches that really ran; a sampled launch that was skipped gives its slot back
         if (sample_slot[k] < 0) continue;
-        if (k < done) { float t = 0; CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev[2 * sample_slot[k] + 1])); s->ms_force_sampled += t; s->nforce_sampled_acc++; }
+        if (k < done) {
+          float t = 0;
+          CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev[2 * sample_slot[k] + 1])); s->ms_force_sampled += t; s->nforce_sampled_acc++;
+          if (eam) { CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev_mid[sample_slot[k]])); s->ms_pass1_sampled += t; }
+        }
         else nsampled = std::min(nsampled, sample_slot[k]);
       }
       const bool final_ran = done == m && (int64_t)m == remaining;
@@ -1009,7 +1021,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         // lattice, whose rows all have one length; it is confirmed ONCE on evolved positions, at the first rebuild
         // that comes 20 or more time steps later (the timing builds its own lists; the state is left as a build leaves it)
         if (s->kernel_req == MD_KERNEL_AUTO && s->tune_stage == 1 && s->nsteps_total - s->tune_step >= 20) {
-          rc = autotune(s, 3, nullptr);
+          rc = autotune(s, 5, nullptr);
           if (rc) return rc;
         }
         rc = build(s, false);   // also clears the flags
@@ -1047,8 +1059,9 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         const int64_t step = nsteps - remaining + k;
         const bool sample = step % sample_every == 0 && nsampled < md_system_impl::NSAMPLE;
         sample_slot[k] = -1;
-        if (sample) { sample_slot[k] = nsampled; CK(cudaEventRecord(s->pev[2 * nsampled], s->stream)); }
+        if (sample) { sample_slot[k] = nsampled; CK(cudaEventRecord(s->pev[2 * nsampled], s->stream)); if (eam) s->mid_event = s->pev_mid[nsampled]; }
         rc = compute_forces_device(s, false, M);
+        s->mid_event = nullptr;
         if (rc) return rc;
         if (sample) { CK(cudaEventRecord(s->pev[2 * nsampled + 1], s->stream)); ++nsampled; }
         rc = final_integrate(true);
@@ -1061,7 +1074,11 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
       if (done < 0 || done > m || (!stopped && done != m)) return fail(s, MD_ERR_CUDA, "md_run: inconsistent step count from the device (%d of %d)", done, m);
       for (int k = 0; k < m; ++k) {
         if (sample_slot[k] < 0) continue;
-        if (k < done) { float t = 0; CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev[2 * sample_slot[k] + 1])); s->ms_force_sampled += t; s->nforce_sampled_acc++; }
+        if (k < done) {
+          float t = 0;
+          CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev[2 * sample_slot[k] + 1])); s->ms_force_sampled += t; s->nforce_sampled_acc++;
+          if (eam) { CK(cudaEventElapsedTime(&t, s->pev[2 * sample_slot[k]], s->pev_mid[sample_slot[k]])); s->ms_pass1_sampled += t; }
+        }
         else nsampled = std::min(nsampled, sample_slot[k]);
       }
       s->nsteps_total += done;
@@ -1221,7 +1238,7 @@ int md_get_stats(md_system* s, md_stats* out) {
   out->ms_build = s->ms_build; out->ms_force = s->ms_force; out->ms_run = s->ms_run;
   out->launches_last_run = s->launches_last_run; out->launches_total = s->launches;
   out->ms_force_sampled = s->ms_force_sampled; out->nforce_sampled = s->nforce_sampled;
-  out->ms_build_in_run = s->ms_build_in_run; out->nbuilds_in_run = s->nbuilds_in_run;
+  out->ms_build_in_run = s->ms_build_in_run; out->nbuilds_in_run = s->nbuilds_in_run; out->ms_force_pass1_sampled = s->ms_pass1_sampled;
   return MD_OK;
 }
 

@@ -44,6 +44,7 @@ class md_stats(ctypes.Structure):
         ("ms_force_sampled", ctypes.c_double), ("nforce_sampled", ctypes.c_int64),
         ("ms_build_in_run", ctypes.c_double), ("nbuilds_in_run", ctypes.c_int64),
         ("max_row", ctypes.c_int32), ("reserved0", ctypes.c_int32), ("mean_row", ctypes.c_double),
+        ("ms_force_pass1_sampled", ctypes.c_double),
     ]
 
     def as_dict(self) -> dict:
