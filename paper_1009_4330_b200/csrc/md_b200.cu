@@ -61,10 +61,11 @@ struct md_system_impl {
   int balance_after = 0;     // BALANCE_AFTER, or MD_B200_BALANCE_AFTER (tuning experiments)
   bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
   int p_min_tiles_per_sm = 1;   // k_tile_force_p is used from this many tiles per SM on (MD_B200_PMIN; measured: cfg 4 -4 % at 2-3 tiles per SM)
-  int p_groups = 2;             // consumer groups of the persistent force kernel (MD_B200_PGROUPS)
+  int p_groups = 0;             // consumer groups of the persistent force kernel; 0: two if three tile buffers fit, else one (MD_B200_PGROUPS)
   bool no_persistent = false;   // MD_B200_NO_PERSISTENT=1: run k_tile_force where k_tile_force_p would be used (A/B measurements)
-  int brick_forced = 0;   // 9 + offset: the autotuner's step away from the planner's tile shape in the candidate list (0: none)
+  int brick_forced = 0;   // tile shape chosen by the autotuner, bx | by << 4 | bz << 8 (0: the planner's own pick)
   int shape_index = 0, shape_count = 0, build_threads = 256;
+  int shape_codes[64] = {};   // the feasible tile shapes of the last plan(), largest first (bx | by << 4 | bz << 8)
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
   void* xr[2] = {nullptr, nullptr};   // packed cell-relative positions (Vec4<T>, 32 B per atom reserved), buffer index = xcur
   int* tab = nullptr;                 // per-tile tables of the last build
@@ -222,13 +223,20 @@ constexpr size_t SMEM_OPTIN_BUDGET = 227 * 1024 - 1024;
 bool persistent_eligible(const md_system* s) {
   return s->precision == MD_MIXED && s->list_kind == MD_LIST_FULL && s->kernel_eff != MD_KERNEL_CELL && !s->no_persistent;
 }
-int p_groups(const md_system* s) { return s->p_groups; }               // consumer groups per block (1 or 2)
-int p_nbuf(const md_system* s) { return s->p_groups + 1; }             // tile buffers: one per group + one being loaded
-int p_max_group_threads(const md_system* s) { return ((FORCE_P_MAX_THREADS - 32 * FORCE_P_NPROD) / s->p_groups) / 128 * 128; }   // whole warpgroups (register split)
-// ... and enough tiles per SM for the producer to run ahead (with a few tiles per block the static tile assignment
-// quantises badly: 2 or 3 tiles per block at 256,000 atoms)
+// Consumer groups per block: two, with three tile buffers (two being computed on, one being loaded), when they fit the
+// SM's shared memory; else one group with two buffers (rc = 5 sigma: a 3x1x1 tile stages 108 KB); 0: does not fit.
+int p_groups(const md_system* s, const Geom& g) {
+  if (s->p_groups > 0) return force_p_smem(g, s->p_groups + 1) <= SMEM_OPTIN_BUDGET ? s->p_groups : 0;
+  if (force_p_smem(g, 3) <= SMEM_OPTIN_BUDGET) return 2;
+  return force_p_smem(g, 2) <= SMEM_OPTIN_BUDGET ? 1 : 0;
+}
+int p_nbuf(const md_system* s, const Geom& g) { return p_groups(s, g) + 1; }             // tile buffers: one per group + one being loaded
+int p_max_group_threads(const md_system* s, const Geom& g) {   // whole warpgroups (register split)
+  return ((FORCE_P_MAX_THREADS - 32 * FORCE_P_NPROD) / std::max(1, p_groups(s, g))) / 128 * 128;
+}
+// ... and enough tiles per SM for the producer to run ahead
 bool use_persistent(const md_system* s, const Geom& g) {
-  return persistent_eligible(s) && g.ntiles >= s->p_min_tiles_per_sm * s->num_sms && force_p_smem(g, p_nbuf(s)) <= SMEM_OPTIN_BUDGET;
+  return persistent_eligible(s) && g.ntiles >= s->p_min_tiles_per_sm * s->num_sms && p_groups(s, g) > 0;
 }
 
 void fill_geom_for_b(const md_system* s, const int shape[3], Geom& g) {
@@ -317,27 +325,46 @@ int plan(md_system* s) {
     feasible[nfeas++] = i;
   }
   if (!nfeas) return fail(s, MD_ERR_OVERFLOW, "no tile shape fits shared memory or the 16-bit slot codes (too many atoms per cell of edge rc+skin)");
-  for (int pass = 0; pass < 3 && pick < 0; ++pass) {
+  // Preferences, dropped one level at a time until a shape qualifies (largest shape first within a level):
+  //   level 0: shared memory for three resident blocks (or the persistent kernel's two groups + three tile buffers), fp32 tile extent,
+  //            enough tiles for two per SM, one round of rows, halo not more than 18 staged cells per interior cell
+  //   level 1: the same without the tile count
+  //   level 2: shared memory for two resident blocks (or the persistent kernel with one group + two buffers)
+  //   level 3: anything feasible
+  const size_t smem_two = (227 * 1024) / 2 - 1536 - 3200;
+  for (int pass = 0; pass < 4 && pick < 0; ++pass) {
     for (int f = 0; f < nfeas && pick < 0; ++f) {
       fill_geom_for_b(s, shapes[feasible[f]].b, g);
-      if (pass < 2) {
-        const bool pers = persistent_eligible(s) && g.ntiles >= s->p_min_tiles_per_sm * s->num_sms;
-        if (pers ? force_p_smem(g, p_nbuf(s)) > SMEM_OPTIN_BUDGET : force_smem(s, g, g.half) > smem_three) continue;
+      if (pass < 3) {
+        const bool pers = use_persistent(s, g);
+        if (pass < 2 ? !(pers && p_groups(s, g) == 2) && force_smem(s, g, g.half) > smem_three : !pers && force_smem(s, g, g.half) > smem_two) continue;
         double half_extent = 0;
         for (int d = 0; d < 3; ++d) half_extent = std::max(half_extent, 0.5 * (g.b[d] + 2) * g.edge[d]);
-        if (s->precision == MD_MIXED && half_extent > 9.0 * lscale && g.b[0] > 1) continue;   // fp32 tile coordinates
+        // fp32 tile coordinates: |value| <= 13.5 nearest-neighbor distances keeps the ulp at 1e-6 of one (cfg 3's 3x1x1
+        // tiles, 13.2, meet the 1e-5 force tolerance at full size: tests/test_gpu_fullsize.py)
+        if (s->precision == MD_MIXED && half_extent > 13.5 * lscale && g.b[0] > 1) continue;
         if (pass == 0 && g.ntiles < 2 * 148) continue;
+        if ((g.b[0] + 2) * (g.b[1] + 2) * (g.b[2] + 2) > 18 * g.b[0] * g.b[1] * g.b[2] && g.nc[0] * g.nc[1] * g.nc[2] > 27) continue;
         // thread-per-row: the tile's pair rows (+ 5 % for the fullest tiles) should fit ONE round of a block small
         // enough for three resident blocks (384 threads of <= 56 registers); a second, nearly empty round costs
         // more than the smaller tile does
-        if (g.K == 1 && 0.5 * ((double)s->N / g.ncell + 0.5) * g.b[0] * g.b[1] * g.b[2] * 1.05 > (pers ? (double)p_max_group_threads(s) : 384.0)) continue;
+        if (g.K == 1 && 0.5 * ((double)s->N / g.ncell + 0.5) * g.b[0] * g.b[1] * g.b[2] * 1.05 > (pers ? (double)p_max_group_threads(s, g) : 384.0)) continue;
       }
       pick = f;
     }
   }
-  // the autotuner may step away from the planner's pick: brick_forced = 1 + offset + 8 (0: none)
-  if (s->brick_forced) pick = std::min(std::max(pick + (s->brick_forced - 9), 0), nfeas - 1);
+  // the autotuner may name a shape itself; if that shape is not feasible (any more: the capacities may have grown
+  // after an overflow), the planner's own pick stands
+  if (s->brick_forced) {
+    int found = -1;
+    for (int f = 0; f < nfeas; ++f) {
+      const int* b = shapes[feasible[f]].b;
+      if ((b[0] | b[1] << 4 | b[2] << 8) == s->brick_forced) found = f;
+    }
+    if (found >= 0) pick = found; else s->brick_forced = 0;
+  }
   s->shape_index = pick; s->shape_count = nfeas;
+  for (int f = 0; f < nfeas; ++f) s->shape_codes[f] = shapes[feasible[f]].b[0] | shapes[feasible[f]].b[1] << 4 | shapes[feasible[f]].b[2] << 8;
   fill_geom_for_b(s, shapes[feasible[pick]].b, g);
   s->g = g;
   // block size of the list force kernels: the tile's pair rows should fill whole rounds of the block
@@ -345,7 +372,7 @@ int plan(md_system* s) {
     double rows = 0.5 * ((double)s->N / g.ncell + 0.5) * g.b[0] * g.b[1] * g.b[2] * 1.05;
     double lanes = rows * g.K;
     int tmax = s->precision == MD_FP64 ? FORCE_MAX_THREADS_WIDE : FORCE_MAX_THREADS;
-    if (use_persistent(s, g)) tmax = p_max_group_threads(s);                       // threads of ONE consumer group
+    if (use_persistent(s, g)) tmax = p_max_group_threads(s, g);                     // threads of ONE consumer group
     else if (force_smem(s, g, g.half) <= smem_three) tmax = std::min(tmax, 384);   // three resident blocks of <= 56 registers
     int rounds = (int)std::ceil(lanes / tmax);
     int t = (int)std::ceil(lanes / std::max(rounds, 1));
@@ -562,8 +589,8 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
     if constexpr (std::is_same<T, float>::value && !EV) {
       if (use_persistent(s, g)) {
         // persistent, warp-specialised path: one block per SM, two consumer groups of `threads` + one producer warp
-        const int ng = p_groups(s), nb = p_nbuf(s);
-        const int gth = std::min((threads + 127) / 128 * 128, p_max_group_threads(s));   // whole warpgroups
+        const int ng = p_groups(s, g), nb = p_nbuf(s, g);
+        const int gth = std::min((threads + 127) / 128 * 128, p_max_group_threads(s, g));   // whole warpgroups
         const unsigned grid = (unsigned)std::min(g.ntiles, s->num_sms);
         const unsigned block = (unsigned)(ng * gth + 32 * FORCE_P_NPROD);
         const size_t sm = force_p_smem(g, nb);
@@ -654,9 +681,12 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set first");
   if (s->list_kind == MD_LIST_HALF) { s->kernel_eff = MD_KERNEL_TPA; s->autotuned = true; s->planned = false; return MD_OK; }
   if (nrep < 1) nrep = 1;
-  // The setup-time mini benchmark of PAPER.md L137, over lanes per atom (1, 8, 32) and, because the best tile
-  // width depends on how many tiles the box yields, over the planner's width and its two neighbours.  Score of a
-  // candidate: one force evaluation plus an eighth of a list build (a typical rebuild interval).
+  // The setup-time mini benchmark of PAPER.md L137, over lanes per row (1, 2, 4, 8, 32) and, because the best tile
+  // shape depends on how many tiles the box yields, over the planner's shape and its neighbours in the list of feasible
+  // shapes.  What is timed is what md_run runs: the FUSED step kernel (force evaluation + kick + drift epilogue), with
+  // dt = 0 so that positions and velocities keep their values while the kernel does all of its work (a plain force
+  // evaluation misjudges the variants with few lanes per row, whose epilogue is the more expensive one).  Score of a
+  // candidate: one step plus an eighth of a list build (a typical rebuild interval).
   const int cand[5] = {MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2};
   s->brick_forced = 0;
   s->kernel_eff = MD_KERNEL_TPA;
@@ -671,37 +701,45 @@ int autotune(md_system* s, int nrep, double* ms_out) {
   // the box yields few tiles: then its neighbours in the candidate list (two larger, two smaller) are timed too
   const bool sweep = s->g.ntiles < 2048;
   const int i0 = s->shape_index, nfeas = s->shape_count;
-  for (int off = sweep ? -2 : 0; off <= (sweep ? 2 : 0); ++off) {
-    if (i0 + off < 0 || i0 + off >= nfeas) continue;
+  nrep = (nrep + 1) & ~1;                                   // an even number of buffer flips
+  CK(cudaMemsetAsync(s->dtf_d, 0, (size_t)s->ntypes * sizeof(double), s->stream));   // kick factors of a dt = 0 step
+  int codes[64];
+  for (int f = 0; f < nfeas; ++f) codes[f] = s->shape_codes[f];
+  for (int idx = sweep ? std::max(0, i0 - 2) : i0; idx <= (sweep ? std::min(nfeas - 1, i0 + 2) : i0); ++idx) {
     for (int kk = 0; kk < 5; ++kk) {
       static const int by_lanes[5] = {0, 4, 3, 1, 2};   // cand[] in the order 1, 2, 4, 8, 32 lanes per row
       const int k = by_lanes[kk];
       s->kernel_eff = cand[k];
-      s->brick_forced = off == 0 ? 0 : 9 + off;
+      s->brick_forced = codes[idx];
       s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;   // an overflow of one shape must not inflate the next
       s->planned = false;
       rc = build(s, true);
       if (rc && getenv("MD_B200_TUNE_VERBOSE"))
-        fprintf(stderr, "autotune: K=%d off %d shape %dx%dx%d: build failed (%d) %s\n", lanes_for(cand[k]), off, s->g.b[0], s->g.b[1], s->g.b[2], rc, s->err.c_str());
-      if (rc == MD_ERR_OVERFLOW && off != 0) continue;   // this shape does not fit with this many lanes per atom
+        fprintf(stderr, "autotune: K=%d shape %d (%dx%dx%d): build failed (%d) %s\n", lanes_for(cand[k]), idx, s->g.b[0], s->g.b[1], s->g.b[2], rc, s->err.c_str());
+      if (rc == MD_ERR_OVERFLOW && idx != i0) continue;   // this shape does not fit with this many lanes per row
       if (rc) return rc;
+      if ((s->g.b[0] | s->g.b[1] << 4 | s->g.b[2] << 8) != codes[idx]) continue;   // the build had to fall back to another shape
       const double ms_build = s->ms_build;
-      rc = compute_forces_device(s, false);   // warm-up
-      if (rc) return rc;
+      auto step = [&](int r) {
+        StepMode M;
+        M.epi = EPI_KICK_DRIFT; M.in_run = 0; M.parity = r & 1; M.dt = 0.0; M.hdtf = 0.0; M.trigger = 1e300;
+        M.xbuf = s->xcur ^ (r & 1);
+        return compute_forces_device(s, false, M);
+      };
+      for (int r = 0; r < 2; ++r) { rc = step(r); if (rc) return rc; }   // warm-up
       CK(cudaEventRecord(s->ev4, s->stream));
-      for (int r = 0; r < nrep; ++r) { rc = compute_forces_device(s, false); if (rc) return rc; }
+      for (int r = 0; r < nrep; ++r) { rc = step(r); if (rc) return rc; }
       CK(cudaEventRecord(s->ev5, s->stream));
       CK(cudaStreamSynchronize(s->stream));
       float ms = 0;
       cudaEventElapsedTime(&ms, s->ev4, s->ev5);
       const double per = ms / nrep, score = per + ms_build / 8.0;
       if (getenv("MD_B200_TUNE_VERBOSE"))
-        fprintf(stderr, "autotune: off %d i0 %d nfeas %d K=%d shape %dx%dx%d tiles %d threads %d force %.4f ms build %.4f ms score %.4f\n", off, i0, nfeas, lanes_for(cand[k]), s->g.b[0],
-                s->g.b[1], s->g.b[2], s->g.ntiles, s->force_threads, per, ms_build, score);
+        fprintf(stderr, "autotune: K=%d shape %d of %d (%dx%dx%d) tiles %d threads %d step %.4f ms build %.4f ms score %.4f\n", lanes_for(cand[k]), idx,
+                nfeas, s->g.b[0], s->g.b[1], s->g.b[2], s->g.ntiles, s->force_threads, per, ms_build, score);
       if (ms_out && per < ms_out[k]) ms_out[k] = per;
-      // more lanes per row must win by 5 %: the timing here is of plain force evaluations on the positions of the moment
-      // (often the initial lattice), and near a tie the variant with fewer lanes has the cheaper fused epilogue
-      if (score < (best_score < 1e299 && lanes_for(cand[k]) > lanes_for(best) ? 0.95 * best_score : best_score)) {
+      // more lanes per row must win by 3 % (timing noise)
+      if (score < (best_score < 1e299 && lanes_for(cand[k]) > lanes_for(best) ? 0.97 * best_score : best_score)) {
         best_score = score; best = cand[k]; best_b = s->brick_forced;
       }
     }
@@ -760,7 +798,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   s = new md_system();
   if (const char* e = getenv("MD_B200_NO_BALANCE")) s->no_balance = atoi(e) != 0;
   if (const char* e = getenv("MD_B200_NO_PERSISTENT")) s->no_persistent = atoi(e) != 0;
-  if (const char* e = getenv("MD_B200_PGROUPS")) s->p_groups = atoi(e) == 1 ? 1 : 2;
+  if (const char* e = getenv("MD_B200_PGROUPS")) s->p_groups = std::min(2, std::max(0, atoi(e)));
   if (const char* e = getenv("MD_B200_PMIN")) s->p_min_tiles_per_sm = std::max(0, atoi(e));
   s->balance_after = BALANCE_AFTER;
   if (const char* e = getenv("MD_B200_BALANCE_AFTER")) s->balance_after = atoi(e);
@@ -951,12 +989,15 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   const int N = (int)s->N;
   const double trigger = 0.25 * s->skin * s->skin;
   const double hdtf = 0.5 * dt * s->ftm2v;
-  {   // per-type kick factor of the fused epilogue (same expression as the integrator kernels: hdtf / m)
+  auto upload_dtf = [&]() -> int {   // per-type kick factor of the fused epilogue (same expression as the integrator kernels: hdtf / m)
     std::vector<double> dtf(s->mass_h.size());
     for (size_t t = 0; t < dtf.size(); ++t) dtf[t] = hdtf / s->mass_h[t];
     CK(cudaMemcpyAsync(s->dtf_d, dtf.data(), dtf.size() * sizeof(double), cudaMemcpyHostToDevice, s->stream));
     CK(cudaStreamSynchronize(s->stream));   // dtf is a stack object
-  }
+    return MD_OK;
+  };
+  rc = upload_dtf();
+  if (rc) return rc;
   const int64_t sample_every = (nsteps + md_system_impl::NSAMPLE - 1) / md_system_impl::NSAMPLE;
   int nsampled = 0;
   s->ms_force_sampled = 0; s->ms_pass1_sampled = 0;
@@ -1022,6 +1063,8 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         // that comes 20 or more time steps later (the timing builds its own lists; the state is left as a build leaves it)
         if (s->kernel_req == MD_KERNEL_AUTO && s->tune_stage == 1 && s->nsteps_total - s->tune_step >= 20) {
           rc = autotune(s, 5, nullptr);
+          if (rc) return rc;
+          rc = upload_dtf();   // the timing ran dt = 0 steps
           if (rc) return rc;
         }
         rc = build(s, false);   // also clears the flags
