@@ -231,12 +231,12 @@ def _flush_l2(torch, scratch):
     scratch.add_(1)      # writes 2 x L2 bytes on the same stream, outside the event-timed region
 
 
-def time_workload(torch, md, w, stream, steps: int, warmup: int, kernel: int, list_kind: int, host_io: bool):
+def time_workload(torch, md, w, stream, steps: int, warmup: int, kernel: int, list_kind: int, host_io: bool, options: dict | None = None):
     """Runs ``warmup`` + ``steps`` passes of the whole hot path for workload ``w``.  Returns per-pass
     device times (ms, CUDA events on ``stream``), the stats of the last pass and launches per pass."""
     N = w.natoms
     with torch.cuda.stream(stream):
-        s = md.from_workload(w, kernel=kernel, list_kind=list_kind, stream=int(stream.cuda_stream))
+        s = md.from_workload(w, kernel=kernel, list_kind=list_kind, stream=int(stream.cuda_stream), options=options)
         if host_io:
             x_in = torch.from_numpy(w.x).pin_memory(); v_in = torch.from_numpy(w.v).pin_memory()
             x_out = torch.empty((N, 3), dtype=torch.float64).pin_memory()
@@ -295,7 +295,8 @@ def run_ours(args, rk) -> None:
     if rk.is_root:
         sampler.start()
     t_region0 = time.perf_counter()
-    dev_run = time_workload(torch, md, w, stream, args.steps, args.warmup, kernel, list_kind, host_io=False)
+    options = {kv.split("=")[0]: int(kv.split("=")[1], 0) for kv in args.opt}
+    dev_run = time_workload(torch, md, w, stream, args.steps, args.warmup, kernel, list_kind, host_io=False, options=options)
     torch.cuda.synchronize(); mdist.barrier(rk)
     t_region1 = time.perf_counter()
     clocks = sampler.stop(t_region0, t_region1) if rk.is_root else None
@@ -304,7 +305,7 @@ def run_ours(args, rk) -> None:
     value, tmax = mdist.aggregate_throughput(rk, units, sum(dev_run["ms"]) * 1e-3)
 
     mdist.barrier(rk)
-    e2e_run = time_workload(torch, md, w, stream, args.steps, min(args.warmup, 3), kernel, list_kind, host_io=True)
+    e2e_run = time_workload(torch, md, w, stream, args.steps, min(args.warmup, 3), kernel, list_kind, host_io=True, options=options)
     e2e_value, _ = mdist.aggregate_throughput(rk, units, sum(e2e_run["wall_ms"]) * 1e-3)
     launches = mdist.all_sum(rk, dev_run["launches"])
 
@@ -417,6 +418,8 @@ def main() -> None:
     ap.add_argument("--all-configs", dest="all_configs", action="store_true", default=True)
     ap.add_argument("--no-all-configs", dest="all_configs", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="md_set_option tuning knob for the bench workload (include/md_b200.h), e.g. --opt tile_shape=0x334; repeatable")
     args = ap.parse_args()
     if args.impl == "reference":
         rank = int(os.environ.get("RANK", "0"))

@@ -114,25 +114,50 @@ typedef struct md_stats {
 } md_stats;
 
 /* Creates a system: orthogonal periodic box [0,Lx) x [0,Ly) x [0,Lz), N atoms with type ids in
- * 0..ntypes-1 (caller order, host or device pointer) and per-type masses (host pointer).
- * stream: a cudaStream_t (void*), NULL for the default stream.  (north_star md_create) */
+ * 0..ntypes-1 (caller order, host or device pointer; ids outside the range are refused) and per-type masses
+ * (host pointer).  stream: a cudaStream_t (void*), NULL for the default stream.
+ * ("N atoms in a periodic box"; north_star md_create(box, N, types)) */
 int md_create(md_system** out, const double box[3], int64_t N, const int32_t* types, int ntypes,
               const double* mass, void* cuda_stream);
+/* Frees the handle and all device memory it owns.  NULL is allowed.  (north_star: the handle owns the device state) */
 void md_destroy(md_system* s);
 
-/* LJ reduced units: (1, 1).  LAMMPS-metal (A, eV, amu, ps): ftm2v = 1/1.0364269e-4, mvv2e = 1.0364269e-4. */
+/* Unit factors of the integrator (PAPER.md L52 NVE; reading s14 of DESIGN.md: the paper runs LAMMPS "metal" units for
+ * the EAM workload, App. A): a = f/m * ftm2v, KE = 1/2 m v^2 * mvv2e.  LJ reduced units: (1, 1).
+ * LAMMPS-metal (A, eV, amu, ps): ftm2v = 1/1.0364269e-4, mvv2e = 1.0364269e-4.  Both must be positive. */
 int md_set_units(md_system* s, double ftm2v, double mvv2e);
-/* MD_FP64 or MD_MIXED.  Invalidates the neighbor list. */
+/* MD_FP64 or MD_MIXED ("single, double and mixed precision"; reading s15).  Invalidates the
+ * neighbor list and the variant choice. */
 int md_set_precision(md_system* s, int mode);
-/* N x 3 doubles, caller order, host or device.  Positions may lie outside the box (they are wrapped at
- * the next build).  Setting positions invalidates the neighbor list and the cached forces. */
+/* Positions (north_star: resident on the device): N x 3 doubles, caller order, host or device.  They may
+ * lie outside the box (wrapped at the next build, reading s5); a non-finite value is reported by the next build as
+ * MD_ERR_NONFINITE.  Setting positions invalidates the neighbor list and the cached forces. */
 int md_set_positions(md_system* s, const double* x);
+/* Velocities (PAPER.md L52 velocity Verlet; reading s17: generated by the caller): N x 3 doubles, caller order,
+ * host or device. */
 int md_set_velocities(md_system* s, const double* v);
-/* One parameter set for all type pairs (single-species potentials; types select masses).
- * Fails with MD_ERR_BOX_TOO_SMALL unless every box edge >= 3 (rc + skin).  (north_star md_set_pair) */
+/* Pair style, its parameters (see MD_PAIR_*), cutoff rc and skin (PAPER.md L86-98 neighbor lists with a skin, App. A
+ * L256/L260; north_star md_set_pair(style, params, rc, skin)).  One parameter set for all type pairs (types select
+ * masses).  The interaction is r^2 < rc^2 strictly (reading s3).  Fails with MD_ERR_BOX_TOO_SMALL unless every box
+ * edge >= 3 (rc + skin) (reading s19), MD_ERR_BAD_ARGUMENT for a wrong parameter count or a non-finite value. */
 int md_set_pair(md_system* s, int style, const double* params, int nparams, double rc, double skin);
-/* list_kind: MD_LIST_FULL | MD_LIST_HALF; kernel: MD_KERNEL_*.  HALF needs TPA.  Invalidates the list. */
+/* list_kind: MD_LIST_FULL | MD_LIST_HALF (PAPER.md L76 Newton's third law, L104 full list; reading s6);
+ * kernel: MD_KERNEL_* (PAPER.md L88-122 TpA/BpA, L64-82 cell list, L137 choice by timing).  HALF needs TPA or AUTO.
+ * Invalidates the list. */
 int md_set_neighbor(md_system* s, int list_kind, int kernel);
+
+/* Tuning knobs for measurements (profiles/; none is needed in normal use: the planner and md_autotune set
+ * all of them; SURVEY.md 8(f)-1 sweeps use them).  Invalidates the list and the variant choice.  Names:
+ *   "tile_shape"  bx | by << 4 | bz << 8 cells per tile (4 >= bx >= by >= bz >= 1), 0: planner
+ *   "force_threads"  block size of the list force kernels, 0: planner
+ *   "persistent_groups"  consumer groups of the persistent force kernel: 1, 2, or 0 = automatic
+ *   "persistent_min_tiles_per_sm"  the persistent kernel is used from this many tiles per SM on (default 1)
+ *   "no_persistent"  1: run the one-block-per-tile kernel everywhere
+ *   "balance_after"  apply the row balancing to a list that has lived this many steps (default 48; <= 0: at every build)
+ *   "no_balance"  1: never
+ *   "tune_verbose"  1: md_autotune prints every candidate's timing to stderr
+ * Unknown names and values out of range return MD_ERR_BAD_ARGUMENT. */
+int md_set_option(md_system* s, const char* name, int64_t value);
 
 /* Wrap into the box, bin into cells of edge >= rc+skin, counting-sort and reorder atoms, build the
  * Verlet list from the 27-cell stencil (fp64 distance test r^2 < (rc+skin)^2), reset x0.
@@ -150,16 +175,20 @@ int md_compute_forces(md_system* s, double* f_out, double* energy_out, double vi
  * rebuild decisions.  (north_star md_run) */
 int md_run(md_system* s, int64_t nsteps, double dt);
 
-/* Current state in caller order (host or device buffers of N x 3 doubles).  Positions are as stored:
- * inside the box at the last build, possibly slightly outside since. */
+/* Current positions in caller order (host or device buffer of N x 3 doubles, reading s5): as stored,
+ * i.e. inside the box at the last build, possibly slightly outside since.  MD_ERR_NOT_READY before md_set_positions. */
 int md_get_positions(md_system* s, double* x);
+/* Current velocities in caller order: at whole time steps after md_run. */
 int md_get_velocities(md_system* s, double* v);
-/* Forces of the last evaluation (md_compute_forces or the last step of md_run). */
+/* Forces of the last evaluation (md_compute_forces, or the last step of md_run: PAPER.md L52, the forces that belong
+ * to the final positions).  MD_ERR_NOT_READY if there is none. */
 int md_get_forces(md_system* s, double* f);
 
-/* The current neighbor list in CALLER ids, for pair-set parity: numneigh[N] and neigh[N x stride]
- * (host or device int32 buffers).  Rows longer than stride are truncated (numneigh still holds the true
- * length).  Half lists hold each unordered pair in exactly one of the two rows. */
+/* The current neighbor list in CALLER ids, for pair-set parity (numneigh[i], neighbors[i][jj];
+ * north_star (2): "neighbor pair sets identical"): numneigh[N] and neigh[N x stride] (host or device int32 buffers),
+ * exactly the pairs with |x_i - x_j|^2 < (rc+skin)^2 in fp64 at the current positions among the stored rows.  Rows
+ * longer than stride are truncated (numneigh still holds the true length).  Half lists hold each unordered pair in
+ * exactly one of the two rows.  Builds the list first if it is not valid. */
 int md_get_neighbors(md_system* s, int32_t* numneigh, int32_t* neigh, int64_t stride);
 
 /* The STORED list rows as they are, for checking the build itself (north_star (2)).
@@ -175,15 +204,22 @@ int md_get_neighbor_rows(md_system* s, int32_t* row_owner, int32_t* numrow, int3
  * (NVE; the metric a time-stepping caller reads back.) */
 int md_kinetic_energy(md_system* s, double* ke_out);
 
-/* Setup-time mini benchmark of PAPER.md L137: on the current positions, builds the list and times nrep
- * force evaluations with each of TPA, SUBWARP, WARP, SUBWARP4 and SUBWARP2, at the planner's tile width and its two
- * neighbours; keeps the combination with the lowest (force evaluation + 1/8 list build) time, and
- * reports the best force time of each variant (ms per evaluation, in the order TPA, SUBWARP, WARP,
- * SUBWARP4, SUBWARP2) if ms_out is not NULL.  MD_KERNEL_AUTO runs it once before the first build. */
+/* Setup-time mini benchmark of PAPER.md L137 ("the faster variant is chosen by timing at setup"): on the current
+ * positions, builds the list and times nrep (rounded up to an even number) FUSED time-step kernels with dt = 0 (force
+ * evaluation + kick + drift epilogue: what md_run runs; positions and velocities keep their values) with each of TPA,
+ * SUBWARP, WARP, SUBWARP4 and SUBWARP2 and, on boxes with fewer than 2048 tiles, at the planner's tile shape and its
+ * neighbours in the list of feasible shapes; keeps the combination with the lowest (step + 1/8 list build) time and
+ * reports the best step time of each variant (ms, in the order TPA, SUBWARP, WARP, SUBWARP4, SUBWARP2) if ms_out is
+ * not NULL.  MD_KERNEL_AUTO runs it before the first build and once more inside md_run, at the first rebuild that comes
+ * 20 or more time steps later (the caller's positions are often a perfect lattice).  Half lists always use TPA. */
 int md_autotune(md_system* s, int nrep, double ms_out[5]);
 
+/* Counters, geometry and timers (see md_stats; what bench.py reports).  Counts the exact neighbor
+ * statistics on demand and reads the kinetic energy, so it synchronises the stream. */
 int md_get_stats(md_system* s, md_stats* out);
-const char* md_last_error(const md_system* s); /* s may be NULL: error of a failed md_create */
+/* Text of the last failure of this handle (north_star: errors are codes, never throws).  s may be NULL: the error of
+ * a failed md_create on this thread. */
+const char* md_last_error(const md_system* s);
 
 #ifdef __cplusplus
 }

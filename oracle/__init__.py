@@ -23,6 +23,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 
 PAIR_LJ = 1
 PAIR_EAM = 2
+PAIR_BUCK_COUL = 3   # params: dict(k=Coulomb constant, types=int32[N], q=float[ntypes], coef=float[ntypes, ntypes, 3] = A, rho, C)
 
 
 def build(force: bool = False) -> str:
@@ -35,15 +36,33 @@ def build(force: bool = False) -> str:
 
 
 class _Pair(ctypes.Structure):
-    _fields_ = [("style", ctypes.c_int), ("p", ctypes.c_double * 5), ("rc", ctypes.c_double)]
+    _fields_ = [("style", ctypes.c_int), ("p", ctypes.c_double * 5), ("rc", ctypes.c_double),
+                ("type", ctypes.POINTER(ctypes.c_int32)), ("ntypes", ctypes.c_int),
+                ("coef", ctypes.POINTER(ctypes.c_double)), ("qtype", ctypes.POINTER(ctypes.c_double))]
 
 
 def _pair(style: int, params, rc: float) -> _Pair:
     p = _Pair()
     p.style = int(style)
+    p.rc = float(rc)
+    if style == PAIR_BUCK_COUL:
+        types = np.ascontiguousarray(params["types"], dtype=np.int32)
+        q = np.ascontiguousarray(params["q"], dtype=np.float64)
+        coef = np.ascontiguousarray(params["coef"], dtype=np.float64)
+        nt = len(q)
+        if coef.shape != (nt, nt, 3) or types.min() < 0 or types.max() >= nt:
+            raise ValueError("buck/coul: coef must be [ntypes, ntypes, 3] and types must lie in 0..ntypes-1")
+        if not np.array_equal(coef, coef.transpose(1, 0, 2)):
+            raise ValueError("buck/coul: the coefficient table must be symmetric in the two types")
+        p.p[0] = float(params["k"])
+        p._keep = (types, q, coef)               # the struct only holds pointers
+        p.type = types.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+        p.ntypes = nt
+        p.coef = coef.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        p.qtype = q.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        return p
     for k, val in enumerate(params):
         p.p[k] = float(val)
-    p.rc = float(rc)
     return p
 
 

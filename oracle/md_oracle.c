@@ -21,6 +21,10 @@
  *                 (App. A, refs 11,12; the functional form is
  *                 BASELINE.json cfg 4: phi = A exp(-p(r/r0-1)),
  *                 rho = exp(-q(r/r0-1)), F = -B sqrt(rho); reading s12, s13)
+ *   Buckingham + cutoff Coulomb (App. A, the "silicate (cutoff)" workload, LAMMPS
+ *                 style buck/coul/cut named there): per type pair (a,b)
+ *                 u(r) = A_ab exp(-r/rho_ab) - C_ab / r^6 + k q_a q_b / r,  r^2 < rc^2, plain truncation of all three
+ *                 terms at one cutoff; charges per TYPE (the paper's silicate has one charge per species).
  *   NVE           velocity Verlet ("NVE ... integrators"):
  *                 v += dt/2 f/m ftm2v; x += dt v; f = F(x); v += dt/2 f/m ftm2v
  *   neighbor list loop of PAPER.md L88-104 (TpA pseudo-code): for each i, for
@@ -52,11 +56,17 @@
 
 #define ORC_PAIR_LJ 1
 #define ORC_PAIR_EAM 2
+#define ORC_PAIR_BUCK_COUL 3
 
 typedef struct {
-  int style;        /* ORC_PAIR_LJ or ORC_PAIR_EAM */
-  double p[5];      /* LJ: eps, sigma ; EAM: A, p, B, q, r0 */
+  int style;        /* ORC_PAIR_LJ, ORC_PAIR_EAM or ORC_PAIR_BUCK_COUL */
+  double p[5];      /* LJ: eps, sigma ; EAM: A, p, B, q, r0 ; BUCK_COUL: k (the Coulomb constant, e.g. 14.399645 eV A / e^2) */
   double rc;
+  /* ORC_PAIR_BUCK_COUL only (NULL / 0 otherwise) */
+  const int32_t* type;   /* [N] type of every atom, 0..ntypes-1 */
+  int ntypes;
+  const double* coef;    /* [ntypes][ntypes][3]: A, rho, C of the type pair (symmetric) */
+  const double* qtype;   /* [ntypes] charge of a type */
 } orc_pair;
 
 int orc_max_threads(void) {
@@ -85,6 +95,24 @@ static void lj_pair(const orc_pair* P, double r2, double* u, double* fpair) {
   double s6 = s2 * s2 * s2;
   *u = 4.0 * eps * (s6 * s6 - s6);
   *fpair = 24.0 * eps * (2.0 * s6 * s6 - s6) / r2;
+}
+
+/* Buckingham + cutoff Coulomb for the type pair (ta, tb): u and fpair = -(1/r) du/dr.
+ * du/dr = -(A/rho) exp(-r/rho) + 6 C / r^7 - k qa qb / r^2. */
+static void buck_coul_pair(const orc_pair* P, int ta, int tb, double r2, double* u, double* fpair) {
+  const double* c = P->coef + 3 * ((size_t)ta * P->ntypes + tb);
+  double A = c[0], rho = c[1], C = c[2], kqq = P->p[0] * P->qtype[ta] * P->qtype[tb];
+  double r = sqrt(r2), r6 = r2 * r2 * r2;
+  double ex = A * exp(-r / rho);
+  *u = ex - C / r6 + kqq / r;
+  *fpair = (ex / rho - 6.0 * C / (r6 * r) + kqq / r2) / r;
+}
+
+/* the pairwise (non-EAM) styles: one term of atoms i and j */
+static void lj_pair(const orc_pair* P, double r2, double* u, double* fpair);
+static void pairwise(const orc_pair* P, int64_t i, int64_t j, double r2, double* u, double* fpair) {
+  if (P->style == ORC_PAIR_BUCK_COUL) buck_coul_pair(P, P->type[i], P->type[j], r2, u, fpair);
+  else lj_pair(P, r2, u, fpair);
 }
 
 /* EAM pieces (BASELINE.json cfg 4). */
@@ -130,14 +158,14 @@ void orc_forces_brute(int64_t N, const double* x, const double* box, const orc_p
   double rc2 = P->rc * P->rc, e = 0.0, w[6] = {0, 0, 0, 0, 0, 0};
   int64_t np = 0;
   zero(f, 3 * N);
-  if (P->style == ORC_PAIR_LJ) {
+  if (P->style != ORC_PAIR_EAM) {
     for (int64_t i = 0; i < N; ++i)
       for (int64_t j = i + 1; j < N; ++j) {
         double D[3], r2 = 0.0;
         for (int a = 0; a < 3; ++a) { D[a] = min_image(x[3 * i + a] - x[3 * j + a], box[a]); r2 += D[a] * D[a]; }
         if (r2 < rc2) {
           double u, fp;
-          lj_pair(P, r2, &u, &fp);
+          pairwise(P, i, j, r2, &u, &fp);
           for (int a = 0; a < 3; ++a) { f[3 * i + a] += fp * D[a]; f[3 * j + a] -= fp * D[a]; }
           e += u; add_virial(w, D, fp); ++np;
         }
@@ -181,12 +209,12 @@ void orc_forces_sample(int64_t N, const double* x, const double* box, const orc_
   for (int64_t s = 0; s < ns; ++s) {
     int64_t i = ids[s];
     double fi[3] = {0, 0, 0}, e = 0.0;
-    if (P->style == ORC_PAIR_LJ) {
+    if (P->style != ORC_PAIR_EAM) {
       for (int64_t j = 0; j < N; ++j) {
         if (j == i) continue;
         double D[3], r2 = 0.0;
         for (int a = 0; a < 3; ++a) { D[a] = min_image(x[3 * i + a] - x[3 * j + a], box[a]); r2 += D[a] * D[a]; }
-        if (r2 < rc2) { double u, fp; lj_pair(P, r2, &u, &fp); for (int a = 0; a < 3; ++a) fi[a] += fp * D[a]; e += 0.5 * u; }
+        if (r2 < rc2) { double u, fp; pairwise(P, i, j, r2, &u, &fp); for (int a = 0; a < 3; ++a) fi[a] += fp * D[a]; e += 0.5 * u; }
       }
     } else {
       double rho_i = 0.0;
@@ -356,7 +384,7 @@ void orc_forces_list(int64_t N, const double* x, const double* box, const orc_pa
       for (int a = 0; a < 3; ++a) { D[a] = min_image(x[3 * i + a] - x[3 * j + a], box[a]); r2 += D[a] * D[a]; }
       if (r2 < rc2) {
         double u, fp;
-        if (P->style == ORC_PAIR_LJ) lj_pair(P, r2, &u, &fp);
+        if (P->style != ORC_PAIR_EAM) pairwise(P, i, j, r2, &u, &fp);
         else { double r = sqrt(r2); u = eam_phi(P, r); fp = -((dF[i] + dF[j]) * eam_drho(P, r) + eam_dphi(P, r)) / r; }
         for (int a = 0; a < 3; ++a) ftmp[a] += fp * D[a];
         e += 0.5 * u;

@@ -64,6 +64,9 @@ struct md_system_impl {
   int p_groups = 0;             // consumer groups of the persistent force kernel; 0: two if three tile buffers fit, else one (MD_B200_PGROUPS)
   bool no_persistent = false;   // MD_B200_NO_PERSISTENT=1: run k_tile_force where k_tile_force_p would be used (A/B measurements)
   int brick_forced = 0;   // tile shape chosen by the autotuner, bx | by << 4 | bz << 8 (0: the planner's own pick)
+  int opt_tile_shape = 0;     // md_set_option("tile_shape"): bx | by << 4 | bz << 8, 0: planner
+  int opt_force_threads = 0;  // md_set_option("force_threads"): block size of the list force kernels, 0: planner
+  bool tune_verbose = false;  // md_set_option("tune_verbose")
   int shape_index = 0, shape_count = 0, build_threads = 256;
   int shape_codes[64] = {};   // the feasible tile shapes of the last plan(), largest first (bx | by << 4 | bz << 8)
   double *f = nullptr, *x0 = nullptr, *rho = nullptr, *fp = nullptr;
@@ -314,7 +317,7 @@ int plan(md_system* s) {
   // of pass 0 (all), pass 1 (all but the tile count) or pass 2 (none)
   int feasible[64], nfeas = 0, pick = -1;
   int forced_shape[3] = {0, 0, 0};
-  if (const char* e = getenv("MD_B200_BRICK_XYZ")) sscanf(e, "%d,%d,%d", &forced_shape[0], &forced_shape[1], &forced_shape[2]);
+  if (s->opt_tile_shape) { forced_shape[0] = s->opt_tile_shape & 15; forced_shape[1] = (s->opt_tile_shape >> 4) & 15; forced_shape[2] = (s->opt_tile_shape >> 8) & 15; }
   for (int i = 0; i < nshapes; ++i) {
     fill_geom_for_b(s, shapes[i].b, g);
     if (g.b[0] != shapes[i].b[0] || g.b[1] != shapes[i].b[1] || g.b[2] != shapes[i].b[2]) continue;   // wider than the box
@@ -378,7 +381,7 @@ int plan(md_system* s) {
     int t = (int)std::ceil(lanes / std::max(rounds, 1));
     t = ((t + 31) / 32) * 32;
     s->force_threads = std::min(std::max(t, 32), tmax);
-    if (const char* e = getenv("MD_B200_THREADS")) s->force_threads = std::min(std::max(atoi(e) / 32 * 32, 32), tmax);
+    if (s->opt_force_threads) s->force_threads = std::min(std::max(s->opt_force_threads / 32 * 32, 32), tmax);
   }
   // pair constants
   PairParams& P = s->P;
@@ -714,7 +717,7 @@ int autotune(md_system* s, int nrep, double* ms_out) {
       s->cap_scale_tile = s->cap_scale_int = s->cap_scale_row = 1.0;   // an overflow of one shape must not inflate the next
       s->planned = false;
       rc = build(s, true);
-      if (rc && getenv("MD_B200_TUNE_VERBOSE"))
+      if (rc && s->tune_verbose)
         fprintf(stderr, "autotune: K=%d shape %d (%dx%dx%d): build failed (%d) %s\n", lanes_for(cand[k]), idx, s->g.b[0], s->g.b[1], s->g.b[2], rc, s->err.c_str());
       if (rc == MD_ERR_OVERFLOW && idx != i0) continue;   // this shape does not fit with this many lanes per row
       if (rc) return rc;
@@ -734,7 +737,7 @@ int autotune(md_system* s, int nrep, double* ms_out) {
       float ms = 0;
       cudaEventElapsedTime(&ms, s->ev4, s->ev5);
       const double per = ms / nrep, score = per + ms_build / 8.0;
-      if (getenv("MD_B200_TUNE_VERBOSE"))
+      if (s->tune_verbose)
         fprintf(stderr, "autotune: K=%d shape %d of %d (%dx%dx%d) tiles %d threads %d step %.4f ms build %.4f ms score %.4f\n", lanes_for(cand[k]), idx,
                 nfeas, s->g.b[0], s->g.b[1], s->g.b[2], s->g.ntiles, s->force_threads, per, ms_build, score);
       if (ms_out && per < ms_out[k]) ms_out[k] = per;
@@ -796,12 +799,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   for (int t = 0; t < ntypes; ++t)
     if (!(mass[t] > 0.0)) return fail(nullptr, MD_ERR_BAD_ARGUMENT, "md_create: masses must be positive");
   s = new md_system();
-  if (const char* e = getenv("MD_B200_NO_BALANCE")) s->no_balance = atoi(e) != 0;
-  if (const char* e = getenv("MD_B200_NO_PERSISTENT")) s->no_persistent = atoi(e) != 0;
-  if (const char* e = getenv("MD_B200_PGROUPS")) s->p_groups = std::min(2, std::max(0, atoi(e)));
-  if (const char* e = getenv("MD_B200_PMIN")) s->p_min_tiles_per_sm = std::max(0, atoi(e));
   s->balance_after = BALANCE_AFTER;
-  if (const char* e = getenv("MD_B200_BALANCE_AFTER")) s->balance_after = atoi(e);
   auto bail = [&](int code) { std::string e = s->err; md_destroy(s); g_create_error = e; return code; };
   {
     int dev = 0, sms = 0;
@@ -881,6 +879,38 @@ int md_set_units(md_system* s, double ftm2v, double mvv2e) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (!(ftm2v > 0.0) || !(mvv2e > 0.0)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_units: factors must be positive");
   s->ftm2v = ftm2v; s->mvv2e = mvv2e;
+  return MD_OK;
+}
+
+int md_set_option(md_system* s, const char* name, int64_t value) {
+  if (!s || !name) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_option: NULL") : MD_ERR_BAD_ARGUMENT;
+  const std::string n(name);
+  if (n == "tile_shape") {
+    const int bx = (int)(value & 15), by = (int)((value >> 4) & 15), bz = (int)((value >> 8) & 15);
+    if (value != 0 && (value < 0 || value > 0xfff || bx < 1 || bx > 4 || by < 1 || by > bx || bz < 1 || bz > by))
+      return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_option: tile_shape wants bx | by << 4 | bz << 8 with 4 >= bx >= by >= bz >= 1, or 0");
+    s->opt_tile_shape = (int)value;
+  } else if (n == "force_threads") {
+    if (value < 0 || value > 1024) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_option: force_threads wants 0..1024");
+    s->opt_force_threads = (int)value;
+  } else if (n == "balance_after") {
+    s->balance_after = (int)std::max<int64_t>(-1, std::min<int64_t>(value, 1 << 30));
+  } else if (n == "no_balance") {
+    s->no_balance = value != 0;
+  } else if (n == "no_persistent") {
+    s->no_persistent = value != 0;
+  } else if (n == "persistent_groups") {
+    if (value < 0 || value > 2) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_option: persistent_groups wants 0 (automatic), 1 or 2");
+    s->p_groups = (int)value;
+  } else if (n == "persistent_min_tiles_per_sm") {
+    if (value < 0) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_option: persistent_min_tiles_per_sm wants >= 0");
+    s->p_min_tiles_per_sm = (int)std::min<int64_t>(value, 1 << 20);
+  } else if (n == "tune_verbose") {
+    s->tune_verbose = value != 0;
+  } else {
+    return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_option: unknown option '%s'", name);
+  }
+  s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->tune_stage = 0; s->brick_forced = 0;
   return MD_OK;
 }
 

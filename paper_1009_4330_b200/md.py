@@ -27,7 +27,7 @@ EXPORTS = [
     "md_create", "md_destroy", "md_set_units", "md_set_precision", "md_set_positions", "md_set_velocities",
     "md_set_pair", "md_set_neighbor", "md_build_neighbors", "md_compute_forces", "md_run", "md_get_positions",
     "md_get_velocities", "md_get_forces", "md_get_neighbors", "md_get_neighbor_rows", "md_kinetic_energy", "md_autotune",
-    "md_get_stats", "md_last_error",
+    "md_get_stats", "md_last_error", "md_set_option",
 ]
 
 
@@ -88,6 +88,7 @@ def _load():
     L.md_get_neighbors.argtypes = [vp, ip, ip, ctypes.c_int64]
     L.md_get_neighbor_rows.argtypes = [vp, ip, ip, ip, ctypes.c_int64]
     L.md_kinetic_energy.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    L.md_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int64]
     L.md_autotune.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     L.md_get_stats.argtypes = [vp, ctypes.POINTER(md_stats)]
     L.md_last_error.argtypes = [vp]
@@ -206,6 +207,9 @@ class System:
         self._ck(lib.md_get_neighbor_rows(self._h, _addr(row_owner, np.int32, self.natoms), _addr(numrow, np.int32, self.natoms),
                                           _addr(entries, np.int32, self.natoms * stride), stride))
 
+    def md_set_option(self, name: str, value: int):
+        self._ck(lib.md_set_option(self._h, name.encode(), int(value)))
+
     def md_kinetic_energy(self) -> float:
         ke = ctypes.c_double(0.0)
         self._ck(lib.md_kinetic_energy(self._h, ctypes.byref(ke)))
@@ -223,12 +227,14 @@ class System:
 
 
 def from_workload(w, precision: int | None = None, list_kind: int = MD_LIST_FULL, kernel: int = MD_KERNEL_TPA,
-                  x=None, stream: int | None = None) -> System:
+                  x=None, stream: int | None = None, options: dict | None = None) -> System:
     """Convenience: a System configured from a ``workloads.Workload`` (marshalling only)."""
     s = System(w.box, w.natoms, w.types, w.mass, stream=stream)
     s.md_set_units(w.ftm2v, w.mvv2e)
     s.md_set_precision(w.precision if precision is None else precision)
     s.md_set_neighbor(list_kind, kernel)
+    for name, value in (options or {}).items():
+        s.md_set_option(name, value)
     s.md_set_pair(w.style, w.params, w.rc, w.skin)
     s.md_set_positions(np.ascontiguousarray(w.x if x is None else x))
     s.md_set_velocities(np.ascontiguousarray(w.v))

@@ -458,6 +458,31 @@ def test_error_paths():
         md.System(np.array([1.0, -1.0, 1.0]), 4, np.zeros(4, np.int32), np.array([1.0]))
     with pytest.raises(md.MDError):
         md.System(box, 0, np.zeros(0, np.int32), np.array([1.0]))
+    for name, value in [("no_such_option", 1), ("tile_shape", 0x135), ("tile_shape", 0x511), ("persistent_groups", 3), ("force_threads", -32)]:
+        with pytest.raises(md.MDError) as e:
+            s.md_set_option(name, value)
+        assert e.value.code == md.MD_ERR_BAD_ARGUMENT
+
+
+@pytest.mark.parametrize("options", [{"tile_shape": 0x111}, {"tile_shape": 0x112, "no_persistent": 1}, {"persistent_groups": 1},
+                                     {"force_threads": 64, "balance_after": 0}])
+def test_tuning_options_change_the_plan_not_the_result(options):
+    """md_set_option knobs (tile shape, block size, persistent-kernel layout, row balancing) must leave forces and energy
+    within the mixed-precision tolerance of the brute-force oracle."""
+    w = wl.make(2, n_override=8)
+    x = wl.perturbed(w, 0.12)
+    fo, Eo = oracle.forces_brute(x, w.box, w.style, w.params, w.rc)[:2]
+    s = md.from_workload(w, x=x, options=options)
+    f = np.zeros((w.natoms, 3))
+    E, _ = s.md_compute_forces(f, energy=True)
+    assert _rel_rms(f, fo) < 1e-5 and abs(E - Eo) < 1e-6 * abs(Eo)
+    if "tile_shape" in options:
+        b = options["tile_shape"]
+        assert s.md_get_stats()["brick"] == [b & 15, (b >> 4) & 15, (b >> 8) & 15]
+    s.md_run(30, w.dt)
+    xg = np.zeros((w.natoms, 3)); s.md_get_positions(xg); s.md_get_forces(f)
+    assert _rel_rms(f, oracle.forces(xg, w.box, w.style, w.params, w.rc)[0]) < 1e-5
+    s.close()
 
 
 def test_sparse_gas_empty_cells_and_zero_steps():
