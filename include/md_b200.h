@@ -63,6 +63,11 @@ typedef struct md_system md_system; /* opaque */
 #define MD_PAIR_EAM_FS 2  /* params = {A, p, B, q, r0}: phi = A exp(-p(r/r0-1)), rho = exp(-q(r/r0-1)),
                              F(rho) = -B sqrt(rho), F'(0) := 0; E = sum_i F(rho_i) + 1/2 sum_ij phi (L260) */
 
+#define MD_PAIR_BUCK_COUL 3 /* params = {k}: u_ab = A_ab exp(-r/rho_ab) - C_ab/r^6 + k q_a q_b / r, all three terms cut plainly at rc
+                             (App. A "silicate (cutoff)", LAMMPS buck/coul/cut).  Per type pair
+                             A, rho, C by md_set_pair_coeff, per type charge by md_set_type_charges; at most 4 types;
+                             k = 14.399645 eV A / e^2 in metal units */
+
 /* neighbor-list kinds */
 #define MD_LIST_FULL 0    /* both (i,j) and (j,i): each kernel row writes only f[i] (L104) */
 #define MD_LIST_HALF 1    /* each pair once; -F scattered to j with atomics (Newton's third law, L76) */
@@ -137,10 +142,17 @@ int md_set_positions(md_system* s, const double* x);
  * host or device. */
 int md_set_velocities(md_system* s, const double* v);
 /* Pair style, its parameters (see MD_PAIR_*), cutoff rc and skin (PAPER.md L86-98 neighbor lists with a skin, App. A
- * L256/L260; north_star md_set_pair(style, params, rc, skin)).  One parameter set for all type pairs (types select
- * masses).  The interaction is r^2 < rc^2 strictly (reading s3).  Fails with MD_ERR_BOX_TOO_SMALL unless every box
+ * L256/L260; north_star md_set_pair(style, params, rc, skin)).  MD_PAIR_LJ126 and MD_PAIR_EAM_FS take one parameter set for all
+ * type pairs (types select masses); MD_PAIR_BUCK_COUL takes per-type-pair coefficients through md_set_pair_coeff.  The interaction is r^2 < rc^2 strictly (reading s3).  Fails with MD_ERR_BOX_TOO_SMALL unless every box
  * edge >= 3 (rc + skin) (reading s19), MD_ERR_BAD_ARGUMENT for a wrong parameter count or a non-finite value. */
 int md_set_pair(md_system* s, int style, const double* params, int nparams, double rc, double skin);
+/* MD_PAIR_BUCK_COUL only: the coefficients {A, rho, C} (n = 3) of the type pair (a, b) and, by symmetry, (b, a)
+ * (App. A "26 pair force styles": per-type-pair coefficients as in LAMMPS pair_coeff).  Every pair of
+ * the system's types must be set before the next force evaluation (MD_ERR_NOT_READY otherwise); rho must be positive. */
+int md_set_pair_coeff(md_system* s, int type_a, int type_b, const double* coeff, int n);
+/* MD_PAIR_BUCK_COUL only: the charge of every atom type, n = ntypes values (the paper's silicate carries one charge per
+ * species, App. A).  Host pointer. */
+int md_set_type_charges(md_system* s, const double* q, int n);
 /* list_kind: MD_LIST_FULL | MD_LIST_HALF (PAPER.md L76 Newton's third law, L104 full list; reading s6);
  * kernel: MD_KERNEL_* (PAPER.md L88-122 TpA/BpA, L64-82 cell list, L137 choice by timing).  HALF needs TPA or AUTO.
  * Invalidates the list. */

@@ -36,6 +36,10 @@ struct md_system_impl {
   int precision = MD_FP64;
   int style = 0;
   double params[5] = {0, 0, 0, 0, 0};
+  // MD_PAIR_BUCK_COUL: per type pair A, rho, C (md_set_pair_coeff) and per type charge (md_set_type_charges)
+  double pair_coef[MAX_PAIR_TYPES][MAX_PAIR_TYPES][3] = {};
+  bool pair_coef_set[MAX_PAIR_TYPES][MAX_PAIR_TYPES] = {};
+  double qtype[MAX_PAIR_TYPES] = {0, 0, 0, 0};
   double rc = 0, skin = 0;
   int list_kind = MD_LIST_FULL;
   int kernel_req = MD_KERNEL_TPA;
@@ -391,6 +395,15 @@ int plan(md_system* s) {
     double eps = s->params[0], sg = s->params[1];
     double s6 = std::pow(sg, 6), s12 = s6 * s6;
     P.lj1 = 48.0 * eps * s12; P.lj2 = 24.0 * eps * s6; P.lj3 = 4.0 * eps * s12; P.lj4 = 4.0 * eps * s6;
+  } else if (s->style == MD_PAIR_BUCK_COUL) {
+    if (s->ntypes > MAX_PAIR_TYPES) return fail(s, MD_ERR_BAD_ARGUMENT, "MD_PAIR_BUCK_COUL supports at most %d atom types", MAX_PAIR_TYPES);
+    for (int a = 0; a < s->ntypes; ++a)
+      for (int b = 0; b < s->ntypes; ++b) {
+        if (!s->pair_coef_set[a][b]) return fail(s, MD_ERR_NOT_READY, "md_set_pair_coeff has not been called for the type pair (%d, %d)", a, b);
+        double* e = P.bc[MAX_PAIR_TYPES * a + b];
+        e[0] = s->pair_coef[a][b][0]; e[1] = 1.0 / s->pair_coef[a][b][1]; e[2] = s->pair_coef[a][b][2];
+        e[3] = s->params[0] * s->qtype[a] * s->qtype[b];
+      }
   } else {
     P.A = s->params[0]; P.p = s->params[1]; P.B = s->params[2]; P.q = s->params[3];
     P.inv_r0 = 1.0 / s->params[4]; P.p_r0 = P.p * P.inv_r0; P.q_r0 = P.q * P.inv_r0;
@@ -627,6 +640,10 @@ int launch_force_T(md_system* s, const StepMode& M) {
   A.dt = M.dt; A.half_dt_ftm2v = M.hdtf; A.trigger = M.trigger; A.flags = s->flags_d;
   if (s->style == MD_PAIR_LJ126) {
     int rc = launch_force_variant<T, LJBody, 0, EV>(s, A);
+    if (rc) return rc;
+    if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
+  } else if (s->style == MD_PAIR_BUCK_COUL) {
+    int rc = launch_force_variant<T, BuckCoulBody, 0, EV>(s, A);
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
   } else {
@@ -936,7 +953,7 @@ int md_set_velocities(md_system* s, const double* v) {
 
 int md_set_pair(md_system* s, int style, const double* params, int nparams, double rc, double skin) {
   if (!s || !params) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: NULL") : MD_ERR_BAD_ARGUMENT;
-  int need = style == MD_PAIR_LJ126 ? 2 : (style == MD_PAIR_EAM_FS ? 5 : -1);
+  int need = style == MD_PAIR_LJ126 ? 2 : (style == MD_PAIR_EAM_FS ? 5 : (style == MD_PAIR_BUCK_COUL ? 1 : -1));
   if (need < 0) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: unknown style %d", style);
   if (nparams != need) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: style %d takes %d parameters, got %d", style, need, nparams);
   if (!(rc > 0.0) || !(skin >= 0.0) || !std::isfinite(rc) || !std::isfinite(skin)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: bad rc/skin");
@@ -950,6 +967,30 @@ int md_set_pair(md_system* s, int style, const double* params, int nparams, doub
   for (int k = 0; k < 5; ++k) s->params[k] = k < need ? params[k] : 0.0;
   s->rc = rc; s->skin = skin;
   s->pair_set = true; s->planned = false; s->list_valid = false; s->forces_valid = false; s->autotuned = false; s->tune_stage = 0; s->brick_forced = 0;
+  return MD_OK;
+}
+
+int md_set_pair_coeff(md_system* s, int type_a, int type_b, const double* c, int n) {
+  if (!s || !c) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair_coeff: NULL") : MD_ERR_BAD_ARGUMENT;
+  if (type_a < 0 || type_b < 0 || type_a >= s->ntypes || type_b >= s->ntypes || type_a >= MAX_PAIR_TYPES || type_b >= MAX_PAIR_TYPES)
+    return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair_coeff: types must lie in 0..min(ntypes, %d)-1", MAX_PAIR_TYPES);
+  if (n != 3) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair_coeff: MD_PAIR_BUCK_COUL takes 3 coefficients {A, rho, C}, got %d", n);
+  if (!std::isfinite(c[0]) || !std::isfinite(c[1]) || !std::isfinite(c[2]) || !(c[1] > 0.0))
+    return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair_coeff: coefficients must be finite and rho positive");
+  for (int k = 0; k < 3; ++k) s->pair_coef[type_a][type_b][k] = s->pair_coef[type_b][type_a][k] = c[k];
+  s->pair_coef_set[type_a][type_b] = s->pair_coef_set[type_b][type_a] = true;
+  s->planned = false; s->forces_valid = false;
+  return MD_OK;
+}
+
+int md_set_type_charges(md_system* s, const double* q, int n) {
+  if (!s || !q) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_type_charges: NULL") : MD_ERR_BAD_ARGUMENT;
+  if (n != s->ntypes || n > MAX_PAIR_TYPES) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_type_charges: wants ntypes (<= %d) charges", MAX_PAIR_TYPES);
+  for (int k = 0; k < n; ++k) {
+    if (!std::isfinite(q[k])) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_type_charges: non-finite charge");
+    s->qtype[k] = q[k];
+  }
+  s->planned = false; s->forces_valid = false;
   return MD_OK;
 }
 

@@ -605,9 +605,10 @@ __global__ void k_permute(Geom g, int N, const int* __restrict__ perm, const dou
     vo[d * ld + n] = vi[d * ld + k];
     r[d] = (T)(p - cell_anchor_1d(g, d, cell_index_1d(g, d, p)));
   }
-  xr[n] = make_v4<T>(r[0], r[1], r[2], (T)0);
+  const int ty = typei[k];
+  xr[n] = make_v4<T>(r[0], r[1], r[2], (T)ty);   // w: the atom's type (read by the multi-type pair styles; EAM overwrites it with -F')
   ido[n] = idi[k];
-  typeo[n] = typei[k];
+  typeo[n] = ty;
 }
 
 // caller order <-> sorted order
@@ -1211,6 +1212,7 @@ __device__ __forceinline__ d64x2 pk_mul(d64x2 x, d64x2 y) { return d64x2{x.a * y
 __device__ __forceinline__ d64x2 pk_fma(d64x2 x, d64x2 y, d64x2 z) { return d64x2{fma(x.a, y.a, z.a), fma(x.b, y.b, z.b)}; }
 template <typename T> __device__ __forceinline__ typename Pk<T>::type pk_splat(T a) { return pk_make(a, a); }
 
+constexpr int MAX_PAIR_TYPES = 4;   // types a multi-type pair style can tell apart (the staged record carries the type in w)
 struct PairParams {    // host-prepared constants, in double; kernels convert once
   double rc2;
   double lj1, lj2, lj3, lj4;             // 48 eps s^12, 24 eps s^6, 4 eps s^12, 4 eps s^6
@@ -1218,6 +1220,8 @@ struct PairParams {    // host-prepared constants, in double; kernels convert on
   // the same rounded to fp32 once on the host (fill_float_copies): the mixed-precision bodies read these straight
   // from the constant bank instead of converting the doubles inside the list loop
   float f_rc2, f_lj1, f_lj2, f_lj3, f_lj4, f_A, f_p_r0, f_q_r0, f_p, f_q;
+  // Buckingham + cutoff Coulomb: per type pair (ta, tb), entry 4 ta + tb: A, 1/rho, C, k q_a q_b
+  double bc[MAX_PAIR_TYPES * MAX_PAIR_TYPES][4];
   __host__ void fill_float_copies() {
     f_rc2 = (float)rc2; f_lj1 = (float)lj1; f_lj2 = (float)lj2; f_lj3 = (float)lj3; f_lj4 = (float)lj4;
     f_A = (float)A; f_p_r0 = (float)p_r0; f_q_r0 = (float)q_r0; f_p = (float)p; f_q = (float)q;
@@ -1249,6 +1253,13 @@ __device__ __forceinline__ void virial2(PK dx, PK dy, PK dz, PK fp, PK* p) {
 // LJ 12-6 force (+ energy, virial when EV).  PAPER.md L102 calcPairForce, App. A L256.
 template <typename T, bool EV>
 struct LJBody {
+  // the w component of a staged record: the row's own atoms enter the list loop with own_w(w), every gathered atom j
+  // with its staged w, and pair2 receives own_w(w_i) - w_j (the direct cell-list kernel: cell_own_w(w_i) + w_j)
+  static __device__ __forceinline__ T own_w(T w) { return -w; }
+  static __device__ __forceinline__ T mutual_w(T a, T b) { return a + b; }
+  static __device__ __forceinline__ T cell_own_w(T w) { return w; }
+  template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
+  static constexpr bool TABLE = false;
   static constexpr int NT = EV ? 10 : 3;   // fx fy fz [e wxx wyy wzz wxy wxz wyz]
   using PK = typename Pk<T>::type;
   T rc2, lj1, lj2, lj3, lj4;
@@ -1283,6 +1294,13 @@ struct LJBody {
 // EAM pass 1: rho_i = sum_j exp(-q (r/r0 - 1))            (a6)
 template <typename T, bool EV>
 struct EamDensityBody {
+  // the w component of a staged record: the row's own atoms enter the list loop with own_w(w), every gathered atom j
+  // with its staged w, and pair2 receives own_w(w_i) - w_j (the direct cell-list kernel: cell_own_w(w_i) + w_j)
+  static __device__ __forceinline__ T own_w(T w) { return -w; }
+  static __device__ __forceinline__ T mutual_w(T a, T b) { return a + b; }
+  static __device__ __forceinline__ T cell_own_w(T w) { return w; }
+  template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
+  static constexpr bool TABLE = false;
   static constexpr int NT = 1;
   using PK = typename Pk<T>::type;
   T rc2, q_r0, q;
@@ -1304,6 +1322,13 @@ struct EamDensityBody {
 // EAM pass 2: F_i = -sum_j [ (F'_i + F'_j) rho'(r) + phi'(r) ] D / r      (a7); wsum = F'_i + F'_j.
 template <typename T, bool EV>
 struct EamForceBody {
+  // the w component of a staged record: the row's own atoms enter the list loop with own_w(w), every gathered atom j
+  // with its staged w, and pair2 receives own_w(w_i) - w_j (the direct cell-list kernel: cell_own_w(w_i) + w_j)
+  static __device__ __forceinline__ T own_w(T w) { return -w; }
+  static __device__ __forceinline__ T mutual_w(T a, T b) { return a + b; }
+  static __device__ __forceinline__ T cell_own_w(T w) { return w; }
+  template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
+  static constexpr bool TABLE = false;
   static constexpr int NT = EV ? 10 : 3;
   using PK = typename Pk<T>::type;
   T rc2, q_r0, q, p_r0, pp, A;
@@ -1339,6 +1364,73 @@ struct EamForceBody {
     p[0] = pk_fma(fp, dx, p[0]); p[1] = pk_fma(fp, dy, p[1]); p[2] = pk_fma(fp, dz, p[2]);
     if constexpr (EV) {
       p[3] = pk_add(p[3], phi);
+      virial2(dx, dy, dz, fp, p);
+    }
+  }
+};
+
+// Buckingham + cutoff Coulomb (App. A, LAMMPS style buck/coul/cut):
+//   u_ab(r) = A_ab exp(-r/rho_ab) - C_ab / r^6 + k q_a q_b / r,  r^2 < rc^2;  F_i = fpair D,
+//   fpair = [ (A/rho) r exp(-r/rho) - 6 C / r^6 + k q_a q_b / r ] / r^2.
+// The type of an atom travels in the w component of its staged record; the row's own atoms carry -4 t_i, so the
+// list loop hands pair2 the value -(4 t_i + t_j): the index of the type pair's coefficients in a 16-entry table
+// in shared memory (one 128-bit load per atom of the row and list entry; 256 bits in fp64).
+template <typename T, bool EV>
+struct BuckCoulBody {
+  static constexpr int NT = EV ? 10 : 3;
+  using PK = typename Pk<T>::type;
+  using V4 = typename Vec4<T>::type;
+  static constexpr bool TABLE = true;
+  static __device__ __forceinline__ T own_w(T w) { return (T)(-MAX_PAIR_TYPES) * w; }
+  static __device__ __forceinline__ T mutual_w(T a, T b) { return a + b * (T)(1.0 / MAX_PAIR_TYPES); }   // -(4 t0 + t1)
+  static __device__ __forceinline__ T cell_own_w(T w) { return (T)MAX_PAIR_TYPES * w; }
+  T rc2;
+  const V4* tab = nullptr;
+  __device__ explicit BuckCoulBody(const PairParams& P) : rc2(MDK_PP(rc2)) {}
+  // fills the shared-memory table (all threads of the block call it; the caller synchronises before the first use)
+  __device__ __forceinline__ void attach(V4* t) { tab = t; }
+  static __device__ __forceinline__ void fill(const PairParams& P, V4* t) {
+    for (int k = threadIdx.x; k < MAX_PAIR_TYPES * MAX_PAIR_TYPES; k += blockDim.x)
+      t[k] = make_v4<T>((T)P.bc[k][0], (T)P.bc[k][1], (T)P.bc[k][2], (T)P.bc[k][3]);
+  }
+  __device__ __forceinline__ V4 coef(T w) const {
+    int k = (int)((w < (T)0 ? -w : w) + (T)0.25);                      // |w| = 4 t_i + t_j exactly; the quarter guards the cast
+    k = k < MAX_PAIR_TYPES * MAX_PAIR_TYPES ? k : 0;                   // pad and dummy entries carry any w: they are out of range anyway
+    return tab[k];
+  }
+  __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T wsum, bool ok, T (&p)[NT]) const {
+    const bool in = ok && r2 < rc2;
+    const V4 c = coef(wsum);
+    const T rinv = t_rsqrt<T>(r2), r = r2 * rinv, r2i = rinv * rinv, r6i = r2i * r2i * r2i;
+    const T ex = c.x * t_exp<T>(-r * c.y);
+    const T fp = in ? (ex * r * c.y - (T)6 * c.z * r6i + c.w * rinv) * r2i : (T)0;
+    p[0] += fp * dx; p[1] += fp * dy; p[2] += fp * dz;
+    if constexpr (EV) {
+      p[3] += in ? ex - c.z * r6i + c.w * rinv : (T)0;
+      p[4] += dx * dx * fp; p[5] += dy * dy * fp; p[6] += dz * dz * fp;
+      p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
+    }
+  }
+  // 1/r := 0 beyond the cutoff zeroes the Coulomb term and, through 1/r^2, the whole force factor; the energy is masked
+  __device__ __forceinline__ void pair2(PK dx, PK dy, PK dz, PK r2, PK wsum, PK (&p)[NT]) const {
+    const T ra = pk_lo(r2), rb = pk_hi(r2);
+    const V4 ca = coef(pk_lo(wsum)), cb = coef(pk_hi(wsum));
+    const bool ina = ra < rc2, inb = rb < rc2;
+    const T ia = t_rsqrt<T>(ra), ib = t_rsqrt<T>(rb);
+    const PK r = pk_mul(r2, pk_make(ia, ib));
+    const PK irho = pk_make(ca.y, cb.y);
+    const PK arg = pk_mul(r, irho);
+    const PK ex = pk_mul(pk_make(ca.x, cb.x), pk_make(t_exp<T>(-pk_lo(arg)), t_exp<T>(-pk_hi(arg))));
+    const PK rinv = pk_make(ina ? ia : (T)0, inb ? ib : (T)0);
+    const PK r2i = pk_mul(rinv, rinv);
+    const PK r6i = pk_mul(pk_mul(r2i, r2i), r2i);
+    const PK c6 = pk_mul(pk_make(ca.z, cb.z), r6i), coul = pk_mul(pk_make(ca.w, cb.w), rinv);
+    // (A/rho) r e^{-r/rho} - 6 C/r^6 + kqq/r, times 1/r^2 (zero beyond the cutoff)
+    const PK fp = pk_mul(pk_fma(pk_mul(ex, arg), pk_splat<T>((T)1), pk_fma(pk_splat<T>((T)-6), c6, coul)), r2i);
+    p[0] = pk_fma(fp, dx, p[0]); p[1] = pk_fma(fp, dy, p[1]); p[2] = pk_fma(fp, dz, p[2]);
+    if constexpr (EV) {
+      const PK m = pk_make(ina ? (T)1 : (T)0, inb ? (T)1 : (T)0);
+      p[3] = pk_fma(m, pk_add(pk_sub(ex, c6), coul), p[3]);
       virial2(dx, dy, dz, fp, p);
     }
   }
@@ -1404,7 +1496,8 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
 #pragma unroll
     for (int d = 0; d < 3; ++d) { xx[d] = A.x[d * ld + gi]; x0v[d] = A.x0[d * ld + gi]; }
   }
-  const double dtf = A.dtf_type[A.type[gi]];   // dt/2 ftm2v / m of the atom's type (a tiny table, L1-resident)
+  const int ty = A.type[gi];
+  const double dtf = A.dtf_type[ty];   // dt/2 ftm2v / m of the atom's type (a tiny table, L1-resident)
   double d2 = 0.0;
   T r[3];
 #pragma unroll
@@ -1421,7 +1514,7 @@ __device__ __forceinline__ double atom_epilogue(const ForceArgs& A, int gi, cons
   if (A.epi == EPI_KICK_DRIFT) {
 #pragma unroll
     for (int d = 0; d < 3; ++d) { A.x_new[d * ld + gi] = xx[d]; A.v[d * ld + gi] = vv[d]; }
-    reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(r[0], r[1], r[2], (T)0);
+    reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(r[0], r[1], r[2], (T)ty);
   } else {
 #pragma unroll
     for (int d = 0; d < 3; ++d) { A.f[d * ld + gi] = tot[d]; A.v[d * ld + gi] = vv[d]; }
@@ -1480,11 +1573,11 @@ __device__ __forceinline__ double atom_epilogue2(const ForceArgs& A, int gi, boo
     if (A.epi == EPI_KICK_DRIFT) {
 #pragma unroll
       for (int d = 0; d < 3; ++d) { A.x_new[d * ld + gi] = xa[d]; A.v[d * ld + gi] = va[d]; }
-      reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(ra[0], ra[1], ra[2], (T)0);
+      reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi] = make_v4<T>(ra[0], ra[1], ra[2], (T)tya);
       if (act1) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) { A.x_new[d * ld + gi + 1] = xb[d]; A.v[d * ld + gi + 1] = vb[d]; }
-        reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi + 1] = make_v4<T>(rb[0], rb[1], rb[2], (T)0);
+        reinterpret_cast<typename Vec4<T>::type*>(A.xr_new)[gi + 1] = make_v4<T>(rb[0], rb[1], rb[2], (T)tyb);
       }
     } else {
 #pragma unroll
@@ -1633,6 +1726,8 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
   const unsigned mbar = smem_addr(&mbar_storage);
   const int tileid = blockIdx.x;
   if (threadIdx.x == 0) mbar_init(mbar, 1);
+  __shared__ __align__(16) unsigned char pair_tab[Body::TABLE ? MAX_PAIR_TYPES * MAX_PAIR_TYPES * sizeof(V4) : 16];   // per-type-pair coefficients
+  if constexpr (Body::TABLE) Body::fill(A.P, reinterpret_cast<V4*>(pair_tab));
   tile_load(g, tileid, A.tab, tt);
   const int pcap = prow_cap(g);
   const unsigned st_base = smem_addr(st);
@@ -1694,7 +1789,8 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
     if (threadIdx.x == 0) st[tt.n_slots] = make_v4<T>((T)1e15, (T)1e15, (T)1e15, (T)0);   // the dummy slot
   }
   __syncthreads();
-  const Body body(A.P);
+  Body body(A.P);
+  body.attach(reinterpret_cast<V4*>(pair_tab));
   const size_t ld = A.ld;
   const size_t slots_cap = (size_t)pcap * K;
   const uint4* tlist = A.list + (size_t)tileid * g.chunk_cap * slots_cap;
@@ -1718,7 +1814,7 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
       V4 pi0 = lds_v4_scalars<T>(st_base + (unsigned)slot0 * (unsigned)sizeof(V4));
       V4 pi1 = lds_v4_scalars<T>(st_base + (unsigned)(slot0 + 1) * (unsigned)sizeof(V4));   // a pad slot if there is no partner: far from everything
       if (!act1) { pi1.x = (T)-1e15; pi1.y = (T)-1e15; pi1.z = (T)-1e15; pi1.w = (T)0; }    // ... and from the dummy slot too
-      pi0.w = -pi0.w; pi1.w = -pi1.w;
+      pi0.w = Body::own_w(pi0.w); pi1.w = Body::own_w(pi1.w);
       const int n = (!HALF && base == 0) ? n_first : A.numneigh[(size_t)tileid * pcap + r];
       const int nq = (n + 7) >> 3;                          // words of this row
       if (act1 && s == 0) {
@@ -1728,7 +1824,7 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
         for (int k = 0; k < NT; ++k) p[k] = pk_splat<T>((T)0);
         const T ex = pi0.x - pi1.x, ey = pi0.y - pi1.y, ez = pi0.z - pi1.z;
         const T r2 = ex * ex + ey * ey + ez * ez;
-        body.pair2(pk_make(ex, -ex), pk_make(ey, -ey), pk_make(ez, -ez), pk_splat<T>(r2), pk_splat<T>(pi0.w + pi1.w), p);
+        body.pair2(pk_make(ex, -ex), pk_make(ey, -ey), pk_make(ez, -ez), pk_splat<T>(r2), pk_splat<T>(Body::mutual_w(pi0.w, pi1.w)), p);
 #pragma unroll
         for (int k = 0; k < NT; ++k) {
           tot0[k] += (double)pk_lo(p[k]);
@@ -1996,6 +2092,8 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  __shared__ __align__(16) unsigned char pair_tab[Body::TABLE ? MAX_PAIR_TYPES * MAX_PAIR_TYPES * sizeof(V4) : 16];   // per-type-pair coefficients
+  if constexpr (Body::TABLE) Body::fill(A.P, reinterpret_cast<V4*>(pair_tab));
   __syncthreads();
   const int ntl = ((int)g.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this block
   const int pcap = prow_cap(g);
@@ -2057,7 +2155,8 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   // ---------------- consumer groups ----------------
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(FORCE_P_CONSUMER_REGS));
   const int grp = wid / gwarps, gt = (int)threadIdx.x - grp * gthreads;
-  const Body body(A.P);
+  Body body(A.P);
+  body.attach(reinterpret_cast<V4*>(pair_tab));
   const size_t ld = A.ld;
   const size_t slots_cap = (size_t)pcap * K;
   double d2max = 0.0;
@@ -2113,7 +2212,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
         V4 pi0 = lds_v4_scalars<T>(st_base + (unsigned)slot0 * 16u);
         V4 pi1 = lds_v4_scalars<T>(st_base + (unsigned)(slot0 + 1) * 16u);   // a pad slot if there is no partner
         if (!act1) { pi1.x = -1e15f; pi1.y = -1e15f; pi1.z = -1e15f; pi1.w = 0.f; }
-        pi0.w = -pi0.w; pi1.w = -pi1.w;
+        pi0.w = Body::own_w(pi0.w); pi1.w = Body::own_w(pi1.w);
         const int n = base == 0 ? n_first : A.numneigh[(size_t)tile * pcap + r];
         const int nq = (n + 7) >> 3;                          // words of this row
         if (act1 && s == 0) {
@@ -2123,7 +2222,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
           for (int q = 0; q < NT; ++q) p[q] = pk_splat<T>(0.f);
           const T ex = pi0.x - pi1.x, ey = pi0.y - pi1.y, ez = pi0.z - pi1.z;
           const T r2 = ex * ex + ey * ey + ez * ez;
-          body.pair2(pk_make(ex, -ex), pk_make(ey, -ey), pk_make(ez, -ez), pk_splat<T>(r2), pk_splat<T>(pi0.w + pi1.w), p);
+          body.pair2(pk_make(ex, -ex), pk_make(ey, -ey), pk_make(ez, -ez), pk_splat<T>(r2), pk_splat<T>(Body::mutual_w(pi0.w, pi1.w)), p);
 #pragma unroll
           for (int q = 0; q < NT; ++q) { tot0[q] += (double)pk_lo(p[q]); tot1[q] += (double)pk_hi(p[q]); }
         }
@@ -2223,11 +2322,14 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
                xs[slot] = (T)(x[gi] + off[0]);
                ys[slot] = (T)(x[ld + gi] + off[1]);
                zs[slot] = (T)(x[2 * ld + gi] + off[2]);
-               ws[slot] = fpin ? (T)fpin[gi] : (T)0;
+               ws[slot] = fpin ? (T)fpin[gi] : (T)A.type[gi];   // F'(rho_j) in EAM pass 2, else the atom's type
              },
              [&](int slot) { xs[slot] = (T)1e15; ys[slot] = (T)1e15; zs[slot] = (T)1e15; ws[slot] = (T)0; });
+  __shared__ __align__(16) unsigned char pair_tab[Body::TABLE ? MAX_PAIR_TYPES * MAX_PAIR_TYPES * sizeof(V4) : 16];   // per-type-pair coefficients
+  if constexpr (Body::TABLE) Body::fill(A.P, reinterpret_cast<V4*>(pair_tab));
   __syncthreads();
-  const Body body(A.P);
+  Body body(A.P);
+  body.attach(reinterpret_cast<V4*>(pair_tab));
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   double ev[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   double d2max = 0.0;
@@ -2239,7 +2341,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
       const bool act = r0 + lane < c;
       const int a = act ? s_lo + r0 + lane : s_lo;
       const int gi = g_lo + r0 + lane;
-      const T xi = xs[a], yi = ys[a], zi = zs[a], wi = ws[a];
+      const T xi = xs[a], yi = ys[a], zi = zs[a], wi = Body::cell_own_w(ws[a]);
       double tot[NT];
 #pragma unroll
       for (int k = 0; k < NT; ++k) tot[k] = 0.0;
@@ -2330,7 +2432,8 @@ __global__ void k_initial_integrate(Geom g, int N, size_t ld, double* __restrict
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   double d2 = 0.0;
   if (n < N) {
-    double dtf = half_dt_ftm2v / mass[type[n]];
+    const int ty = type[n];
+    double dtf = half_dt_ftm2v / mass[ty];
     T r[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
@@ -2343,7 +2446,7 @@ __global__ void k_initial_integrate(Geom g, int N, size_t ld, double* __restrict
       d2 += dd * dd;
       r[d] = (T)(xx - cell_anchor_1d(g, d, cell_index_1d(g, d, p0)));
     }
-    xr[n] = make_v4<T>(r[0], r[1], r[2], (T)0);
+    xr[n] = make_v4<T>(r[0], r[1], r[2], (T)ty);
   }
   block_max_to_flag(d2, red, flag);
 }

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libmd_b200.so")
 MD_OK = 0
 MD_ERR_BAD_ARGUMENT, MD_ERR_BOX_TOO_SMALL, MD_ERR_CUDA, MD_ERR_OVERFLOW, MD_ERR_NOT_READY, MD_ERR_NONFINITE = -1, -2, -3, -4, -5, -6
 MD_FP64, MD_MIXED = 0, 1
-MD_PAIR_LJ126, MD_PAIR_EAM_FS = 1, 2
+MD_PAIR_LJ126, MD_PAIR_EAM_FS, MD_PAIR_BUCK_COUL = 1, 2, 3
 MD_LIST_FULL, MD_LIST_HALF = 0, 1
 MD_KERNEL_AUTO, MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_CELL, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2 = 0, 1, 2, 3, 4, 5, 6
 KERNEL_NAMES = {0: "auto", 1: "tpa", 2: "subwarp8", 3: "warp", 4: "cell", 5: "subwarp4", 6: "subwarp2"}
@@ -27,7 +27,7 @@ EXPORTS = [
     "md_create", "md_destroy", "md_set_units", "md_set_precision", "md_set_positions", "md_set_velocities",
     "md_set_pair", "md_set_neighbor", "md_build_neighbors", "md_compute_forces", "md_run", "md_get_positions",
     "md_get_velocities", "md_get_forces", "md_get_neighbors", "md_get_neighbor_rows", "md_kinetic_energy", "md_autotune",
-    "md_get_stats", "md_last_error", "md_set_option",
+    "md_get_stats", "md_last_error", "md_set_option", "md_set_pair_coeff", "md_set_type_charges",
 ]
 
 
@@ -89,6 +89,8 @@ def _load():
     L.md_get_neighbor_rows.argtypes = [vp, ip, ip, ip, ctypes.c_int64]
     L.md_kinetic_energy.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.md_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int64]
+    L.md_set_pair_coeff.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+    L.md_set_type_charges.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
     L.md_autotune.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     L.md_get_stats.argtypes = [vp, ctypes.POINTER(md_stats)]
     L.md_last_error.argtypes = [vp]
@@ -173,6 +175,14 @@ class System:
         p = (ctypes.c_double * len(params))(*[float(q) for q in params])
         self._ck(lib.md_set_pair(self._h, style, p, len(params), rc, skin))
 
+    def md_set_pair_coeff(self, type_a: int, type_b: int, coeff):
+        c = (ctypes.c_double * len(coeff))(*[float(q) for q in coeff])
+        self._ck(lib.md_set_pair_coeff(self._h, int(type_a), int(type_b), c, len(coeff)))
+
+    def md_set_type_charges(self, q):
+        c = (ctypes.c_double * len(q))(*[float(v) for v in q])
+        self._ck(lib.md_set_type_charges(self._h, c, len(q)))
+
     def md_set_neighbor(self, list_kind: int, kernel: int):
         self._ck(lib.md_set_neighbor(self._h, list_kind, kernel))
 
@@ -236,6 +246,12 @@ def from_workload(w, precision: int | None = None, list_kind: int = MD_LIST_FULL
     for name, value in (options or {}).items():
         s.md_set_option(name, value)
     s.md_set_pair(w.style, w.params, w.rc, w.skin)
+    if w.style == MD_PAIR_BUCK_COUL:
+        nt = len(w.mass)
+        for a in range(nt):
+            for b in range(a, nt):
+                s.md_set_pair_coeff(a, b, w.pair_coef[a][b])
+        s.md_set_type_charges(w.qtype)
     s.md_set_positions(np.ascontiguousarray(w.x if x is None else x))
     s.md_set_velocities(np.ascontiguousarray(w.v))
     return s

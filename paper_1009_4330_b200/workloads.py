@@ -27,6 +27,7 @@ FTM2V_METAL = 1.0 / 1.0364269e-4
 
 PAIR_LJ = 1
 PAIR_EAM = 2
+PAIR_BUCK_COUL = 3
 PREC_FP64 = 0
 PREC_MIXED = 1
 
@@ -121,6 +122,8 @@ class Workload:
     mvv2e: float
     kT: float
     seed: int
+    qtype: np.ndarray | None = None       # PAIR_BUCK_COUL: charge of every type
+    pair_coef: np.ndarray | None = None   # PAIR_BUCK_COUL: [ntypes, ntypes, 3] = A, rho, C of every type pair (symmetric)
 
     @property
     def natoms(self) -> int:
@@ -142,9 +145,51 @@ _TABLE = {
 }
 
 
+# cfg 6: a synthetic stand-in for the paper's "silicate (cutoff)" workload (App. A: buck/coul/cut,
+# 0.09 atoms per A^3, two charged species), whose data file and parameters are not in the container.  Rock-salt sites of
+# spacing 2.25 A (0.0878 per A^3), anions (type 0) and cations (type 1) alternating, seeded displacements of 0.1 A;
+# Buckingham coefficients of the magnitude of the BKS silica potential.  rc = 8 A, not the paper's 15 A: a cell of edge
+# rc + skin must hold fewer than 8191/27 atoms for the tile's 16-bit slot codes (known limits).
+K_COULOMB_METAL = 14.399645             # eV A / e^2
+SILICATE_A0 = 2.25
+SILICATE_Q = (-1.2, 1.2)
+SILICATE_MASS = (15.9994, 28.0855)
+SILICATE_COEF = {(0, 0): (1388.77, 0.3623, 175.0), (0, 1): (18003.76, 0.2052, 133.54), (1, 1): (0.0, 1.0, 0.0)}
+
+
+def make_silicate_like(n: int = 48, seed_offset: int = 0, rc: float = 8.0, skin: float = 1.0, nsteps: int = 100) -> Workload:
+    seed = 43306 + 1000 * seed_offset
+    iz, iy, ix = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    site = np.stack([ix.ravel(), iy.ravel(), iz.ravel()], axis=1)
+    types = ((site.sum(axis=1)) % 2).astype(np.int32)
+    box = np.array([n * SILICATE_A0] * 3, dtype=np.float64)
+    N = site.shape[0]
+    ids = np.arange(N, dtype=np.uint64)
+    x = site.astype(np.float64) * SILICATE_A0 + uniform_displacements(seed, ids, 0.1)
+    x -= np.floor(x / box) * box
+    mass = np.array(SILICATE_MASS)
+    kT = KB_METAL * 300.0
+    v = thermal_velocities(seed, ids, mass[types], kT, MVV2E_METAL)
+    coef = np.zeros((2, 2, 3))
+    for (a, b), c in SILICATE_COEF.items():
+        coef[a, b] = coef[b, a] = c
+    return Workload(name="Buckingham + cutoff Coulomb, two species, %d atoms mixed" % N, cfg=6, x=np.ascontiguousarray(x), v=v, box=box,
+                    types=types, mass=mass, style=PAIR_BUCK_COUL, params=(K_COULOMB_METAL,), rc=rc, skin=skin, dt=0.001, nsteps=nsteps,
+                    precision=PREC_MIXED, ftm2v=FTM2V_METAL, mvv2e=MVV2E_METAL, kT=kT, seed=seed, qtype=np.array(SILICATE_Q), pair_coef=coef)
+
+
+def oracle_params(w: Workload):
+    """The pair parameters of ``w`` in the form the CPU oracle's wrapper takes them (packing only)."""
+    if w.style == PAIR_BUCK_COUL:
+        return dict(k=w.params[0], types=w.types, q=w.qtype, coef=w.pair_coef)
+    return w.params
+
+
 def make(cfg: int, n_override: int | None = None, seed_offset: int = 0) -> Workload:
-    """Build config ``cfg`` (1..5) of BASELINE.json.  ``n_override`` shrinks the
+    """Build config ``cfg`` (1..5) of BASELINE.json (6: the synthetic two-species workload of SURVEY.md 8(f)-2).  ``n_override`` shrinks the
     lattice (unit cells per edge) for tests; ``seed_offset`` decorrelates replicas."""
+    if cfg == 6:
+        return make_silicate_like(48 if n_override is None else int(n_override), seed_offset)
     name, style, n, rc, skin, dt, nsteps, prec, permuted = _TABLE[cfg]
     if n_override is not None:
         n = int(n_override)

@@ -428,6 +428,75 @@ def test_half_list_run_matches_oracle_trajectory(cfg, n, nsteps):
     s.close()
 
 
+# ---- Buckingham + cutoff Coulomb, two charged species (App. A) ---------------------
+
+BC_VARIANTS = [("tpa", 1, 0), ("subwarp4", 5, 0), ("warp", 3, 0), ("cell", 4, 0), ("half", 1, 1)]
+
+
+@pytest.mark.parametrize("name,kernel,list_kind", BC_VARIANTS)
+def test_buck_coul_fp64_forces_energy_virial(name, kernel, list_kind):
+    w = wl.make(6, n_override=12)                       # 1,728 ions, box = 3 (rc + skin)
+    fo, Eo, Wo, npairs, _ = oracle.forces_brute(w.x, w.box, w.style, wl.oracle_params(w), w.rc)
+    s = md.from_workload(w, precision=md.MD_FP64, kernel=kernel, list_kind=list_kind)
+    f = np.zeros((w.natoms, 3))
+    E, W = s.md_compute_forces(f, energy=True, virial=True)
+    assert _fp64_force_err(f, fo) < 1e-12
+    assert abs(E - Eo) < 1e-12 * abs(Eo) and np.abs(W - Wo).max() < 1e-11 * np.abs(Wo).max()
+    s.close()
+
+
+@pytest.mark.parametrize("name,kernel,list_kind", BC_VARIANTS)
+def test_buck_coul_mixed_forces_energy(name, kernel, list_kind):
+    w = wl.make(6, n_override=12)
+    fo, Eo = oracle.forces_brute(w.x, w.box, w.style, wl.oracle_params(w), w.rc)[:2]
+    s = md.from_workload(w, precision=md.MD_MIXED, kernel=kernel, list_kind=list_kind)
+    f = np.zeros((w.natoms, 3))
+    E, _ = s.md_compute_forces(f, energy=True)
+    assert _rel_rms(f, fo) < 1e-5
+    assert abs(E - Eo) < 1e-6 * abs(Eo)
+    s.close()
+
+
+def test_buck_coul_type_pairs_and_charges_reach_the_kernel():
+    """Two ions of every type combination through the API: the coefficient table is indexed by (t_i, t_j)."""
+    box = np.array([40.0, 40.0, 40.0])
+    coef = {(0, 0): (100.0, 0.5, 3.0), (0, 1): (75.0, 0.45, 2.0), (1, 1): (50.0, 0.4, 1.0)}
+    q = (0.3, -0.6)
+    for ta, tb in [(0, 0), (0, 1), (1, 0), (1, 1)]:
+        for prec, tol in [(md.MD_FP64, 1e-13), (md.MD_MIXED, 2e-6)]:
+            s = md.System(box, 2, np.array([ta, tb], np.int32), np.array([1.0, 2.0]))
+            s.md_set_precision(prec)
+            s.md_set_pair(md.MD_PAIR_BUCK_COUL, (14.399645,), 6.0, 1.0)
+            with pytest.raises(md.MDError) as e:       # coefficients missing
+                s.md_set_positions(np.array([[5.0, 5, 5], [7.0, 5, 5]])); s.md_compute_forces()
+            assert e.value.code == md.MD_ERR_NOT_READY
+            for (a, b), c in coef.items():
+                s.md_set_pair_coeff(a, b, c)
+            s.md_set_type_charges(q)
+            x = np.array([[39.0, 5.0, 5.0], [1.0, 5.0, 5.0]])                     # r = 2 across the periodic face
+            s.md_set_positions(x)
+            f = np.zeros((2, 3))
+            E, _ = s.md_compute_forces(f, energy=True)
+            A, rho, C = coef[min(ta, tb), max(ta, tb)]
+            P = dict(k=14.399645, types=[ta, tb], q=q, coef=np.array([[coef[0, 0], coef[0, 1]], [coef[0, 1], coef[1, 1]]]))
+            fo, Eo = oracle.forces_brute(x, box, oracle.PAIR_BUCK_COUL, P, 6.0)[:2]
+            assert abs(E - Eo) < tol * max(1.0, abs(Eo)) and np.abs(f - fo).max() < tol * max(1.0, np.abs(fo).max())
+            s.close()
+
+
+def test_buck_coul_run_matches_oracle_trajectory():
+    w = wl.make(6, n_override=12)
+    s = md.from_workload(w, precision=md.MD_FP64)
+    s.md_run(20, w.dt)
+    x, v = np.zeros((w.natoms, 3)), np.zeros((w.natoms, 3))
+    s.md_get_positions(x); s.md_get_velocities(v)
+    ref = oracle.run_nve(w.x, w.v, w.box, w.mass[w.types], w.style, wl.oracle_params(w), w.rc, w.skin, w.dt, 20,
+                         ftm2v=w.ftm2v, mvv2e=w.mvv2e)
+    assert np.abs(_minimg(x - ref["x"], w.box)).max() < 1e-9
+    assert np.abs(v - ref["v"]).max() < 1e-8 * np.abs(ref["v"]).max()
+    s.close()
+
+
 # ---- errors and degenerate inputs ------------------------------------------------------------------------------
 
 def test_error_paths():
