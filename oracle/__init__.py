@@ -237,3 +237,25 @@ def run_nve(x, v, box, mass_per_atom, style, params, rc, skin, dt, nsteps, ftm2v
     if trace:
         out.update(pe=pe, ke=ke)
     return out
+
+
+def run_nvt(x, v, box, mass_per_atom, style, params, rc, skin, dt, nsteps, kT, tau, ftm2v=1.0, mvv2e=1.0, thermo=(0.0, 0.0)):
+    """Velocity Verlet with one Nose-Hoover thermostat (md_oracle.c header; reading s25).
+    Returns dict(x, v, f, nbuild, thermo=(xi, eta), h[nsteps+1] conserved quantity, ke[nsteps+1])."""
+    x, v, box, m = _c(x).copy(), _c(v).copy(), _c(box), _c(mass_per_atom)
+    N = x.shape[0]
+    f = np.zeros((N, 3))
+    h = np.zeros(nsteps + 1)
+    ke = np.zeros(nsteps + 1)
+    th = np.array(thermo, dtype=np.float64)
+    P = _pair(style, params, rc)
+    L = lib()
+    L.orc_run_nvt.restype = ctypes.c_int64
+    dp = ctypes.POINTER(ctypes.c_double)
+    L.orc_run_nvt.argtypes = [ctypes.c_int64, dp, dp, dp, dp, dp, ctypes.POINTER(_Pair), ctypes.c_double, ctypes.c_double,
+                              ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, dp, dp]
+    nb = L.orc_run_nvt(N, _d(x), _d(v), _d(f), _d(box), _d(m), ctypes.byref(P), float(skin), float(dt), int(nsteps),
+                       float(ftm2v), float(mvv2e), float(kT), float(tau), _d(th), _d(h), _d(ke))
+    if nb < 0:
+        raise ValueError("box smaller than 3 (rc+skin) in some dimension")
+    return dict(x=x, v=v, f=f, nbuild=int(nb), thermo=(float(th[0]), float(th[1])), h=h, ke=ke)

@@ -27,6 +27,11 @@
  *                 terms at one cutoff; charges per TYPE (the paper's silicate has one charge per species).
  *   NVE           velocity Verlet ("NVE ... integrators"):
  *                 v += dt/2 f/m ftm2v; x += dt v; f = F(x); v += dt/2 f/m ftm2v
+ *   NVT           ("NVE, NVT, and NPT integrators"; reading s25) one Nose-Hoover
+ *                 thermostat: dv/dt = f/m - xi v, dxi/dt = G = (2 KE - g kT)/Q, deta/dt = xi, Q = g kT tau^2,
+ *                 g = 3N - 3, integrated by the symmetric splitting  TH(dt/2) kick drift force kick TH(dt/2)  with
+ *                 TH(h): xi += h/2 G(KE); s = exp(-xi h); v *= s; KE *= s^2; eta += xi h; xi += h/2 G(KE).
+ *                 Conserved: H = KE + PE + Q xi^2 / 2 + g kT eta.
  *   neighbor list loop of PAPER.md L88-104 (TpA pseudo-code): for each i, for
  *                 jj < numneigh[i]: j = neighbors[i][jj]; cutoff test (L159);
  *                 ftmp += pair force; f[i] = ftmp      -- a FULL list.
@@ -456,6 +461,81 @@ int64_t orc_run_nve(int64_t N, double* x, double* v, double* f, const double* bo
       for (int a = 0; a < 3; ++a) v[3 * i + a] += dtf * f[3 * i + a];
     }
   }
+  orc_list_free(l);
+  free(x0);
+  return nbuild;
+}
+
+/* ---- NVT: velocity Verlet with one Nose-Hoover thermostat (header comment; reading s25) ------------------ */
+
+static double kinetic(int64_t N, const double* v, const double* mass, double mvv2e) {
+  double ke = 0.0;
+  for (int64_t i = 0; i < N; ++i) ke += 0.5 * mass[i] * (v[3 * i] * v[3 * i] + v[3 * i + 1] * v[3 * i + 1] + v[3 * i + 2] * v[3 * i + 2]);
+  return ke * mvv2e;
+}
+
+/* TH(h): returns the velocity scale factor; updates xi, eta and KE */
+static double thermostat_half(double* xi, double* eta, double* ke, double h, double gkT, double Q) {
+  *xi += 0.5 * h * (2.0 * *ke - gkT) / Q;
+  double sc = exp(-*xi * h);
+  *ke *= sc * sc;
+  *eta += *xi * h;
+  *xi += 0.5 * h * (2.0 * *ke - gkT) / Q;
+  return sc;
+}
+
+/* nsteps of NVT from (x, v) with thermostat state thermo[2] = {xi, eta} (in/out).  kT and tau in the caller's energy
+ * and time units.  h_trace[nsteps+1] (may be NULL): the conserved quantity at every whole step.  Returns the number of
+ * list builds, -1 if the box is too small.  Same list route and rebuild rule as orc_run_nve. */
+int64_t orc_run_nvt(int64_t N, double* x, double* v, double* f, const double* box, const double* mass,
+                    const orc_pair* P, double skin, double dt, int64_t nsteps, double ftm2v, double mvv2e,
+                    double kT, double tau, double* thermo, double* h_trace, double* ke_trace) {
+  double rl = P->rc + skin, trigger = 0.25 * skin * skin;
+  double gkT = (3.0 * (double)N - 3.0) * kT, Q = gkT * tau * tau;
+  double* x0 = (double*)malloc((size_t)(3 * N) * sizeof(double));
+  for (int64_t i = 0; i < N; ++i)
+    for (int a = 0; a < 3; ++a) x[3 * i + a] -= box[a] * floor(x[3 * i + a] / box[a]);
+  orc_list* l = orc_list_build(N, x, box, rl);
+  if (!l) { free(x0); return -1; }
+  memcpy(x0, x, (size_t)(3 * N) * sizeof(double));
+  int64_t nbuild = 1;
+  double pe, xi = thermo[0], eta = thermo[1];
+  orc_forces_list(N, x, box, P, l, f, &pe, NULL, NULL, NULL);
+  for (int64_t step = 0;; ++step) {
+    double ke = kinetic(N, v, mass, mvv2e);
+    if (h_trace) h_trace[step] = ke + pe + 0.5 * Q * xi * xi + gkT * eta;
+    if (ke_trace) ke_trace[step] = ke;
+    if (step == nsteps) break;
+    double sc = thermostat_half(&xi, &eta, &ke, 0.5 * dt, gkT, Q);
+    double dmax = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+      double dtf = 0.5 * dt * ftm2v / mass[i], d2 = 0.0;
+      for (int a = 0; a < 3; ++a) {
+        v[3 * i + a] = sc * v[3 * i + a] + dtf * f[3 * i + a];
+        x[3 * i + a] += dt * v[3 * i + a];
+        double d = x[3 * i + a] - x0[3 * i + a];
+        d2 += d * d;
+      }
+      if (d2 > dmax) dmax = d2;
+    }
+    if (dmax > trigger) {
+      for (int64_t i = 0; i < N; ++i)
+        for (int a = 0; a < 3; ++a) x[3 * i + a] -= box[a] * floor(x[3 * i + a] / box[a]);
+      orc_list_free(l);
+      l = orc_list_build(N, x, box, rl);
+      memcpy(x0, x, (size_t)(3 * N) * sizeof(double));
+      ++nbuild;
+    }
+    orc_forces_list(N, x, box, P, l, f, &pe, NULL, NULL, NULL);
+    for (int64_t i = 0; i < N; ++i) {
+      double dtf = 0.5 * dt * ftm2v / mass[i];
+      for (int a = 0; a < 3; ++a) v[3 * i + a] += dtf * f[3 * i + a];
+    }
+    ke = kinetic(N, v, mass, mvv2e);
+    sc = thermostat_half(&xi, &eta, &ke, 0.5 * dt, gkT, Q);
+    for (int64_t i = 0; i < 3 * N; ++i) v[i] *= sc;
+  }
+  thermo[0] = xi; thermo[1] = eta;
   orc_list_free(l);
   free(x0);
   return nbuild;
