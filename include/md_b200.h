@@ -68,6 +68,10 @@ typedef struct md_system md_system; /* opaque */
                              A, rho, C by md_set_pair_coeff, per type charge by md_set_type_charges; at most 4 types;
                              k = 14.399645 eV A / e^2 in metal units */
 
+/* thermostats (md_set_thermostat) */
+#define MD_THERMO_NONE 0         /* NVE */
+#define MD_THERMO_NOSE_HOOVER 1  /* NVT: one Nose-Hoover thermostat */
+
 /* neighbor-list kinds */
 #define MD_LIST_FULL 0    /* both (i,j) and (j,i): each kernel row writes only f[i] (L104) */
 #define MD_LIST_HALF 1    /* each pair once; -F scattered to j with atomics (Newton's third law, L76) */
@@ -186,6 +190,16 @@ int md_compute_forces(md_system* s, double* f_out, double* energy_out, double vi
  * [rebuild iff max |x-x0|^2 > (skin/2)^2]; f = F(x); v += dt/2 f/m ftm2v.  Asynchronous apart from the
  * rebuild decisions.  (north_star md_run) */
 int md_run(md_system* s, int64_t nsteps, double dt);
+
+/* NVT ("NVE, NVT, and NPT integrators"; reading s25 of DESIGN.md): with
+ * MD_THERMO_NOSE_HOOVER md_run integrates dv/dt = f/m - xi v, dxi/dt = (2 KE - g kT)/Q, Q = g kT tau^2, g = 3N - 3, by the
+ * symmetric splitting TH(dt/2) kick drift force kick TH(dt/2), TH(h): xi += h/2 G; v *= exp(-xi h); eta += xi h; xi += h/2 G.
+ * kT in the caller's energy units (k_B T), tau in its time units.  Resets the thermostat state (xi = eta = 0), which
+ * otherwise persists across md_run calls.  MD_THERMO_NONE returns to NVE. */
+int md_set_thermostat(md_system* s, int kind, double kT, double tau);
+/* out = {xi, eta, Q xi^2 / 2 + g kT eta}: the thermostat's state and its share of the conserved quantity
+ * H = KE + PE + Q xi^2 / 2 + g kT eta (host doubles). */
+int md_get_thermostat(md_system* s, double out[3]);
 
 /* Current positions in caller order (host or device buffer of N x 3 doubles, reading s5): as stored,
  * i.e. inside the box at the last build, possibly slightly outside since.  MD_ERR_NOT_READY before md_set_positions. */

@@ -91,6 +91,11 @@ struct md_system_impl {
   size_t list_words = 0;
   double* mass_d = nullptr;
   double* dtf_d = nullptr;       // [ntypes]: dt/2 ftm2v / mass of the current md_run
+  // NVT (md_set_thermostat): one Nose-Hoover thermostat; state xi, eta persists across md_run calls
+  int thermostat = MD_THERMO_NONE;
+  double thermo_kT = 0, thermo_tau = 0, thermo_xi = 0, thermo_eta = 0;
+  double* thermo_d = nullptr;    // 8 doubles: xi, eta, KE, scale, g kT, Q
+  double* ke_partial_d = nullptr;   // one kinetic-energy partial per block of k_final_integrate_ke
   std::vector<double> mass_h;
   double* ev_partials = nullptr;
   size_t ev_tiles_alloc = 0;
@@ -673,17 +678,17 @@ int compute_forces_device(md_system* s, bool ev, const StepMode& M = StepMode())
 
 int autotune(md_system* s, int nrep, double* ms_out);
 
-int initial_integrate(md_system* s, double dt, double hdtf, bool in_run = false) {
+int initial_integrate(md_system* s, double dt, double hdtf, bool in_run = false, const double* vscale = nullptr) {
   const Flags* rf = in_run ? s->flags_d : nullptr;
   const int N = (int)s->N;
   if (s->precision == MD_FP64)
     CK(launch(s, k_initial_integrate<double>, blocks_for(N, 256), 256, 0, s->g, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
               (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, (double4*)s->xr[s->xcur], dt, hdtf,
-              &s->flags_d->max_disp2_bits[0], rf));
+              &s->flags_d->max_disp2_bits[0], rf, vscale));
   else
     CK(launch(s, k_initial_integrate<float>, blocks_for(N, 256), 256, 0, s->g, N, s->ld, s->x[s->xcur], s->v[s->cur], (const double*)s->f,
               (const double*)s->x0, (const int*)s->type[s->cur], (const double*)s->mass_d, (float4*)s->xr[s->xcur], dt, hdtf,
-              &s->flags_d->max_disp2_bits[0], rf));
+              &s->flags_d->max_disp2_bits[0], rf, vscale));
   return MD_OK;
 }
 
@@ -844,6 +849,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   CKC(dalloc(&s->cell_of, s->ld)); CKC(dalloc(&s->rank, s->ld)); CKC(dalloc(&s->perm, s->ld)); CKC(dalloc(&s->mkey, s->ld));
   CKC(dalloc(&s->nstat_d, (size_t)4));
   CKC(dalloc(&s->mass_d, (size_t)ntypes)); CKC(dalloc(&s->dtf_d, (size_t)ntypes));
+  CKC(dalloc(&s->thermo_d, (size_t)8)); CKC(dalloc(&s->ke_partial_d, (size_t)blocks_for(N, 256)));
   s->mass_h.assign(mass, mass + ntypes); CKC(dalloc(&s->scalars_d, 16)); CKC(dalloc(&s->io_d, 3 * s->ld));
   CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
@@ -877,7 +883,7 @@ void md_destroy(md_system* s) {
   cudaFree(s->tab);
   cudaFree(s->f); cudaFree(s->x0); cudaFree(s->rho); cudaFree(s->fp); cudaFree(s->cell_of); cudaFree(s->rank); cudaFree(s->perm); cudaFree(s->mkey);
   cudaFree(s->nstat_d); cudaFree(s->export_buf);
-  cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d); cudaFree(s->dtf_d);
+  cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d); cudaFree(s->dtf_d); cudaFree(s->thermo_d); cudaFree(s->ke_partial_d);
   cudaFree(s->ev_partials); cudaFree(s->scalars_d); cudaFree(s->io_d); cudaFree(s->io_i); cudaFree(s->types_caller); cudaFree(s->flags_d);
   if (s->flags_h) cudaFreeHost(s->flags_h);
   if (s->scalars_h) cudaFreeHost(s->scalars_h);
@@ -994,6 +1000,23 @@ int md_set_type_charges(md_system* s, const double* q, int n) {
   return MD_OK;
 }
 
+int md_set_thermostat(md_system* s, int kind, double kT, double tau) {
+  if (!s) return MD_ERR_BAD_ARGUMENT;
+  if (kind != MD_THERMO_NONE && kind != MD_THERMO_NOSE_HOOVER) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_thermostat: unknown kind %d", kind);
+  if (kind == MD_THERMO_NOSE_HOOVER && (!(kT > 0.0) || !(tau > 0.0) || !std::isfinite(kT) || !std::isfinite(tau) || s->N < 2))
+    return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_thermostat: kT and tau must be positive (and N >= 2)");
+  s->thermostat = kind; s->thermo_kT = kT; s->thermo_tau = tau; s->thermo_xi = 0.0; s->thermo_eta = 0.0;
+  return MD_OK;
+}
+
+int md_get_thermostat(md_system* s, double out[3]) {
+  if (!s || !out) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_get_thermostat: NULL") : MD_ERR_BAD_ARGUMENT;
+  const double gkT = (3.0 * (double)s->N - 3.0) * s->thermo_kT, Q = gkT * s->thermo_tau * s->thermo_tau;
+  out[0] = s->thermo_xi; out[1] = s->thermo_eta;
+  out[2] = s->thermostat == MD_THERMO_NOSE_HOOVER ? 0.5 * Q * s->thermo_xi * s->thermo_xi + gkT * s->thermo_eta : 0.0;
+  return MD_OK;
+}
+
 int md_set_neighbor(md_system* s, int list_kind, int kernel) {
   if (!s) return MD_ERR_BAD_ARGUMENT;
   if (list_kind != MD_LIST_FULL && list_kind != MD_LIST_HALF) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_neighbor: unknown list kind");
@@ -1073,7 +1096,8 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   int nsampled = 0;
   s->ms_force_sampled = 0; s->ms_pass1_sampled = 0;
   const bool eam = s->style == MD_PAIR_EAM_FS;
-  const bool fused = s->list_kind != MD_LIST_HALF;
+  const bool nvt = s->thermostat == MD_THERMO_NOSE_HOOVER;
+  const bool fused = s->list_kind != MD_LIST_HALF && !nvt;
   if (nsteps > 0 && fused) {
     // Velocity Verlet with ONE launch per time step (two for EAM): the force kernel of step n also does the
     // second half kick of step n and the first half kick + drift of step n+1, writing the new positions to
@@ -1155,18 +1179,43 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
     // every later kernel of the batch then does nothing either.  The host reads {steps_done, stop} once per batch; the
     // step that stopped has had its first half (kick + drift) applied, so the host rebuilds, evaluates the forces and
     // finishes it before it enqueues the next batch.
+    // NVT (reading s25): TH(dt/2) before the first kick and after the second; the thermostat's scalar state lives on the
+    // device (thermo_d), the kinetic energy it needs comes out of the second kick's kernel as per-block partials
+    const unsigned nb256 = blocks_for(N, 256);
     auto final_integrate = [&](bool in_run) -> int {
-      CK(launch(s, k_final_integrate, blocks_for(N, 256), 256, 0, N, s->ld, s->v[s->cur], (const double*)s->f, (const int*)s->type[s->cur],
-                (const double*)s->mass_d, hdtf, in_run ? s->flags_d : (Flags*)nullptr));
+      Flags* rf = in_run ? s->flags_d : (Flags*)nullptr;
+      if (!nvt) {
+        CK(launch(s, k_final_integrate, nb256, 256, 0, N, s->ld, s->v[s->cur], (const double*)s->f, (const int*)s->type[s->cur],
+                  (const double*)s->mass_d, hdtf, rf));
+        return MD_OK;
+      }
+      CK(launch(s, k_final_integrate_ke, nb256, 256, 0, N, s->ld, s->v[s->cur], (const double*)s->f, (const int*)s->type[s->cur],
+                (const double*)s->mass_d, hdtf, s->ke_partial_d, rf));
+      CK(launch(s, k_nh_reduce, 1, 256, 0, (int)nb256, (const double*)s->ke_partial_d, s->mvv2e, s->thermo_d, 0.5 * dt, (const Flags*)rf));
+      CK(launch(s, k_scale_velocities, nb256, 256, 0, N, s->ld, s->v[s->cur], (const double*)(s->thermo_d + 3), (const Flags*)rf));
       return MD_OK;
     };
+    auto first_half = [&](bool in_run) -> int {   // TH(dt/2) (NVT), then kick + drift + displacement flag
+      if (nvt) CK(launch(s, k_nh_half, 1, 1, 0, s->thermo_d, 0.5 * dt, in_run ? (const Flags*)s->flags_d : (const Flags*)nullptr));
+      return initial_integrate(s, dt, hdtf, in_run, nvt ? s->thermo_d + 3 : nullptr);
+    };
     CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
+    if (nvt && nsteps > 0) {
+      // thermostat constants and state; the current kinetic energy (a kick by zero gives the partials)
+      const double gkT = (3.0 * (double)s->N - 3.0) * s->thermo_kT;
+      const double th[8] = {s->thermo_xi, s->thermo_eta, 0.0, 1.0, gkT, gkT * s->thermo_tau * s->thermo_tau, 0.0, 0.0};
+      CK(cudaMemcpyAsync(s->thermo_d, th, sizeof th, cudaMemcpyHostToDevice, s->stream));
+      CK(cudaStreamSynchronize(s->stream));   // th is a stack object
+      CK(launch(s, k_final_integrate_ke, nb256, 256, 0, N, s->ld, s->v[s->cur], (const double*)s->f, (const int*)s->type[s->cur],
+                (const double*)s->mass_d, 0.0, s->ke_partial_d, (Flags*)nullptr));
+      CK(launch(s, k_nh_reduce, 1, 256, 0, (int)nb256, (const double*)s->ke_partial_d, s->mvv2e, s->thermo_d, 0.0, (const Flags*)nullptr));
+    }
     int64_t remaining = nsteps;
     while (remaining > 0) {
       const int m = (int)std::min<int64_t>(s->batch, remaining);
       int sample_slot[64];
       for (int k = 0; k < m; ++k) {
-        rc = initial_integrate(s, dt, hdtf, true);
+        rc = first_half(true);
         if (rc) return rc;
         StepMode M;
         M.epi = EPI_FORCES; M.in_run = 1; M.parity = 0; M.trigger = trigger;
@@ -1213,6 +1262,11 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
         CK(cudaMemsetAsync(&s->flags_d->steps_done, 0, sizeof(int), s->stream));
         if (done == s->batch) s->batch = std::min(32, s->batch + 2);
       }
+    }
+    if (nvt && nsteps > 0) {   // thermostat state back to the handle
+      CK(cudaMemcpyAsync(s->scalars_h + 9, s->thermo_d, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+      CK(cudaStreamSynchronize(s->stream));
+      s->thermo_xi = s->scalars_h[9]; s->thermo_eta = s->scalars_h[10];
     }
     s->forces_valid = true;
   }

@@ -1947,7 +1947,7 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
       for (int o = 16; o > 0; o >>= 1) d2max = fmax(d2max, __shfl_xor_sync(0xffffffffu, d2max, o));
       if ((threadIdx.x & 31) == 0 && d2max > A.trigger) atomic_max_double_bits(&A.flags->max_disp2_bits[1 - A.parity], d2max);
     }
-    if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
+    if (A.in_run && A.epi != EPI_FORCES && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);   // fused steps only: the unfused paths count in their last kernel
   }
 }
 
@@ -2288,7 +2288,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
       for (int o = 16; o > 0; o >>= 1) d2max = fmax(d2max, __shfl_xor_sync(0xffffffffu, d2max, o));
       if (lane == 0 && d2max > A.trigger) atomic_max_double_bits(&A.flags->max_disp2_bits[1 - A.parity], d2max);
     }
-    if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
+    if (A.in_run && A.epi != EPI_FORCES && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);   // fused steps only: the unfused paths count in their last kernel
   }
 }
 
@@ -2397,7 +2397,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
   }
   if constexpr (MODE == 0) {
     if (A.epi == EPI_KICK_DRIFT) block_max_to_flag(d2max, red, &A.flags->max_disp2_bits[1 - A.parity]);
-    if (A.in_run && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);
+    if (A.in_run && A.epi != EPI_FORCES && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&A.flags->steps_done, 1);   // fused steps only: the unfused paths count in their last kernel
   }
 }
 
@@ -2426,18 +2426,19 @@ template <typename T>
 __global__ void k_initial_integrate(Geom g, int N, size_t ld, double* __restrict__ x, double* __restrict__ v, const double* __restrict__ f,
                                     const double* __restrict__ x0, const int* __restrict__ type, const double* __restrict__ mass,
                                     typename Vec4<T>::type* __restrict__ xr, double dt, double half_dt_ftm2v, unsigned long long* flag,
-                                    const Flags* run_flags) {
+                                    const Flags* run_flags, const double* __restrict__ vscale) {
   __shared__ double red[32];
   if (run_flags && run_flags->stop) return;   // a batched step after the one that found the list stale: do nothing
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   double d2 = 0.0;
+  const double sc = vscale ? *vscale : 1.0;   // NVT: the thermostat's velocity scale of this half step (k_nh_half)
   if (n < N) {
     const int ty = type[n];
     double dtf = half_dt_ftm2v / mass[ty];
     T r[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-      double vv = v[d * ld + n] + dtf * f[d * ld + n];
+      double vv = sc * v[d * ld + n] + dtf * f[d * ld + n];
       double xx = x[d * ld + n] + dt * vv;
       v[d * ld + n] = vv;
       x[d * ld + n] = xx;
@@ -2462,6 +2463,72 @@ __global__ void k_final_integrate(int N, size_t ld, double* __restrict__ v, cons
   double dtf = half_dt_ftm2v / mass[type[n]];
 #pragma unroll
   for (int d = 0; d < 3; ++d) v[d * ld + n] += dtf * f[d * ld + n];
+}
+
+// ---------------------------------------------------------------------------------------------------
+// NVT (reading s25): one Nose-Hoover thermostat, TH(dt/2) kick drift force kick TH(dt/2),
+//   TH(h): xi += h/2 G(KE); s = exp(-xi h); v *= s; KE *= s^2; eta += xi h; xi += h/2 G(KE),  G = (2 KE - g kT)/Q.
+// Thermostat state on the device: th[0] xi, th[1] eta, th[2] KE (energy units), th[3] velocity scale of the last TH,
+// th[4] g kT, th[5] Q.  The per-atom work fuses into the integrator kernels; the scalar update is one thread.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void nh_half(double* th, double h) {
+  double xi = th[0], ke = th[2];
+  const double gkT = th[4], Q = th[5];
+  xi += 0.5 * h * (2.0 * ke - gkT) / Q;
+  const double sc = exp(-xi * h);
+  ke *= sc * sc;
+  th[1] += xi * h;
+  xi += 0.5 * h * (2.0 * ke - gkT) / Q;
+  th[0] = xi; th[2] = ke; th[3] = sc;
+}
+__global__ void k_nh_half(double* th, double h, const Flags* run_flags) {
+  if (run_flags && run_flags->stop) return;
+  nh_half(th, h);
+}
+// second kick + this block's share of the kinetic energy after it (deterministic: one partial per block, no atomics)
+__global__ void __launch_bounds__(256) k_final_integrate_ke(int N, size_t ld, double* __restrict__ v, const double* __restrict__ f,
+                                                            const int* __restrict__ type, const double* __restrict__ mass, double half_dt_ftm2v,
+                                                            double* __restrict__ partial, Flags* run_flags) {
+  __shared__ double red[32];
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (run_flags) {
+    if (run_flags->stop) return;
+    if (n == 0) atomicAdd(&run_flags->steps_done, 1);
+  }
+  double ke[1] = {0.0};
+  if (n < N) {
+    const double m = mass[type[n]], dtf = half_dt_ftm2v / m;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double vv = v[d * ld + n] + dtf * f[d * ld + n];
+      v[d * ld + n] = vv;
+      ke[0] += 0.5 * m * vv * vv;
+    }
+  }
+  block_sum<1>(ke, red);
+  if (threadIdx.x == 0) partial[blockIdx.x] = ke[0];
+}
+// one block: KE = mvv2e * sum of the partials in index order; then TH(h) if h > 0
+__global__ void __launch_bounds__(256) k_nh_reduce(int nblocks, const double* __restrict__ partial, double mvv2e, double* th, double h,
+                                                   const Flags* run_flags) {
+  __shared__ double red[32];
+  if (run_flags && run_flags->stop) return;
+  double s[1] = {0.0};
+  for (int b = threadIdx.x; b < nblocks; b += blockDim.x) s[0] += partial[b];
+  block_sum<1>(s, red);
+  if (threadIdx.x == 0) {
+    th[2] = s[0] * mvv2e;
+    th[3] = 1.0;
+    if (h > 0.0) nh_half(th, h);
+  }
+}
+__global__ void k_scale_velocities(int N, size_t ld, double* __restrict__ v, const double* __restrict__ vscale, const Flags* run_flags) {
+  if (run_flags && run_flags->stop) return;
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= N) return;
+  const double sc = *vscale;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) v[d * ld + n] *= sc;
 }
 
 __global__ void k_kinetic(int N, size_t ld, const double* __restrict__ v, const int* __restrict__ type,

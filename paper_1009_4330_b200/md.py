@@ -20,6 +20,7 @@ MD_ERR_BAD_ARGUMENT, MD_ERR_BOX_TOO_SMALL, MD_ERR_CUDA, MD_ERR_OVERFLOW, MD_ERR_
 MD_FP64, MD_MIXED = 0, 1
 MD_PAIR_LJ126, MD_PAIR_EAM_FS, MD_PAIR_BUCK_COUL = 1, 2, 3
 MD_LIST_FULL, MD_LIST_HALF = 0, 1
+MD_THERMO_NONE, MD_THERMO_NOSE_HOOVER = 0, 1
 MD_KERNEL_AUTO, MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_CELL, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2 = 0, 1, 2, 3, 4, 5, 6
 KERNEL_NAMES = {0: "auto", 1: "tpa", 2: "subwarp8", 3: "warp", 4: "cell", 5: "subwarp4", 6: "subwarp2"}
 
@@ -27,7 +28,7 @@ EXPORTS = [
     "md_create", "md_destroy", "md_set_units", "md_set_precision", "md_set_positions", "md_set_velocities",
     "md_set_pair", "md_set_neighbor", "md_build_neighbors", "md_compute_forces", "md_run", "md_get_positions",
     "md_get_velocities", "md_get_forces", "md_get_neighbors", "md_get_neighbor_rows", "md_kinetic_energy", "md_autotune",
-    "md_get_stats", "md_last_error", "md_set_option", "md_set_pair_coeff", "md_set_type_charges",
+    "md_get_stats", "md_last_error", "md_set_option", "md_set_pair_coeff", "md_set_type_charges", "md_set_thermostat", "md_get_thermostat",
 ]
 
 
@@ -89,6 +90,8 @@ def _load():
     L.md_get_neighbor_rows.argtypes = [vp, ip, ip, ip, ctypes.c_int64]
     L.md_kinetic_energy.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.md_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int64]
+    L.md_set_thermostat.argtypes = [vp, ctypes.c_int, ctypes.c_double, ctypes.c_double]
+    L.md_get_thermostat.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.md_set_pair_coeff.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
     L.md_set_type_charges.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
     L.md_autotune.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
@@ -182,6 +185,14 @@ class System:
     def md_set_type_charges(self, q):
         c = (ctypes.c_double * len(q))(*[float(v) for v in q])
         self._ck(lib.md_set_type_charges(self._h, c, len(q)))
+
+    def md_set_thermostat(self, kind: int, kT: float = 0.0, tau: float = 0.0):
+        self._ck(lib.md_set_thermostat(self._h, int(kind), float(kT), float(tau)))
+
+    def md_get_thermostat(self):
+        out = (ctypes.c_double * 3)()
+        self._ck(lib.md_get_thermostat(self._h, out))
+        return {"xi": out[0], "eta": out[1], "energy": out[2]}
 
     def md_set_neighbor(self, list_kind: int, kernel: int):
         self._ck(lib.md_set_neighbor(self._h, list_kind, kernel))

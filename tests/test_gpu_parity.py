@@ -497,6 +497,54 @@ def test_buck_coul_run_matches_oracle_trajectory():
     s.close()
 
 
+# ---- NVT, one Nose-Hoover thermostat (reading s25) -----------------------------------
+
+@pytest.mark.parametrize("cfg,n,nsteps,kT_factor,tau,list_kind", [(1, 7, 60, 0.5, 0.1, 0), (1, 7, 40, 0.5, 0.1, 1), (4, 6, 40, 2.0, 0.02, 0)])
+def test_nvt_run_matches_oracle_trajectory(cfg, n, nsteps, kT_factor, tau, list_kind):
+    w = wl.make(cfg, n_override=n)
+    kT = kT_factor * w.kT
+    s = md.from_workload(w, precision=md.MD_FP64, kernel=md.MD_KERNEL_TPA, list_kind=list_kind)
+    s.md_set_thermostat(md.MD_THERMO_NOSE_HOOVER, kT, tau)
+    half = nsteps // 2
+    s.md_run(half, w.dt)                       # in two pieces: the thermostat state persists across calls
+    s.md_run(nsteps - half, w.dt)
+    x, v = np.zeros((w.natoms, 3)), np.zeros((w.natoms, 3))
+    s.md_get_positions(x); s.md_get_velocities(v)
+    ref = oracle.run_nvt(w.x, w.v, w.box, np.full(w.natoms, w.mass[0]), w.style, w.params, w.rc, w.skin, w.dt, nsteps,
+                         kT=kT, tau=tau, ftm2v=w.ftm2v, mvv2e=w.mvv2e)
+    assert np.abs(_minimg(x - ref["x"], w.box)).max() < 1e-9
+    assert np.abs(v - ref["v"]).max() < 1e-8 * np.abs(ref["v"]).max()
+    th = s.md_get_thermostat()
+    assert th["xi"] == pytest.approx(ref["thermo"][0], rel=1e-8) and th["eta"] == pytest.approx(ref["thermo"][1], rel=1e-8)
+    assert abs(ref["thermo"][0]) * tau > 1e-3             # the thermostat acted
+    ke = s.md_kinetic_energy()
+    assert ke == pytest.approx(ref["ke"][-1], rel=1e-9)
+    # conserved quantity through the API: KE + PE + thermostat share equals the oracle's H
+    E, _ = s.md_compute_forces(energy=True)
+    assert ke + E + th["energy"] == pytest.approx(ref["h"][-1], rel=1e-9)
+    assert abs(s.md_get_stats()["nbuilds"] - ref["nbuild"]) <= 2
+    s.md_set_thermostat(md.MD_THERMO_NONE)
+    s.close()
+
+
+def test_nvt_mixed_precision_thermalises_and_rejects_bad_arguments():
+    w = wl.make(2, n_override=8)
+    s = md.from_workload(w, kernel=md.MD_KERNEL_AUTO)
+    for kT, tau in [(-1.0, 0.1), (1.0, 0.0), (float("nan"), 0.1)]:
+        with pytest.raises(md.MDError) as e:
+            s.md_set_thermostat(md.MD_THERMO_NOSE_HOOVER, kT, tau)
+        assert e.value.code == md.MD_ERR_BAD_ARGUMENT
+    s.md_set_thermostat(md.MD_THERMO_NOSE_HOOVER, 0.8, 0.2)
+    s.md_run(600, w.dt)
+    g = 3 * w.natoms - 3
+    T = [2.0 * s.md_kinetic_energy() / g]
+    for _ in range(10):
+        s.md_run(40, w.dt)
+        T.append(2.0 * s.md_kinetic_energy() / g)
+    assert np.mean(T) == pytest.approx(0.8, rel=0.06)
+    s.close()
+
+
 # ---- errors and degenerate inputs ------------------------------------------------------------------------------
 
 def test_error_paths():
