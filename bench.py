@@ -162,7 +162,7 @@ def roofline_block(cfg: int, w, st: dict, value: float, hbm_gbs: float, peak_src
         p1 = st["ms_force_pass1_sampled"] / nf
         r["ms_pass1_density"] = p1
         r["ms_pass2_force"] = ms_force - p1
-    t = ncu_summary.traffic(os.path.join(ROOT, PROFILE_MD % cfg))
+    t = ncu_summary.traffic(os.path.join(ROOT, PROFILE_MD % cfg), sections=2 if w.style == wl.PAIR_EAM else 1)
     if t is not None:
         r["traffic"] = t
         r["traffic_source"] = (PROFILE_MD % cfg) + " (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum; both passes summed for EAM)"

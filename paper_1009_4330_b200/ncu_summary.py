@@ -111,17 +111,19 @@ def launches(args) -> None:
         print("\n" + args.note)
 
 
-def traffic(path: str):
-    """DRAM bytes per launch recorded by ``full`` in a summary file (first kernel section), or None."""
+def traffic(path: str, sections: int = 1):
+    """DRAM bytes per launch recorded by ``full`` in a summary file: the sum over the first ``sections`` kernel
+    sections (2 for EAM: density pass + force pass), or None if the file or a section is missing."""
+    found = []
     try:
         with open(path) as fh:
             for line in fh:
                 m = re.match(r"dram_bytes_per_launch:\s*([0-9.eE+]+)", line)
                 if m:
-                    return float(m.group(1))
+                    found.append(float(m.group(1)))
     except OSError:
-        pass
-    return None
+        return None
+    return sum(found[:sections]) if len(found) >= sections else None
 
 
 def main() -> None:
