@@ -23,6 +23,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 
 PAIR_LJ = 1
 PAIR_EAM = 2
+PAIR_EAM_TAB = 4     # params: dict(dr, drho, rho_r=float[nr], phi_r=float[nr], F_rho=float[nrho]): tables on uniform grids from 0
 PAIR_BUCK_COUL = 3   # params: dict(k=Coulomb constant, types=int32[N], q=float[ntypes], coef=float[ntypes, ntypes, 3] = A, rho, C)
 
 
@@ -38,7 +39,10 @@ def build(force: bool = False) -> str:
 class _Pair(ctypes.Structure):
     _fields_ = [("style", ctypes.c_int), ("p", ctypes.c_double * 5), ("rc", ctypes.c_double),
                 ("type", ctypes.POINTER(ctypes.c_int32)), ("ntypes", ctypes.c_int),
-                ("coef", ctypes.POINTER(ctypes.c_double)), ("qtype", ctypes.POINTER(ctypes.c_double))]
+                ("coef", ctypes.POINTER(ctypes.c_double)), ("qtype", ctypes.POINTER(ctypes.c_double)),
+                ("nr", ctypes.c_int), ("nrho", ctypes.c_int), ("dr", ctypes.c_double), ("drho", ctypes.c_double),
+                ("tab_rho", ctypes.POINTER(ctypes.c_double)), ("tab_phi", ctypes.POINTER(ctypes.c_double)),
+                ("tab_F", ctypes.POINTER(ctypes.c_double))]
 
 
 def _pair(style: int, params, rc: float) -> _Pair:
@@ -60,6 +64,17 @@ def _pair(style: int, params, rc: float) -> _Pair:
         p.ntypes = nt
         p.coef = coef.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
         p.qtype = q.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        return p
+    if style == PAIR_EAM_TAB:
+        rho_r = np.ascontiguousarray(params["rho_r"], dtype=np.float64)
+        phi_r = np.ascontiguousarray(params["phi_r"], dtype=np.float64)
+        F_rho = np.ascontiguousarray(params["F_rho"], dtype=np.float64)
+        if len(rho_r) != len(phi_r) or len(rho_r) < 5 or len(F_rho) < 5:
+            raise ValueError("tabulated EAM: rho_r and phi_r must have the same length >= 5, F_rho >= 5")
+        p._keep = (rho_r, phi_r, F_rho)
+        dp = ctypes.POINTER(ctypes.c_double)
+        p.nr, p.nrho, p.dr, p.drho = len(rho_r), len(F_rho), float(params["dr"]), float(params["drho"])
+        p.tab_rho, p.tab_phi, p.tab_F = rho_r.ctypes.data_as(dp), phi_r.ctypes.data_as(dp), F_rho.ctypes.data_as(dp)
         return p
     for k, val in enumerate(params):
         p.p[k] = float(val)
@@ -149,7 +164,7 @@ def forces_brute(x, box, style, params, rc):
     E = ctypes.c_double(0.0)
     W = np.zeros(6)
     npairs = ctypes.c_int64(0)
-    rho = np.zeros(N) if style == PAIR_EAM else None
+    rho = np.zeros(N) if style in (PAIR_EAM, PAIR_EAM_TAB) else None
     P = _pair(style, params, rc)
     lib().orc_forces_brute(N, _d(x), _d(box), ctypes.byref(P), _d(f), ctypes.byref(E), _d(W),
                            ctypes.byref(npairs), _d(rho) if rho is not None else None)
@@ -208,7 +223,7 @@ class NeighborList:
         E = ctypes.c_double(0.0)
         W = np.zeros(6)
         npairs = ctypes.c_int64(0)
-        rho = np.zeros(self.N) if style == PAIR_EAM else None
+        rho = np.zeros(self.N) if style in (PAIR_EAM, PAIR_EAM_TAB) else None
         P = _pair(style, params, rc)
         lib().orc_forces_list(self.N, _d(x), _d(self.box), ctypes.byref(P), self._h, _d(f), ctypes.byref(E), _d(W),
                               ctypes.byref(npairs), _d(rho) if rho is not None else None)

@@ -21,6 +21,11 @@
  *                 (App. A, refs 11,12; the functional form is
  *                 BASELINE.json cfg 4: phi = A exp(-p(r/r0-1)),
  *                 rho = exp(-q(r/r0-1)), F = -B sqrt(rho); reading s12, s13)
+ *   tabulated EAM (SURVEY.md 8(f)-2 "then tabulated/spline EAM (what the paper's EAM run actually used)"; App. A
+ *                 L260; reading s26): rho(r), phi(r) on a uniform grid r_k = k dr and F(rho) on rho_k = k drho, each
+ *                 interpolated by the cubic Hermite polynomial of its interval with node slopes from centred differences
+ *                 (4th order inside, 2nd order next to the ends, one-sided at the ends); the force uses the DERIVATIVE OF
+ *                 THE INTERPOLANT, so it is the exact gradient of the interpolated energy.  Same E and F_i as analytic EAM.
  *   Buckingham + cutoff Coulomb (App. A, the "silicate (cutoff)" workload, LAMMPS
  *                 style buck/coul/cut named there): per type pair (a,b)
  *                 u(r) = A_ab exp(-r/rho_ab) - C_ab / r^6 + k q_a q_b / r,  r^2 < rc^2, plain truncation of all three
@@ -62,6 +67,7 @@
 #define ORC_PAIR_LJ 1
 #define ORC_PAIR_EAM 2
 #define ORC_PAIR_BUCK_COUL 3
+#define ORC_PAIR_EAM_TAB 4
 
 typedef struct {
   int style;        /* ORC_PAIR_LJ, ORC_PAIR_EAM or ORC_PAIR_BUCK_COUL */
@@ -72,7 +78,14 @@ typedef struct {
   int ntypes;
   const double* coef;    /* [ntypes][ntypes][3]: A, rho, C of the type pair (symmetric) */
   const double* qtype;   /* [ntypes] charge of a type */
+  /* ORC_PAIR_EAM_TAB only: tables on uniform grids starting at 0 */
+  int nr, nrho;
+  double dr, drho;
+  const double* tab_rho;  /* [nr]  rho(k dr) */
+  const double* tab_phi;  /* [nr]  phi(k dr) */
+  const double* tab_F;    /* [nrho] F(k drho) */
 } orc_pair;
+#define IS_EAM(P) ((P)->style == ORC_PAIR_EAM || (P)->style == ORC_PAIR_EAM_TAB)
 
 int orc_max_threads(void) {
 #ifdef _OPENMP
@@ -120,14 +133,51 @@ static void pairwise(const orc_pair* P, int64_t i, int64_t j, double r2, double*
   else lj_pair(P, r2, u, fpair);
 }
 
-/* EAM pieces (BASELINE.json cfg 4). */
-static double eam_phi(const orc_pair* P, double r) { return P->p[0] * exp(-P->p[1] * (r / P->p[4] - 1.0)); }
-static double eam_dphi(const orc_pair* P, double r) { return -(P->p[1] / P->p[4]) * eam_phi(P, r); }
-static double eam_rho(const orc_pair* P, double r) { return exp(-P->p[3] * (r / P->p[4] - 1.0)); }
-static double eam_drho(const orc_pair* P, double r) { return -(P->p[3] / P->p[4]) * eam_rho(P, r); }
-static double eam_F(const orc_pair* P, double rho) { return rho > 0.0 ? -P->p[2] * sqrt(rho) : 0.0; }
+/* Tabulated functions (header; reading s26): node slope by centred differences, cubic Hermite inside the interval.
+ * Returns the value, *dy the derivative with respect to x. */
+static double tab_slope(const double* y, int n, double h, int k) {
+  if (k <= 0) return (y[1] - y[0]) / h;
+  if (k >= n - 1) return (y[n - 1] - y[n - 2]) / h;
+  if (k == 1 || k == n - 2) return (y[k + 1] - y[k - 1]) / (2.0 * h);
+  return (y[k - 2] - 8.0 * y[k - 1] + 8.0 * y[k + 1] - y[k + 2]) / (12.0 * h);
+}
+static double tab_eval(const double* y, int n, double h, double x, double* dy) {
+  int k = (int)floor(x / h);
+  if (k < 0) k = 0;
+  if (k > n - 2) k = n - 2;
+  double u = x / h - (double)k;
+  double y0 = y[k], D = y[k + 1] - y[k], m0 = h * tab_slope(y, n, h, k), m1 = h * tab_slope(y, n, h, k + 1);
+  double c2 = 3.0 * D - 2.0 * m0 - m1, c3 = -2.0 * D + m0 + m1;
+  if (dy) *dy = (m0 + u * (2.0 * c2 + 3.0 * c3 * u)) / h;
+  return y0 + u * (m0 + u * (c2 + c3 * u));
+}
+
+/* EAM pieces (BASELINE.json cfg 4); the tabulated style evaluates its tables instead. */
+static double eam_phi(const orc_pair* P, double r) {
+  if (P->style == ORC_PAIR_EAM_TAB) return tab_eval(P->tab_phi, P->nr, P->dr, r, NULL);
+  return P->p[0] * exp(-P->p[1] * (r / P->p[4] - 1.0));
+}
+static double eam_dphi(const orc_pair* P, double r) {
+  if (P->style == ORC_PAIR_EAM_TAB) { double d; tab_eval(P->tab_phi, P->nr, P->dr, r, &d); return d; }
+  return -(P->p[1] / P->p[4]) * eam_phi(P, r);
+}
+static double eam_rho(const orc_pair* P, double r) {
+  if (P->style == ORC_PAIR_EAM_TAB) return tab_eval(P->tab_rho, P->nr, P->dr, r, NULL);
+  return exp(-P->p[3] * (r / P->p[4] - 1.0));
+}
+static double eam_drho(const orc_pair* P, double r) {
+  if (P->style == ORC_PAIR_EAM_TAB) { double d; tab_eval(P->tab_rho, P->nr, P->dr, r, &d); return d; }
+  return -(P->p[3] / P->p[4]) * eam_rho(P, r);
+}
+static double eam_F(const orc_pair* P, double rho) {
+  if (P->style == ORC_PAIR_EAM_TAB) return tab_eval(P->tab_F, P->nrho, P->drho, rho, NULL);
+  return rho > 0.0 ? -P->p[2] * sqrt(rho) : 0.0;
+}
 /* F'(0) := 0 (reading s13) */
-static double eam_dF(const orc_pair* P, double rho) { return rho > 0.0 ? -P->p[2] / (2.0 * sqrt(rho)) : 0.0; }
+static double eam_dF(const orc_pair* P, double rho) {
+  if (P->style == ORC_PAIR_EAM_TAB) { double d; tab_eval(P->tab_F, P->nrho, P->drho, rho, &d); return d; }
+  return rho > 0.0 ? -P->p[2] / (2.0 * sqrt(rho)) : 0.0;
+}
 
 static void zero(double* a, int64_t n) { for (int64_t k = 0; k < n; ++k) a[k] = 0.0; }
 
@@ -163,7 +213,7 @@ void orc_forces_brute(int64_t N, const double* x, const double* box, const orc_p
   double rc2 = P->rc * P->rc, e = 0.0, w[6] = {0, 0, 0, 0, 0, 0};
   int64_t np = 0;
   zero(f, 3 * N);
-  if (P->style != ORC_PAIR_EAM) {
+  if (!IS_EAM(P)) {
     for (int64_t i = 0; i < N; ++i)
       for (int64_t j = i + 1; j < N; ++j) {
         double D[3], r2 = 0.0;
@@ -214,7 +264,7 @@ void orc_forces_sample(int64_t N, const double* x, const double* box, const orc_
   for (int64_t s = 0; s < ns; ++s) {
     int64_t i = ids[s];
     double fi[3] = {0, 0, 0}, e = 0.0;
-    if (P->style != ORC_PAIR_EAM) {
+    if (!IS_EAM(P)) {
       for (int64_t j = 0; j < N; ++j) {
         if (j == i) continue;
         double D[3], r2 = 0.0;
@@ -363,7 +413,7 @@ void orc_forces_list(int64_t N, const double* x, const double* box, const orc_pa
   double rc2 = P->rc * P->rc, e = 0.0, w0 = 0, w1 = 0, w2 = 0, w3 = 0, w4 = 0, w5 = 0;
   int64_t np2 = 0;
   double* dF = NULL;
-  if (P->style == ORC_PAIR_EAM) {
+  if (IS_EAM(P)) {
     double* rho = (double*)malloc((size_t)N * sizeof(double));
     dF = (double*)malloc((size_t)N * sizeof(double));
 #pragma omp parallel for schedule(static) reduction(+ : e)
@@ -389,7 +439,7 @@ void orc_forces_list(int64_t N, const double* x, const double* box, const orc_pa
       for (int a = 0; a < 3; ++a) { D[a] = min_image(x[3 * i + a] - x[3 * j + a], box[a]); r2 += D[a] * D[a]; }
       if (r2 < rc2) {
         double u, fp;
-        if (P->style != ORC_PAIR_EAM) pairwise(P, i, j, r2, &u, &fp);
+        if (!IS_EAM(P)) pairwise(P, i, j, r2, &u, &fp);
         else { double r = sqrt(r2); u = eam_phi(P, r); fp = -((dF[i] + dF[j]) * eam_drho(P, r) + eam_dphi(P, r)) / r; }
         for (int a = 0; a < 3; ++a) ftmp[a] += fp * D[a];
         e += 0.5 * u;
