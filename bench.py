@@ -378,6 +378,17 @@ def run_ours(args, rk) -> None:
             "force_ms_per_launch": msf,
             "force_GBps_survey_bytes": (4.0 * sc["mean_neighbors"] + 52) * w6.natoms / (msf * 1e-3) / 1e9 if msf > 0 else None,
             "note": "next-row workload (SURVEY 8(f)-2): parity in tests/test_gpu_parity.py::test_buck_coul_*; rc 8 A instead of the paper's 15 A (DESIGN.md, known limits)"}
+        # SURVEY.md 8(f)-2, second half: cfg 4 with its potential given as 2001-point tables
+        w7 = wl.make(7)
+        r = time_workload(torch, md, w7, stream, 5, 3, md.MD_KERNEL_AUTO if args.kernel == "auto" else kernel, md.MD_LIST_FULL, host_io=False)
+        sc = r["stats"]
+        msf = sc["ms_force_sampled"] / max(1, sc["nforce_sampled"])
+        per_config["cfg7_eam_tabulated"] = {
+            "workload": w7.name, "value": w7.natoms * w7.nsteps * len(r["ms"]) / (sum(r["ms"]) * 1e-3), "unit": UNIT, "passes_timed": len(r["ms"]),
+            "ms_per_pass": sum(r["ms"]) / len(r["ms"]), "time_steps": w7.nsteps, "builds": sc["nbuilds_in_run"],
+            "variant": md.KERNEL_NAMES[sc["kernel_variant"]], "brick": sc["brick"], "tiles": sc["ntiles"], "mean_neighbors": sc["mean_neighbors"],
+            "force_ms_per_launch": msf, "ms_pass1_density": sc["ms_force_pass1_sampled"] / max(1, sc["nforce_sampled"]),
+            "note": "next-row workload (SURVEY 8(f)-2): parity in tests/test_gpu_parity.py::test_tabulated_eam_*; table lookups through the read-only path"}
         per_config["clocks"] = sampler2.stop(t_pc0, time.perf_counter())
         # the paper's comparison (Eq. 1): neighbor-list kernel against the direct cell-list kernel, and
         # the half list (Newton's third law, atomics), on the bench workload itself

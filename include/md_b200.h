@@ -63,6 +63,10 @@ typedef struct md_system md_system; /* opaque */
 #define MD_PAIR_EAM_FS 2  /* params = {A, p, B, q, r0}: phi = A exp(-p(r/r0-1)), rho = exp(-q(r/r0-1)),
                              F(rho) = -B sqrt(rho), F'(0) := 0; E = sum_i F(rho_i) + 1/2 sum_ij phi (L260) */
 
+#define MD_PAIR_EAM_TAB 4  /* params = {dr, drho}: the same two-pass EAM with rho(r), phi(r) on the grid r_k = k dr and F(rho) on
+                             rho_k = k drho, given by md_set_eam_tables (App. A: what the paper's
+                             EAM run used; reading s26): cubic Hermite interpolation per interval with centred-difference node
+                             slopes; the force uses the derivative of the interpolant */
 #define MD_PAIR_BUCK_COUL 3 /* params = {k}: u_ab = A_ab exp(-r/rho_ab) - C_ab/r^6 + k q_a q_b / r, all three terms cut plainly at rc
                              (App. A "silicate (cutoff)", LAMMPS buck/coul/cut).  Per type pair
                              A, rho, C by md_set_pair_coeff, per type charge by md_set_type_charges; at most 4 types;
@@ -154,6 +158,10 @@ int md_set_pair(md_system* s, int style, const double* params, int nparams, doub
  * (App. A "26 pair force styles": per-type-pair coefficients as in LAMMPS pair_coeff).  Every pair of
  * the system's types must be set before the next force evaluation (MD_ERR_NOT_READY otherwise); rho must be positive. */
 int md_set_pair_coeff(md_system* s, int type_a, int type_b, const double* coeff, int n);
+/* MD_PAIR_EAM_TAB only (after md_set_pair): the tables rho_r[nr], phi_r[nr] at r = 0, dr, 2 dr, ... and F_rho[nrho] at
+ * rho = 0, drho, ... (host pointers; copied).  The r grid must reach the cutoff (checked at the next build); distances
+ * and densities beyond a table's end are evaluated with its last interval's cubic.  (App. A; reading s26) */
+int md_set_eam_tables(md_system* s, const double* rho_r, const double* phi_r, int nr, const double* F_rho, int nrho);
 /* MD_PAIR_BUCK_COUL only: the charge of every atom type, n = ntypes values (the paper's silicate carries one charge per
  * species, App. A).  Host pointer. */
 int md_set_type_charges(md_system* s, const double* q, int n);

@@ -40,6 +40,10 @@ struct md_system_impl {
   double pair_coef[MAX_PAIR_TYPES][MAX_PAIR_TYPES][3] = {};
   bool pair_coef_set[MAX_PAIR_TYPES][MAX_PAIR_TYPES] = {};
   double qtype[MAX_PAIR_TYPES] = {0, 0, 0, 0};
+  // MD_PAIR_EAM_TAB: per-interval cubic coefficients of rho(r), phi(r) (float4 and double4 copies) and F(rho) (double4)
+  int eam_nr = 0, eam_nrho = 0;
+  float4* tab_rho_f = nullptr; float4* tab_phi_f = nullptr;
+  double4* tab_rho_dd = nullptr; double4* tab_phi_dd = nullptr; double4* tab_F_dd = nullptr;
   double rc = 0, skin = 0;
   int list_kind = MD_LIST_FULL;
   int kernel_req = MD_KERNEL_TPA;
@@ -400,6 +404,15 @@ int plan(md_system* s) {
     double eps = s->params[0], sg = s->params[1];
     double s6 = std::pow(sg, 6), s12 = s6 * s6;
     P.lj1 = 48.0 * eps * s12; P.lj2 = 24.0 * eps * s6; P.lj3 = 4.0 * eps * s12; P.lj4 = 4.0 * eps * s6;
+  } else if (s->style == MD_PAIR_EAM_TAB) {
+    if (!s->tab_F_dd) return fail(s, MD_ERR_NOT_READY, "md_set_eam_tables has not been called");
+    const double rmax = (s->eam_nr - 1) * s->params[0];
+    if (rmax < s->rc) return fail(s, MD_ERR_BAD_ARGUMENT, "the EAM tables end at r = %g, before the cutoff %g", rmax, s->rc);
+    P.tab_rho = s->precision == MD_FP64 ? (const void*)s->tab_rho_dd : (const void*)s->tab_rho_f;
+    P.tab_phi = s->precision == MD_FP64 ? (const void*)s->tab_phi_dd : (const void*)s->tab_phi_f;
+    P.tab_F = s->tab_F_dd;
+    P.tab_nr = s->eam_nr; P.tab_nrho = s->eam_nrho;
+    P.inv_dr = 1.0 / s->params[0]; P.inv_drho = 1.0 / s->params[1];
   } else if (s->style == MD_PAIR_BUCK_COUL) {
     if (s->ntypes > MAX_PAIR_TYPES) return fail(s, MD_ERR_BAD_ARGUMENT, "MD_PAIR_BUCK_COUL supports at most %d atom types", MAX_PAIR_TYPES);
     for (int a = 0; a < s->ntypes; ++a)
@@ -652,15 +665,17 @@ int launch_force_T(md_system* s, const StepMode& M) {
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
   } else {
-    int rc = launch_force_variant<T, EamDensityBody, 1, EV>(s, A);   // pass 1: rho, F'(rho), sum F(rho)
+    const bool tab = s->style == MD_PAIR_EAM_TAB;
+    int rc = tab ? launch_force_variant<T, EamTabDensityBody, 1, EV>(s, A)
+                 : launch_force_variant<T, EamDensityBody, 1, EV>(s, A);   // pass 1: rho, F'(rho), sum F(rho)
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 0));
     if (g.half && s->kernel_eff != MD_KERNEL_CELL)   // half list: rho was scattered with atomics, so F'(rho) needs its own pass
-      CK(launch(s, k_eam_embed<T>, blocks_for(s->N, 256), 256, 0, (int)s->N, s->P.B, (const double*)s->rho, s->fp, (T*)s->xr[xb],
+      CK(launch(s, k_eam_embed<T>, blocks_for(s->N, 256), 256, 0, (int)s->N, s->P, (const double*)s->rho, s->fp, (T*)s->xr[xb],
                 EV ? s->scalars_d : (double*)nullptr));
     if (s->mid_event) CK(cudaEventRecord(s->mid_event, s->stream));
     A.fp_in = s->fp;
-    rc = launch_force_variant<T, EamForceBody, 0, EV>(s, A);          // pass 2: forces
+    rc = tab ? launch_force_variant<T, EamTabForceBody, 0, EV>(s, A) : launch_force_variant<T, EamForceBody, 0, EV>(s, A);   // pass 2: forces
     if (rc) return rc;
     if (EV) CK(launch(s, k_reduce_ev, 1, 256, 0, g.ntiles, (const double*)s->ev_partials, s->scalars_d, 1));
   }
@@ -884,6 +899,7 @@ void md_destroy(md_system* s) {
   cudaFree(s->f); cudaFree(s->x0); cudaFree(s->rho); cudaFree(s->fp); cudaFree(s->cell_of); cudaFree(s->rank); cudaFree(s->perm); cudaFree(s->mkey);
   cudaFree(s->nstat_d); cudaFree(s->export_buf);
   cudaFree(s->numneigh); cudaFree(s->cell_count); cudaFree(s->cell_start); cudaFree(s->list); cudaFree(s->mass_d); cudaFree(s->dtf_d); cudaFree(s->thermo_d); cudaFree(s->ke_partial_d);
+  cudaFree(s->tab_rho_f); cudaFree(s->tab_phi_f); cudaFree(s->tab_rho_dd); cudaFree(s->tab_phi_dd); cudaFree(s->tab_F_dd);
   cudaFree(s->ev_partials); cudaFree(s->scalars_d); cudaFree(s->io_d); cudaFree(s->io_i); cudaFree(s->types_caller); cudaFree(s->flags_d);
   if (s->flags_h) cudaFreeHost(s->flags_h);
   if (s->scalars_h) cudaFreeHost(s->scalars_h);
@@ -959,13 +975,14 @@ int md_set_velocities(md_system* s, const double* v) {
 
 int md_set_pair(md_system* s, int style, const double* params, int nparams, double rc, double skin) {
   if (!s || !params) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: NULL") : MD_ERR_BAD_ARGUMENT;
-  int need = style == MD_PAIR_LJ126 ? 2 : (style == MD_PAIR_EAM_FS ? 5 : (style == MD_PAIR_BUCK_COUL ? 1 : -1));
+  int need = style == MD_PAIR_LJ126 ? 2 : (style == MD_PAIR_EAM_FS ? 5 : (style == MD_PAIR_BUCK_COUL ? 1 : (style == MD_PAIR_EAM_TAB ? 2 : -1)));
   if (need < 0) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: unknown style %d", style);
   if (nparams != need) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: style %d takes %d parameters, got %d", style, need, nparams);
   if (!(rc > 0.0) || !(skin >= 0.0) || !std::isfinite(rc) || !std::isfinite(skin)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: bad rc/skin");
   for (int k = 0; k < need; ++k)
     if (!std::isfinite(params[k])) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: non-finite parameter");
   if (style == MD_PAIR_EAM_FS && !(params[4] > 0.0)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: r0 must be positive");
+  if (style == MD_PAIR_EAM_TAB && (!(params[0] > 0.0) || !(params[1] > 0.0))) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair: dr and drho must be positive");
   for (int d = 0; d < 3; ++d)
     if (s->box[d] < 3.0 * (rc + skin))
       return fail(s, MD_ERR_BOX_TOO_SMALL, "box edge %d = %g < 3 (rc+skin) = %g", d, s->box[d], 3.0 * (rc + skin));
@@ -985,6 +1002,48 @@ int md_set_pair_coeff(md_system* s, int type_a, int type_b, const double* c, int
     return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_pair_coeff: coefficients must be finite and rho positive");
   for (int k = 0; k < 3; ++k) s->pair_coef[type_a][type_b][k] = s->pair_coef[type_b][type_a][k] = c[k];
   s->pair_coef_set[type_a][type_b] = s->pair_coef_set[type_b][type_a] = true;
+  s->planned = false; s->forces_valid = false;
+  return MD_OK;
+}
+
+// per-interval cubic of a uniform table (reading s26): node slopes by centred differences (4th order inside, 2nd order next
+// to the ends, one-sided at the ends), Hermite cubic c0 + c1 u + c2 u^2 + c3 u^3 on [k, k+1]
+static void table_cubics(const double* y, int n, double h, std::vector<double>& c) {
+  auto slope = [&](int k) {
+    if (k <= 0) return (y[1] - y[0]) / h;
+    if (k >= n - 1) return (y[n - 1] - y[n - 2]) / h;
+    if (k == 1 || k == n - 2) return (y[k + 1] - y[k - 1]) / (2.0 * h);
+    return (y[k - 2] - 8.0 * y[k - 1] + 8.0 * y[k + 1] - y[k + 2]) / (12.0 * h);
+  };
+  c.resize(4 * (size_t)(n - 1));
+  for (int k = 0; k < n - 1; ++k) {
+    const double D = y[k + 1] - y[k], m0 = h * slope(k), m1 = h * slope(k + 1);
+    c[4 * k] = y[k]; c[4 * k + 1] = m0; c[4 * k + 2] = 3.0 * D - 2.0 * m0 - m1; c[4 * k + 3] = -2.0 * D + m0 + m1;
+  }
+}
+
+int md_set_eam_tables(md_system* s, const double* rho_r, const double* phi_r, int nr, const double* F_rho, int nrho) {
+  if (!s || !rho_r || !phi_r || !F_rho) return s ? fail(s, MD_ERR_BAD_ARGUMENT, "md_set_eam_tables: NULL") : MD_ERR_BAD_ARGUMENT;
+  if (nr < 5 || nrho < 5 || nr > (1 << 24) || nrho > (1 << 24)) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_eam_tables: tables need 5 .. 2^24 entries");
+  if (s->style != MD_PAIR_EAM_TAB) return fail(s, MD_ERR_NOT_READY, "md_set_eam_tables: call md_set_pair(MD_PAIR_EAM_TAB, {dr, drho}, ...) first");
+  for (int k = 0; k < nr; ++k) if (!std::isfinite(rho_r[k]) || !std::isfinite(phi_r[k])) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_eam_tables: non-finite entry");
+  for (int k = 0; k < nrho; ++k) if (!std::isfinite(F_rho[k])) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_eam_tables: non-finite entry");
+  std::vector<double> cr, cp, cF;
+  table_cubics(rho_r, nr, s->params[0], cr);
+  table_cubics(phi_r, nr, s->params[0], cp);
+  table_cubics(F_rho, nrho, s->params[1], cF);
+  std::vector<float> fr(cr.begin(), cr.end()), fpv(cp.begin(), cp.end());
+  cudaFree(s->tab_rho_f); cudaFree(s->tab_phi_f); cudaFree(s->tab_rho_dd); cudaFree(s->tab_phi_dd); cudaFree(s->tab_F_dd);
+  s->tab_rho_f = s->tab_phi_f = nullptr; s->tab_rho_dd = s->tab_phi_dd = s->tab_F_dd = nullptr;
+  CK(dalloc(&s->tab_rho_f, (size_t)nr - 1)); CK(dalloc(&s->tab_phi_f, (size_t)nr - 1));
+  CK(dalloc(&s->tab_rho_dd, (size_t)nr - 1)); CK(dalloc(&s->tab_phi_dd, (size_t)nr - 1)); CK(dalloc(&s->tab_F_dd, (size_t)nrho - 1));
+  CK(cudaMemcpyAsync(s->tab_rho_f, fr.data(), fr.size() * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->tab_phi_f, fpv.data(), fpv.size() * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->tab_rho_dd, cr.data(), cr.size() * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->tab_phi_dd, cp.data(), cp.size() * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->tab_F_dd, cF.data(), cF.size() * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaStreamSynchronize(s->stream));   // the staging vectors are locals
+  s->eam_nr = nr; s->eam_nrho = nrho;
   s->planned = false; s->forces_valid = false;
   return MD_OK;
 }
@@ -1095,7 +1154,7 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
   const int64_t sample_every = (nsteps + md_system_impl::NSAMPLE - 1) / md_system_impl::NSAMPLE;
   int nsampled = 0;
   s->ms_force_sampled = 0; s->ms_pass1_sampled = 0;
-  const bool eam = s->style == MD_PAIR_EAM_FS;
+  const bool eam = s->style == MD_PAIR_EAM_FS || s->style == MD_PAIR_EAM_TAB;
   const bool nvt = s->thermostat == MD_THERMO_NOSE_HOOVER;
   const bool fused = s->list_kind != MD_LIST_HALF && !nvt;
   if (nsteps > 0 && fused) {

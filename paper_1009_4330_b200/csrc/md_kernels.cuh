@@ -1220,6 +1220,13 @@ struct PairParams {    // host-prepared constants, in double; kernels convert on
   // the same rounded to fp32 once on the host (fill_float_copies): the mixed-precision bodies read these straight
   // from the constant bank instead of converting the doubles inside the list loop
   float f_rc2, f_lj1, f_lj2, f_lj3, f_lj4, f_A, f_p_r0, f_q_r0, f_p, f_q;
+  // tabulated EAM (reading s26): per interval k of the uniform grids the cubic c0 + c1 u + c2 u^2 + c3 u^3, u = x/h - k
+  // (host: md_set_eam_tables); rho(r) and phi(r) in the pair-math precision, F(rho) in double.  NULL: analytic EAM
+  const void* tab_rho;     // [tab_nr - 1] Vec4<T>
+  const void* tab_phi;     // [tab_nr - 1] Vec4<T>
+  const double4* tab_F;    // [tab_nrho - 1]
+  int tab_nr, tab_nrho;
+  double inv_dr, inv_drho;
   // Buckingham + cutoff Coulomb: per type pair (ta, tb), entry 4 ta + tb: A, 1/rho, C, k q_a q_b
   double bc[MAX_PAIR_TYPES * MAX_PAIR_TYPES][4];
   __host__ void fill_float_copies() {
@@ -1364,6 +1371,123 @@ struct EamForceBody {
     p[0] = pk_fma(fp, dx, p[0]); p[1] = pk_fma(fp, dy, p[1]); p[2] = pk_fma(fp, dz, p[2]);
     if constexpr (EV) {
       p[3] = pk_add(p[3], phi);
+      virial2(dx, dy, dz, fp, p);
+    }
+  }
+};
+
+// Embedding function of one atom: F(rho) and F'(rho).  Analytic (BASELINE.json cfg 4): F = -B sqrt(rho), F'(0) := 0
+// (reading s13); tabulated (reading s26): the cubic of rho's interval and its derivative.
+__device__ __forceinline__ void eam_embed(const PairParams& P, double rho, double& F, double& dF) {
+  if (P.tab_F) {
+    const double t = rho * P.inv_drho;
+    int k = (int)floor(t);
+    k = k < 0 ? 0 : (k > P.tab_nrho - 2 ? P.tab_nrho - 2 : k);
+    const double u = t - (double)k;
+    const double4 c = P.tab_F[k];
+    F = c.x + u * (c.y + u * (c.z + u * c.w));
+    dF = (c.y + u * (2.0 * c.z + 3.0 * c.w * u)) * P.inv_drho;
+  } else {
+    const double sq = sqrt(rho);
+    F = -P.B * sq;
+    dF = rho > 0.0 ? -P.B / (2.0 * sq) : 0.0;
+  }
+}
+
+// Tabulated EAM (SURVEY.md 8(f)-2 second half; App. A: what the paper's EAM run used; reading s26).  The same
+// two passes as the analytic style with rho(r), rho'(r), phi(r), phi'(r) from per-interval cubics: one 16-byte (fp64: 32)
+// table load per function, atom of the row and list entry, through the read-only path (the tables are a few tens of KB).
+template <typename T>
+struct TabLookup {
+  using V4 = typename Vec4<T>::type;
+  T inv_dr;
+  int kmax;
+  __device__ __forceinline__ int interval(T r, T& u) const {
+    const T t = r * inv_dr;
+    int k = (int)t;
+    k = k > kmax ? kmax : (k < 0 ? 0 : k);   // (r = NaN for the self term r2 = 0 of the cell-list variant: any interval will do, the term is dropped)
+    u = t - (T)k;
+    return k;
+  }
+  static __device__ __forceinline__ V4 load(const void* tab, int k) {
+    if constexpr (sizeof(T) == 4) return __ldg(reinterpret_cast<const float4*>(tab) + k);
+    else { const double2* q = reinterpret_cast<const double2*>(tab) + 2 * (size_t)k; const double2 a = __ldg(q), b = __ldg(q + 1); return make_double4(a.x, a.y, b.x, b.y); }
+  }
+  static __device__ __forceinline__ T value(const V4& c, T u) { return c.x + u * (c.y + u * (c.z + u * c.w)); }
+  __device__ __forceinline__ T slope(const V4& c, T u) const { return (c.y + u * ((T)2 * c.z + (T)3 * c.w * u)) * inv_dr; }
+};
+
+template <typename T, bool EV>
+struct EamTabDensityBody {
+  static constexpr int NT = 1;
+  using PK = typename Pk<T>::type;
+  static __device__ __forceinline__ T own_w(T w) { return -w; }
+  static __device__ __forceinline__ T mutual_w(T a, T b) { return a + b; }
+  static __device__ __forceinline__ T cell_own_w(T w) { return w; }
+  template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
+  static constexpr bool TABLE = false;
+  T rc2;
+  TabLookup<T> L;
+  const void* tab_rho;
+  __device__ explicit EamTabDensityBody(const PairParams& P) : rc2(MDK_PP(rc2)), L{(T)P.inv_dr, P.tab_nr - 2}, tab_rho(P.tab_rho) {}
+  __device__ __forceinline__ T rho_of(T r2) const {
+    T u;
+    const int k = L.interval(r2 * t_rsqrt<T>(r2), u);
+    return TabLookup<T>::value(TabLookup<T>::load(tab_rho, k), u);
+  }
+  __device__ __forceinline__ void pair(T, T, T, T r2, T, bool ok, T (&p)[NT]) const { p[0] += (ok && r2 < rc2) ? rho_of(r2) : (T)0; }
+  __device__ __forceinline__ void pair2(PK, PK, PK, PK r2, PK, PK (&p)[NT]) const {
+    const T ra = pk_lo(r2), rb = pk_hi(r2);
+    // (an entry beyond the cutoff may lie beyond the table too: its interval is clamped and its value dropped)
+    const T ea = ra < rc2 ? rho_of(ra) : (T)0, eb = rb < rc2 ? rho_of(rb) : (T)0;
+    p[0] = pk_add(p[0], pk_make(ea, eb));
+  }
+};
+
+template <typename T, bool EV>
+struct EamTabForceBody {
+  static constexpr int NT = EV ? 10 : 3;
+  using PK = typename Pk<T>::type;
+  using V4 = typename Vec4<T>::type;
+  static __device__ __forceinline__ T own_w(T w) { return -w; }
+  static __device__ __forceinline__ T mutual_w(T a, T b) { return a + b; }
+  static __device__ __forceinline__ T cell_own_w(T w) { return w; }
+  template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
+  static constexpr bool TABLE = false;
+  T rc2;
+  TabLookup<T> L;
+  const void *tab_rho, *tab_phi;
+  __device__ explicit EamTabForceBody(const PairParams& P)
+      : rc2(MDK_PP(rc2)), L{(T)P.inv_dr, P.tab_nr - 2}, tab_rho(P.tab_rho), tab_phi(P.tab_phi) {}
+  // fpair = -[ (F'_i + F'_j) rho'(r) + phi'(r) ] / r and phi(r) of one term; zero beyond the cutoff
+  __device__ __forceinline__ void term(T r2, T wsum, T& fp, T& phi) const {
+    const bool in = r2 < rc2;
+    const T rinv = t_rsqrt<T>(r2);
+    T u;
+    const int k = L.interval(r2 * rinv, u);
+    const V4 cr = TabLookup<T>::load(tab_rho, k), cp = TabLookup<T>::load(tab_phi, k);
+    fp = in ? -(wsum * L.slope(cr, u) + L.slope(cp, u)) * rinv : (T)0;
+    phi = in ? TabLookup<T>::value(cp, u) : (T)0;
+  }
+  __device__ __forceinline__ void pair(T dx, T dy, T dz, T r2, T wsum, bool ok, T (&p)[NT]) const {
+    T fp, phi;
+    term(r2, wsum, fp, phi);
+    if (!ok) { fp = (T)0; phi = (T)0; }
+    p[0] += fp * dx; p[1] += fp * dy; p[2] += fp * dz;
+    if constexpr (EV) {
+      p[3] += phi;
+      p[4] += dx * dx * fp; p[5] += dy * dy * fp; p[6] += dz * dz * fp;
+      p[7] += dx * dy * fp; p[8] += dx * dz * fp; p[9] += dy * dz * fp;
+    }
+  }
+  __device__ __forceinline__ void pair2(PK dx, PK dy, PK dz, PK r2, PK wsum, PK (&p)[NT]) const {
+    T fa, fb, pa, pb;
+    term(pk_lo(r2), pk_lo(wsum), fa, pa);
+    term(pk_hi(r2), pk_hi(wsum), fb, pb);
+    const PK fp = pk_make(fa, fb);
+    p[0] = pk_fma(fp, dx, p[0]); p[1] = pk_fma(fp, dy, p[1]); p[2] = pk_fma(fp, dz, p[2]);
+    if constexpr (EV) {
+      p[3] = pk_add(p[3], pk_make(pa, pb));
       virial2(dx, dy, dz, fp, p);
     }
   }
@@ -1923,12 +2047,12 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
           for (int a = 0; a < 2; ++a) {
             if (a == 1 && !act1) break;
             const double rho = a ? tot1[0] : tot0[0];
-            const double sq = sqrt(rho);
-            const double fpv = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
+            double Fv, fpv;
+            eam_embed(A.P, rho, Fv, fpv);
             A.rho[gi + a] = rho;
             A.fp_out[gi + a] = fpv;
             reinterpret_cast<T*>(const_cast<void*>(A.xr))[4 * (size_t)(gi + a) + 3] = (T)(-fpv);   // read back as pj.w by pass 2
-            if constexpr (EV) ev[0] += -A.P.B * sq;                  // embedding energy F(rho_i)
+            if constexpr (EV) ev[0] += Fv;                           // embedding energy F(rho_i)
           }
         }
       }
@@ -1954,17 +2078,17 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
 // EAM with a half list, between the two passes: rho (accumulated with atomics by pass 1) -> F'(rho), the packed
 // w = -F'(rho) that pass 2 gathers, and the embedding energy (one partial per block, added to ev_partials[.][0]).
 template <typename T>
-__global__ void __launch_bounds__(256) k_eam_embed(int N, double B, const double* __restrict__ rho, double* __restrict__ fp, T* __restrict__ xr4,
+__global__ void __launch_bounds__(256) k_eam_embed(int N, PairParams P, const double* __restrict__ rho, double* __restrict__ fp, T* __restrict__ xr4,
                                                    double* __restrict__ ev_out) {
   __shared__ double red[32];
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   double e[1] = {0.0};
   if (n < N) {
-    const double r = rho[n], sq = sqrt(r);
-    const double fpv = r > 0.0 ? -B / (2.0 * sq) : 0.0;
+    double Fv, fpv;
+    eam_embed(P, rho[n], Fv, fpv);
     fp[n] = fpv;
     xr4[4 * (size_t)n + 3] = (T)(-fpv);
-    e[0] = -B * sq;
+    e[0] = Fv;
   }
   if (ev_out) {
     block_sum<1>(e, red);
@@ -2269,8 +2393,8 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
           for (int a = 0; a < 2; ++a) {
             if (a == 1 && !act1) break;
             const double rho = a ? tot1[0] : tot0[0];
-            const double sq = sqrt(rho);
-            const double fpv = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;   // F'(0) := 0 (reading s13)
+            double Fv, fpv;
+            eam_embed(A.P, rho, Fv, fpv);
             A.rho[gi + a] = rho;
             A.fp_out[gi + a] = fpv;
             reinterpret_cast<T*>(const_cast<void*>(A.xr))[4 * (size_t)(gi + a) + 3] = (T)(-fpv);   // read back as pj.w by pass 2
@@ -2381,10 +2505,11 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_cell_force(ForceArgs A) {
             for (int k = 0; k < 7; ++k) ev[k] += 0.5 * tot[3 + k];
         } else {
           const double rho = tot[0];
-          const double sq = sqrt(rho);
+          double Fv, fpv;
+          eam_embed(A.P, rho, Fv, fpv);
           A.rho[gi] = rho;
-          A.fp_out[gi] = rho > 0.0 ? -A.P.B / (2.0 * sq) : 0.0;
-          if constexpr (EV) ev[0] += -A.P.B * sq;
+          A.fp_out[gi] = fpv;
+          if constexpr (EV) ev[0] += Fv;
         }
       }
     }

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libmd_b200.so")
 MD_OK = 0
 MD_ERR_BAD_ARGUMENT, MD_ERR_BOX_TOO_SMALL, MD_ERR_CUDA, MD_ERR_OVERFLOW, MD_ERR_NOT_READY, MD_ERR_NONFINITE = -1, -2, -3, -4, -5, -6
 MD_FP64, MD_MIXED = 0, 1
-MD_PAIR_LJ126, MD_PAIR_EAM_FS, MD_PAIR_BUCK_COUL = 1, 2, 3
+MD_PAIR_LJ126, MD_PAIR_EAM_FS, MD_PAIR_BUCK_COUL, MD_PAIR_EAM_TAB = 1, 2, 3, 4
 MD_LIST_FULL, MD_LIST_HALF = 0, 1
 MD_THERMO_NONE, MD_THERMO_NOSE_HOOVER = 0, 1
 MD_KERNEL_AUTO, MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_CELL, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2 = 0, 1, 2, 3, 4, 5, 6
@@ -28,7 +28,7 @@ EXPORTS = [
     "md_create", "md_destroy", "md_set_units", "md_set_precision", "md_set_positions", "md_set_velocities",
     "md_set_pair", "md_set_neighbor", "md_build_neighbors", "md_compute_forces", "md_run", "md_get_positions",
     "md_get_velocities", "md_get_forces", "md_get_neighbors", "md_get_neighbor_rows", "md_kinetic_energy", "md_autotune",
-    "md_get_stats", "md_last_error", "md_set_option", "md_set_pair_coeff", "md_set_type_charges", "md_set_thermostat", "md_get_thermostat",
+    "md_get_stats", "md_last_error", "md_set_option", "md_set_pair_coeff", "md_set_type_charges", "md_set_thermostat", "md_get_thermostat", "md_set_eam_tables",
 ]
 
 
@@ -90,6 +90,8 @@ def _load():
     L.md_get_neighbor_rows.argtypes = [vp, ip, ip, ip, ctypes.c_int64]
     L.md_kinetic_energy.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.md_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int64]
+    L.md_set_eam_tables.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), ctypes.c_int,
+                                    ctypes.POINTER(ctypes.c_double), ctypes.c_int]
     L.md_set_thermostat.argtypes = [vp, ctypes.c_int, ctypes.c_double, ctypes.c_double]
     L.md_get_thermostat.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.md_set_pair_coeff.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
@@ -194,6 +196,13 @@ class System:
         self._ck(lib.md_get_thermostat(self._h, out))
         return {"xi": out[0], "eta": out[1], "energy": out[2]}
 
+    def md_set_eam_tables(self, rho_r, phi_r, F_rho):
+        dp = ctypes.POINTER(ctypes.c_double)
+        a, b, c = (np.ascontiguousarray(t, dtype=np.float64) for t in (rho_r, phi_r, F_rho))
+        if len(a) != len(b):
+            raise ValueError("rho_r and phi_r must have the same length")
+        self._ck(lib.md_set_eam_tables(self._h, a.ctypes.data_as(dp), b.ctypes.data_as(dp), len(a), c.ctypes.data_as(dp), len(c)))
+
     def md_set_neighbor(self, list_kind: int, kernel: int):
         self._ck(lib.md_set_neighbor(self._h, list_kind, kernel))
 
@@ -257,6 +266,8 @@ def from_workload(w, precision: int | None = None, list_kind: int = MD_LIST_FULL
     for name, value in (options or {}).items():
         s.md_set_option(name, value)
     s.md_set_pair(w.style, w.params, w.rc, w.skin)
+    if w.style == MD_PAIR_EAM_TAB:
+        s.md_set_eam_tables(w.tables["rho_r"], w.tables["phi_r"], w.tables["F_rho"])
     if w.style == MD_PAIR_BUCK_COUL:
         nt = len(w.mass)
         for a in range(nt):

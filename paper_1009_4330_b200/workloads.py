@@ -28,6 +28,7 @@ FTM2V_METAL = 1.0 / 1.0364269e-4
 PAIR_LJ = 1
 PAIR_EAM = 2
 PAIR_BUCK_COUL = 3
+PAIR_EAM_TAB = 4
 PREC_FP64 = 0
 PREC_MIXED = 1
 
@@ -124,6 +125,7 @@ class Workload:
     seed: int
     qtype: np.ndarray | None = None       # PAIR_BUCK_COUL: charge of every type
     pair_coef: np.ndarray | None = None   # PAIR_BUCK_COUL: [ntypes, ntypes, 3] = A, rho, C of every type pair (symmetric)
+    tables: dict | None = None            # PAIR_EAM_TAB: dict(dr, drho, rho_r, phi_r, F_rho)
 
     @property
     def natoms(self) -> int:
@@ -178,16 +180,33 @@ def make_silicate_like(n: int = 48, seed_offset: int = 0, rc: float = 8.0, skin:
                     precision=PREC_MIXED, ftm2v=FTM2V_METAL, mvv2e=MVV2E_METAL, kT=kT, seed=seed, qtype=np.array(SILICATE_Q), pair_coef=coef)
 
 
+def make_eam_tabulated(n_cells: int = 40, n_table: int = 2001, rmax: float = 6.0, rhomax: float = 60.0, seed_offset: int = 0) -> Workload:
+    """cfg 4 with its potential given as TABLES (App. A: the paper's EAM run read a tabulated
+    Cu potential file, which is not in the container): the Finnis-Sinclair functions of BASELINE.json cfg 4 sampled on
+    ``n_table`` points of [0, rmax] A and [0, rhomax].  An input table, like the lattice: the interpolation is the method's."""
+    w = make(4, n_override=n_cells, seed_offset=seed_offset)
+    A, p, B, q, r0 = EAM_PARAMS
+    dr, drho = rmax / (n_table - 1), rhomax / (n_table - 1)
+    r, rh = np.arange(n_table) * dr, np.arange(n_table) * drho
+    tables = dict(dr=dr, drho=drho, rho_r=np.exp(-q * (r / r0 - 1.0)), phi_r=A * np.exp(-p * (r / r0 - 1.0)), F_rho=-B * np.sqrt(rh))
+    return dataclasses.replace(w, name="EAM Cu tabulated (%d-point tables) %d atoms mixed" % (n_table, w.natoms), cfg=7, style=PAIR_EAM_TAB,
+                               params=(dr, drho), tables=tables)
+
+
 def oracle_params(w: Workload):
     """The pair parameters of ``w`` in the form the CPU oracle's wrapper takes them (packing only)."""
     if w.style == PAIR_BUCK_COUL:
         return dict(k=w.params[0], types=w.types, q=w.qtype, coef=w.pair_coef)
+    if w.style == PAIR_EAM_TAB:
+        return w.tables
     return w.params
 
 
 def make(cfg: int, n_override: int | None = None, seed_offset: int = 0) -> Workload:
     """Build config ``cfg`` (1..5) of BASELINE.json (6: the synthetic two-species workload of SURVEY.md 8(f)-2).  ``n_override`` shrinks the
     lattice (unit cells per edge) for tests; ``seed_offset`` decorrelates replicas."""
+    if cfg == 7:
+        return make_eam_tabulated(40 if n_override is None else int(n_override), seed_offset=seed_offset)
     if cfg == 6:
         return make_silicate_like(48 if n_override is None else int(n_override), seed_offset)
     name, style, n, rc, skin, dt, nsteps, prec, permuted = _TABLE[cfg]

@@ -497,6 +497,59 @@ def test_buck_coul_run_matches_oracle_trajectory():
     s.close()
 
 
+# ---- SURVEY.md 8(f)-2, second half: tabulated EAM (App. A; reading s26) -------------------------------
+
+@pytest.mark.parametrize("name,kernel,list_kind", [("tpa", 1, 0), ("subwarp4", 5, 0), ("warp", 3, 0), ("cell", 4, 0), ("half", 1, 1)])
+@pytest.mark.parametrize("precision", [0, 1])   # MD_FP64, MD_MIXED
+def test_tabulated_eam_forces_energy_virial(name, kernel, list_kind, precision):
+    w = wl.make_eam_tabulated(6, n_table=1501)
+    x = wl.perturbed(w, 0.2)
+    fo, Eo, Wo, _, rho_o = oracle.forces_brute(x, w.box, w.style, wl.oracle_params(w), w.rc)
+    s = md.from_workload(w, precision=precision, kernel=kernel, list_kind=list_kind, x=x)
+    f = np.zeros((w.natoms, 3))
+    E, W = s.md_compute_forces(f, energy=True, virial=True)
+    if precision == md.MD_FP64:
+        assert _fp64_force_err(f, fo) < 1e-11
+        assert abs(E - Eo) < 1e-12 * abs(Eo) and np.abs(W - Wo).max() < 1e-10 * np.abs(Wo).max()
+    else:
+        assert _rel_rms(f, fo) < 1e-5 and abs(E - Eo) < 1e-6 * abs(Eo)
+    s.close()
+
+
+def test_tabulated_eam_run_and_table_checks():
+    w = wl.make_eam_tabulated(6, n_table=1501)
+    s = md.from_workload(w, precision=md.MD_FP64)
+    s.md_run(30, w.dt)
+    x, v = np.zeros((w.natoms, 3)), np.zeros((w.natoms, 3))
+    s.md_get_positions(x); s.md_get_velocities(v)
+    ref = oracle.run_nve(w.x, w.v, w.box, np.full(w.natoms, w.mass[0]), w.style, wl.oracle_params(w), w.rc, w.skin, w.dt, 30,
+                         ftm2v=w.ftm2v, mvv2e=w.mvv2e)
+    assert np.abs(_minimg(x - ref["x"], w.box)).max() < 1e-10 and np.abs(v - ref["v"]).max() < 1e-9 * np.abs(ref["v"]).max()
+    s.close()
+    # a coarse table is a different potential: the GPU must follow the TABLE, not the analytic form it was sampled from
+    wc = wl.make_eam_tabulated(6, n_table=61)
+    xc = wl.perturbed(wc, 0.2)
+    ft = oracle.forces_brute(xc, wc.box, wc.style, wl.oracle_params(wc), wc.rc)[0]
+    fa = oracle.forces_brute(xc, wc.box, oracle.PAIR_EAM, wl.EAM_PARAMS, wc.rc)[0]
+    s = md.from_workload(wc, precision=md.MD_FP64, x=xc)
+    f = np.zeros((wc.natoms, 3))
+    s.md_compute_forces(f)
+    assert _fp64_force_err(f, ft) < 1e-11 and _fp64_force_err(f, fa) > 1e-6
+    s.close()
+    # tables that end before the cutoff, or are missing, are refused
+    s = md.System(w.box, w.natoms, w.types, w.mass)
+    s.md_set_pair(md.MD_PAIR_EAM_TAB, (0.004, 0.05), w.rc, w.skin)
+    s.md_set_positions(w.x)
+    with pytest.raises(md.MDError) as e:
+        s.md_compute_forces()
+    assert e.value.code == md.MD_ERR_NOT_READY
+    s.md_set_eam_tables(np.ones(100), np.ones(100), np.ones(100))          # reaches r = 0.396 only
+    with pytest.raises(md.MDError) as e:
+        s.md_compute_forces()
+    assert e.value.code == md.MD_ERR_BAD_ARGUMENT
+    s.close()
+
+
 # ---- NVT, one Nose-Hoover thermostat (reading s25) -----------------------------------
 
 @pytest.mark.parametrize("cfg,n,nsteps,kT_factor,tau,list_kind", [(1, 7, 60, 0.5, 0.1, 0), (1, 7, 40, 0.5, 0.1, 1), (4, 6, 40, 2.0, 0.02, 0)])
