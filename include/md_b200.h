@@ -8,11 +8,12 @@
  *
  *   cell binning + counting sort + spatial reorder      ("spatially ordered")
  *   Verlet neighbor-list build, full or half            (numneigh[i], neighbors[i][jj])
- *   pair forces: LJ 12-6 and two-pass EAM               (App. A)
- *     thread-per-atom (TpA, L88-104), sub-warp/warp-per-atom with shuffle
+ *   pair forces: LJ 12-6, two-pass EAM (analytic and tabulated), Buckingham + cutoff Coulomb
+ *                                                       (App. A)
+ *     one thread (TpA, L88-104), 2 / 4 / 8 lanes or a warp per list row with shuffle
  *     reduction (the paper's block-per-atom BpA, L105-122), direct cell list (L64-82),
  *     chosen by a setup-time mini benchmark (L137)
- *   velocity-Verlet NVE, positions/velocities/forces resident on the device (L50-58)
+ *   velocity-Verlet NVE and Nose-Hoover NVT, positions/velocities/forces resident on the device (L50-58)
  *   rebuild iff max_i |x_i - x0_i|^2 > (skin/2)^2, decided on the device.
  *
  * Conventions
