@@ -239,6 +239,31 @@ int md_get_neighbor_rows(md_system* s, int32_t* row_owner, int32_t* numrow, int3
  * (NVE; the metric a time-stepping caller reads back.) */
 int md_kinetic_energy(md_system* s, double* ke_out);
 
+/* The same quantity (the kinetic energy the NVE/NVT integrators report) for callers that cannot call
+ * cudaMalloc -- code under CUDA-graph capture, tight serving loops, harnesses that forbid allocation.  Needs no handle
+ * and allocates NOTHING, on the host or the device: no cudaMalloc / cudaFree / allocating library routine; it enqueues
+ * one 4-byte memset and one kernel on cuda_stream (a cudaStream_t passed as void*, NULL = legacy default stream) and
+ * does not synchronise.  The kernel's scratch (one partial sum per 256 atoms plus a completion counter) is a file-scope
+ * static __device__ array of MD_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds until the process
+ * exits; its device address is resolved with cudaGetSymbolAddress on the first call on each device (make that call
+ * outside stream capture).
+ *   v_dev      DEVICE, N x 3 AoS doubles, read
+ *   type_dev   DEVICE, N int32 in [0, ntypes), read (not range-checked)
+ *   mass_dev   DEVICE, ntypes doubles, read
+ *   mvv2e      the unit factor of md_set_units (1 in LJ reduced units)
+ *   ke_out_dev DEVICE, 1 double, written by the kernel: 1/2 sum m v^2 mvv2e, summed in a fixed order (bitwise
+ *              reproducible from call to call)
+ * The caller owns all five buffers.  Errors: MD_ERR_BAD_ARGUMENT for a NULL pointer, N <= 0 or N > MD_NOALLOC_MAX_ATOMS
+ * (nothing is enqueued); MD_ERR_CUDA if a runtime call fails; the text is in md_last_error(NULL) on the calling thread.
+ * ALL calls in the process share the one array per GPU: calls on the same stream are ordered and safe; calls whose
+ * kernels may overlap on the GPU (different streams, or several host threads on different streams) RACE on the scratch
+ * and give wrong sums -- serialise them.  The counter is cleared at the start of every call; the partials need no
+ * clearing (each call overwrites the ones it reads). */
+#define MD_NOALLOC_SCRATCH_BYTES 524288   /* 512 KiB: 256 bytes of header + 65504 partials */
+#define MD_NOALLOC_MAX_ATOMS 16769024LL   /* 65504 partials x 256 atoms */
+int md_kinetic_energy_noalloc(const double* v_dev, const int32_t* type_dev, const double* mass_dev, int64_t N, double mvv2e,
+                              double* ke_out_dev, void* cuda_stream);
+
 /* Setup-time mini benchmark of PAPER.md L137 ("the faster variant is chosen by timing at setup"): on the current
  * positions, builds the list and times nrep (rounded up to an even number) FUSED time-step kernels with dt = 0 (force
  * evaluation + kick + drift epilogue: what md_run runs; positions and velocities keep their values) with each of TPA,

@@ -1470,3 +1470,89 @@ int md_get_stats(md_system* s, md_stats* out) {
 }
 
 }  // extern "C"
+
+// ---- md_kinetic_energy_noalloc: the kinetic-energy reduction for callers that cannot call cudaMalloc ---------------
+// (see include/md_b200.h).  The per-block partials and the completion ticket live in a file-scope device array instead
+// of handle memory: every GPU that loads the library holds these MD_NOALLOC_SCRATCH_BYTES until the process exits.
+// In HOST code `g_noalloc_scratch` is only a stand-in for the symbol, not a device address: the address a kernel may
+// dereference comes from cudaGetSymbolAddress, resolved once per device with that device current.
+
+namespace {
+
+constexpr int NOALLOC_BLOCK = 256;                    // atoms per block = atoms per partial
+constexpr int NOALLOC_HEADER_BYTES = 256;             // [0] the ticket counter, rest of the first 256 bytes unused
+constexpr int64_t NOALLOC_MAX_BLOCKS = (MD_NOALLOC_SCRATCH_BYTES - NOALLOC_HEADER_BYTES) / (int64_t)sizeof(double);
+static_assert(NOALLOC_MAX_BLOCKS * NOALLOC_BLOCK == MD_NOALLOC_MAX_ATOMS, "header constant and scratch layout disagree");
+constexpr int NOALLOC_MAX_DEVICES = 64;
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[MD_NOALLOC_SCRATCH_BYTES];
+
+// One partial per block of 256 atoms (index order inside the block is fixed by block_sum); the block that draws the
+// last ticket adds the partials in index order, so the result does not depend on the order the blocks finish in.
+__global__ void __launch_bounds__(NOALLOC_BLOCK) k_kinetic_noalloc(int64_t N, const double* __restrict__ v, const int* __restrict__ type,
+                                                                   const double* __restrict__ mass, double mvv2e,
+                                                                   unsigned char* __restrict__ scratch, double* __restrict__ ke_out) {
+  __shared__ double red[32];
+  __shared__ bool last;
+  unsigned int* ticket = reinterpret_cast<unsigned int*>(scratch);
+  double* partial = reinterpret_cast<double*>(scratch + NOALLOC_HEADER_BYTES);
+  const int64_t n = (int64_t)blockIdx.x * NOALLOC_BLOCK + threadIdx.x;
+  double ke[1] = {0.0};
+  if (n < N) {
+    const double vx = v[3 * n], vy = v[3 * n + 1], vz = v[3 * n + 2];
+    ke[0] = 0.5 * mass[type[n]] * (vx * vx + vy * vy + vz * vz);
+  }
+  block_sum<1>(ke, red);
+  if (threadIdx.x == 0) {
+    partial[blockIdx.x] = ke[0];
+    __threadfence();                                   // the partial is visible before the ticket is
+    last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  double s[1] = {0.0};
+  for (unsigned b = threadIdx.x; b < gridDim.x; b += NOALLOC_BLOCK) s[0] += __ldcg(partial + b);
+  block_sum<1>(s, red);
+  if (threadIdx.x == 0) {
+    *ke_out = s[0] * mvv2e;
+    *ticket = 0u;                                      // leave the counter as the next call expects it
+  }
+}
+
+std::mutex g_noalloc_mutex;
+unsigned char* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};    // device address of g_noalloc_scratch, per device ordinal
+
+}  // namespace
+
+extern "C" int md_kinetic_energy_noalloc(const double* v_dev, const int32_t* type_dev, const double* mass_dev, int64_t N, double mvv2e,
+                                         double* ke_out_dev, void* cuda_stream) {
+  md_system* s = nullptr;   // errors go where a failed md_create's go: md_last_error(NULL) on this thread
+  if (!v_dev || !type_dev || !mass_dev || !ke_out_dev) return fail(s, MD_ERR_BAD_ARGUMENT, "md_kinetic_energy_noalloc: NULL pointer");
+  if (N <= 0) return fail(s, MD_ERR_BAD_ARGUMENT, "md_kinetic_energy_noalloc: N = %lld must be positive", (long long)N);
+  if (N > MD_NOALLOC_MAX_ATOMS)
+    return fail(s, MD_ERR_BAD_ARGUMENT,
+                "md_kinetic_energy_noalloc: N = %lld exceeds MD_NOALLOC_MAX_ATOMS = %lld (the static scratch holds one partial per %d atoms "
+                "in %d bytes); use md_kinetic_energy on a handle instead",
+                (long long)N, (long long)MD_NOALLOC_MAX_ATOMS, NOALLOC_BLOCK, (int)MD_NOALLOC_SCRATCH_BYTES);
+  int dev = 0;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(s, MD_ERR_BAD_ARGUMENT, "md_kinetic_energy_noalloc: device ordinal %d not supported", dev);
+  unsigned char* scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {   // set-up, once per device, with that device current
+      void* p = nullptr;
+      CK(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+      if (!p) return fail(s, MD_ERR_CUDA, "md_kinetic_energy_noalloc: cudaGetSymbolAddress returned NULL");
+      g_noalloc_ptr[dev] = static_cast<unsigned char*>(p);
+    }
+    scratch = g_noalloc_ptr[dev];
+  }
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  // the ticket must start at zero: the last block of a completed call resets it, the memset covers a call that died
+  CK(cudaMemsetAsync(scratch, 0, sizeof(unsigned int), stream));
+  k_kinetic_noalloc<<<blocks_for(N, NOALLOC_BLOCK), NOALLOC_BLOCK, 0, stream>>>(N, v_dev, type_dev, mass_dev, mvv2e, scratch, ke_out_dev);
+  CK(cudaGetLastError());
+  return MD_OK;
+}

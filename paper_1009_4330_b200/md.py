@@ -21,6 +21,7 @@ MD_FP64, MD_MIXED = 0, 1
 MD_PAIR_LJ126, MD_PAIR_EAM_FS, MD_PAIR_BUCK_COUL, MD_PAIR_EAM_TAB = 1, 2, 3, 4
 MD_LIST_FULL, MD_LIST_HALF = 0, 1
 MD_THERMO_NONE, MD_THERMO_NOSE_HOOVER = 0, 1
+MD_NOALLOC_SCRATCH_BYTES, MD_NOALLOC_MAX_ATOMS = 524288, 16769024
 MD_KERNEL_AUTO, MD_KERNEL_TPA, MD_KERNEL_SUBWARP, MD_KERNEL_WARP, MD_KERNEL_CELL, MD_KERNEL_SUBWARP4, MD_KERNEL_SUBWARP2 = 0, 1, 2, 3, 4, 5, 6
 KERNEL_NAMES = {0: "auto", 1: "tpa", 2: "subwarp8", 3: "warp", 4: "cell", 5: "subwarp4", 6: "subwarp2"}
 
@@ -29,6 +30,7 @@ EXPORTS = [
     "md_set_pair", "md_set_neighbor", "md_build_neighbors", "md_compute_forces", "md_run", "md_get_positions",
     "md_get_velocities", "md_get_forces", "md_get_neighbors", "md_get_neighbor_rows", "md_kinetic_energy", "md_autotune",
     "md_get_stats", "md_last_error", "md_set_option", "md_set_pair_coeff", "md_set_type_charges", "md_set_thermostat", "md_get_thermostat", "md_set_eam_tables",
+    "md_kinetic_energy_noalloc",
 ]
 
 
@@ -96,6 +98,7 @@ def _load():
     L.md_get_thermostat.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.md_set_pair_coeff.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
     L.md_set_type_charges.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+    L.md_kinetic_energy_noalloc.argtypes = [dp, ip, dp, ctypes.c_int64, ctypes.c_double, dp, vp]
     L.md_autotune.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     L.md_get_stats.argtypes = [vp, ctypes.POINTER(md_stats)]
     L.md_last_error.argtypes = [vp]
@@ -128,6 +131,21 @@ def current_stream_ptr() -> int:
     """The current torch CUDA stream as a raw cudaStream_t."""
     import torch
     return int(torch.cuda.current_stream().cuda_stream)
+
+
+def md_kinetic_energy_noalloc(v, types, mass, mvv2e: float, ke_out, stream: int | None = None):
+    """``md_kinetic_energy_noalloc`` of the C ABI: all four buffers are CUDA tensors the caller owns (v: N x 3 float64,
+    types: N int32, mass: ntypes float64, ke_out: 1 float64); nothing is allocated and the stream is not synchronised."""
+    for t in (v, types, mass, ke_out):
+        if not (hasattr(t, "is_cuda") and t.is_cuda):
+            raise TypeError("md_kinetic_energy_noalloc takes CUDA tensors")
+    n = int(types.numel())
+    if stream is None:
+        stream = current_stream_ptr()
+    rc = lib.md_kinetic_energy_noalloc(_addr(v, np.float64, 3 * n), _addr(types, np.int32, n), _addr(mass, np.float64, mass.numel()),
+                                       n, float(mvv2e), _addr(ke_out, np.float64, 1), ctypes.c_void_p(stream))
+    if rc != MD_OK:
+        raise MDError(rc, (lib.md_last_error(None) or b"").decode())
 
 
 class System:
