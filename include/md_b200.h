@@ -180,6 +180,7 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel);
  *   "no_persistent"  1: run the one-block-per-tile kernel everywhere
  *   "balance_after"  apply the row balancing to a list that has lived this many steps (default 48; <= 0: at every build)
  *   "no_balance"  1: never
+ *   "build_graph"  0: md_run enqueues every rebuild launch by launch (default 1: replays the sequence as a CUDA graph)
  *   "tune_verbose"  1: md_autotune prints every candidate's timing to stderr
  * Unknown names and values out of range return MD_ERR_BAD_ARGUMENT. */
 int md_set_option(md_system* s, const char* name, int64_t value);

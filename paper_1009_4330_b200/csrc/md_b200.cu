@@ -62,6 +62,14 @@ struct md_system_impl {
   int cur = 0;    // buffer of v, id, type (flips at every build)
   int xcur = 0;   // buffer of x (flips at every build and at every fused kick+drift step)
   int force_threads = 256, batch = 8;
+  int build_attempts = 0;   // builds in a row that md_run found too small for their capacities
+  // the build's launch sequence as CUDA graphs, one per (cur, xcur) buffer state; captured on capture_stream (the
+  // caller's stream may be the legacy default stream, which cannot be captured) and launched on the caller's stream
+  struct BuildGraph { cudaGraphExec_t exec = nullptr; uint64_t key = 0; int64_t nlaunch = 0; };
+  BuildGraph build_graph[4];
+  cudaStream_t capture_stream = nullptr;
+  uint64_t plan_epoch = 0;    // bumped by every plan(): graphs captured for an older geometry are stale
+  bool opt_build_graph = true;   // md_set_option("build_graph")
   int num_sms = 148;
   bool force_timing_pending = false;
   bool list_balanced = false;
@@ -461,6 +469,7 @@ int plan(md_system* s) {
     CK(dalloc(&s->ev_partials, (size_t)g.ntiles * 8));
   }
   s->planned = true;
+  s->plan_epoch++;
   s->list_valid = false;
   return MD_OK;
 }
@@ -530,66 +539,125 @@ int balance_rows(md_system* s) {
   return MD_OK;
 }
 
+// One build, enqueued on the stream without waiting for it: bin, scan, rank sort, reorder (which flips the buffers), tile
+// tables and the list.  What the kernels found (capacities needed, non-finite coordinates, row statistics) is in
+// flags_d afterwards; build_finish() judges a host copy of it.
+int build_launches(md_system* s, bool do_list) {
+  const Geom& g = s->g;
+  const int N = (int)s->N;
+  CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
+  CK(cudaMemsetAsync(s->cell_count, 0, (size_t)(g.ncell + 1) * sizeof(int), s->stream));
+  int c = s->cur, o = 1 - c, xc = s->xcur, xo = 1 - xc;
+  CK(launch(s, k_bin, blocks_for(N, 256), 256, 0, g, N, s->x[xc], s->x[xc] + s->ld, s->x[xc] + 2 * s->ld, s->cell_of, s->rank,
+            s->cell_count, s->flags_d));
+  {
+    // block sums live in the tail of cell_count's allocation (cell_alloc has SCAN slack, see plan())
+    const unsigned nblk = blocks_for(g.ncell, SCAN_BLOCK);
+    int* bsum = s->cell_count + (g.ncell + 1);
+    CK(launch(s, k_scan_block_sums, nblk, 1024, 0, g.ncell, (const int*)s->cell_count, bsum));
+    CK(launch(s, k_scan_cells, nblk, 1024, 0, g.ncell, (const int*)s->cell_count, (const int*)bsum, s->cell_start));
+  }
+  CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
+            s->perm, s->mkey));
+  CK(launch(s, k_sort_cells, std::min<unsigned>(blocks_for(g.ncell, 8), 148u * 8u), 256, 0, g.ncell, (const int*)s->cell_start,
+            s->perm, s->mkey));   // a warp per cell, grid-stride
+  if (s->precision == MD_FP64)
+    CK(launch(s, k_permute<double>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
+              (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (double4*)s->xr[xo], s->ld));
+  else
+    CK(launch(s, k_permute<float>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
+              (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (float4*)s->xr[xo], s->ld));
+  CK(launch(s, k_tile_tables, g.ntiles, 128, 0, g, (const int*)s->cell_start, s->tab, s->flags_d));
+  s->cur = o; s->xcur = xo;   // host state only: the list is built from the reordered buffers
+  s->forces_valid = false;
+  if (do_list) { int rc = build_list_only(s); if (rc) return rc; }
+  return MD_OK;
+}
+
+// use_graph: replay the sequence as a CUDA graph (md_run's rebuilds: the same dozen launches every few steps, which at
+// small N cost more to launch than to run); the graph of a buffer state is captured the first time that state builds.
+int build_enqueue(md_system* s, bool need_list, bool* did_list, bool use_graph = false) {
+  if (!s->planned) { int rc = plan(s); if (rc) return rc; }
+  const bool do_list = need_list || s->kernel_eff != MD_KERNEL_CELL;
+  *did_list = do_list;
+  CK(cudaEventRecord(s->ev2, s->stream));
+  if (use_graph && s->opt_build_graph && s->capture_stream) {
+    md_system_impl::BuildGraph& G = s->build_graph[s->cur * 2 + s->xcur];
+    const uint64_t key = (s->plan_epoch << 8) | (uint64_t)(s->precision << 4) | (uint64_t)(s->kernel_eff << 1) | (do_list ? 1u : 0u);
+    if (!G.exec || G.key != key) {
+      if (G.exec) { cudaGraphExecDestroy(G.exec); G.exec = nullptr; }
+      const int cur0 = s->cur, xcur0 = s->xcur;
+      const int64_t l0 = s->launches;
+      cudaStream_t user = s->stream;
+      cudaGraph_t graph = nullptr;
+      CK(cudaStreamBeginCapture(s->capture_stream, cudaStreamCaptureModeRelaxed));
+      s->stream = s->capture_stream;
+      const int rc = build_launches(s, do_list);
+      s->stream = user;
+      const cudaError_t e = cudaStreamEndCapture(s->capture_stream, &graph);
+      G.nlaunch = s->launches - l0;
+      s->launches = l0; s->cur = cur0; s->xcur = xcur0;   // nothing has run yet
+      if (rc || e != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        if (rc) return rc;
+        return fail(s, MD_ERR_CUDA, "capturing the build sequence failed: %s", cudaGetErrorString(e));
+      }
+      const cudaError_t ei = cudaGraphInstantiate(&G.exec, graph, 0);
+      cudaGraphDestroy(graph);
+      if (ei != cudaSuccess) { G.exec = nullptr; return fail(s, MD_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(ei)); }
+      G.key = key;
+    }
+    CK(cudaGraphLaunch(G.exec, s->stream));
+    s->launches += G.nlaunch;
+    s->cur ^= 1; s->xcur ^= 1;
+    s->forces_valid = false;
+  } else {
+    int rc = build_launches(s, do_list);
+    if (rc) return rc;
+  }
+  CK(cudaEventRecord(s->ev3, s->stream));
+  return MD_OK;
+}
+
+// Judges a finished build from the host copy F of its flags (the stream has been synchronised since ev3).
+// *again: a capacity was too small; the cap scales are raised and the geometry has to be planned anew.
+int build_finish(md_system* s, const Flags& F, bool did_list, bool* again) {
+  const Geom& g = s->g;
+  float ms = 0;
+  cudaEventElapsedTime(&ms, s->ev2, s->ev3);
+  s->ms_build = ms;
+  s->nbuilds++;
+  *again = false;
+  if (F.nonfinite) return fail(s, MD_ERR_NONFINITE, "a non-finite coordinate reached the binning kernel");
+  if (F.need_tile_cap > g.tile_cap) { s->cap_scale_tile *= 1.1 * (double)F.need_tile_cap / g.tile_cap; *again = true; }
+  if (F.need_interior_cap > g.interior_cap) { s->cap_scale_int *= 1.1 * (double)F.need_interior_cap / g.interior_cap; *again = true; }
+  if (F.need_row_cap > g.row_cap) { s->cap_scale_row *= 1.1 * (double)F.need_row_cap / g.row_cap; *again = true; }
+  if (*again) { s->planned = false; return MD_OK; }
+  s->max_tile_atoms = F.max_tile_atoms;
+  s->max_row = F.max_row;
+  s->mean_row = (double)F.sum_rows / (0.5 * (double)s->N);   // entries per stored pair row
+  s->list_valid = true;
+  s->list_built_for_export = did_list;
+  s->list_balanced = false;
+  s->steps_since_build = 0;
+  s->build_attempts = 0;
+  return MD_OK;
+}
+
 int build(md_system* s, bool need_list) {
   if (!s->have_x || !s->pair_set) return fail(s, MD_ERR_NOT_READY, "positions and pair style must be set before building");
   // nothing of the previous list survives a build, successful or not
   s->list_valid = false; s->forces_valid = false; s->list_built_for_export = false; s->counts_valid = false;
   for (int attempt = 0; attempt < 6; ++attempt) {
-    if (!s->planned) { int rc = plan(s); if (rc) return rc; }
-    const Geom& g = s->g;
-    const int N = (int)s->N;
-    CK(cudaEventRecord(s->ev2, s->stream));
-    CK(cudaMemsetAsync(s->flags_d, 0, sizeof(Flags), s->stream));
-    CK(cudaMemsetAsync(s->cell_count, 0, (size_t)(g.ncell + 1) * sizeof(int), s->stream));
-    int c = s->cur, o = 1 - c, xc = s->xcur, xo = 1 - xc;
-    CK(launch(s, k_bin, blocks_for(N, 256), 256, 0, g, N, s->x[xc], s->x[xc] + s->ld, s->x[xc] + 2 * s->ld, s->cell_of, s->rank,
-              s->cell_count, s->flags_d));
-    {
-      // block sums live in the tail of cell_count's allocation (cell_alloc has SCAN slack, see plan())
-      const unsigned nblk = blocks_for(g.ncell, SCAN_BLOCK);
-      int* bsum = s->cell_count + (g.ncell + 1);
-      CK(launch(s, k_scan_block_sums, nblk, 1024, 0, g.ncell, (const int*)s->cell_count, bsum));
-      CK(launch(s, k_scan_cells, nblk, 1024, 0, g.ncell, (const int*)s->cell_count, (const int*)bsum, s->cell_start));
-    }
-    CK(launch(s, k_fill_perm, blocks_for(N, 256), 256, 0, N, (const int*)s->cell_of, (const int*)s->rank, (const int*)s->cell_start,
-              s->perm, s->mkey));
-    CK(launch(s, k_sort_cells, std::min<unsigned>(blocks_for(g.ncell, 8), 148u * 8u), 256, 0, g.ncell, (const int*)s->cell_start,
-              s->perm, s->mkey));   // a warp per cell, grid-stride
-    if (s->precision == MD_FP64)
-      CK(launch(s, k_permute<double>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
-                (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (double4*)s->xr[xo], s->ld));
-    else
-      CK(launch(s, k_permute<float>, blocks_for(N, 256), 256, 0, g, N, (const int*)s->perm, (const double*)s->x[xc], (const double*)s->v[c],
-                (const int*)s->id[c], (const int*)s->type[c], s->x[xo], s->v[o], s->id[o], s->type[o], s->x0, (float4*)s->xr[xo], s->ld));
-    CK(launch(s, k_tile_tables, g.ntiles, 128, 0, g, (const int*)s->cell_start, s->tab, s->flags_d));
-    s->cur = o; s->xcur = xo;
-    s->forces_valid = false;
-    bool do_list = need_list || s->kernel_eff != MD_KERNEL_CELL;
-    if (do_list) { int rc = build_list_only(s); if (rc) return rc; }
-    CK(cudaEventRecord(s->ev3, s->stream));
+    bool did_list = false, again = false;
+    int rc = build_enqueue(s, need_list, &did_list);
+    if (rc) return rc;
     CK(cudaMemcpyAsync(s->flags_h, s->flags_d, sizeof(Flags), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
-    float ms = 0;
-    cudaEventElapsedTime(&ms, s->ev2, s->ev3);
-    s->ms_build = ms;
-    s->nbuilds++;
-    const Flags& F = *s->flags_h;
-    if (F.nonfinite) return fail(s, MD_ERR_NONFINITE, "a non-finite coordinate reached the binning kernel");
-    bool again = false;
-    {
-      if (F.need_tile_cap > g.tile_cap) { s->cap_scale_tile *= 1.1 * (double)F.need_tile_cap / g.tile_cap; again = true; }
-      if (F.need_interior_cap > g.interior_cap) { s->cap_scale_int *= 1.1 * (double)F.need_interior_cap / g.interior_cap; again = true; }
-      if (F.need_row_cap > g.row_cap) { s->cap_scale_row *= 1.1 * (double)F.need_row_cap / g.row_cap; again = true; }
-    }
-    if (again) { s->planned = false; continue; }
-    s->max_tile_atoms = F.max_tile_atoms;
-    s->max_row = F.max_row;
-    s->mean_row = (double)F.sum_rows / (0.5 * (double)s->N);   // entries per stored pair row
-    s->list_valid = true;
-    s->list_built_for_export = do_list;
-    s->list_balanced = false;
-    s->steps_since_build = 0;
-    if (s->balance_after <= 0 && do_list) { int rcb = balance_rows(s); if (rcb) return rcb; }   // tuning experiments only
+    rc = build_finish(s, *s->flags_h, did_list, &again);
+    if (rc) return rc;
+    if (again) continue;
+    if (s->balance_after <= 0 && did_list) { int rcb = balance_rows(s); if (rcb) return rcb; }   // tuning experiments only
     return MD_OK;
   }
   return fail(s, MD_ERR_OVERFLOW, "tile or neighbor-row capacity still exceeded after re-planning");
@@ -869,6 +937,7 @@ int md_create(md_system** out, const double box[3], int64_t N, const int32_t* ty
   CKC(dalloc(&s->io_i, s->ld)); CKC(dalloc(&s->types_caller, s->ld)); CKC(dalloc(&s->flags_d, 1));
   CKC(cudaMallocHost((void**)&s->flags_h, sizeof(Flags))); CKC(cudaMallocHost((void**)&s->scalars_h, 16 * sizeof(double)));
   CKC(cudaEventCreate(&s->ev0)); CKC(cudaEventCreate(&s->ev1)); CKC(cudaEventCreate(&s->ev2)); CKC(cudaEventCreate(&s->ev3)); CKC(cudaEventCreate(&s->ev4)); CKC(cudaEventCreate(&s->ev5));
+  CKC(cudaStreamCreateWithFlags(&s->capture_stream, cudaStreamNonBlocking));
   for (int k = 0; k < 2 * md_system_impl::NSAMPLE; ++k) CKC(cudaEventCreate(&s->pev[k]));
   for (int k = 0; k < md_system_impl::NSAMPLE; ++k) CKC(cudaEventCreate(&s->pev_mid[k]));
   CKC(cudaMemcpyAsync(s->mass_d, mass, ntypes * sizeof(double), cudaMemcpyHostToDevice, s->stream));
@@ -903,6 +972,8 @@ void md_destroy(md_system* s) {
   cudaFree(s->ev_partials); cudaFree(s->scalars_d); cudaFree(s->io_d); cudaFree(s->io_i); cudaFree(s->types_caller); cudaFree(s->flags_d);
   if (s->flags_h) cudaFreeHost(s->flags_h);
   if (s->scalars_h) cudaFreeHost(s->scalars_h);
+  for (auto& G : s->build_graph) if (G.exec) cudaGraphExecDestroy(G.exec);
+  if (s->capture_stream) cudaStreamDestroy(s->capture_stream);
   if (s->ev0) cudaEventDestroy(s->ev0);
   if (s->ev1) cudaEventDestroy(s->ev1);
   if (s->ev2) cudaEventDestroy(s->ev2);
@@ -944,6 +1015,8 @@ int md_set_option(md_system* s, const char* name, int64_t value) {
   } else if (n == "persistent_min_tiles_per_sm") {
     if (value < 0) return fail(s, MD_ERR_BAD_ARGUMENT, "md_set_option: persistent_min_tiles_per_sm wants >= 0");
     s->p_min_tiles_per_sm = (int)std::min<int64_t>(value, 1 << 20);
+  } else if (n == "build_graph") {
+    s->opt_build_graph = value != 0;
   } else if (n == "tune_verbose") {
     s->tune_verbose = value != 0;
   } else {
@@ -1169,6 +1242,9 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
     s->forces_valid = false;
     int64_t remaining = nsteps;
     int parity = 0;
+    // a rebuild is enqueued without waiting for it (pending): the next batch follows on the stream, its kernels judge
+    // the build's flags themselves (list_is_stale) and the host does so with the flags it reads after that batch
+    bool pending = false, pending_list = false;
     while (remaining > 0) {
       const int m = (int)std::min<int64_t>(s->batch, remaining);
       int sample_slot[64];
@@ -1192,6 +1268,15 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
       const int done = s->flags_h->steps_done;
       const bool stopped = s->flags_h->stop != 0;
       if (done < 0 || done > m || (!stopped && done != m)) return fail(s, MD_ERR_CUDA, "md_run: inconsistent step count from the device (%d of %d)", done, m);
+      if (pending) {
+        bool again = false;
+        rc = build_finish(s, *s->flags_h, pending_list, &again);
+        if (rc) return rc;
+        s->ms_build_in_run += s->ms_build;
+        pending = false;
+        // a capacity was too small: no step of this batch ran; the stopped branch below plans anew and builds again
+        if (again && (done != 0 || !stopped)) return fail(s, MD_ERR_CUDA, "md_run: steps ran on an overflowed build");
+      }
       for (int k = 0; k < m; ++k) {   // timings of the launches that really ran; a sampled launch that was skipped gives its slot back
         if (sample_slot[k] < 0) continue;
         if (k < done) {
@@ -1221,9 +1306,17 @@ int md_run(md_system* s, int64_t nsteps, double dt) {
           rc = upload_dtf();   // the timing ran dt = 0 steps
           if (rc) return rc;
         }
-        rc = build(s, false);   // also clears the flags
-        if (rc) return rc;
-        s->ms_build_in_run += s->ms_build;
+        if (s->balance_after <= 0) {   // tuning experiments only: balance right after every build
+          rc = build(s, false);   // also clears the flags
+          if (rc) return rc;
+          s->ms_build_in_run += s->ms_build;
+        } else {
+          if (++s->build_attempts > 6) return fail(s, MD_ERR_OVERFLOW, "tile or neighbor-row capacity still exceeded after re-planning");
+          s->list_valid = false; s->forces_valid = false; s->list_built_for_export = false; s->counts_valid = false;
+          rc = build_enqueue(s, false, &pending_list, true);   // also clears the flags
+          if (rc) return rc;
+          pending = true;
+        }
         parity = 0;
       } else if (remaining > 0) {
         if (s->steps_since_build >= s->balance_after && s->kernel_eff != MD_KERNEL_CELL) { rc = balance_rows(s); if (rc) return rc; }

@@ -1597,7 +1597,11 @@ struct ForceArgs {
 __device__ __forceinline__ bool list_is_stale(const ForceArgs& A) {
   if (!A.in_run) return false;
   const double d2 = __longlong_as_double((long long)A.flags->max_disp2_bits[A.parity]);
-  const bool stale = A.flags->stop != 0 || d2 > A.trigger;
+  // the build before this batch is judged here too (md_run does not wait for it): a tile or row that outgrew its
+  // capacity, or a non-finite coordinate, stops the batch before its first step
+  const bool bad_build = A.flags->need_tile_cap > A.g.tile_cap || A.flags->need_interior_cap > A.g.interior_cap ||
+                         A.flags->need_row_cap > A.g.row_cap || A.flags->nonfinite != 0;
+  const bool stale = A.flags->stop != 0 || d2 > A.trigger || bad_build;
   if (stale && threadIdx.x == 0 && blockIdx.x == 0) atomicExch(&A.flags->stop, 1);
   return stale;
 }

@@ -598,6 +598,44 @@ def test_nvt_mixed_precision_thermalises_and_rejects_bad_arguments():
     s.close()
 
 
+@pytest.mark.parametrize("build_graph", [1, 0])
+def test_capacity_overflow_inside_a_run_replans_and_matches_oracle(build_graph):
+    """md_run does not wait for its rebuilds: the step kernels that follow one on the stream judge its flags themselves
+    (a tile or row that outgrew its capacity stops the batch before its first step) and the host plans anew after the
+    batch.  A converging flow (v_x = -c sin(2 pi x / L) on a dilute lattice) piles the atoms up around x = L/2 until the
+    rows outgrow the capacity planned for the uniform start; the trajectory must still be the oracle's.  With and
+    without the CUDA-graph replay of the build sequence."""
+    n, a, c, dt, nsteps = 16, 1.5, 2.0, 0.004, 450
+    L = n * a
+    g = (np.arange(n) + 0.5) * a
+    x = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3).copy()
+    x += np.random.default_rng(3).uniform(-0.05, 0.05, x.shape)
+    v = np.zeros_like(x)
+    v[:, 0] = -c * np.sin(2 * np.pi * x[:, 0] / L)
+    box = np.array([L, L, L])
+    N = len(x)
+    s = md.System(box, N, np.zeros(N, np.int32), np.array([1.0]))
+    s.md_set_precision(md.MD_FP64)
+    s.md_set_pair(md.MD_PAIR_LJ126, (1.0, 1.0), 2.5, 0.3)
+    s.md_set_neighbor(md.MD_LIST_FULL, md.MD_KERNEL_TPA)
+    s.md_set_option("build_graph", build_graph)
+    s.md_set_positions(x); s.md_set_velocities(v)
+    s.md_build_neighbors()
+    st0 = s.md_get_stats()
+    s.md_run(nsteps, dt)
+    st1 = s.md_get_stats()
+    assert st1["row_capacity"] > st0["row_capacity"] and st1["max_row"] > st0["row_capacity"]      # the plan was outgrown in the run
+    ref = oracle.run_nve(x, v, box, np.ones(N), oracle.PAIR_LJ, (1.0, 1.0), 2.5, 0.3, dt, nsteps)
+    xg, vg, fg = (np.zeros((N, 3)) for _ in range(3))
+    s.md_get_positions(xg); s.md_get_velocities(vg); s.md_get_forces(fg)
+    assert np.abs(_minimg(xg - ref["x"], box)).max() < 1e-9 and np.abs(vg - ref["v"]).max() < 1e-8
+    assert st1["nsteps_total"] == nsteps
+    assert ref["nbuild"] <= st1["nbuilds"] - st0["nbuilds"] <= ref["nbuild"] + 8             # the overflowed builds are done twice
+    fo = oracle.forces(xg, box, oracle.PAIR_LJ, (1.0, 1.0), 2.5)[0]
+    assert _fp64_force_err(fg, fo) < 1e-12
+    s.close()
+
+
 # ---- errors and degenerate inputs ------------------------------------------------------------------------------
 
 def test_error_paths():
