@@ -181,6 +181,7 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel);
  *   "balance_after"  apply the row balancing to a list that has lived this many steps (default 48; <= 0: at every build)
  *   "no_balance"  1: never
  *   "build_graph"  0: md_run enqueues every rebuild launch by launch (default 1: replays the sequence as a CUDA graph)
+ *   "pdl"  0: md_run launches its step kernels without programmatic dependent launch (default 1)
  *   "tune_verbose"  1: md_autotune prints every candidate's timing to stderr
  * Unknown names and values out of range return MD_ERR_BAD_ARGUMENT. */
 int md_set_option(md_system* s, const char* name, int64_t value);

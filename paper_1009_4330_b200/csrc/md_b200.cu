@@ -70,6 +70,7 @@ struct md_system_impl {
   cudaStream_t capture_stream = nullptr;
   uint64_t plan_epoch = 0;    // bumped by every plan(): graphs captured for an older geometry are stale
   bool opt_build_graph = true;   // md_set_option("build_graph")
+  bool opt_pdl = true;           // md_set_option("pdl"): programmatic dependent launch of the step kernels
   int num_sms = 148;
   bool force_timing_pending = false;
   bool list_balanced = false;
@@ -200,6 +201,27 @@ cudaError_t launch(md_system* s, Kern kern, unsigned grid, unsigned block, size_
   kern<<<grid, block, smem, s->stream>>>(args...);
   s->launches++;
   return cudaGetLastError();
+}
+
+// A step kernel of md_run's batches: programmatic dependent launch, so that the launch itself (grid set-up, block
+// scheduling) overlaps the tail of the previous step kernel; the kernels call pdl_wait_then_release() before they read
+// anything (md_kernels.cuh).
+template <class Kern, class... Args>
+cudaError_t launch_pdl(md_system* s, bool pdl, Kern kern, unsigned grid, unsigned block, size_t smem, Args... args) {
+  if (!pdl) return launch(s, kern, grid, block, smem, args...);
+  if (grid == 0) return cudaSuccess;
+  if (smem > 40 * 1024) {
+    cudaError_t e = opt_in_smem(kern);
+    if (e != cudaSuccess) return e;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = s->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  s->launches++;
+  return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
 inline unsigned blocks_for(int64_t n, int block) { return (unsigned)((n + block - 1) / block); }
@@ -680,6 +702,7 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
   const bool half = g.half != 0;
   // the energy/virial and fp64 instantiations are compiled for more registers, hence smaller blocks
   const int threads = (EV || sizeof(T) == 8) ? std::min(s->force_threads, FORCE_MAX_THREADS_WIDE) : s->force_threads;
+  const bool pdl = A.in_run != 0 && s->opt_pdl;   // the fused step launches of md_run's batches
   if (s->kernel_eff == MD_KERNEL_CELL) {
     CK(launch(s, k_cell_force<T, Body, MODE, EV>, g.ntiles, BUILD_THREADS, cell_smem(s, g), A));
   } else if (half) {
@@ -692,23 +715,27 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
       if (use_persistent(s, g)) {
         // persistent, warp-specialised path: one block per SM, two consumer groups of `threads` + one producer warp
         const int ng = p_groups(s, g), nb = p_nbuf(s, g);
-        const int gth = std::min((threads + 127) / 128 * 128, p_max_group_threads(s, g));   // whole warpgroups
+        // all the consumer warps the register budget allows: the kernel deals 32-lane tasks to whichever warp is free,
+        // so the tile's row count no longer has to match a group's size
+        const int gth = p_max_group_threads(s, g);   // whole warpgroups
+        (void)threads;
         const unsigned grid = (unsigned)std::min(g.ntiles, s->num_sms);
         const unsigned block = (unsigned)(ng * gth + 32 * FORCE_P_NPROD);
         const size_t sm = force_p_smem(g, nb);
-        if (g.K == 1) CK(launch(s, k_tile_force_p<Body, 1, MODE>, grid, block, sm, A, gth, ng, nb));
-        else if (g.K == 2) CK(launch(s, k_tile_force_p<Body, 2, MODE>, grid, block, sm, A, gth, ng, nb));
-        else if (g.K == 4) CK(launch(s, k_tile_force_p<Body, 4, MODE>, grid, block, sm, A, gth, ng, nb));
-        else if (g.K == 8) CK(launch(s, k_tile_force_p<Body, 8, MODE>, grid, block, sm, A, gth, ng, nb));
-        else CK(launch(s, k_tile_force_p<Body, 32, MODE>, grid, block, sm, A, gth, ng, nb));
+        if (g.K == 1) CK(launch_pdl(s, pdl, k_tile_force_p<Body, 1, MODE>, grid, block, sm, A, gth, ng, nb));
+        else if (g.K == 2) CK(launch_pdl(s, pdl, k_tile_force_p<Body, 2, MODE>, grid, block, sm, A, gth, ng, nb));
+        else if (g.K == 4) CK(launch_pdl(s, pdl, k_tile_force_p<Body, 4, MODE>, grid, block, sm, A, gth, ng, nb));
+        else if (g.K == 8) CK(launch_pdl(s, pdl, k_tile_force_p<Body, 8, MODE>, grid, block, sm, A, gth, ng, nb));
+        else CK(launch_pdl(s, pdl, k_tile_force_p<Body, 32, MODE>, grid, block, sm, A, gth, ng, nb));
         return MD_OK;
       }
     }
-    if (g.K == 1) CK(launch(s, k_tile_force<T, Body, 1, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
-    else if (g.K == 2) CK(launch(s, k_tile_force<T, Body, 2, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
-    else if (g.K == 4) CK(launch(s, k_tile_force<T, Body, 4, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
-    else if (g.K == 8) CK(launch(s, k_tile_force<T, Body, 8, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
-    else CK(launch(s, k_tile_force<T, Body, 32, MODE, EV, false>, g.ntiles, threads, force_smem(s, g, false), A));
+    const unsigned nt = (unsigned)g.ntiles, th = (unsigned)threads;
+    if (g.K == 1) CK(launch_pdl(s, pdl, k_tile_force<T, Body, 1, MODE, EV, false>, nt, th, force_smem(s, g, false), A));
+    else if (g.K == 2) CK(launch_pdl(s, pdl, k_tile_force<T, Body, 2, MODE, EV, false>, nt, th, force_smem(s, g, false), A));
+    else if (g.K == 4) CK(launch_pdl(s, pdl, k_tile_force<T, Body, 4, MODE, EV, false>, nt, th, force_smem(s, g, false), A));
+    else if (g.K == 8) CK(launch_pdl(s, pdl, k_tile_force<T, Body, 8, MODE, EV, false>, nt, th, force_smem(s, g, false), A));
+    else CK(launch_pdl(s, pdl, k_tile_force<T, Body, 32, MODE, EV, false>, nt, th, force_smem(s, g, false), A));
   }
   return MD_OK;
 }
@@ -1017,6 +1044,8 @@ int md_set_option(md_system* s, const char* name, int64_t value) {
     s->p_min_tiles_per_sm = (int)std::min<int64_t>(value, 1 << 20);
   } else if (n == "build_graph") {
     s->opt_build_graph = value != 0;
+  } else if (n == "pdl") {
+    s->opt_pdl = value != 0;
   } else if (n == "tune_verbose") {
     s->tune_verbose = value != 0;
   } else {

@@ -1592,6 +1592,15 @@ struct ForceArgs {
   Flags* flags;
 };
 
+// Programmatic dependent launch (step kernels inside md_run are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization): the next launch of the stream may be set up and its blocks
+// scheduled while this grid is still running; nothing the previous grid wrote may be read before pdl_wait().  Both are
+// no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_wait_then_release() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 // true if this launch must do nothing: an earlier step of the batch moved some atom farther than
 // skin/2 from its position at the last build, so the host has to rebuild first (reading s4).
 __device__ __forceinline__ bool list_is_stale(const ForceArgs& A) {
@@ -1765,6 +1774,14 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned
                "r"(mbar)
                : "memory");
 }
+__device__ __forceinline__ bool mbar_test(unsigned mbar, unsigned parity) {   // has the phase of this parity completed? (does not block)
+  unsigned ok = 0;
+  asm volatile("{ .reg .pred p; mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+               : "=r"(ok)
+               : "r"(mbar), "r"(parity)
+               : "memory");
+  return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
   unsigned ok = 0;
   while (!ok)
@@ -1839,6 +1856,7 @@ __global__ void __maxnreg__((EV || sizeof(T) == 8) ? 96 : FORCE_MAX_REGS) k_tile
   using V4 = typename Vec4<T>::type;
   using PK = typename Pk<T>::type;
   constexpr int NT = Body::NT;
+  pdl_wait_then_release();
   if (list_is_stale(A)) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   TileTables& tt = *reinterpret_cast<TileTables*>(smem_raw);
@@ -2121,8 +2139,9 @@ constexpr int FORCE_P_MAX_REGS = 72;              // registers per thread at lau
 constexpr int FORCE_P_MAX_THREADS = 896;          // consumer threads + the producer warps
 constexpr int FORCE_P_CONSUMER_REGS = 80;         // after the register split below: (896 x 72 - 128 x 24) / 768
 constexpr int FORCE_P_NPROD = 4;                  // producer warps
+constexpr int FORCE_P_CLAIM_BYTES = 512;          // per buffer: one claim word per post-processing chunk (tile_cap < 16384: <= 128 chunks)
 __host__ __device__ inline size_t force_p_buf_bytes(const Geom& g) {
-  return (size_t)tile_tab_stride(g) * 4 + (size_t)force_capA(g) * 16 + (((size_t)g.interior_cap * 2 + 15) & ~(size_t)15);
+  return (size_t)tile_tab_stride(g) * 4 + (size_t)force_capA(g) * 16 + (((size_t)g.interior_cap * 2 + 15) & ~(size_t)15) + FORCE_P_CLAIM_BYTES;
 }
 __host__ __device__ inline size_t force_p_smem(const Geom& g, int nbuf) { return 128 + (size_t)nbuf * force_p_buf_bytes(g); }
 __host__ __device__ inline int force_p_chunks(const Geom& g) { return ((g.tile_cap >> 2) + 1 + 31) >> 5; }   // chunks of 32 quads of slots
@@ -2150,48 +2169,58 @@ struct TileView {
   __device__ __forceinline__ const unsigned short* qc() const { return reinterpret_cast<const unsigned short*>(h + TILE_HDR + TILE_CELL_INTS * tcs); }
 };
 
-// post-processing of one chunk (32 quads of staged slots) of a landed tile: cell offsets added in place, pad slots and
-// the dummy slot set far away, pair row -> cells map.  One warp per chunk.
+// post-processing of one chunk (32 quads = 128 staged slots) of a landed tile: cell offsets added in place, pad slots and
+// the dummy slot set far away, pair row -> cells map.  One warp per chunk; consecutive lanes take consecutive slots, so
+// every 128-bit access of the warp is four conflict-free wavefronts (a quad of slots per lane made it sixteen, and the
+// tile's post-processing cost 2 us of the shared-memory pipe that the gathers of the list loop live on).
 __device__ __forceinline__ void force_p_post_chunk(const TileView& tv, float4* st, unsigned short* scell, int ch, int lane) {
-  const int nq = tv.n_slots() >> 2;
-  const int q = ch * 32 + lane;
-  if (q < nq) {
-    const int t = tv.qc()[q];
-    const int c = tv.cnt(t), k0 = 4 * q - tv.start(t);
-    const float ox = tv.off(0, t), oy = tv.off(1, t), oz = tv.off(2, t);
-    const bool interior = (tv.meta(t) >> 24) != 0;
-    unsigned sc[2] = {0xffffffffu, 0xffffffffu};
+  const int ns = tv.n_slots();
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int slot = 4 * q + u;
-      if (k0 + u < c) {
+  for (int u = 0; u < 4; ++u) {
+    const int slot = ch * 128 + u * 32 + lane;
+    if (slot < ns) {
+      const int t = tv.qc()[slot >> 2];
+      const int c = tv.cnt(t), kk = slot - tv.start(t);       // index within the cell (cells are padded to quads of slots)
+      if (kk < c) {
         float4 v = st[slot];
-        v.x += ox; v.y += oy; v.z += oz;
+        v.x += tv.off(0, t); v.y += tv.off(1, t); v.z += tv.off(2, t);
         st[slot] = v;
-        sc[u >> 1] = (u & 1) ? ((sc[u >> 1] & 0xffffu) | ((unsigned)t << 16)) : ((sc[u >> 1] & 0xffff0000u) | (unsigned)t);
       } else {
         st[slot] = make_float4(1e15f, 1e15f, 1e15f, 0.f);
       }
+      // indexed by interior slot; a pair of slots is one list row (the cell's rows are padded to 2, not 4)
+      if ((tv.meta(t) >> 24) != 0 && (kk & ~1) < c) scell[tv.rstart(t) + kk] = kk < c ? (unsigned short)t : (unsigned short)0xffffu;
+    } else if (slot == ns) {
+      st[ns] = make_float4(1e15f, 1e15f, 1e15f, 0.f);   // the dummy slot
     }
-    if (interior) {   // indexed by interior slot; a pair of slots is one list row (the cell's rows are padded to 2, not 4)
-      unsigned* sp = reinterpret_cast<unsigned*>(scell + tv.rstart(t) + k0);
-      if (k0 < c) sp[0] = sc[0];
-      if (k0 + 2 < c) sp[1] = sc[1];
-    }
-  } else if (q == nq) {
-    st[tv.n_slots()] = make_float4(1e15f, 1e15f, 1e15f, 0.f);   // the dummy slot
   }
 }
 
-#ifndef MDK_FORCE_P_PRODUCER_POST
-#define MDK_FORCE_P_PRODUCER_POST 1   // 1: the producer warps post-process the landed tile; 0: the consumer warps do (chunks dealt on arrival)
-#endif
+// The post-processing chunks of a landed tile are shared between the producer warps, which walk them from the front, and
+// the consumer warps that would otherwise wait for the tile (at the start of a launch all of them do), which walk them
+// from the back.  A chunk belongs to whoever first moves its claim word from the tile's generation `gen` to gen + 1:
+// one word per chunk, because two dozen warps hammering ONE shared counter serialise (measured: 1.8 us for 28 chunks).
+__device__ __forceinline__ void force_p_post_share(const TileView& tv, float4* st, unsigned short* scell, int* claim, int gen, int nchunks,
+                                                   unsigned ready_b, int lane, int first, int step, bool from_back) {
+  for (int i = first; i < nchunks; i += step) {
+    const int ch = from_back ? nchunks - 1 - i : i;
+    int won = 0;
+    if (lane == 0 && *reinterpret_cast<volatile int*>(claim + ch) == gen) won = atomicCAS(claim + ch, gen, gen + 1) == gen;
+    won = __shfl_sync(0xffffffffu, won, 0);
+    if (!won) continue;
+    force_p_post_chunk(tv, st, scell, ch, lane);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(ready_b);   // release: the consumers' wait acquires the chunk
+  }
+}
+
 template <class Body, int K, int MODE>
 __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gthreads, int NG, int NB) {
   constexpr int NP = FORCE_P_NPROD;
   using T = float;
   using V4 = float4;
   constexpr int NT = Body::NT;
+  pdl_wait_then_release();
   if (list_is_stale(A)) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Geom& g = A.g;
@@ -2207,21 +2236,28 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   auto empty = [&](int b) { return smem0 + 8u * (unsigned)(2 * MB + b); };
   auto ready = [&](int b) { return smem0 + 8u * (unsigned)(3 * MB + b); };
   int* ctr = reinterpret_cast<int*>(smem_raw + 8 * 4 * MB);
+  int* next_task = ctr + MB;   // the consumers' task counter
+  volatile int* fin = ctr + MB + 1;   // per buffer: tasks finished in it since the launch began (never reset)
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int gwarps = gthreads >> 5;
   const int nchunks = force_p_chunks(g);
+  const int tasks_per_tile = (prow_cap(g) * K + 31) >> 5;
   if (threadIdx.x == 0) {
     for (int b = 0; b < NB; ++b) {
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(full(b)), "r"(1) : "memory");
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tabfull(b)), "r"(1) : "memory");
-      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(empty(b)), "r"(gwarps) : "memory");
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(empty(b)), "r"(tasks_per_tile) : "memory");
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(ready(b)), "r"(nchunks) : "memory");
       ctr[b] = 0;
     }
+    *next_task = 0;
+    for (int b = 0; b < MB; ++b) fin[b] = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __shared__ __align__(16) unsigned char pair_tab[Body::TABLE ? MAX_PAIR_TYPES * MAX_PAIR_TYPES * sizeof(V4) : 16];   // per-type-pair coefficients
   if constexpr (Body::TABLE) Body::fill(A.P, reinterpret_cast<V4*>(pair_tab));
+  auto claims = [&](int b) { return reinterpret_cast<int*>(smem_raw + 128 + (size_t)(b + 1) * buf_bytes - FORCE_P_CLAIM_BYTES); };
+  for (int i = threadIdx.x; i < NB * (FORCE_P_CLAIM_BYTES / 4); i += blockDim.x) claims(i / (FORCE_P_CLAIM_BYTES / 4))[i % (FORCE_P_CLAIM_BYTES / 4)] = 0;
   __syncthreads();
   const int ntl = ((int)g.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this block
   const int pcap = prow_cap(g);
@@ -2238,17 +2274,26 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
     const int pw = wid - NG * gwarps;
     if (pw >= NP) return;
     const V4* __restrict__ xr = reinterpret_cast<const V4*>(A.xr);
+    // the table of tile k is requested as early as its buffer is free: by the first producer thread, either ahead of time
+    // (while the cells of tile k - 1 are in flight, if the buffer is free by then) or at the top of iteration k
+    auto request_table = [&](int k) {
+      const int b = k % NB;
+      ctr[b] = 0;
+      mbar_expect_tx(tabfull(b), (unsigned)tab_ints * 4u);
+      bulk_g2s(smem0 + 128u + (unsigned)b * buf_bytes, A.tab + (size_t)((int)blockIdx.x + k * (int)gridDim.x) * tab_ints, (unsigned)tab_ints * 4u,
+               tabfull(b));
+    };
+    int requested = 0;   // tables requested so far (meaningful in the first producer thread only)
     for (int k = 0; k < ntl; ++k) {
       const int b = k % NB, j = k / NB;
       const int tile = (int)blockIdx.x + k * (int)gridDim.x;
       unsigned char* bufp = smem_raw + 128 + (size_t)b * buf_bytes;
       const unsigned buf = smem0 + 128u + (unsigned)b * buf_bytes;
       TileView tv{reinterpret_cast<const int*>(bufp), tcs};
-      if (j > 0) mbar_wait(empty(b), (unsigned)((j - 1) & 1));
-      if (pw == 0 && lane == 0) {
-        ctr[b] = 0;
-        mbar_expect_tx(tabfull(b), (unsigned)tab_ints * 4u);
-        bulk_g2s(buf, A.tab + (size_t)tile * tab_ints, (unsigned)tab_ints * 4u, tabfull(b));
+      if (pw == 0 && lane == 0 && requested <= k) {
+        if (j > 0) mbar_wait(empty(b), (unsigned)((j - 1) & 1));
+        request_table(k);
+        requested = k + 1;
       }
       mbar_wait(tabfull(b), (unsigned)(j & 1));
       int c0[3], w[3];
@@ -2261,71 +2306,72 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
         const int c = tv.cnt(t);
         if (c > 0) bulk_g2s(st_a + (unsigned)tv.start(t) * 16u, xr + tv.gstart(t), (unsigned)c * 16u, full(b));
       }
-#if MDK_FORCE_P_PRODUCER_POST
-      // the tile's post-processing, off the consumers' critical path (7 % of their time when they did it themselves):
-      // the producers run a tile ahead of the consumers, so they can afford to wait for the copies here
+      if (pw == 0 && lane == 0 && k + 1 < ntl) {   // the next tile's table, if its buffer is free already
+        const int b1 = (k + 1) % NB, j1 = (k + 1) / NB;
+        if (j1 == 0 || mbar_test(empty(b1), (unsigned)((j1 - 1) & 1))) { request_table(k + 1); requested = k + 2; }
+      }
+      // the tile's post-processing, off the consumers' critical path (7 % of their time when they did all of it themselves):
+      // the producers run a tile ahead of the consumers in the steady state, so they can afford to wait for the copies here
       mbar_wait(full(b), (unsigned)(j & 1));
       {
         float4* stp = reinterpret_cast<float4*>(bufp + (size_t)tab_ints * 4);
         unsigned short* scp = reinterpret_cast<unsigned short*>(stp + capA);
-        for (int ch = pw; ch < nchunks; ch += NP) {
-          force_p_post_chunk(tv, stp, scp, ch, lane);
-          __syncwarp();
-          if (lane == 0) mbar_arrive(ready(b));   // release: the consumers' wait acquires the chunk
-        }
+        force_p_post_share(tv, stp, scp, claims(b), j, nchunks, ready(b), lane, pw, NP, false);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // these generic stores precede the buffer's next bulk copies
       }
-#endif
     }
     return;
   }
 
   // ---------------- consumer groups ----------------
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(FORCE_P_CONSUMER_REGS));
-  const int grp = wid / gwarps, gt = (int)threadIdx.x - grp * gthreads;
   Body body(A.P);
   body.attach(reinterpret_cast<V4*>(pair_tab));
   const size_t ld = A.ld;
   const size_t slots_cap = (size_t)pcap * K;
+  // Work is dealt to the consumer WARPS, not to groups: a task is 32 consecutive lane slots (32 / K pair rows) of one
+  // tile, handed out in tile order from a shared counter.  A block's tiles rarely divide evenly among two groups (cfg 4:
+  // three tiles per SM left one group idle for a third of the launch), and a tile's rows rarely fill a group.
+  const int tpt = ((int)slots_cap + 31) >> 5;   // tasks per tile (the trailing ones of a tile are empty: pcap is a capacity)
+  const int ntasks = ntl * tpt;
   double d2max = 0.0;
-  for (int k = grp; k < ntl; k += NG) {
+  for (;;) {
+    int task = 0;
+    if (lane == 0) task = atomicAdd(next_task, 1);
+    task = __shfl_sync(0xffffffffu, task, 0);
+    if (task >= ntasks) break;
+    const int k = task / tpt, tc = task - k * tpt;
     const int b = k % NB, j = k / NB;
     const int tile = (int)blockIdx.x + k * (int)gridDim.x;
     const uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
-    // while the tile lands: this thread's row length and first list word of the first round
+    const int sidx = tc * 32 + lane;
+    const int r = sidx / K, s = sidx % K;                   // pair row, lane of the row
+    // while the tile lands: this lane's row length and first list word
     int n_first = 0;
     uint4 w_first = make_uint4(0, 0, 0, 0);
-    if (gt < pcap * K) {
-      n_first = A.numneigh[(size_t)tile * pcap + gt / K];
-      w_first = ld_stream(tlist + gt);
+    if (sidx < (int)slots_cap) {
+      n_first = A.numneigh[(size_t)tile * pcap + r];
+      w_first = ld_stream(tlist + sidx);
     }
     unsigned char* bufp = smem_raw + 128 + (size_t)b * buf_bytes;
     TileView tv{reinterpret_cast<const int*>(bufp), tcs};
     V4* st = reinterpret_cast<V4*>(bufp + (size_t)tab_ints * 4);
     unsigned short* scell = reinterpret_cast<unsigned short*>(st + capA);
     const unsigned st_base = smem_addr(st);
-#if !MDK_FORCE_P_PRODUCER_POST
-    mbar_wait(tabfull(b), (unsigned)(j & 1));
-    mbar_wait(full(b), (unsigned)(j & 1));
-    // chunks of 32 quads of slots dealt to whichever warps of the group get here first (the warps of a group finish
-    // their previous tile at different times: no group barrier)
-    for (;;) {
-      int ch = 0;
-      if (lane == 0) ch = atomicAdd(&ctr[b], 1);
-      ch = __shfl_sync(0xffffffffu, ch, 0);
-      if (ch >= nchunks) break;
-      force_p_post_chunk(tv, st, scell, ch, lane);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(ready(b));   // release: the waits below acquire the chunk
+    // A parity wait is only right for a waiter at most one phase ahead of the barrier, and tasks are dealt without regard
+    // to what has landed (with few tasks per tile a free warp can be handed a tile whose buffer still holds the tile
+    // NB before it, or the one 2 NB before): first make sure the buffer's previous tile is finished, by count
+    while (fin[b] < j * tpt) __nanosleep(32);
+    if (!mbar_test(ready(b), (unsigned)(j & 1))) {   // the tile is not ready: help with its post-processing instead of waiting
+      mbar_wait(tabfull(b), (unsigned)(j & 1));
+      mbar_wait(full(b), (unsigned)(j & 1));
+      force_p_post_share(tv, st, scell, claims(b), j, nchunks, ready(b), lane, tc, tpt, true);
+      mbar_wait(ready(b), (unsigned)(j & 1));
     }
-#endif
-    mbar_wait(ready(b), (unsigned)(j & 1));
     int c0[3], wdt[3];
     tile_dims(g, tile, c0, wdt);
     const int nlanes = (tv.n_int_slots() >> 1) * K;
-    for (int base = 0; base < nlanes; base += gthreads) {   // uniform trip count: the shuffles below need full groups
-      const int sidx = base + gt;
-      const int r = sidx / K, s = sidx % K;                   // pair row, lane of the row
+    {
       unsigned cells = 0xffffffffu;
       if (sidx < nlanes) cells = reinterpret_cast<const unsigned*>(scell)[r];
       const unsigned cell = cells & 0xffffu;
@@ -2341,8 +2387,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
         V4 pi1 = lds_v4_scalars<T>(st_base + (unsigned)(slot0 + 1) * 16u);   // a pad slot if there is no partner
         if (!act1) { pi1.x = -1e15f; pi1.y = -1e15f; pi1.z = -1e15f; pi1.w = 0.f; }
         pi0.w = Body::own_w(pi0.w); pi1.w = Body::own_w(pi1.w);
-        const int n = base == 0 ? n_first : A.numneigh[(size_t)tile * pcap + r];
-        const int nq = (n + 7) >> 3;                          // words of this row
+        const int nq = (n_first + 7) >> 3;                    // words of this row
         if (act1 && s == 0) {
           // the pair's mutual term (the two atoms are never entries of their own row)
           typename Pk<T>::type p[NT];
@@ -2375,7 +2420,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
 #else
         const int mine = nq > s ? (nq - s + K - 1) / K : 0;   // words q = s, s+K, ...
 #endif
-        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi0, pi1, tot0, tot1, w_first, base == 0);
+        list_loop<T, Body>(body, st_base, tlist + sidx, slots_cap, mine, pi0, pi1, tot0, tot1, w_first, true);
       }
       if constexpr (K > 1) {
 #pragma unroll
@@ -2406,10 +2451,14 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
         }
       }
     }
-    // the group is done with this buffer: hand it back to the producer (its next writes are bulk copies)
+    // this task is done with the buffer: the producer may refill it when all tasks of the tile have said so (its next
+    // writes are bulk copies)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncwarp();
-    if (lane == 0) mbar_arrive(empty(b));
+    if (lane == 0) {
+      mbar_arrive(empty(b));
+      atomicAdd(const_cast<int*>(fin) + b, 1);
+    }
   }
   if constexpr (MODE == 0) {
     if (A.epi == EPI_KICK_DRIFT) {   // a4: device-side max-displacement reduction (see k_tile_force)
