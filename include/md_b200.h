@@ -182,6 +182,8 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel);
  *   "no_balance"  1: never
  *   "build_graph"  0: md_run enqueues every rebuild launch by launch (default 1: replays the sequence as a CUDA graph)
  *   "pdl"  0: md_run launches its step kernels without programmatic dependent launch (default 1)
+ *   "tab_smem"  0: MD_PAIR_EAM_TAB reads its coefficient tables through L1/L2 (default 1: staged in shared memory when
+ *               a table is at most 48 KB)
  *   "tune_verbose"  1: md_autotune prints every candidate's timing to stderr
  * Unknown names and values out of range return MD_ERR_BAD_ARGUMENT. */
 int md_set_option(md_system* s, const char* name, int64_t value);

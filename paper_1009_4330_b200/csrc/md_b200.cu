@@ -71,6 +71,7 @@ struct md_system_impl {
   uint64_t plan_epoch = 0;    // bumped by every plan(): graphs captured for an older geometry are stale
   bool opt_build_graph = true;   // md_set_option("build_graph")
   bool opt_pdl = true;           // md_set_option("pdl"): programmatic dependent launch of the step kernels
+  bool opt_tab_smem = true;      // md_set_option("tab_smem"): tabulated EAM stages its coefficient tables in shared memory
   int num_sms = 148;
   bool force_timing_pending = false;
   bool list_balanced = false;
@@ -271,10 +272,18 @@ bool persistent_eligible(const md_system* s) {
 }
 // Consumer groups per block: two, with three tile buffers (two being computed on, one being loaded), when they fit the
 // SM's shared memory; else one group with two buffers (rc = 5 sigma: a 3x1x1 tile stages 108 KB); 0: does not fit.
+// Tabulated EAM: the two coefficient tables (rho, phi: 16 bytes per interval) are staged in shared memory behind the
+// tile buffers when they are small enough to leave room for two buffers; bytes of ONE table, 0: read through L1/L2.
+size_t p_table_bytes(const md_system* s) {
+  if (s->style != MD_PAIR_EAM_TAB || s->precision != MD_MIXED || !s->opt_tab_smem || s->eam_nr < 2) return 0;
+  const size_t one = (size_t)(s->eam_nr - 1) * 16;
+  return one <= 48 * 1024 ? one : 0;
+}
 int p_groups(const md_system* s, const Geom& g) {
-  if (s->p_groups > 0) return force_p_smem(g, s->p_groups + 1) <= SMEM_OPTIN_BUDGET ? s->p_groups : 0;
-  if (force_p_smem(g, 3) <= SMEM_OPTIN_BUDGET) return 2;
-  return force_p_smem(g, 2) <= SMEM_OPTIN_BUDGET ? 1 : 0;
+  const size_t extra = 2 * p_table_bytes(s);
+  if (s->p_groups > 0) return force_p_smem(g, s->p_groups + 1) + extra <= SMEM_OPTIN_BUDGET ? s->p_groups : 0;
+  if (force_p_smem(g, 3) + extra <= SMEM_OPTIN_BUDGET) return 2;
+  return force_p_smem(g, 2) + extra <= SMEM_OPTIN_BUDGET ? 1 : 0;
 }
 int p_nbuf(const md_system* s, const Geom& g) { return p_groups(s, g) + 1; }             // tile buffers: one per group + one being loaded
 int p_max_group_threads(const md_system* s, const Geom& g) {   // whole warpgroups (register split)
@@ -721,7 +730,7 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
         (void)threads;
         const unsigned grid = (unsigned)std::min(g.ntiles, s->num_sms);
         const unsigned block = (unsigned)(ng * gth + 32 * FORCE_P_NPROD);
-        const size_t sm = force_p_smem(g, nb);
+        const size_t sm = force_p_smem(g, nb) + 2 * p_table_bytes(s);
         if (g.K == 1) CK(launch_pdl(s, pdl, k_tile_force_p<Body, 1, MODE>, grid, block, sm, A, gth, ng, nb));
         else if (g.K == 2) CK(launch_pdl(s, pdl, k_tile_force_p<Body, 2, MODE>, grid, block, sm, A, gth, ng, nb));
         else if (g.K == 4) CK(launch_pdl(s, pdl, k_tile_force_p<Body, 4, MODE>, grid, block, sm, A, gth, ng, nb));
@@ -750,6 +759,7 @@ int launch_force_T(md_system* s, const StepMode& M) {
   A.epi = M.epi; A.in_run = M.in_run; A.parity = M.parity;
   A.v = s->v[s->cur]; A.x_new = s->x[xb ^ 1]; A.xr_new = s->xr[xb ^ 1]; A.x0 = s->x0; A.type = s->type[s->cur]; A.mass = s->mass_d;
   A.dtf_type = s->dtf_d;
+  A.tab_smem_bytes = (int)p_table_bytes(s);
   A.dt = M.dt; A.half_dt_ftm2v = M.hdtf; A.trigger = M.trigger; A.flags = s->flags_d;
   if (s->style == MD_PAIR_LJ126) {
     int rc = launch_force_variant<T, LJBody, 0, EV>(s, A);
@@ -1051,6 +1061,8 @@ int md_set_option(md_system* s, const char* name, int64_t value) {
     s->opt_build_graph = value != 0;
   } else if (n == "pdl") {
     s->opt_pdl = value != 0;
+  } else if (n == "tab_smem") {
+    s->opt_tab_smem = value != 0;
   } else if (n == "tune_verbose") {
     s->tune_verbose = value != 0;
   } else {

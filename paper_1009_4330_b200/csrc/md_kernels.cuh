@@ -1267,6 +1267,8 @@ struct LJBody {
   static __device__ __forceinline__ T cell_own_w(T w) { return w; }
   template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
   static constexpr bool TABLE = false;
+  static constexpr int SMEM_TABLES = 0;   // no coefficient tables to stage (tabulated EAM has)
+  __device__ __forceinline__ void attach_tables(unsigned, unsigned) {}
   static constexpr int NT = EV ? 10 : 3;   // fx fy fz [e wxx wyy wzz wxy wxz wyz]
   using PK = typename Pk<T>::type;
   T rc2, lj1, lj2, lj3, lj4;
@@ -1308,6 +1310,8 @@ struct EamDensityBody {
   static __device__ __forceinline__ T cell_own_w(T w) { return w; }
   template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
   static constexpr bool TABLE = false;
+  static constexpr int SMEM_TABLES = 0;   // no coefficient tables to stage (tabulated EAM has)
+  __device__ __forceinline__ void attach_tables(unsigned, unsigned) {}
   static constexpr int NT = 1;
   using PK = typename Pk<T>::type;
   T rc2, q_r0, q;
@@ -1336,6 +1340,8 @@ struct EamForceBody {
   static __device__ __forceinline__ T cell_own_w(T w) { return w; }
   template <class TAB> __device__ __forceinline__ void attach(TAB*) {}
   static constexpr bool TABLE = false;
+  static constexpr int SMEM_TABLES = 0;   // no coefficient tables to stage (tabulated EAM has)
+  __device__ __forceinline__ void attach_tables(unsigned, unsigned) {}
   static constexpr int NT = EV ? 10 : 3;
   using PK = typename Pk<T>::type;
   T rc2, q_r0, q, p_r0, pp, A;
@@ -1397,6 +1403,7 @@ __device__ __forceinline__ void eam_embed(const PairParams& P, double rho, doubl
 // Tabulated EAM (SURVEY.md 8(f)-2 second half; App. A: what the paper's EAM run used; reading s26).  The same
 // two passes as the analytic style with rho(r), rho'(r), phi(r), phi'(r) from per-interval cubics: one 16-byte (fp64: 32)
 // table load per function, atom of the row and list entry, through the read-only path (the tables are a few tens of KB).
+template <typename T> __device__ __forceinline__ typename Vec4<T>::type lds_v4(unsigned a);   // defined with the force kernels' helpers
 template <typename T>
 struct TabLookup {
   using V4 = typename Vec4<T>::type;
@@ -1408,6 +1415,13 @@ struct TabLookup {
     k = k > kmax ? kmax : (k < 0 ? 0 : k);   // (r = NaN for the self term r2 = 0 of the cell-list variant: any interval will do, the term is dropped)
     u = t - (T)k;
     return k;
+  }
+  // smem != 0: the table has been staged in shared memory at that address (k_tile_force_p); else the read-only path
+  static __device__ __forceinline__ V4 load(const void* tab, unsigned smem, int k) {
+    if constexpr (sizeof(T) == 4) {
+      if (smem) return lds_v4<T>(smem + 16u * (unsigned)k);
+    }
+    return load(tab, k);
   }
   static __device__ __forceinline__ V4 load(const void* tab, int k) {
     if constexpr (sizeof(T) == 4) return __ldg(reinterpret_cast<const float4*>(tab) + k);
@@ -1429,11 +1443,14 @@ struct EamTabDensityBody {
   T rc2;
   TabLookup<T> L;
   const void* tab_rho;
+  unsigned s_rho = 0;   // shared-memory address of the staged table, 0: not staged
+  static constexpr int SMEM_TABLES = 1;
+  __device__ __forceinline__ void attach_tables(unsigned base, unsigned) { s_rho = base; }
   __device__ explicit EamTabDensityBody(const PairParams& P) : rc2(MDK_PP(rc2)), L{(T)P.inv_dr, P.tab_nr - 2}, tab_rho(P.tab_rho) {}
   __device__ __forceinline__ T rho_of(T r2) const {
     T u;
     const int k = L.interval(r2 * t_rsqrt<T>(r2), u);
-    return TabLookup<T>::value(TabLookup<T>::load(tab_rho, k), u);
+    return TabLookup<T>::value(TabLookup<T>::load(tab_rho, s_rho, k), u);
   }
   __device__ __forceinline__ void pair(T, T, T, T r2, T, bool ok, T (&p)[NT]) const { p[0] += (ok && r2 < rc2) ? rho_of(r2) : (T)0; }
   __device__ __forceinline__ void pair2(PK, PK, PK, PK r2, PK, PK (&p)[NT]) const {
@@ -1457,6 +1474,9 @@ struct EamTabForceBody {
   T rc2;
   TabLookup<T> L;
   const void *tab_rho, *tab_phi;
+  unsigned s_rho = 0, s_phi = 0;   // shared-memory addresses of the staged tables, 0: not staged
+  static constexpr int SMEM_TABLES = 2;
+  __device__ __forceinline__ void attach_tables(unsigned base, unsigned table_bytes) { s_rho = base; s_phi = base ? base + table_bytes : 0u; }
   __device__ explicit EamTabForceBody(const PairParams& P)
       : rc2(MDK_PP(rc2)), L{(T)P.inv_dr, P.tab_nr - 2}, tab_rho(P.tab_rho), tab_phi(P.tab_phi) {}
   // fpair = -[ (F'_i + F'_j) rho'(r) + phi'(r) ] / r and phi(r) of one term; zero beyond the cutoff
@@ -1465,7 +1485,7 @@ struct EamTabForceBody {
     const T rinv = t_rsqrt<T>(r2);
     T u;
     const int k = L.interval(r2 * rinv, u);
-    const V4 cr = TabLookup<T>::load(tab_rho, k), cp = TabLookup<T>::load(tab_phi, k);
+    const V4 cr = TabLookup<T>::load(tab_rho, s_rho, k), cp = TabLookup<T>::load(tab_phi, s_phi, k);
     fp = in ? -(wsum * L.slope(cr, u) + L.slope(cp, u)) * rinv : (T)0;
     phi = in ? TabLookup<T>::value(cp, u) : (T)0;
   }
@@ -1505,6 +1525,8 @@ struct BuckCoulBody {
   using PK = typename Pk<T>::type;
   using V4 = typename Vec4<T>::type;
   static constexpr bool TABLE = true;
+  static constexpr int SMEM_TABLES = 0;   // no coefficient tables to stage (tabulated EAM has)
+  __device__ __forceinline__ void attach_tables(unsigned, unsigned) {}
   static __device__ __forceinline__ T own_w(T w) { return (T)(-MAX_PAIR_TYPES) * w; }
   static __device__ __forceinline__ T mutual_w(T a, T b) { return a + b * (T)(1.0 / MAX_PAIR_TYPES); }   // -(4 t0 + t1)
   static __device__ __forceinline__ T cell_own_w(T w) { return (T)MAX_PAIR_TYPES * w; }
@@ -1588,6 +1610,7 @@ struct ForceArgs {
   double* v; double* x_new; const double* x0;
   const int* type; const double* mass;
   const double* dtf_type;  // [ntypes]: half_dt_ftm2v / mass[t] (host-prepared per md_run)
+  int tab_smem_bytes;      // tabulated EAM in k_tile_force_p: bytes of ONE coefficient table staged behind the tile buffers (0: none)
   double dt, half_dt_ftm2v, trigger;
   Flags* flags;
 };
@@ -2256,6 +2279,20 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   }
   __shared__ __align__(16) unsigned char pair_tab[Body::TABLE ? MAX_PAIR_TYPES * MAX_PAIR_TYPES * sizeof(V4) : 16];   // per-type-pair coefficients
   if constexpr (Body::TABLE) Body::fill(A.P, reinterpret_cast<V4*>(pair_tab));
+  // tabulated EAM (reading s26): the per-interval cubics of rho(r) (and phi(r) in pass 2) are copied behind the tile
+  // buffers once per launch; the bodies then look them up with one 128-bit shared-memory load instead of a global one
+  if constexpr (Body::SMEM_TABLES > 0) {
+    if (A.tab_smem_bytes) {
+      float4* dst = reinterpret_cast<float4*>(smem_raw + 128 + (size_t)NB * buf_bytes);
+      const int n4 = A.tab_smem_bytes / 16;
+      const float4* src0 = reinterpret_cast<const float4*>(A.P.tab_rho);
+      const float4* src1 = reinterpret_cast<const float4*>(A.P.tab_phi);
+      for (int i = threadIdx.x; i < n4; i += blockDim.x) {
+        dst[i] = __ldg(src0 + i);
+        if (Body::SMEM_TABLES > 1) dst[n4 + i] = __ldg(src1 + i);
+      }
+    }
+  }
   auto claims = [&](int b) { return reinterpret_cast<int*>(smem_raw + 128 + (size_t)(b + 1) * buf_bytes - FORCE_P_CLAIM_BYTES); };
   for (int i = threadIdx.x; i < NB * (FORCE_P_CLAIM_BYTES / 4); i += blockDim.x) claims(i / (FORCE_P_CLAIM_BYTES / 4))[i % (FORCE_P_CLAIM_BYTES / 4)] = 0;
   __syncthreads();
@@ -2327,6 +2364,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(FORCE_P_CONSUMER_REGS));
   Body body(A.P);
   body.attach(reinterpret_cast<V4*>(pair_tab));
+  body.attach_tables(A.tab_smem_bytes ? smem0 + 128u + (unsigned)NB * buf_bytes : 0u, (unsigned)A.tab_smem_bytes);
   const size_t ld = A.ld;
   const size_t slots_cap = (size_t)pcap * K;
   // Work is dealt to the consumer WARPS, not to groups: a task is 32 consecutive lane slots (32 / K pair rows) of one

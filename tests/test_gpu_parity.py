@@ -550,6 +550,47 @@ def test_tabulated_eam_run_and_table_checks():
     s.close()
 
 
+@pytest.mark.parametrize("kernel,shape", [(1, 0x111), (5, 0x112), (6, 0x122), (3, 0x111)])
+def test_persistent_kernel_on_a_small_box_many_tiles_per_block(kernel, shape):
+    """The persistent force kernel normally needs a box of a few hundred tiles; persistent_min_tiles_per_sm = 0 runs it on
+    any box.  16,384 atoms in one-cell (or two-, four-cell) tiles give every block several tiles, so that the tile
+    buffers are reused, tasks of three tiles are in flight at once and consumer warps help with the post-processing."""
+    w = wl.make(2, n_override=16)
+    x = wl.perturbed(w, 0.12)
+    s = md.from_workload(w, x=x, kernel=kernel, options={"persistent_min_tiles_per_sm": 0, "tile_shape": shape})
+    f = np.zeros((w.natoms, 3))
+    s.md_compute_forces(f)                                           # no energy: the persistent kernel
+    assert _rel_rms(f, oracle.forces(x, w.box, w.style, w.params, w.rc)[0]) < 1e-5
+    st = s.md_get_stats()
+    assert st["ntiles"] > 3 * 148 or shape != 0x111
+    f2 = np.zeros_like(f)
+    s.md_compute_forces(f2)
+    assert np.array_equal(f, f2)                                     # tasks are dealt dynamically, the arithmetic is not
+    s.md_run(25, w.dt)
+    xg = np.zeros((w.natoms, 3)); s.md_get_positions(xg); s.md_get_forces(f)
+    assert _rel_rms(f, oracle.forces(xg, w.box, w.style, w.params, w.rc)[0]) < 1e-5
+    s.close()
+
+
+def test_tabulated_eam_tables_staged_in_shared_memory():
+    """MD_PAIR_EAM_TAB in the persistent kernel copies its coefficient tables behind the tile buffers (option tab_smem);
+    the lookups must return what the read-only path returns: bitwise the same forces, both within tolerance of the oracle."""
+    w = wl.make_eam_tabulated(8, n_table=2001)
+    x = wl.perturbed(w, 0.2)
+    fo = oracle.forces(x, w.box, w.style, wl.oracle_params(w), w.rc)[0]
+    out = {}
+    for tab_smem in (1, 0):
+        s = md.from_workload(w, precision=md.MD_MIXED, x=x, options={"persistent_min_tiles_per_sm": 0, "tab_smem": tab_smem})
+        f = np.zeros((w.natoms, 3))
+        s.md_compute_forces(f)
+        assert _rel_rms(f, fo) < 1e-5
+        s.md_run(10, w.dt)
+        s.md_get_forces(f)
+        out[tab_smem] = f
+        s.close()
+    assert np.array_equal(out[0], out[1])
+
+
 # ---- SURVEY.md 8(f)-4: NVT, one Nose-Hoover thermostat (PAPER.md L52; reading s25) -----------------------------------
 
 @pytest.mark.parametrize("cfg,n,nsteps,kT_factor,tau,list_kind", [(1, 7, 60, 0.5, 0.1, 0), (1, 7, 40, 0.5, 0.1, 1), (4, 6, 40, 2.0, 0.02, 0)])
