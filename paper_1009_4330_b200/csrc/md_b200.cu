@@ -727,7 +727,6 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
         // all the consumer warps the register budget allows: the kernel deals 32-lane tasks to whichever warp is free,
         // so the tile's row count no longer has to match a group's size
         const int gth = p_max_group_threads(s, g);   // whole warpgroups
-        (void)threads;
         const unsigned grid = (unsigned)std::min(g.ntiles, s->num_sms);
         const unsigned block = (unsigned)(ng * gth + 32 * FORCE_P_NPROD);
         const size_t sm = force_p_smem(g, nb) + 2 * p_table_bytes(s);

@@ -2251,16 +2251,15 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   const unsigned buf_bytes = (unsigned)force_p_buf_bytes(g);
   const unsigned smem0 = smem_addr(smem_raw);
   // per buffer: `tabfull` (the table has landed), `full` (the coordinates have landed), `ready` (the cell offsets
-  // have been added: the list loop may start), `empty` (the consumers are done: the producer may refill), and a
-  // work counter `ctr` for the post-processing chunks
+  // have been added: the list loop may start), `empty` (all tasks of the tile are done: the producer may refill);
+  // behind the mbarriers, in the 128-byte header: the consumers' task counter and the per-buffer finished-task counts
   constexpr int MB = FORCE_P_MAX_NBUF;
   auto full = [&](int b) { return smem0 + 8u * (unsigned)b; };
   auto tabfull = [&](int b) { return smem0 + 8u * (unsigned)(MB + b); };
   auto empty = [&](int b) { return smem0 + 8u * (unsigned)(2 * MB + b); };
   auto ready = [&](int b) { return smem0 + 8u * (unsigned)(3 * MB + b); };
-  int* ctr = reinterpret_cast<int*>(smem_raw + 8 * 4 * MB);
-  int* next_task = ctr + MB;   // the consumers' task counter
-  volatile int* fin = ctr + MB + 1;   // per buffer: tasks finished in it since the launch began (never reset)
+  int* next_task = reinterpret_cast<int*>(smem_raw + 8 * 4 * MB);   // the consumers' task counter
+  volatile int* fin = next_task + 1;   // per buffer: tasks finished in it since the launch began (never reset)
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int gwarps = gthreads >> 5;
   const int nchunks = force_p_chunks(g);
@@ -2271,7 +2270,6 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tabfull(b)), "r"(1) : "memory");
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(empty(b)), "r"(tasks_per_tile) : "memory");
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(ready(b)), "r"(nchunks) : "memory");
-      ctr[b] = 0;
     }
     *next_task = 0;
     for (int b = 0; b < MB; ++b) fin[b] = 0;
@@ -2315,7 +2313,6 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
     // (while the cells of tile k - 1 are in flight, if the buffer is free by then) or at the top of iteration k
     auto request_table = [&](int k) {
       const int b = k % NB;
-      ctr[b] = 0;
       mbar_expect_tx(tabfull(b), (unsigned)tab_ints * 4u);
       bulk_g2s(smem0 + 128u + (unsigned)b * buf_bytes, A.tab + (size_t)((int)blockIdx.x + k * (int)gridDim.x) * tab_ints, (unsigned)tab_ints * 4u,
                tabfull(b));
