@@ -175,7 +175,8 @@ int md_set_neighbor(md_system* s, int list_kind, int kernel);
  * all of them; SURVEY.md 8(f)-1 sweeps use them).  Invalidates the list and the variant choice.  Names:
  *   "tile_shape"  bx | by << 4 | bz << 8 cells per tile (4 >= bx >= by >= bz >= 1), 0: planner
  *   "force_threads"  block size of the list force kernels, 0: planner
- *   "persistent_groups"  consumer groups of the persistent force kernel: 1, 2, or 0 = automatic
+ *   "persistent_groups"  tile buffers of the persistent force kernel minus one: 1 (two buffers), 2 (three), 0 = automatic
+ *               (the name dates from the version that dealt tiles to that many fixed groups of consumer warps)
  *   "persistent_min_tiles_per_sm"  the persistent kernel is used from this many tiles per SM on (default 1)
  *   "no_persistent"  1: run the one-block-per-tile kernel everywhere
  *   "balance_after"  apply the row balancing to a list that has lived this many steps (default 48; <= 0: at every build)

@@ -79,7 +79,7 @@ struct md_system_impl {
   int balance_after = 0;     // BALANCE_AFTER, or MD_B200_BALANCE_AFTER (tuning experiments)
   bool no_balance = false;   // MD_B200_NO_BALANCE=1: skip the row-balancing pass (for A/B measurements)
   int p_min_tiles_per_sm = 1;   // k_tile_force_p is used from this many tiles per SM on (MD_B200_PMIN; measured: cfg 4 -4 % at 2-3 tiles per SM)
-  int p_groups = 0;             // consumer groups of the persistent force kernel; 0: two if three tile buffers fit, else one (MD_B200_PGROUPS)
+  int p_groups = 0;             // tile buffers of the persistent force kernel minus one; 0: two (three buffers) if they fit, else one
   bool no_persistent = false;   // MD_B200_NO_PERSISTENT=1: run k_tile_force where k_tile_force_p would be used (A/B measurements)
   int brick_forced = 0;   // tile shape chosen by the autotuner, bx | by << 4 | bz << 8 (0: the planner's own pick)
   int opt_tile_shape = 0;     // md_set_option("tile_shape"): bx | by << 4 | bz << 8, 0: planner
@@ -270,8 +270,6 @@ constexpr size_t SMEM_OPTIN_BUDGET = 227 * 1024 - 1024;
 bool persistent_eligible(const md_system* s) {
   return s->precision == MD_MIXED && s->list_kind == MD_LIST_FULL && s->kernel_eff != MD_KERNEL_CELL && !s->no_persistent;
 }
-// Consumer groups per block: two, with three tile buffers (two being computed on, one being loaded), when they fit the
-// SM's shared memory; else one group with two buffers (rc = 5 sigma: a 3x1x1 tile stages 108 KB); 0: does not fit.
 // Tabulated EAM: the two coefficient tables (rho, phi: 16 bytes per interval) are staged in shared memory behind the
 // tile buffers when they are small enough to leave room for two buffers; bytes of ONE table, 0: read through L1/L2.
 size_t p_table_bytes(const md_system* s) {
@@ -279,6 +277,8 @@ size_t p_table_bytes(const md_system* s) {
   const size_t one = (size_t)(s->eam_nr - 1) * 16;
   return one <= 48 * 1024 ? one : 0;
 }
+// Tile buffers per block minus one (historically: consumer groups): two, i.e. three buffers, when they fit the
+// SM's shared memory; else one, i.e. two buffers (rc = 5 sigma: a 3x1x1 tile stages 108 KB); 0: does not fit.
 int p_groups(const md_system* s, const Geom& g) {
   const size_t extra = 2 * p_table_bytes(s);
   if (s->p_groups > 0) return force_p_smem(g, s->p_groups + 1) + extra <= SMEM_OPTIN_BUDGET ? s->p_groups : 0;
@@ -722,7 +722,7 @@ int launch_force_variant(md_system* s, const ForceArgs& A) {
   } else {
     if constexpr (std::is_same<T, float>::value && !EV) {
       if (use_persistent(s, g)) {
-        // persistent, warp-specialised path: one block per SM, two consumer groups of `threads` + one producer warp
+        // persistent, warp-specialised path: one block per SM, ng * gth consumer threads (tasks dealt to warps) + the producer warps
         const int ng = p_groups(s, g), nb = p_nbuf(s, g);
         // all the consumer warps the register budget allows: the kernel deals 32-lane tasks to whichever warp is free,
         // so the tile's row count no longer has to match a group's size
