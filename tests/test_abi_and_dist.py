@@ -53,6 +53,37 @@ def test_argument_errors_without_a_gpu():
     assert md.lib.md_set_units(None, 1.0, 1.0) == md.MD_ERR_BAD_ARGUMENT
 
 
+def test_noalloc_entry_point_checks_its_arguments_before_any_cuda_call():
+    """md_kinetic_energy_noalloc rejects NULL pointers and sizes outside (0, MD_NOALLOC_MAX_ATOMS] with a clear message,
+    and the limit in the binding is the header's."""
+    from paper_1009_4330_b200 import md
+    text = open(os.path.join(ROOT, "include", "md_b200.h")).read()
+    assert int(re.search(r"#define MD_NOALLOC_MAX_ATOMS (\d+)LL", text).group(1)) == md.MD_NOALLOC_MAX_ATOMS
+    assert int(re.search(r"#define MD_NOALLOC_SCRATCH_BYTES (\d+)", text).group(1)) == md.MD_NOALLOC_SCRATCH_BYTES
+    assert md.MD_NOALLOC_MAX_ATOMS == (md.MD_NOALLOC_SCRATCH_BYTES - 256) // 8 * 256
+    fake = 4096     # never dereferenced: the checks come first
+    f = md.lib.md_kinetic_energy_noalloc
+    assert f(None, fake, fake, 10, 1.0, fake, None) == md.MD_ERR_BAD_ARGUMENT and b"NULL" in md.lib.md_last_error(None)
+    assert f(fake, fake, fake, 10, 1.0, None, None) == md.MD_ERR_BAD_ARGUMENT
+    assert f(fake, fake, fake, 0, 1.0, fake, None) == md.MD_ERR_BAD_ARGUMENT and b"positive" in md.lib.md_last_error(None)
+    assert f(fake, fake, fake, md.MD_NOALLOC_MAX_ATOMS + 1, 1.0, fake, None) == md.MD_ERR_BAD_ARGUMENT
+    msg = md.lib.md_last_error(None).decode()
+    assert "MD_NOALLOC_MAX_ATOMS" in msg and str(md.MD_NOALLOC_MAX_ATOMS + 1) in msg
+
+
+def test_roofline_traffic_is_read_from_the_committed_ncu_summaries():
+    """bench.py takes roofline.traffic from the `dram_bytes_per_launch:` lines that ncu_summary wrote into profiles/."""
+    from paper_1009_4330_b200 import ncu_summary
+    prof = os.path.join(ROOT, "profiles")
+    t5 = ncu_summary.traffic(os.path.join(prof, "r02_ncu_full_force_cfg5.md"))
+    assert t5 is not None and 5e8 < t5 < 3e9                      # a 4 M-atom LJ force launch moves about a gigabyte
+    one = ncu_summary.traffic(os.path.join(prof, "r02_ncu_full_force_cfg4.md"), sections=1)
+    two = ncu_summary.traffic(os.path.join(prof, "r02_ncu_full_force_cfg4.md"), sections=2)
+    assert one is not None and two is not None and two > one      # EAM: density pass + force pass
+    assert ncu_summary.traffic(os.path.join(prof, "r02_ncu_full_force_cfg4.md"), sections=3) is None
+    assert ncu_summary.traffic(os.path.join(prof, "no_such_file.md")) is None
+
+
 def test_product_path_never_imports_the_oracle():
     for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_1009_4330_b200")):
         for fn in files:
