@@ -15,6 +15,8 @@
  *     chosen by a setup-time mini benchmark (L137)
  *   velocity-Verlet NVE and Nose-Hoover NVT, positions/velocities/forces resident on the device (L50-58)
  *   rebuild iff max_i |x_i - x0_i|^2 > (skin/2)^2, decided on the device.
+ *   md_run keeps the host out of the loop: one fused launch per time step (two for EAM) with programmatic dependent
+ *   launch, the rebuild flag read once per batch of steps, rebuilds enqueued without waiting and replayed as a CUDA graph.
  *
  * Conventions
  *   - Every call returns MD_OK (0) or a negative MD_ERR_*; nothing throws or

@@ -2147,17 +2147,19 @@ __global__ void __launch_bounds__(256) k_eam_embed(int N, PairParams P, const do
 // Measured on B200 at cfg 5: the prologue of k_tile_force (table loads -> barrier -> ~140 small bulk copies ->
 // mbarrier wait -> offset pass -> barrier) is a chain of dependent round trips worth 0.16 ms of a 0.51 ms
 // launch, with a third of the resident warps waiting in it at any time.  Here
-//   * one PRODUCER warp walks the block's tiles ahead of the others: one bulk copy brings the tile's table
+//   * four PRODUCER warps walk the block's tiles ahead of the others: one bulk copy brings the tile's table
 //     (k_tile_tables: cell starts, counts, offsets, quad map) into shared memory, then one bulk copy per tile
-//     cell stages the packed coordinates, all counted on the buffer's `full` mbarrier;
-//   * two CONSUMER groups of `gthreads` threads each take the block's tiles alternately; a group waits for its
-//     buffer, adds the cell offsets in place (shared memory only), runs the list loop and the fused epilogue,
-//     and hands the buffer back through the `empty` mbarrier;
-//   * three tile buffers: two being computed on, one being loaded.
-// Tiles of a block: blockIdx.x + k gridDim.x; tile k uses buffer k % 3 and group k % 2.
-// Shared memory: mbarriers (128 B) | 3 x { table[tile_tab_stride] ints | st[capA] float4 | scell[interior_cap] u16 }.
+//     cell stages the packed coordinates, all counted on the buffer's `full` mbarrier; then they add the cell
+//     offsets in place in chunks of 128 slots, each chunk counted on the buffer's `ready` mbarrier;
+//   * 24 CONSUMER warps take 32-lane tasks (32 / K pair rows of one tile) from a shared counter, in tile order: a warp
+//     waits for its tile (helping with the tile's chunks meanwhile), runs the list loop and the fused epilogue, and
+//     counts the task on the buffer's `empty` mbarrier, which the producers wait for before they refill the buffer;
+//   * three tile buffers (two where three do not fit).
+// Tiles of a block: blockIdx.x + k gridDim.x; tile k uses buffer k % NB.
+// Shared memory: header (128 B: mbarriers, task counter, finished-task counts) | NB x { table[tile_tab_stride] ints |
+// st[capA] float4 | scell[interior_cap] u16 | claim words } | (tabulated EAM: the coefficient tables).
 // ---------------------------------------------------------------------------------------------------
-constexpr int FORCE_P_MAX_NBUF = 3;               // tile buffers: ngroups being computed on + one being loaded
+constexpr int FORCE_P_MAX_NBUF = 3;               // tile buffers
 constexpr int FORCE_P_MAX_REGS = 72;              // registers per thread at launch: up to 896 threads per block
 constexpr int FORCE_P_MAX_THREADS = 896;          // consumer threads + the producer warps
 constexpr int FORCE_P_CONSUMER_REGS = 80;         // after the register split below: (896 x 72 - 128 x 24) / 768
@@ -2263,7 +2265,8 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int gwarps = gthreads >> 5;
   const int nchunks = force_p_chunks(g);
-  const int tasks_per_tile = (prow_cap(g) * K + 31) >> 5;
+  constexpr int ROUNDS = K >= 32 ? 4 : 1;   // 32-lane rounds per task: a warp per row takes four rows at a time (the dealing costs as much as a short row)
+  const int tasks_per_tile = (prow_cap(g) * K + 32 * ROUNDS - 1) / (32 * ROUNDS);
   if (threadIdx.x == 0) {
     for (int b = 0; b < NB; ++b) {
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(full(b)), "r"(1) : "memory");
@@ -2357,7 +2360,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
     return;
   }
 
-  // ---------------- consumer groups ----------------
+  // ---------------- consumer warps ----------------
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(FORCE_P_CONSUMER_REGS));
   Body body(A.P);
   body.attach(reinterpret_cast<V4*>(pair_tab));
@@ -2367,7 +2370,7 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
   // Work is dealt to the consumer WARPS, not to groups: a task is 32 consecutive lane slots (32 / K pair rows) of one
   // tile, handed out in tile order from a shared counter.  A block's tiles rarely divide evenly among two groups (cfg 4:
   // three tiles per SM left one group idle for a third of the launch), and a tile's rows rarely fill a group.
-  const int tpt = ((int)slots_cap + 31) >> 5;   // tasks per tile (the trailing ones of a tile are empty: pcap is a capacity)
+  const int tpt = tasks_per_tile;               // (the trailing tasks of a tile are empty: pcap is a capacity)
   const int ntasks = ntl * tpt;
   double d2max = 0.0;
   for (;;) {
@@ -2379,8 +2382,9 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
     const int b = k % NB, j = k / NB;
     const int tile = (int)blockIdx.x + k * (int)gridDim.x;
     const uint4* tlist = A.list + (size_t)tile * g.chunk_cap * slots_cap;
-    const int sidx = tc * 32 + lane;
-    const int r = sidx / K, s = sidx % K;                   // pair row, lane of the row
+    int sidx = tc * (32 * ROUNDS) + lane;
+    int r = sidx / K;                                       // pair row
+    const int s = sidx % K;                                 // lane of the row (the same in every round)
     // while the tile lands: this lane's row length and first list word
     int n_first = 0;
     uint4 w_first = make_uint4(0, 0, 0, 0);
@@ -2406,7 +2410,17 @@ __global__ void __maxnreg__(FORCE_P_MAX_REGS) k_tile_force_p(ForceArgs A, int gt
     int c0[3], wdt[3];
     tile_dims(g, tile, c0, wdt);
     const int nlanes = (tv.n_int_slots() >> 1) * K;
-    {
+#pragma unroll 1
+    for (int rr = 0; rr < ROUNDS; ++rr) {
+      if (rr > 0) {
+        sidx += 32;
+        r = sidx / K;
+        n_first = 0;
+        if (sidx < (int)slots_cap) {
+          n_first = A.numneigh[(size_t)tile * pcap + r];
+          w_first = ld_stream(tlist + sidx);
+        }
+      }
       unsigned cells = 0xffffffffu;
       if (sidx < nlanes) cells = reinterpret_cast<const unsigned*>(scell)[r];
       const unsigned cell = cells & 0xffffu;
