@@ -415,6 +415,9 @@ def run_ours(args, rk) -> None:
                    "variant": md.KERNEL_NAMES[st["kernel_variant"]], "mean_neighbors": st["mean_neighbors"],
                    "builds_per_step": st["nbuilds_in_run"], "tiles": st["ntiles"], "brick": st["brick"],
                    "parallelism": "replicas x%d (no collective)" % rk.world,
+                   "launch": ("one fused kernel per time step (two for EAM) with programmatic dependent launch; rebuild flag read "
+                              "once per batch of steps; rebuilds enqueued without waiting, replayed as a CUDA graph"
+                              + ("; options " + ",".join(args.opt) if args.opt else "")),
                    "l2": "L2 flushed between passes (2x126 MB write)" if dev_run["flushed_l2"] else
                          "inputs larger than L2 (state + list >> 126 MB)"},
         "clocks": clocks, "roofline": roofline, "roofline_build": roofline_build,
